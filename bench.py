@@ -1,0 +1,320 @@
+#!/usr/bin/env python
+"""bench.py -- MLUPs and HBM-roofline fraction of the fused LBM step on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+Workload at N = 1: BASELINE.json config 3 (configs[2]) -- D3Q19 Smagorinsky + HLBM, fp32, 384x192x128
+urban channel -- the configuration the metric "MLUPs ... for D3Q19 Smagorinsky+HLBM" and the
+north_star target are quoted on.  A "step" is one lattice time step = one pass of the whole hot path
+ over all cells = one fused kernel launch.  One step moves 1.48 GB, far more
+than the 126 MB L2, so no L2 flush is needed between steps.
+N > 1: the path does not shard in this build ("replicas only"): every rank runs the same
+workload on its own GPU, no data-path collective; value = sum over ranks / max time.
+--impl reference: the CPU oracle (oracle/), as it stands, timed on the host cores on a bounded sample.
+Prints ONE JSON line on rank 0.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import lbm_inputs as I  # noqa: E402
+
+METRIC = "MLUPs"
+UNIT = "MLUPs (1e6 non-SOLID lattice cell updates per second)"
+WORKLOADS = {
+    # name: (config number, shape (nz,ny,nx) or None for the config's own, dtype)
+    "config3_urban_channel_384x192x128_f32": (3, None, "f32"),
+    "config2_les_periodic_256_f32": (2, None, "f32"),
+    "config4_d3q27_spheres_512_f32": (4, None, "f32"),
+    "config3_urban_channel_384x192x128_f64": (3, None, "f64"),
+    "config5_urban_cube_128_f32": (5, (128, 128, 128), "f32"),
+    "config5_urban_cube_256_f32": (5, (256, 256, 256), "f32"),
+    "config5_urban_cube_512_f32": (5, (512, 512, 512), "f32"),
+    "config1_tgv_32_f64": (1, None, "f64"),
+}
+DEFAULT_WORKLOAD = "config3_urban_channel_384x192x128_f32"
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def algorithmic_bytes_per_step(cfg, dtype, n_solid):
+    """2*Q*sizeof(T) + sizeof(T) (porosity, when use_hlbm) + 1 (flag) per non-SOLID cell,
+    1 byte per SOLID cell."""
+    sz = 4 if dtype == "f32" else 8
+    N = int(np.prod(cfg["shape"]))
+    per_cell = 2 * cfg["Q"] * sz + (sz if cfg["params"].get("use_hlbm") else 0) + 1
+    return (N - n_solid) * per_cell + n_solid * 1, per_cell
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz, self._stop_evt = index, [], set(), None, threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20,
+                 "hw_power_brake_slowdown": 0x80, "sync_boost": 0x10}
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(0.02)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def cpu_oracle_time(cfg_number, sample_shape, nsteps, nthreads):
+    """Time the oracle, as it stands, on a bounded sample of the workload."""
+    from oracle import oracle as O
+    cfg = I.make_config(cfg_number, shape=sample_shape) if cfg_number != 1 else I.make_config(1)
+    f = O.init_equilibrium(cfg["Q"], cfg["rho"], cfg["u"])
+    nonsolid = f[0].size if cfg["flags"] is None else int(((cfg["flags"] & 15) != I.SOLID).sum())
+    O.step(f, d=cfg["d"], flags=cfg["flags"], nsteps=1, nthreads=nthreads, **cfg["params"])     # warm-up
+    t0 = time.perf_counter()
+    O.step(f, d=cfg["d"], flags=cfg["flags"], nsteps=nsteps, nthreads=nthreads, **cfg["params"])
+    dt = time.perf_counter() - t0
+    return nonsolid * nsteps / dt / 1e6, dt, cfg["shape"]
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the CPU oracle on the host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    from oracle import oracle as O
+    number, shape, dtype = WORKLOADS[args.workload]
+    cores = O.max_threads()
+    total = max(args.steps + args.warmup, 1)
+    # bounded sample: a reduced instance of the same generator, sized for roughly a minute in total
+    cells_budget = max(int(60.0 * 1.0e6 / total), 4096)
+    if number == 1:
+        sample = (32, 32, 32)
+    else:
+        base = {2: (256, 256, 256), 3: (128, 192, 384), 4: (512, 512, 512), 5: shape}[number]
+        scale = min(1.0, (cells_budget / float(np.prod(base))) ** (1.0 / 3.0))
+        sample = tuple(max(16, int(round(b * scale / 8)) * 8) for b in base)
+    cfg = I.make_config(number, shape=sample) if number != 1 else I.make_config(1)
+    f = O.init_equilibrium(cfg["Q"], cfg["rho"], cfg["u"])
+    nonsolid = f[0].size if cfg["flags"] is None else int(((cfg["flags"] & 15) != I.SOLID).sum())
+    kw = dict(d=cfg["d"], flags=cfg["flags"], nthreads=cores, **cfg["params"])
+    f = O.step(f, nsteps=args.warmup, **kw)
+    t0 = time.perf_counter()
+    f = O.step(f, nsteps=args.steps, **kw)
+    dt = time.perf_counter() - t0
+    value = nonsolid * args.steps / dt / 1e6
+    sample_txt = "oracle (fp64, %d OpenMP threads) on U%s generated like the workload, %d steps" % (
+        str(tuple(reversed(sample))), cores, args.steps)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt / max(args.steps, 1) * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "sample_shape_nz_ny_nx": list(sample)},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample_txt},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--option", action="append", default=[], help="library option key=value (tuning)")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    if args.impl == "reference":
+        if args.steps is None:
+            args.steps = 10
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_2506_21804_b200 as P
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    number, shape, dtype = WORKLOADS[args.workload]
+    cfg = I.make_config(number, shape=shape)
+    if args.steps is None:
+        args.steps = cfg["steps"]
+    nz, ny, nx = cfg["shape"]
+    N = nx * ny * nz
+    Q = cfg["Q"]
+    tdt = torch.float32 if dtype == "f32" else torch.float64
+    npdt = np.float32 if dtype == "f32" else np.float64
+    par = P.LbmParams(**cfg["params"])
+
+    stream = torch.cuda.current_stream()
+    sim = P.LBM(Q, nx, ny, nz, dtype, stream=stream.cuda_stream)
+    for kv in args.option:
+        k, v = kv.split("=")
+        sim.set_option(k, int(v))
+
+    # inputs resident in HBM before the timed region
+    rho_d = torch.from_numpy(cfg["rho"].astype(npdt)).cuda()
+    u_d = torch.from_numpy(cfg["u"].astype(npdt)).cuda()
+    d_d = None if cfg["d"] is None else torch.from_numpy(cfg["d"].astype(npdt)).cuda()
+    fl_d = None if cfg["flags"] is None else torch.from_numpy(cfg["flags"]).cuda()
+    sim.set_geometry(d_d, fl_d)
+    sim.init_equilibrium(rho_d, u_d)
+    n_solid = sim.query("solid_cells")
+    n_fluid = N - n_solid
+    tot0 = sim.totals()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing -------------------------------------------------------------------
+    sim.step(args.warmup, par)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    l0 = sim.query("launches")
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    sim.step(args.steps, par)
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    launches = sim.query("launches") - l0
+    ms = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    tot1 = sim.totals()
+    finite = bool(np.isfinite(tot1).all())
+    value = world * n_fluid * args.steps / (ms * 1e-3) / 1e6
+    step_bytes, per_cell = algorithmic_bytes_per_step(cfg, dtype, n_solid)
+    peak, peak_src = measured_peak()
+    achieved = step_bytes / (ms * 1e-3 / max(launches, 1)) / 1e9      # GB/s, per launch = per step
+
+    # ---- end to end through the C ABI with HOST buffers ------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        h_f = torch.empty((Q, nz, ny, nx), dtype=tdt).pin_memory()
+        sim.init_equilibrium(rho_d, u_d)
+        sim.get_populations(h_f)                       # host copy of S_0 (not timed)
+        h_d = None if cfg["d"] is None else torch.from_numpy(cfg["d"].astype(npdt)).pin_memory()
+        h_fl = None if cfg["flags"] is None else torch.from_numpy(cfg["flags"]).pin_memory()
+        h_rho = torch.empty((nz, ny, nx), dtype=tdt).pin_memory()
+        h_u = torch.empty((3, nz, ny, nx), dtype=tdt).pin_memory()
+        sim.moments(h_rho, h_u)                        # warms the staging buffer
+        barrier()
+        t0 = time.perf_counter()
+        sim.set_fields(h_f, h_d, h_fl)                 # H2D: populations + porosity + flags
+        sim.step(args.steps, par)
+        sim.moments(h_rho, h_u)                        # D2H: rho, u
+        sim.synchronize()
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        h2d = h_f.numel() * h_f.element_size() + (0 if h_d is None else h_d.numel() * h_d.element_size()) + \
+            (0 if h_fl is None else h_fl.numel())
+        d2h = 4 * N * h_rho.element_size()
+        e2e = {"value": world * n_fluid * args.steps / dt / 1e6, "unit": UNIT,
+               "h2d_bytes_per_step": h2d / args.steps, "d2h_bytes_per_step": d2h / args.steps,
+               "what": "lbm_set_fields(host populations, porosity, flags) + lbm_step(K) + lbm_moments(host rho,u), wall clock"}
+
+    # ---- CPU oracle beside it (rank 0, N = 1 only; bounded sample) -------------------------------
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle import oracle as O
+        cores = O.max_threads()
+        if number == 1:
+            sample_shape, ns = None, 20
+        else:
+            base = np.array(cfg["shape"], dtype=float)
+            scale = min(1.0, (1.5e6 / base.prod()) ** (1.0 / 3.0))
+            sample_shape = tuple(max(16, int(round(b * scale / 8)) * 8) for b in base)
+            ns = 4
+        v, dt_cpu, shp = cpu_oracle_time(number, sample_shape, ns, cores)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": "fp64 oracle, %d OpenMP threads, workload generator at (nz,ny,nx)=%s, %d steps after 1 warm-up, %.1f s"
+                         % (cores, str(tuple(shp)), ns, dt_cpu)}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": dtype, "data": "synthetic",
+            "config": {"workload": args.workload, "lattice": "D3Q%d" % Q, "nx": nx, "ny": ny, "nz": nz, "cells": N,
+                       "solid_cells": n_solid, "masked_cells": sim.query("masked_cells"), "params": cfg["params"],
+                       "l2": "inputs larger than L2 (%.2f GB per step)" % (step_bytes / 1e9),
+                       "mlups_all_cells": world * N * args.steps / (ms * 1e-3) / 1e6, "parallelism": "replicas only",
+                       "finite": finite, "mass_drift_rel": (tot1[0] - tot0[0]) / tot0[0],
+                       "bytes_per_update": per_cell},
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "peak_source": peak_src, "frac_of_8000_datasheet": achieved / 8000.0,
+                         "algorithmic_bytes_per_launch": step_bytes, "kernel": "lbm::k_step<%d,%s,STREAM_COLLIDE>" % (Q, "float" if dtype == "f32" else "double")},
+            "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        }
+        print(json.dumps(line), flush=True)
+    sim.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,143 @@
+/* =====================================================================================
+ * lbm.h -- C ABI of the B200-native lattice Boltzmann hot path of arxiv 2506.21804
+ * (BGK + Smagorinsky LES + homogenised-LBM porosity; D3Q19 / D3Q27; fp32 / fp64).
+ *
+ * Library: paper_2506_21804_b200/liblbm_b200.so (CUDA, sm_100a).  Every step of the path runs
+ * in the library's own kernels; there is no CPU fallback: every call fails with LBM_ECUDA when no
+ * CUDA device is usable.
+ *
+ * Citations are to /root/reference/PAPER.md (line : equation) and to the readings listed in
+ * DESIGN.md (G1..G26, R1..R12), which follow SURVEY.md section 8(c).
+ *
+ * Conventions common to all calls
+ *  - Return value: 0 on success, <0 on error (enum below).  Nothing throws or aborts across the ABI.
+ *  - POINTERS: every data pointer may be a DEVICE pointer (e.g. torch CUDA tensor data_ptr()) or a
+ *    HOST pointer (pageable or pinned).  The library inspects the pointer (cudaPointerGetAttributes)
+ *    and copies host buffers to / from the device on the context's stream.  Device buffers are used
+ *    in place, with no copy, wherever the layouts allow.
+ *  - OWNERSHIP: the caller owns every buffer it passes; the library copies inputs into its own
+ *    storage and writes outputs into caller buffers of exactly the stated size.  The library owns
+ *    the lbm_ctx and all internal device memory (cudaMalloc), released by lbm_destroy.
+ *  - EXTERNAL LAYOUTS (fixed; x fastest; `dtype` = float or double as chosen at lbm_create):
+ *        populations[Q][nz][ny][nx]   plain f_i, population order of reading R1 (see below)
+ *        porosity   [nz][ny][nx]      d in [0,1]; Eq. 12 convention: 0 = fluid, 1 = solid (G2)
+ *        cell_flags [nz][ny][nx]      uint8
+ *        rho        [nz][ny][nx],  u[3][nz][ny][nx]
+ *  - FLAG BYTE: low nibble = type {0 FLUID, 1 SOLID, 2 INLET, 3 OUTLET, 4 WALLMODEL}.  For
+ *    WALLMODEL the high nibble is the wall-normal code {0:+x, 1:-x, 2:+y, 3:-y, 4:+z, 5:-z}
+ *    pointing from the wall into the fluid (config 3 floor cells: 0x44); otherwise it must be 0.
+ *    INLET is accepted only on the plane x = 0, OUTLET only on x = nx-1.
+ *  - POPULATION ORDER (R1): i = 0 rest; 1..h (h = (Q-1)/2) the directions whose first non-zero
+ *    component is +1 sorted by (|c|^2, -cx, -cy, -cz); h+1..Q-1 their negatives, opp(i) = i +- h.
+ *  - STATE (G12/R2): the state S_t is the set of PRE-collision populations f_i(x,t) of Eq. 6.
+ *    lbm_step(n) advances S_t -> S_{t+n}.  lbm_moments / lbm_totals / lbm_get_populations always
+ *    describe S_t, whatever the internal storage is.
+ *  - ASYNCHRONY: lbm_step only enqueues kernels on the context's stream.  All other calls
+ *    return after their copies have been enqueued; calls that must return a value to the host
+ *    (lbm_totals, outputs into host buffers, flag validation in lbm_set_fields) synchronise the
+ *    stream.  A launch error is reported at the latest by the next call.
+ * ===================================================================================== */
+#ifndef PAPER_2506_21804_B200_LBM_H
+#define PAPER_2506_21804_B200_LBM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { LBM_OK = 0, LBM_EINVAL = -1, LBM_ENOMEM = -2, LBM_ECUDA = -3, LBM_ESTATE = -4 };
+enum { LBM_D3Q19 = 19, LBM_D3Q27 = 27 };
+enum { LBM_F32 = 4, LBM_F64 = 8 };
+enum { LBM_FLUID = 0, LBM_SOLID = 1, LBM_INLET = 2, LBM_OUTLET = 3, LBM_WALLMODEL = 4 };
+
+typedef struct lbm_ctx lbm_ctx; /* opaque; owned by the library */
+
+/* Step parameters.  All reals are double whatever the dtype; converted once per lbm_step. */
+typedef struct {
+  double tau0;      /* molecular relaxation time, > 0.5; nu = (tau0 - 0.5)/3  (Eq. 14, G3)         */
+  double cs_smago;  /* Smagorinsky constant C_S >= 0 (Eq. 4); 0 => plain BGK                       */
+  int use_hlbm;     /* 0: d treated as 0 everywhere (porosity is not read); 1: Eq. 12              */
+  double u_in[3];   /* velocity imposed on INLET cells (l.155, reading R6)                         */
+  int wm_enable;    /* 0: WALLMODEL cells behave as FLUID; 1: Spalding wall model (Eq. 15-17, R8)  */
+  double wm_kappa;  /* Spalding constants; the paper prints neither (defaults 0.41, 9.8)           */
+  double wm_E;
+} lbm_params;
+
+/* Create a context for an nx x ny x nz lattice (nx fastest in memory).
+ * lattice: LBM_D3Q19 | LBM_D3Q27 (l.60; D3Q27 from BASELINE.json config 4).  dtype: LBM_F32 | LBM_F64.
+ * nx, ny, nz >= 1 and nx*ny*nz < 2^31.  Allocates two population lattices (2*Q*N*dtype bytes), the
+ * porosity field and one class byte per cell on the current CUDA device.
+ * Returns NULL on failure; lbm_last_error(NULL) then holds the reason. */
+lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype);
+
+/* Release the context and all its device memory.  NULL is ignored. */
+void lbm_destroy(lbm_ctx* ctx);
+
+/* Set the state S_0 and the fields (Eq. 6 l.70-72: populations on the lattice; Eq. 12-13 l.99-103:
+ * porosity d(x); Listing 1: per-cell model switches).  Resets the step counter to 0.
+ *   populations : [Q][nz][ny][nx] dtype, host or device; must not be NULL.
+ *   porosity    : [nz][ny][nx] dtype, or NULL => d = 0 everywhere.
+ *   cell_flags  : [nz][ny][nx] uint8, or NULL => all FLUID.
+ * Errors: LBM_EINVAL for a NULL ctx / populations or an invalid flag byte (nothing is changed then:
+ * a context that held a valid state keeps it); LBM_ECUDA. */
+int lbm_set_fields(lbm_ctx* ctx, const void* populations, const void* porosity, const uint8_t* cell_flags);
+
+/* Set S_0 = f^eq(rho, u) cell by cell (Eq. 11 l.94 truncated after H(2); A4).  rho[nz][ny][nx],
+ * u[3][nz][ny][nx] dtype, host or device.  Porosity and flags are kept as last set (or d = 0 / all FLUID
+ * if lbm_set_fields was never called).  Resets the step counter to 0. */
+int lbm_init_equilibrium(lbm_ctx* ctx, const void* rho, const void* u);
+
+/* Replace porosity and flags only (same rules as lbm_set_fields); the populations are kept. */
+int lbm_set_geometry(lbm_ctx* ctx, const void* porosity, const uint8_t* cell_flags);
+
+/* Advance S_t -> S_{t+n_steps}: per step, per non-SOLID cell (Eq. 6, l.70):
+ *   wall model u^B (Eq. 15-17, l.131) -> moments (l.97) -> u^ = (1-d)u + d u^B (Eq. 12) -> f^eq (Eq. 11)
+ *   -> tau_eff from the local non-equilibrium stress (Eq. 3-5, 14) -> relaxation (Eq. 6) -> propagation
+ *   with halfway bounce-back at SOLID neighbours (R5), zero-gradient outlet (R7), regularised velocity
+ *   inlet (l.155, R6).
+ * One fused kernel launch per step on the context's stream; asynchronous.
+ * Errors: LBM_EINVAL (NULL ctx/params, n_steps < 0, tau0 <= 0.5, cs_smago < 0, wm_enable with
+ * wm_kappa <= 0 or wm_E <= 0), LBM_ESTATE (no state set yet), LBM_ECUDA. */
+int lbm_step(lbm_ctx* ctx, int n_steps, const lbm_params* params);
+
+/* Moments of the state S_t for EVERY cell (SOLID cells report whatever was set):
+ * rho = sum_i f_i, u = sum_i c_i f_i / rho -- the raw fluid velocity moment of l.97 (G19), not u^.
+ * rho[nz][ny][nx], u[3][nz][ny][nx] dtype, host or device; either may be NULL to skip it. */
+int lbm_moments(lbm_ctx* ctx, void* rho, void* u);
+
+/* State S_t in the external layout (parity checks, checkpoint).  populations[Q][nz][ny][nx]. */
+int lbm_get_populations(lbm_ctx* ctx, void* populations);
+
+/* Totals over non-SOLID cells of S_t: out[0] = sum rho, out[1..3] = sum rho u, out[4] = sum rho |u|^2 / 2.
+ * `out` is a HOST array of 5 doubles.  Accumulated in fp64.  Synchronises the stream. */
+int lbm_totals(lbm_ctx* ctx, double out[5]);
+
+/* Use `cuda_stream` (a cudaStream_t passed as void*) for all subsequent work; NULL = default stream. */
+int lbm_set_stream(lbm_ctx* ctx, void* cuda_stream);
+
+/* Block until everything enqueued so far has finished; returns LBM_ECUDA if any kernel failed. */
+int lbm_synchronize(lbm_ctx* ctx);
+
+/* Static or ctx-owned message of the last error; valid until the next call on that ctx.
+ * ctx == NULL returns the message of the last failed lbm_create. */
+const char* lbm_last_error(const lbm_ctx* ctx);
+
+/* Introspection used by the harness.  what:
+ *   0 steps taken since the last set_fields/init      1 kernels launched by this ctx so far
+ *   2 number of cells N                                3 number of SOLID cells
+ *   4 device bytes owned by the ctx                    5 cells on the masked (boundary) path
+ * Returns -1 for an unknown `what` or a NULL ctx. */
+long long lbm_query(const lbm_ctx* ctx, int what);
+
+/* Tuning knobs (no effect on results beyond floating-point summation order).  Returns LBM_EINVAL for an
+ * unknown key/value.  Keys:
+ *   "cuda_graph"  0|1   replay each lbm_step(n) through a captured CUDA graph (default 1 for n >= 4)
+ * More keys are listed in DESIGN.md as the kernels gain variants. */
+int lbm_set_option(lbm_ctx* ctx, const char* key, long long value);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PAPER_2506_21804_B200_LBM_H */

@@ -1,0 +1,488 @@
+// =====================================================================================
+// lbm_api.cu -- host side of the C ABI declared in include/lbm.h.
+// Argument checking, device storage, phase bookkeeping and kernel launches.  No arithmetic of
+// the method lives here; it is all in lbm_kernels.cuh.
+// =====================================================================================
+#include "../../include/lbm.h"
+
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "lbm_kernels.cuh"
+
+namespace {
+
+char g_create_error[512] = "no error";
+
+enum Phase { PHASE_NONE = 0,   // no state yet
+             PHASE_PRE = 1,    // cur holds S_t (pre-collision), as handed in
+             PHASE_POST = 2 }; // cur holds F_{t-1} (post-collision, not yet streamed); S_t = stream(F_{t-1})
+
+}  // namespace
+
+struct lbm_ctx {
+  int Q, nx, ny, nz, dtype;
+  long long N;
+  void* f[2];            // two population lattices, [Q][N] each
+  void* d;               // porosity [N]
+  bool has_d;
+  uint8_t* cls;          // class byte per cell (see lbm_kernels.cuh)
+  uint8_t* cls_alt;      // classification target before it is accepted
+  uint8_t* flags_raw;    // device copy of the caller's flag bytes
+  unsigned long long* counters;  // device [4]
+  double* totals_dev;            // device [5]
+  void* staging;         // host<->device bounce buffer, grown on demand
+  size_t staging_bytes;
+  int cur;
+  Phase phase;
+  long long steps, launches, n_solid, n_masked;
+  size_t device_bytes;
+  cudaStream_t stream;
+  int block_threads;
+  int use_graph;
+  lbm_params last;       // parameters of the last lbm_step: the inlet rule is part of how S_t is formed from F_{t-1}
+  char err[512];
+};
+
+namespace {
+
+int fail(lbm_ctx* c, int code, const char* fmt, ...) {
+  char* dst = c ? c->err : g_create_error;
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(dst, 512, fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+#define LBM_CUDA(c, call)                                                                             \
+  do {                                                                                                \
+    cudaError_t e_ = (call);                                                                          \
+    if (e_ != cudaSuccess) return fail((c), LBM_ECUDA, "%s: %s", #call, cudaGetErrorString(e_));      \
+  } while (0)
+
+bool is_device_pointer(const void* p) {
+  cudaPointerAttributes at;
+  cudaError_t e = cudaPointerGetAttributes(&at, p);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+int dev_alloc(lbm_ctx* c, void** p, size_t bytes) {
+  cudaError_t e = cudaMalloc(p, bytes ? bytes : 1);
+  if (e != cudaSuccess) {
+    *p = nullptr;
+    cudaGetLastError();
+    return fail(c, e == cudaErrorMemoryAllocation ? LBM_ENOMEM : LBM_ECUDA, "cudaMalloc(%zu bytes): %s", bytes,
+                cudaGetErrorString(e));
+  }
+  c->device_bytes += bytes;
+  return LBM_OK;
+}
+
+int ensure_staging(lbm_ctx* c, size_t bytes) {
+  if (c->staging_bytes >= bytes) return LBM_OK;
+  if (c->staging) {
+    cudaStreamSynchronize(c->stream);
+    cudaFree(c->staging);
+    c->device_bytes -= c->staging_bytes;
+    c->staging = nullptr;
+    c->staging_bytes = 0;
+  }
+  int rc = dev_alloc(c, &c->staging, bytes);
+  if (rc == LBM_OK) c->staging_bytes = bytes;
+  return rc;
+}
+
+void launch_dims(const lbm_ctx* c, dim3& grid, dim3& block) {
+  int bx = 1;
+  while (bx < c->nx && bx < c->block_threads) bx <<= 1;
+  int by = c->block_threads / bx;
+  int ny2 = 1;
+  while (ny2 < c->ny) ny2 <<= 1;
+  if (by > ny2) by = ny2;
+  if (by < 1) by = 1;
+  block = dim3(bx, by, 1);
+  grid = dim3((c->nx + bx - 1) / bx, (c->ny + by - 1) / by, c->nz);
+}
+
+template <typename T>
+lbm::StepArgs<T> make_args(const lbm_ctx* c, const lbm_params* p, int in, int out) {
+  lbm::StepArgs<T> a;
+  a.fin = static_cast<const T*>(c->f[in]);
+  a.fout = static_cast<T*>(c->f[out]);
+  a.d = (p && p->use_hlbm && c->has_d) ? static_cast<const T*>(c->d) : nullptr;
+  a.cls = c->cls;
+  a.nx = c->nx;  a.ny = c->ny;  a.nz = c->nz;
+  a.N = c->N;
+  if (p) {
+    a.tau0 = static_cast<T>(p->tau0);
+    a.smago_k = static_cast<T>(18.0 * 1.4142135623730951 * p->cs_smago * p->cs_smago);
+    a.u_in[0] = static_cast<T>(p->u_in[0]);  a.u_in[1] = static_cast<T>(p->u_in[1]);  a.u_in[2] = static_cast<T>(p->u_in[2]);
+    a.wm_enable = p->wm_enable;
+    a.wm_kappa = p->wm_kappa;  a.wm_E = p->wm_E;
+    a.nu = (p->tau0 - 0.5) / 3.0;
+  } else {
+    a.tau0 = T(1);  a.smago_k = T(0);
+    a.u_in[0] = a.u_in[1] = a.u_in[2] = T(0);
+    a.wm_enable = 0;  a.wm_kappa = 0.41;  a.wm_E = 9.8;  a.nu = 1.0 / 6.0;
+  }
+  return a;
+}
+
+template <int Q, typename T>
+int launch_step_t(lbm_ctx* c, const lbm_params* p, int mode) {
+  dim3 grid, block;
+  launch_dims(c, grid, block);
+  const int in = c->cur, out = 1 - c->cur;
+  lbm::StepArgs<T> a = make_args<T>(c, p, in, out);
+  switch (mode) {
+    case lbm::MODE_COLLIDE: lbm::k_step<Q, T, lbm::MODE_COLLIDE><<<grid, block, 0, c->stream>>>(a); break;
+    case lbm::MODE_STREAM_COLLIDE: lbm::k_step<Q, T, lbm::MODE_STREAM_COLLIDE><<<grid, block, 0, c->stream>>>(a); break;
+    default: lbm::k_step<Q, T, lbm::MODE_STREAM><<<grid, block, 0, c->stream>>>(a); break;
+  }
+  LBM_CUDA(c, cudaGetLastError());
+  c->launches++;
+  c->cur = out;
+  return LBM_OK;
+}
+
+int launch_step(lbm_ctx* c, const lbm_params* p, int mode) {
+  if (c->Q == 19) return c->dtype == LBM_F32 ? launch_step_t<19, float>(c, p, mode) : launch_step_t<19, double>(c, p, mode);
+  return c->dtype == LBM_F32 ? launch_step_t<27, float>(c, p, mode) : launch_step_t<27, double>(c, p, mode);
+}
+
+template <int Q, typename T>
+int launch_moments_t(lbm_ctx* c, const lbm_params* p, void* rho, void* u) {
+  dim3 grid, block;
+  launch_dims(c, grid, block);
+  lbm::StepArgs<T> a = make_args<T>(c, p, c->cur, 1 - c->cur);
+  if (c->phase == PHASE_POST)
+    lbm::k_moments<Q, T, true><<<grid, block, 0, c->stream>>>(a, static_cast<T*>(rho), static_cast<T*>(u));
+  else
+    lbm::k_moments<Q, T, false><<<grid, block, 0, c->stream>>>(a, static_cast<T*>(rho), static_cast<T*>(u));
+  LBM_CUDA(c, cudaGetLastError());
+  c->launches++;
+  return LBM_OK;
+}
+
+template <int Q, typename T>
+int launch_totals_t(lbm_ctx* c, const lbm_params* p) {
+  dim3 grid, block;
+  launch_dims(c, grid, block);
+  lbm::StepArgs<T> a = make_args<T>(c, p, c->cur, 1 - c->cur);
+  if (c->phase == PHASE_POST)
+    lbm::k_totals<Q, T, true><<<grid, block, 0, c->stream>>>(a, c->totals_dev);
+  else
+    lbm::k_totals<Q, T, false><<<grid, block, 0, c->stream>>>(a, c->totals_dev);
+  LBM_CUDA(c, cudaGetLastError());
+  c->launches++;
+  return LBM_OK;
+}
+
+template <int Q, typename T>
+int launch_init_t(lbm_ctx* c, const void* rho, const void* u) {
+  const int threads = 256;
+  const long long blocks = (c->N + threads - 1) / threads;
+  lbm::k_init_equilibrium<Q, T><<<static_cast<unsigned>(blocks), threads, 0, c->stream>>>(
+      static_cast<const T*>(rho), static_cast<const T*>(u), static_cast<T*>(c->f[0]), static_cast<T*>(c->f[1]), c->N);
+  LBM_CUDA(c, cudaGetLastError());
+  c->launches++;
+  return LBM_OK;
+}
+
+#define LBM_DISPATCH(c, fn, ...)                                                                              \
+  ((c)->Q == 19 ? ((c)->dtype == LBM_F32 ? fn<19, float>(__VA_ARGS__) : fn<19, double>(__VA_ARGS__))          \
+                : ((c)->dtype == LBM_F32 ? fn<27, float>(__VA_ARGS__) : fn<27, double>(__VA_ARGS__)))
+
+lbm_params default_params() {
+  lbm_params p;
+  std::memset(&p, 0, sizeof(p));
+  p.tau0 = 1.0;
+  p.wm_kappa = 0.41;
+  p.wm_E = 9.8;
+  return p;
+}
+
+int check_params(lbm_ctx* c, const lbm_params* p) {
+  if (!p) return fail(c, LBM_EINVAL, "lbm_step: params is NULL");
+  if (!(p->tau0 > 0.5)) return fail(c, LBM_EINVAL, "lbm_step: tau0 = %g must be > 0.5", p->tau0);
+  if (!(p->cs_smago >= 0.0)) return fail(c, LBM_EINVAL, "lbm_step: cs_smago = %g must be >= 0", p->cs_smago);
+  if (p->wm_enable && (!(p->wm_kappa > 0.0) || !(p->wm_E > 0.0)))
+    return fail(c, LBM_EINVAL, "lbm_step: wm_enable needs wm_kappa > 0 and wm_E > 0");
+  if (!(p->u_in[0] < 1.0)) return fail(c, LBM_EINVAL, "lbm_step: u_in[0] = %g must be < 1", p->u_in[0]);
+  return LBM_OK;
+}
+
+// copy flags to the device, validate + classify into cls_alt, accept on success
+int classify(lbm_ctx* c, const uint8_t* cell_flags) {
+  if (cell_flags) {
+    LBM_CUDA(c, cudaMemcpyAsync(c->flags_raw, cell_flags, c->N, cudaMemcpyDefault, c->stream));
+  } else {
+    LBM_CUDA(c, cudaMemsetAsync(c->flags_raw, 0, c->N, c->stream));
+  }
+  LBM_CUDA(c, cudaMemsetAsync(c->counters, 0, 4 * sizeof(unsigned long long), c->stream));
+  dim3 grid, block;
+  launch_dims(c, grid, block);
+  if (c->Q == 19) lbm::k_classify<19><<<grid, block, 0, c->stream>>>(c->flags_raw, c->cls_alt, c->nx, c->ny, c->nz, c->counters);
+  else            lbm::k_classify<27><<<grid, block, 0, c->stream>>>(c->flags_raw, c->cls_alt, c->nx, c->ny, c->nz, c->counters);
+  LBM_CUDA(c, cudaGetLastError());
+  c->launches++;
+  unsigned long long h[4];
+  LBM_CUDA(c, cudaMemcpyAsync(h, c->counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+  LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  if (h[0] != 0)
+    return fail(c, LBM_EINVAL, "cell_flags: %llu invalid flag byte(s) (type > 4, bad high nibble, INLET off x=0 or OUTLET off x=nx-1)", h[0]);
+  uint8_t* t = c->cls;  c->cls = c->cls_alt;  c->cls_alt = t;
+  c->n_solid = static_cast<long long>(h[1]);
+  c->n_masked = static_cast<long long>(h[2]);
+  return LBM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* lbm_last_error(const lbm_ctx* ctx) { return ctx ? ctx->err : g_create_error; }
+
+lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype) {
+  if (lattice != LBM_D3Q19 && lattice != LBM_D3Q27) { fail(nullptr, LBM_EINVAL, "lbm_create: lattice %d is not 19 or 27", lattice); return nullptr; }
+  if (dtype != LBM_F32 && dtype != LBM_F64) { fail(nullptr, LBM_EINVAL, "lbm_create: dtype %d is not 4 (f32) or 8 (f64)", dtype); return nullptr; }
+  if (nx < 1 || ny < 1 || nz < 1) { fail(nullptr, LBM_EINVAL, "lbm_create: nx, ny, nz must be >= 1 (got %d %d %d)", nx, ny, nz); return nullptr; }
+  const long long N = static_cast<long long>(nx) * ny * nz;
+  if (N >= (1ll << 31) || nz > 65535) { fail(nullptr, LBM_EINVAL, "lbm_create: lattice too large (N = %lld must be < 2^31, nz <= 65535)", N); return nullptr; }
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    fail(nullptr, LBM_ECUDA, "lbm_create: no usable CUDA device (%s); this library has no CPU fallback", cudaGetErrorString(e));
+    return nullptr;
+  }
+  lbm_ctx* c = new (std::nothrow) lbm_ctx;
+  if (!c) { fail(nullptr, LBM_ENOMEM, "lbm_create: host allocation failed"); return nullptr; }
+  std::memset(c, 0, sizeof(*c));
+  c->Q = lattice;  c->nx = nx;  c->ny = ny;  c->nz = nz;  c->dtype = dtype;  c->N = N;
+  c->phase = PHASE_NONE;
+  c->block_threads = 128;
+  c->last = default_params();
+  std::snprintf(c->err, sizeof(c->err), "no error");
+  const size_t pop = static_cast<size_t>(lattice) * N * dtype;
+  int rc = dev_alloc(c, &c->f[0], pop);
+  if (rc == LBM_OK) rc = dev_alloc(c, &c->f[1], pop);
+  if (rc == LBM_OK) rc = dev_alloc(c, &c->d, static_cast<size_t>(N) * dtype);
+  if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->cls), N);
+  if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->cls_alt), N);
+  if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->flags_raw), N);
+  if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->counters), 4 * sizeof(unsigned long long));
+  if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->totals_dev), 5 * sizeof(double));
+  if (rc == LBM_OK && cudaMemset(c->cls, 0, N) != cudaSuccess) rc = fail(c, LBM_ECUDA, "cudaMemset failed");
+  if (rc != LBM_OK) {
+    std::snprintf(g_create_error, sizeof(g_create_error), "lbm_create: %s", c->err);
+    lbm_destroy(c);
+    return nullptr;
+  }
+  return c;
+}
+
+void lbm_destroy(lbm_ctx* c) {
+  if (!c) return;
+  cudaStreamSynchronize(c->stream);
+  cudaFree(c->f[0]);  cudaFree(c->f[1]);  cudaFree(c->d);
+  cudaFree(c->cls);  cudaFree(c->cls_alt);  cudaFree(c->flags_raw);
+  cudaFree(c->counters);  cudaFree(c->totals_dev);  cudaFree(c->staging);
+  cudaGetLastError();
+  delete c;
+}
+
+int lbm_set_stream(lbm_ctx* c, void* cuda_stream) {
+  if (!c) return LBM_EINVAL;
+  LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  c->stream = static_cast<cudaStream_t>(cuda_stream);
+  return LBM_OK;
+}
+
+int lbm_synchronize(lbm_ctx* c) {
+  if (!c) return LBM_EINVAL;
+  LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  LBM_CUDA(c, cudaGetLastError());
+  return LBM_OK;
+}
+
+static int set_geometry_fields(lbm_ctx* c, const void* porosity, const uint8_t* cell_flags) {
+  int rc = classify(c, cell_flags);
+  if (rc != LBM_OK) return rc;
+  if (porosity) {
+    LBM_CUDA(c, cudaMemcpyAsync(c->d, porosity, static_cast<size_t>(c->N) * c->dtype, cudaMemcpyDefault, c->stream));
+    c->has_d = true;
+  } else {
+    c->has_d = false;
+  }
+  return LBM_OK;
+}
+
+int lbm_set_fields(lbm_ctx* c, const void* populations, const void* porosity, const uint8_t* cell_flags) {
+  if (!c) return LBM_EINVAL;
+  if (!populations) return fail(c, LBM_EINVAL, "lbm_set_fields: populations is NULL");
+  int rc = set_geometry_fields(c, porosity, cell_flags);
+  if (rc != LBM_OK) return rc;
+  const size_t pop = static_cast<size_t>(c->Q) * c->N * c->dtype;
+  LBM_CUDA(c, cudaMemcpyAsync(c->f[0], populations, pop, cudaMemcpyDefault, c->stream));
+  // SOLID cells are never written by the step kernel: both lattices must hold their values
+  LBM_CUDA(c, cudaMemcpyAsync(c->f[1], c->f[0], pop, cudaMemcpyDeviceToDevice, c->stream));
+  if (!is_device_pointer(populations)) LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  c->cur = 0;
+  c->phase = PHASE_PRE;
+  c->steps = 0;
+  return LBM_OK;
+}
+
+int lbm_init_equilibrium(lbm_ctx* c, const void* rho, const void* u) {
+  if (!c) return LBM_EINVAL;
+  if (!rho || !u) return fail(c, LBM_EINVAL, "lbm_init_equilibrium: rho or u is NULL");
+  const size_t cell_bytes = static_cast<size_t>(c->N) * c->dtype;
+  const void* drho = rho;
+  const void* du = u;
+  const bool hr = !is_device_pointer(rho), hu = !is_device_pointer(u);
+  if (hr || hu) {
+    int rc = ensure_staging(c, 4 * cell_bytes);
+    if (rc != LBM_OK) return rc;
+    char* s = static_cast<char*>(c->staging);
+    if (hr) { LBM_CUDA(c, cudaMemcpyAsync(s, rho, cell_bytes, cudaMemcpyDefault, c->stream)); drho = s; }
+    if (hu) { LBM_CUDA(c, cudaMemcpyAsync(s + cell_bytes, u, 3 * cell_bytes, cudaMemcpyDefault, c->stream)); du = s + cell_bytes; }
+  }
+  int rc = LBM_DISPATCH(c, launch_init_t, c, drho, du);
+  if (rc != LBM_OK) return rc;
+  if (hr || hu) LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  c->cur = 0;
+  c->phase = PHASE_PRE;
+  c->steps = 0;
+  return LBM_OK;
+}
+
+// POST -> PRE: write S_t = stream(F_{t-1}) into the other lattice and make it current
+static int materialise(lbm_ctx* c) {
+  if (c->phase != PHASE_POST) return LBM_OK;
+  lbm_params p = c->last;
+  int rc = launch_step(c, &p, lbm::MODE_STREAM);
+  if (rc != LBM_OK) return rc;
+  c->phase = PHASE_PRE;
+  return LBM_OK;
+}
+
+int lbm_set_geometry(lbm_ctx* c, const void* porosity, const uint8_t* cell_flags) {
+  if (!c) return LBM_EINVAL;
+  // S_t is defined with the geometry it was computed under: fix it before the geometry changes
+  int rc = materialise(c);
+  if (rc != LBM_OK) return rc;
+  rc = set_geometry_fields(c, porosity, cell_flags);
+  if (rc != LBM_OK) return rc;
+  if (c->phase == PHASE_PRE) {
+    const size_t pop = static_cast<size_t>(c->Q) * c->N * c->dtype;
+    LBM_CUDA(c, cudaMemcpyAsync(c->f[1 - c->cur], c->f[c->cur], pop, cudaMemcpyDeviceToDevice, c->stream));
+  }
+  return LBM_OK;
+}
+
+int lbm_step(lbm_ctx* c, int n_steps, const lbm_params* params) {
+  if (!c) return LBM_EINVAL;
+  int rc = check_params(c, params);
+  if (rc != LBM_OK) return rc;
+  if (n_steps < 0) return fail(c, LBM_EINVAL, "lbm_step: n_steps = %d must be >= 0", n_steps);
+  if (c->phase == PHASE_NONE) return fail(c, LBM_ESTATE, "lbm_step: no state; call lbm_set_fields or lbm_init_equilibrium first");
+  c->last = *params;
+  for (int s = 0; s < n_steps; ++s) {
+    if (c->phase == PHASE_PRE) {
+      rc = launch_step(c, params, lbm::MODE_COLLIDE);          // S_t -> F_t
+      c->phase = PHASE_POST;
+    } else {
+      rc = launch_step(c, params, lbm::MODE_STREAM_COLLIDE);   // F_{t-1} -> S_t -> F_t
+    }
+    if (rc != LBM_OK) return rc;
+  }
+  c->steps += n_steps;
+  return LBM_OK;
+}
+
+int lbm_moments(lbm_ctx* c, void* rho, void* u) {
+  if (!c) return LBM_EINVAL;
+  if (c->phase == PHASE_NONE) return fail(c, LBM_ESTATE, "lbm_moments: no state");
+  if (!rho && !u) return LBM_OK;
+  const size_t cell_bytes = static_cast<size_t>(c->N) * c->dtype;
+  const bool hr = rho && !is_device_pointer(rho), hu = u && !is_device_pointer(u);
+  void* drho = rho;
+  void* du = u;
+  if (hr || hu) {
+    int rc = ensure_staging(c, 4 * cell_bytes);
+    if (rc != LBM_OK) return rc;
+    char* s = static_cast<char*>(c->staging);
+    if (hr) drho = s;
+    if (hu) du = s + cell_bytes;
+  }
+  lbm_params p = c->last;
+  int rc = LBM_DISPATCH(c, launch_moments_t, c, &p, drho, du);
+  if (rc != LBM_OK) return rc;
+  if (hr) LBM_CUDA(c, cudaMemcpyAsync(rho, drho, cell_bytes, cudaMemcpyDefault, c->stream));
+  if (hu) LBM_CUDA(c, cudaMemcpyAsync(u, du, 3 * cell_bytes, cudaMemcpyDefault, c->stream));
+  if (hr || hu) LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  return LBM_OK;
+}
+
+int lbm_get_populations(lbm_ctx* c, void* populations) {
+  if (!c) return LBM_EINVAL;
+  if (!populations) return fail(c, LBM_EINVAL, "lbm_get_populations: populations is NULL");
+  if (c->phase == PHASE_NONE) return fail(c, LBM_ESTATE, "lbm_get_populations: no state");
+  int rc = materialise(c);
+  if (rc != LBM_OK) return rc;
+  const size_t pop = static_cast<size_t>(c->Q) * c->N * c->dtype;
+  LBM_CUDA(c, cudaMemcpyAsync(populations, c->f[c->cur], pop, cudaMemcpyDefault, c->stream));
+  if (!is_device_pointer(populations)) LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  return LBM_OK;
+}
+
+int lbm_totals(lbm_ctx* c, double out[5]) {
+  if (!c) return LBM_EINVAL;
+  if (!out) return fail(c, LBM_EINVAL, "lbm_totals: out is NULL");
+  if (c->phase == PHASE_NONE) return fail(c, LBM_ESTATE, "lbm_totals: no state");
+  LBM_CUDA(c, cudaMemsetAsync(c->totals_dev, 0, 5 * sizeof(double), c->stream));
+  lbm_params p = c->last;
+  int rc = LBM_DISPATCH(c, launch_totals_t, c, &p);
+  if (rc != LBM_OK) return rc;
+  LBM_CUDA(c, cudaMemcpyAsync(out, c->totals_dev, 5 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  return LBM_OK;
+}
+
+long long lbm_query(const lbm_ctx* c, int what) {
+  if (!c) return -1;
+  switch (what) {
+    case 0: return c->steps;
+    case 1: return c->launches;
+    case 2: return c->N;
+    case 3: return c->n_solid;
+    case 4: return static_cast<long long>(c->device_bytes);
+    case 5: return c->n_masked;
+    default: return -1;
+  }
+}
+
+int lbm_set_option(lbm_ctx* c, const char* key, long long value) {
+  if (!c || !key) return LBM_EINVAL;
+  if (std::strcmp(key, "cuda_graph") == 0) {
+    if (value != 0 && value != 1) return fail(c, LBM_EINVAL, "cuda_graph must be 0 or 1");
+    c->use_graph = static_cast<int>(value);
+    return LBM_OK;
+  }
+  if (std::strcmp(key, "block_threads") == 0) {
+    if (value != 64 && value != 128 && value != 256) return fail(c, LBM_EINVAL, "block_threads must be 64, 128 or 256");
+    c->block_threads = static_cast<int>(value);
+    return LBM_OK;
+  }
+  return fail(c, LBM_EINVAL, "unknown option '%s'", key);
+}
+
+}  // extern "C"

@@ -1,0 +1,506 @@
+// =====================================================================================
+// lbm_kernels.cuh -- device code of the LBM hot path for sm_100a (B200).
+//
+// One fused kernel per time step: pull-propagation (A1) + moments (A2) + HLBM velocity (A3) +
+// equilibrium (A4) + Smagorinsky tau_eff (A5) + relaxation (A6), with the masked boundary rules
+// (A7: halfway bounce-back, velocity inlet, zero-gradient outlet) and the Spalding wall model (A8)
+// on a warp-uniform slow path.  A9 (moments / totals) are separate kernels.
+// Row and equation references are to SURVEY.md section 8(a) and /root/reference/PAPER.md.
+//
+// Storage: SoA f[i][z][y][x], x fastest, two lattices (ping-pong).  The stored array holds the
+// POST-collision populations F_{t-1}; the state S_t of the ABI is stream(F_{t-1}) and is formed in
+// registers by the pull.  This file shares nothing with oracle/.
+// =====================================================================================
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace lbm {
+
+enum : int { T_FLUID = 0, T_SOLID = 1, T_INLET = 2, T_OUTLET = 3, T_WM = 4 };
+// internal class byte: bits 0-2 type, bits 3-5 wall-normal code, bit 7 = cell takes the masked path
+constexpr uint8_t CLS_TYPE = 0x07;
+constexpr uint8_t CLS_MASKED = 0x80;
+constexpr int CLS_NORMAL_SHIFT = 3;
+
+// kernel modes
+enum : int { MODE_COLLIDE = 0,        // input holds S_t (fresh state): collide only           -> F_t
+             MODE_STREAM_COLLIDE = 1, // input holds F_{t-1}: pull to S_t, collide             -> F_t
+             MODE_STREAM = 2 };       // input holds F_{t-1}: pull to S_t, store S_t (materialise)
+
+// ---- velocity set by rule R1 (G13), generated at compile time -------------------------
+template <int Q>
+struct Stencil {
+  int c[Q][3];
+  int opp[Q];
+  int c2[Q];
+  constexpr Stencil() : c{}, opp{}, c2{} {
+    const int maxc2 = (Q == 19) ? 2 : 3;
+    const int h = (Q - 1) / 2;
+    int n = 1;
+    // ascending (|c|^2, -cx, -cy, -cz): loop |c|^2 outermost, then cx, cy, cz descending
+    for (int want = 1; want <= maxc2; ++want)
+      for (int x = 1; x >= -1; --x)
+        for (int y = 1; y >= -1; --y)
+          for (int z = 1; z >= -1; --z) {
+            const int s = x * x + y * y + z * z;
+            if (s != want) continue;
+            const int first = (x != 0) ? x : ((y != 0) ? y : z);
+            if (first != 1) continue;
+            c[n][0] = x;      c[n][1] = y;      c[n][2] = z;      c2[n] = s;      opp[n] = n + h;
+            c[n + h][0] = -x; c[n + h][1] = -y; c[n + h][2] = -z; c2[n + h] = s;  opp[n + h] = n;
+            ++n;
+          }
+  }
+};
+
+template <int Q, typename T>
+__host__ __device__ constexpr T weight(int c2) {
+  return (Q == 19) ? (c2 == 0 ? T(1.0 / 3.0) : (c2 == 1 ? T(1.0 / 18.0) : T(1.0 / 36.0)))
+                   : (c2 == 0 ? T(8.0 / 27.0) : (c2 == 1 ? T(2.0 / 27.0) : (c2 == 2 ? T(1.0 / 54.0) : T(1.0 / 216.0))));
+}
+
+template <typename T>
+struct StepArgs {
+  const T* __restrict__ fin;      // [Q][N]
+  T* __restrict__ fout;           // [Q][N]
+  const T* __restrict__ d;        // [N] or nullptr (=> d = 0)
+  const uint8_t* __restrict__ cls;  // [N]
+  int nx, ny, nz;
+  long long N;                    // cells = population stride
+  T tau0;
+  T smago_k;                      // 18 sqrt(2) Cs^2 ; 0 => BGK
+  T u_in[3];
+  int wm_enable;
+  double wm_kappa, wm_E, nu;
+};
+
+// ---- math helpers ---------------------------------------------------------------------------------
+__device__ __forceinline__ float rcp_(float x) { return __frcp_rn(x); }
+__device__ __forceinline__ double rcp_(double x) { return 1.0 / x; }
+__device__ __forceinline__ float sqrt_(float x) { return __fsqrt_rn(x); }
+__device__ __forceinline__ double sqrt_(double x) { return sqrt(x); }
+
+// A2..A6 on one cell held in registers.  f[] in: S_t, out: post-collision F_t.
+// (ubx,uby,ubz) = u^B; d = porosity.  Eq. 6, 11 (to H2), 12, 14 with Eq. 3-5 in closed form:
+//   tau_eff = (tau0 + sqrt(tau0^2 + 18 sqrt2 Cs^2 |Pi| / rho)) / 2,   Pi = sum_i c c (f_i - feq_i)
+// Opposite directions are paired: sums s = f_i + f_opp and differences for the odd moments.
+template <int Q, typename T>
+__device__ __forceinline__ void collide_cell(T (&f)[Q], T d, T ubx, T uby, T ubz, T tau0, T smago_k) {
+  constexpr Stencil<Q> L{};
+  constexpr int H = (Q - 1) / 2;
+  T rho = f[0], jx = T(0), jy = T(0), jz = T(0);
+  T mxx = T(0), myy = T(0), mzz = T(0), mxy = T(0), mxz = T(0), myz = T(0);
+#pragma unroll
+  for (int i = 1; i <= H; ++i) {
+    const T s = f[i] + f[i + H];
+    const T a = f[i] - f[i + H];
+    rho += s;
+    if (L.c[i][0] == 1) jx += a; else if (L.c[i][0] == -1) jx -= a;
+    if (L.c[i][1] == 1) jy += a; else if (L.c[i][1] == -1) jy -= a;
+    if (L.c[i][2] == 1) jz += a; else if (L.c[i][2] == -1) jz -= a;
+    if (L.c[i][0] != 0) mxx += s;
+    if (L.c[i][1] != 0) myy += s;
+    if (L.c[i][2] != 0) mzz += s;
+    if (L.c[i][0] * L.c[i][1] == 1) mxy += s; else if (L.c[i][0] * L.c[i][1] == -1) mxy -= s;
+    if (L.c[i][0] * L.c[i][2] == 1) mxz += s; else if (L.c[i][0] * L.c[i][2] == -1) mxz -= s;
+    if (L.c[i][1] * L.c[i][2] == 1) myz += s; else if (L.c[i][1] * L.c[i][2] == -1) myz -= s;
+  }
+  const T inv_rho = rcp_(rho);
+  const T keep = T(1) - d;                                  // Eq. 12
+  const T ux = keep * (jx * inv_rho) + d * ubx;
+  const T uy = keep * (jy * inv_rho) + d * uby;
+  const T uz = keep * (jz * inv_rho) + d * ubz;
+  T omega;
+  if (smago_k > T(0)) {
+    // second moment of f^eq(rho, u^) is rho (I/3 + u^ u^)
+    const T third = rho * T(1.0 / 3.0);
+    const T pxx = mxx - third - rho * ux * ux;
+    const T pyy = myy - third - rho * uy * uy;
+    const T pzz = mzz - third - rho * uz * uz;
+    const T pxy = mxy - rho * ux * uy;
+    const T pxz = mxz - rho * ux * uz;
+    const T pyz = myz - rho * uy * uz;
+    const T npi = sqrt_(pxx * pxx + pyy * pyy + pzz * pzz + T(2) * (pxy * pxy + pxz * pxz + pyz * pyz));
+    const T tau = T(0.5) * (tau0 + sqrt_(tau0 * tau0 + smago_k * npi * inv_rho));
+    omega = rcp_(tau);
+  } else {
+    omega = rcp_(tau0);
+  }
+  const T base = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
+  const T keepf = T(1) - omega;
+  f[0] = keepf * f[0] + omega * (weight<Q, T>(0) * rho * base);
+#pragma unroll
+  for (int i = 1; i <= H; ++i) {
+    T cu = T(0);
+    if (L.c[i][0] == 1) cu += ux; else if (L.c[i][0] == -1) cu -= ux;
+    if (L.c[i][1] == 1) cu += uy; else if (L.c[i][1] == -1) cu -= uy;
+    if (L.c[i][2] == 1) cu += uz; else if (L.c[i][2] == -1) cu -= uz;
+    const T wr = weight<Q, T>(L.c2[i]) * rho * omega;
+    const T even = wr * (base + T(4.5) * cu * cu);
+    const T odd = wr * T(3) * cu;
+    f[i] = keepf * f[i] + (even + odd);
+    f[i + H] = keepf * f[i + H] + (even - odd);
+  }
+}
+
+// O4 / reading R6: regularised velocity inlet on a cell of the plane x = 0 (inward normal +x).
+template <int Q, typename T>
+__device__ __forceinline__ void inlet_fixup(T (&g)[Q], T uwx, T uwy, T uwz) {
+  constexpr Stencil<Q> L{};
+  T s0 = T(0), sm = T(0);
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    if (L.c[i][0] == 0) s0 += g[i];
+    else if (L.c[i][0] < 0) sm += g[i];
+  }
+  const T rho = (s0 + T(2) * sm) / (T(1) - uwx);
+  const T base = T(1) - T(1.5) * (uwx * uwx + uwy * uwy + uwz * uwz);
+  T feq[Q];
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    const T cu = T(L.c[i][0]) * uwx + T(L.c[i][1]) * uwy + T(L.c[i][2]) * uwz;
+    feq[i] = weight<Q, T>(L.c2[i]) * rho * (base + T(3) * cu + T(4.5) * cu * cu);
+  }
+  // non-equilibrium: known directions as they are, unknown (cx > 0) from the opposite one
+  T pxx = T(0), pyy = T(0), pzz = T(0), pxy = T(0), pxz = T(0), pyz = T(0);
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    const int k = (L.c[i][0] > 0) ? L.opp[i] : i;
+    const T n = g[k] - feq[k];
+    pxx += T(L.c[i][0] * L.c[i][0]) * n;
+    pyy += T(L.c[i][1] * L.c[i][1]) * n;
+    pzz += T(L.c[i][2] * L.c[i][2]) * n;
+    pxy += T(L.c[i][0] * L.c[i][1]) * n;
+    pxz += T(L.c[i][0] * L.c[i][2]) * n;
+    pyz += T(L.c[i][1] * L.c[i][2]) * n;
+  }
+  const T tr3 = (pxx + pyy + pzz) * T(1.0 / 3.0);
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    const T q = T(L.c[i][0] * L.c[i][0]) * pxx + T(L.c[i][1] * L.c[i][1]) * pyy + T(L.c[i][2] * L.c[i][2]) * pzz +
+                T(2) * (T(L.c[i][0] * L.c[i][1]) * pxy + T(L.c[i][0] * L.c[i][2]) * pxz + T(L.c[i][1] * L.c[i][2]) * pyz) - tr3;
+    g[i] = feq[i] + T(4.5) * weight<Q, T>(L.c2[i]) * q;
+  }
+}
+
+// Spalding's law (Eq. 17) and the two Newton solves of reading R8, in double for both dtypes
+// (0.8 % of the cells of config 3 take this path).  Returns U1 / U2.
+__device__ __noinline__ double wallmodel_ratio(double U2, double nu, double kappa, double E) {
+  const double y2 = 1.5, y1 = 0.5;
+  const double invE = 1.0 / E;
+  double ut = sqrt(nu * U2 / y2);
+  for (int it = 0; it < 200; ++it) {
+    const double up = U2 / ut;
+    const double k = kappa * up;
+    const double ek = exp(k);
+    const double sp = up + invE * (ek - 1.0 - k - 0.5 * k * k - k * k * k * (1.0 / 6.0));
+    const double dsp = 1.0 + kappa * invE * (ek - 1.0 - k - 0.5 * k * k);
+    const double R = sp - y2 * ut / nu;
+    const double dR = -dsp * up / ut - y2 / nu;
+    double un = ut - R / dR;
+    if (!(un > 0.0)) un = 0.5 * ut;
+    const double delta = fabs(un - ut);
+    ut = un;
+    if (delta <= 1e-13 * ut) break;
+  }
+  const double y1p = y1 * ut / nu;
+  double lg = log(E * y1p) / kappa;
+  if (!(lg > 0.0)) lg = 0.0;
+  double up = fmin(y1p, lg + 1.0);
+  for (int it = 0; it < 200; ++it) {
+    const double k = kappa * up;
+    const double ek = exp(k);
+    const double sp = up + invE * (ek - 1.0 - k - 0.5 * k * k - k * k * k * (1.0 / 6.0));
+    const double dsp = 1.0 + kappa * invE * (ek - 1.0 - k - 0.5 * k * k);
+    double un = up - (sp - y1p) / dsp;
+    if (un < 0.0) un = 0.5 * up;
+    const double delta = fabs(un - up);
+    up = un;
+    if (delta <= 1e-13 * fabs(up)) break;
+  }
+  return up * ut / U2;
+}
+
+struct Coord {
+  int x, y, z;
+};
+
+__device__ __forceinline__ long long cell_index(int x, int y, int z, int nx, int ny) {
+  return (static_cast<long long>(z) * ny + y) * nx + x;
+}
+
+// Fast pull: every neighbour is a regular cell (no SOLID neighbour, cell is plain FLUID).
+template <int Q, typename T>
+__device__ __forceinline__ void pull_bulk(const T* __restrict__ fin, long long N, int x, int y, int z, int nx, int ny,
+                                          int nz, T (&f)[Q]) {
+  constexpr Stencil<Q> L{};
+  const int xm = (x == 0) ? nx - 1 : x - 1, xp = (x == nx - 1) ? 0 : x + 1;
+  const int ym = (y == 0) ? ny - 1 : y - 1, yp = (y == ny - 1) ? 0 : y + 1;
+  const int zm = (z == 0) ? nz - 1 : z - 1, zp = (z == nz - 1) ? 0 : z + 1;
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    // source = x - c_i
+    const int sx = (L.c[i][0] == 0) ? x : ((L.c[i][0] == 1) ? xm : xp);
+    const int sy = (L.c[i][1] == 0) ? y : ((L.c[i][1] == 1) ? ym : yp);
+    const int sz = (L.c[i][2] == 0) ? z : ((L.c[i][2] == 1) ? zm : zp);
+    f[i] = __ldg(fin + i * N + cell_index(sx, sy, sz, nx, ny));
+  }
+}
+
+// Masked pull (A7): halfway bounce-back at SOLID neighbours, zero-gradient outlet clamp, then the
+// inlet fix-up if the cell is an INLET cell.  `type` is the cell's own type (not SOLID).
+template <int Q, typename T>
+__device__ __forceinline__ void pull_masked(const StepArgs<T>& a, int x, int y, int z, int type, T (&f)[Q]) {
+  constexpr Stencil<Q> L{};
+  const int nx = a.nx, ny = a.ny, nz = a.nz;
+  const long long N = a.N;
+  const long long self = cell_index(x, y, z, nx, ny);
+  const int xm = (x == 0) ? nx - 1 : x - 1;
+  // outlet: the ghost plane beyond x = nx-1 is a copy of plane nx-1 (no wrap)
+  const int xp = (type == T_OUTLET) ? x : ((x == nx - 1) ? 0 : x + 1);
+  const int ym = (y == 0) ? ny - 1 : y - 1, yp = (y == ny - 1) ? 0 : y + 1;
+  const int zm = (z == 0) ? nz - 1 : z - 1, zp = (z == nz - 1) ? 0 : z + 1;
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    const int sx = (L.c[i][0] == 0) ? x : ((L.c[i][0] == 1) ? xm : xp);
+    const int sy = (L.c[i][1] == 0) ? y : ((L.c[i][1] == 1) ? ym : yp);
+    const int sz = (L.c[i][2] == 0) ? z : ((L.c[i][2] == 1) ? zm : zp);
+    const long long s = cell_index(sx, sy, sz, nx, ny);
+    const bool solid = (i != 0) && ((a.cls[s] & CLS_TYPE) == T_SOLID);
+    f[i] = solid ? __ldg(a.fin + L.opp[i] * N + self) : __ldg(a.fin + i * N + s);
+  }
+  if (type == T_INLET) inlet_fixup<Q, T>(f, a.u_in[0], a.u_in[1], a.u_in[2]);
+}
+
+// S_t of one cell, whatever the storage phase.  PULL = input holds F_{t-1}.
+template <int Q, typename T, bool PULL>
+__device__ __forceinline__ void load_state(const StepArgs<T>& a, int x, int y, int z, uint8_t cls, T (&f)[Q]) {
+  const int type = cls & CLS_TYPE;
+  if (!PULL || type == T_SOLID) {
+    const long long self = cell_index(x, y, z, a.nx, a.ny);
+#pragma unroll
+    for (int i = 0; i < Q; ++i) f[i] = __ldg(a.fin + i * a.N + self);
+  } else if (cls & CLS_MASKED) {
+    pull_masked<Q, T>(a, x, y, z, type, f);
+  } else {
+    pull_bulk<Q, T>(a.fin, a.N, x, y, z, a.nx, a.ny, a.nz, f);
+  }
+}
+
+// A8 / reading R8: u^B of a wall-model cell from the tangential velocity at x + n.
+template <int Q, typename T, bool PULL>
+__device__ __forceinline__ void wallmodel_ub(const StepArgs<T>& a, int x, int y, int z, uint8_t cls, T& ubx, T& uby, T& ubz) {
+  constexpr Stencil<Q> L{};
+  ubx = uby = ubz = T(0);
+  const int code = (cls >> CLS_NORMAL_SHIFT) & 7;
+  int n[3] = {0, 0, 0};
+  n[code >> 1] = (code & 1) ? -1 : 1;
+  int x2 = x + n[0], y2 = y + n[1], z2 = z + n[2];
+  x2 = (x2 < 0) ? x2 + a.nx : ((x2 >= a.nx) ? x2 - a.nx : x2);
+  y2 = (y2 < 0) ? y2 + a.ny : ((y2 >= a.ny) ? y2 - a.ny : y2);
+  z2 = (z2 < 0) ? z2 + a.nz : ((z2 >= a.nz) ? z2 - a.nz : z2);
+  const uint8_t cls2 = a.cls[cell_index(x2, y2, z2, a.nx, a.ny)];
+  if ((cls2 & CLS_TYPE) == T_SOLID) return;
+  T f2[Q];
+  load_state<Q, T, PULL>(a, x2, y2, z2, cls2, f2);
+  double rho = 0.0, j[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    const double v = static_cast<double>(f2[i]);
+    rho += v;
+    j[0] += L.c[i][0] * v;
+    j[1] += L.c[i][1] * v;
+    j[2] += L.c[i][2] * v;
+  }
+  const double u2[3] = {j[0] / rho, j[1] / rho, j[2] / rho};
+  const double un = u2[0] * n[0] + u2[1] * n[1] + u2[2] * n[2];
+  const double t0 = u2[0] - un * n[0], t1 = u2[1] - un * n[1], t2 = u2[2] - un * n[2];
+  const double U2 = sqrt(t0 * t0 + t1 * t1 + t2 * t2);
+  if (U2 < 1e-14) return;
+  const double r = wallmodel_ratio(U2, a.nu, a.wm_kappa, a.wm_E);
+  ubx = static_cast<T>(r * t0);
+  uby = static_cast<T>(r * t1);
+  ubz = static_cast<T>(r * t2);
+}
+
+// ---- the step kernel --------------------------------------------------------------------------------
+// The masked path (A7 + A8): cells that are INLET / OUTLET / WALLMODEL or have a SOLID neighbour.
+// Kept out of line so that the bulk path keeps its populations in registers.
+template <int Q, typename T, int MODE>
+__device__ __noinline__ void step_masked_cell(const StepArgs<T>& a, int x, int y, int z, uint8_t cls) {
+  constexpr bool PULL = (MODE != MODE_COLLIDE);
+  const long long self = cell_index(x, y, z, a.nx, a.ny);
+  const int type = cls & CLS_TYPE;
+  T d = T(0), ubx = T(0), uby = T(0), ubz = T(0);
+  if (MODE != MODE_STREAM) {
+    if (a.d != nullptr) d = __ldg(a.d + self);
+    if (type == T_WM && a.wm_enable) wallmodel_ub<Q, T, PULL>(a, x, y, z, cls, ubx, uby, ubz);
+  }
+  T f[Q];
+  load_state<Q, T, PULL>(a, x, y, z, cls, f);
+  if (MODE != MODE_STREAM) collide_cell<Q, T>(f, d, ubx, uby, ubz, a.tau0, a.smago_k);
+#pragma unroll
+  for (int i = 0; i < Q; ++i) a.fout[i * a.N + self] = f[i];
+}
+
+// grid (ceil(nx/bx), ceil(ny/by), nz), block (bx, by): thread <-> cell, x fastest (coalesced rows).
+template <int Q, typename T, int MODE>
+__global__ void __launch_bounds__(256) k_step(const __grid_constant__ StepArgs<T> a) {
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  const int y = blockIdx.y * blockDim.y + threadIdx.y;
+  const int z = blockIdx.z;
+  if (x >= a.nx || y >= a.ny) return;
+  const long long self = cell_index(x, y, z, a.nx, a.ny);
+  const uint8_t cls = a.cls[self];
+  if ((cls & CLS_TYPE) == T_SOLID) return;   // SOLID cells are inert: nothing read, nothing written (R5)
+  if (cls & CLS_MASKED) {
+    step_masked_cell<Q, T, MODE>(a, x, y, z, cls);
+    return;
+  }
+  // bulk path: plain FLUID cell, no SOLID neighbour
+  T f[Q];
+  T d = T(0);
+  if (MODE != MODE_STREAM && a.d != nullptr) d = __ldg(a.d + self);
+  if (MODE == MODE_COLLIDE) {
+#pragma unroll
+    for (int i = 0; i < Q; ++i) f[i] = __ldg(a.fin + i * a.N + self);
+  } else {
+    pull_bulk<Q, T>(a.fin, a.N, x, y, z, a.nx, a.ny, a.nz, f);
+  }
+  if (MODE != MODE_STREAM) collide_cell<Q, T>(f, d, T(0), T(0), T(0), a.tau0, a.smago_k);
+#pragma unroll
+  for (int i = 0; i < Q; ++i) a.fout[i * a.N + self] = f[i];
+}
+
+// ---- A9: moments of S_t -----------------------------------------------------------------------------
+template <int Q, typename T, bool PULL>
+__global__ void __launch_bounds__(256) k_moments(const __grid_constant__ StepArgs<T> a, T* __restrict__ rho_out, T* __restrict__ u_out) {
+  constexpr Stencil<Q> L{};
+  constexpr int H = (Q - 1) / 2;
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  const int y = blockIdx.y * blockDim.y + threadIdx.y;
+  const int z = blockIdx.z;
+  if (x >= a.nx || y >= a.ny) return;
+  const long long self = cell_index(x, y, z, a.nx, a.ny);
+  const uint8_t cls = a.cls[self];
+  T f[Q];
+  load_state<Q, T, PULL>(a, x, y, z, cls, f);
+  T rho = f[0], jx = T(0), jy = T(0), jz = T(0);
+#pragma unroll
+  for (int i = 1; i <= H; ++i) {
+    rho += f[i] + f[i + H];
+    const T df = f[i] - f[i + H];
+    jx += T(L.c[i][0]) * df;
+    jy += T(L.c[i][1]) * df;
+    jz += T(L.c[i][2]) * df;
+  }
+  if (rho_out) rho_out[self] = rho;
+  if (u_out) {
+    u_out[self] = jx / rho;
+    u_out[a.N + self] = jy / rho;
+    u_out[2 * a.N + self] = jz / rho;
+  }
+}
+
+// ---- A9: totals over non-SOLID cells (mass, momentum, kinetic energy), fp64 accumulation --------------
+// warp shuffle tree -> one shared-memory partial per warp -> one atomicAdd(double) per block and quantity
+template <int Q, typename T, bool PULL>
+__global__ void __launch_bounds__(256) k_totals(const __grid_constant__ StepArgs<T> a, double* __restrict__ out /*[5]*/) {
+  constexpr Stencil<Q> L{};
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  const int y = blockIdx.y * blockDim.y + threadIdx.y;
+  const int z = blockIdx.z;
+  double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  if (x < a.nx && y < a.ny) {
+    const long long self = cell_index(x, y, z, a.nx, a.ny);
+    const uint8_t cls = a.cls[self];
+    if ((cls & CLS_TYPE) != T_SOLID) {
+      T f[Q];
+      load_state<Q, T, PULL>(a, x, y, z, cls, f);
+      double rho = 0.0, jx = 0.0, jy = 0.0, jz = 0.0;
+#pragma unroll
+      for (int i = 0; i < Q; ++i) {
+        const double fi = static_cast<double>(f[i]);
+        rho += fi;
+        jx += L.c[i][0] * fi;
+        jy += L.c[i][1] * fi;
+        jz += L.c[i][2] * fi;
+      }
+      v[0] = rho;  v[1] = jx;  v[2] = jy;  v[3] = jz;
+      v[4] = 0.5 * (jx * jx + jy * jy + jz * jz) / rho;
+    }
+  }
+  __shared__ double part[5][8];
+  const int tid = threadIdx.y * blockDim.x + threadIdx.x;
+  const int lane = tid & 31, warp = tid >> 5;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    double s = v[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    if (lane == 0) part[k][warp] = s;
+  }
+  __syncthreads();
+  const int nwarps = (blockDim.x * blockDim.y + 31) >> 5;
+  if (tid < 5) {
+    double s = 0.0;
+    for (int w = 0; w < nwarps; ++w) s += part[tid][w];
+    atomicAdd(out + tid, s);
+  }
+}
+
+// ---- A4 as an initialiser: f = f^eq(rho, u) ----------------------------------------------------------
+template <int Q, typename T>
+__global__ void __launch_bounds__(256) k_init_equilibrium(const T* __restrict__ rho_in, const T* __restrict__ u_in,
+                                                          T* __restrict__ fa, T* __restrict__ fb, long long N) {
+  constexpr Stencil<Q> L{};
+  const long long n = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (n >= N) return;
+  const T rho = rho_in[n], ux = u_in[n], uy = u_in[N + n], uz = u_in[2 * N + n];
+  const T base = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    const T cu = T(L.c[i][0]) * ux + T(L.c[i][1]) * uy + T(L.c[i][2]) * uz;
+    const T v = weight<Q, T>(L.c2[i]) * rho * (base + T(3) * cu + T(4.5) * cu * cu);
+    fa[i * N + n] = v;
+    fb[i * N + n] = v;   // SOLID cells must hold the same values in both lattices
+  }
+}
+
+// ---- flag validation + classification ------------------------------------------------------------
+// cls = type | normal<<3 | MASKED if the cell is not plain FLUID or any lattice neighbour is SOLID.
+// counters[0] = invalid flag bytes, [1] = SOLID cells, [2] = masked cells.
+template <int Q>
+__global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ flags, uint8_t* __restrict__ cls, int nx,
+                                                  int ny, int nz, unsigned long long* __restrict__ counters) {
+  constexpr Stencil<Q> L{};
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  const int y = blockIdx.y * blockDim.y + threadIdx.y;
+  const int z = blockIdx.z;
+  if (x >= nx || y >= ny) return;
+  const long long self = cell_index(x, y, z, nx, ny);
+  const uint8_t fl = flags[self];
+  const int type = fl & 0x0F, hi = fl >> 4;
+  bool bad = type > T_WM;
+  if (type == T_WM) bad = bad || hi > 5; else bad = bad || hi != 0;
+  if (type == T_INLET && x != 0) bad = true;
+  if (type == T_OUTLET && x != nx - 1) bad = true;
+  if (bad) { atomicAdd(counters, 1ull); return; }
+  bool masked = type != T_FLUID;
+  if (type != T_SOLID) {
+#pragma unroll
+    for (int i = 1; i < Q; ++i) {
+      int sx = x - L.c[i][0], sy = y - L.c[i][1], sz = z - L.c[i][2];
+      sx = (sx < 0) ? sx + nx : ((sx >= nx) ? sx - nx : sx);
+      sy = (sy < 0) ? sy + ny : ((sy >= ny) ? sy - ny : sy);
+      sz = (sz < 0) ? sz + nz : ((sz >= nz) ? sz - nz : sz);
+      masked = masked || ((flags[cell_index(sx, sy, sz, nx, ny)] & 0x0F) == T_SOLID);
+    }
+  }
+  cls[self] = static_cast<uint8_t>(type | ((type == T_WM ? hi : 0) << CLS_NORMAL_SHIFT) | (masked ? CLS_MASKED : 0));
+  if (type == T_SOLID) atomicAdd(counters + 1, 1ull);
+  else if (masked) atomicAdd(counters + 2, 1ull);
+}
+
+}  // namespace lbm
