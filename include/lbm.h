@@ -128,6 +128,7 @@ const char* lbm_last_error(const lbm_ctx* ctx);
  *   0 steps taken since the last set_fields/init      1 kernels launched by this ctx so far
  *   2 number of cells N                                3 number of SOLID cells
  *   4 device bytes owned by the ctx                    5 cells on the masked (boundary) path
+ *   6 cells handled by the list blocks of the vector kernel (masked cells + their vector mates)
  * Returns -1 for an unknown `what` or a NULL ctx. */
 long long lbm_query(const lbm_ctx* ctx, int what);
 

@@ -187,7 +187,10 @@ def make_config(number, shape=None, k_max=None, n_modes=None):
     rho, u, d (or None), flags (or None).  `shape` overrides the size for scaled-down tests;
     config 5 requires `shape`."""
     seed = 1000 + number
-    tau_les = 0.5 + 3.0 * 1e-5
+    tau_les = 0.5 + 3.0 * 1e-5      # nu = 1e-5 (configs 2 and 4)
+    # configs 3 / 5 state no tau0.  With the wall-model coupling of reading R8 the run blows up (oracle and
+    # CUDA path alike) for tau0 <= 0.505; 0.52 (nu = 6.7e-3) keeps all 2000 steps finite (DESIGN.md, G27).
+    tau_urban = 0.52
     if number == 1:
         nz, ny, nx = shape or (32, 32, 32)
         rho, u = taylor_green(nx, ny, nz, u0=0.05)
@@ -208,7 +211,7 @@ def make_config(number, shape=None, k_max=None, n_modes=None):
         u[0][(flags & 0x0F) != SOLID] = 0.05
         return dict(number=number, Q=19, dtype="f32", shape=(nz, ny, nx), steps=2000 if number == 3 else 100,
                     rho=rho, u=u, d=d, flags=flags,
-                    params=dict(tau0=tau_les, cs_smago=0.1, use_hlbm=1, u_in=(0.05, 0.0, 0.0), wm_enable=1,
+                    params=dict(tau0=tau_urban, cs_smago=0.1, use_hlbm=1, u_in=(0.05, 0.0, 0.0), wm_enable=1,
                                 wm_kappa=0.41, wm_E=9.8))
     if number == 4:
         shape = shape or (512, 512, 512)

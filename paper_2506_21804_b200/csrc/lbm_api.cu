@@ -10,6 +10,9 @@
 #include <cstring>
 #include <new>
 
+#include <cub/device/device_select.cuh>
+#include <cub/iterator/counting_input_iterator.cuh>
+
 #include "lbm_kernels.cuh"
 
 namespace {
@@ -30,7 +33,12 @@ struct lbm_ctx {
   bool has_d;
   uint8_t* cls;          // class byte per cell (see lbm_kernels.cuh)
   uint8_t* cls_alt;      // classification target before it is accepted
-  uint8_t* flags_raw;    // device copy of the caller's flag bytes
+  uint8_t* flags_raw;    // device copy of the caller's flag bytes; afterwards the list marks
+  int* list;             // cells of the non-bulk vectors (vector kernel), ascending
+  long long n_list;
+  void* cub_tmp;
+  size_t cub_tmp_bytes;
+  int* list_count_dev;
   unsigned long long* counters;  // device [4]
   double* totals_dev;            // device [5]
   void* staging;         // host<->device bounce buffer, grown on demand
@@ -41,6 +49,7 @@ struct lbm_ctx {
   size_t device_bytes;
   cudaStream_t stream;
   int block_threads;
+  int use_vector;        // 1: 128-bit vector kernel when nx % (32/dtype) == 0 (default); 0: scalar kernel
   int use_graph;
   lbm_params last;       // parameters of the last lbm_step: the inlet rule is part of how S_t is formed from F_{t-1}
   char err[512];
@@ -107,6 +116,7 @@ void launch_dims(const lbm_ctx* c, dim3& grid, dim3& block) {
   while (ny2 < c->ny) ny2 <<= 1;
   if (by > ny2) by = ny2;
   if (by < 1) by = 1;
+  if (bx * by < 32) by = 32 / bx;   // whole warps only: the reductions use full-mask shuffles
   block = dim3(bx, by, 1);
   grid = dim3((c->nx + bx - 1) / bx, (c->ny + by - 1) / by, c->nz);
 }
@@ -120,6 +130,9 @@ lbm::StepArgs<T> make_args(const lbm_ctx* c, const lbm_params* p, int in, int ou
   a.cls = c->cls;
   a.nx = c->nx;  a.ny = c->ny;  a.nz = c->nz;
   a.N = c->N;
+  a.list = c->list;
+  a.n_list = static_cast<int>(c->n_list);
+  a.list_z = 0;
   if (p) {
     a.tau0 = static_cast<T>(p->tau0);
     a.smago_k = static_cast<T>(18.0 * 1.4142135623730951 * p->cs_smago * p->cs_smago);
@@ -135,16 +148,45 @@ lbm::StepArgs<T> make_args(const lbm_ctx* c, const lbm_params* p, int in, int ou
   return a;
 }
 
+// vector kernel: thread <-> V consecutive cells; block (bx quads, by rows)
+template <typename T>
+void launch_dims_vec(const lbm_ctx* c, dim3& grid, dim3& block) {
+  const int V = lbm::VecOf<T>::V;
+  const int nvec = c->nx / V;
+  int bx = 1;
+  while (bx < nvec && bx < 32) bx <<= 1;
+  int by = c->block_threads / bx;
+  int ny2 = 1;
+  while (ny2 < c->ny) ny2 <<= 1;
+  if (by > ny2) by = ny2;
+  if (bx * by < 32) by = 32 / bx;
+  block = dim3(bx, by, 1);
+  grid = dim3((nvec + bx - 1) / bx, (c->ny + by - 1) / by, c->nz);
+}
+
 template <int Q, typename T>
 int launch_step_t(lbm_ctx* c, const lbm_params* p, int mode) {
   dim3 grid, block;
-  launch_dims(c, grid, block);
   const int in = c->cur, out = 1 - c->cur;
   lbm::StepArgs<T> a = make_args<T>(c, p, in, out);
-  switch (mode) {
-    case lbm::MODE_COLLIDE: lbm::k_step<Q, T, lbm::MODE_COLLIDE><<<grid, block, 0, c->stream>>>(a); break;
-    case lbm::MODE_STREAM_COLLIDE: lbm::k_step<Q, T, lbm::MODE_STREAM_COLLIDE><<<grid, block, 0, c->stream>>>(a); break;
-    default: lbm::k_step<Q, T, lbm::MODE_STREAM><<<grid, block, 0, c->stream>>>(a); break;
+  const bool vec = c->use_vector && (c->nx % (2 * lbm::VecOf<T>::V) == 0);   // whole 32-byte sectors per row
+  if (vec) {
+    launch_dims_vec<T>(c, grid, block);
+    const long long per_slice = static_cast<long long>(grid.x) * grid.y * block.x * block.y;
+    a.list_z = static_cast<int>((c->n_list + per_slice - 1) / per_slice);
+    grid.z += a.list_z;
+    switch (mode) {
+      case lbm::MODE_COLLIDE: lbm::k_step_vec<Q, T, lbm::MODE_COLLIDE><<<grid, block, 0, c->stream>>>(a); break;
+      case lbm::MODE_STREAM_COLLIDE: lbm::k_step_vec<Q, T, lbm::MODE_STREAM_COLLIDE><<<grid, block, 0, c->stream>>>(a); break;
+      default: lbm::k_step_vec<Q, T, lbm::MODE_STREAM><<<grid, block, 0, c->stream>>>(a); break;
+    }
+  } else {
+    launch_dims(c, grid, block);
+    switch (mode) {
+      case lbm::MODE_COLLIDE: lbm::k_step<Q, T, lbm::MODE_COLLIDE><<<grid, block, 0, c->stream>>>(a); break;
+      case lbm::MODE_STREAM_COLLIDE: lbm::k_step<Q, T, lbm::MODE_STREAM_COLLIDE><<<grid, block, 0, c->stream>>>(a); break;
+      default: lbm::k_step<Q, T, lbm::MODE_STREAM><<<grid, block, 0, c->stream>>>(a); break;
+    }
   }
   LBM_CUDA(c, cudaGetLastError());
   c->launches++;
@@ -238,6 +280,41 @@ int classify(lbm_ctx* c, const uint8_t* cell_flags) {
   LBM_CUDA(c, cudaStreamSynchronize(c->stream));
   if (h[0] != 0)
     return fail(c, LBM_EINVAL, "cell_flags: %llu invalid flag byte(s) (type > 4, bad high nibble, INLET off x=0 or OUTLET off x=nx-1)", h[0]);
+  // compact list of the cells the vector kernel leaves to its list blocks
+  const int SV = 32 / c->dtype;        // cells per 32-byte sector of a population row
+  long long n_list = 0;
+  if (c->nx % SV == 0) {
+    const long long nsec = c->N / SV;
+    const unsigned blocks = static_cast<unsigned>((nsec + 255) / 256);
+    if (SV == 8) lbm::k_mark_list<8><<<blocks, 256, 0, c->stream>>>(c->cls_alt, c->flags_raw, nsec, c->counters);
+    else         lbm::k_mark_list<4><<<blocks, 256, 0, c->stream>>>(c->cls_alt, c->flags_raw, nsec, c->counters);
+    LBM_CUDA(c, cudaGetLastError());
+    c->launches++;
+    LBM_CUDA(c, cudaMemcpyAsync(h, c->counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+    n_list = static_cast<long long>(h[3]);
+    int* new_list = nullptr;
+    if (n_list > 0) {
+      int rc = dev_alloc(c, reinterpret_cast<void**>(&new_list), static_cast<size_t>(n_list) * sizeof(int));
+      if (rc != LBM_OK) return rc;
+      cub::CountingInputIterator<int> it(0);
+      size_t need = 0;
+      LBM_CUDA(c, cub::DeviceSelect::Flagged(nullptr, need, it, c->flags_raw, new_list, c->list_count_dev,
+                                             static_cast<int>(c->N), c->stream));
+      if (need > c->cub_tmp_bytes) {
+        if (c->cub_tmp) { cudaFree(c->cub_tmp); c->device_bytes -= c->cub_tmp_bytes; c->cub_tmp = nullptr; c->cub_tmp_bytes = 0; }
+        rc = dev_alloc(c, &c->cub_tmp, need);
+        if (rc != LBM_OK) { cudaFree(new_list); return rc; }
+        c->cub_tmp_bytes = need;
+      }
+      LBM_CUDA(c, cub::DeviceSelect::Flagged(c->cub_tmp, need, it, c->flags_raw, new_list, c->list_count_dev,
+                                             static_cast<int>(c->N), c->stream));
+      LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+    }
+    if (c->list) { cudaFree(c->list); c->device_bytes -= static_cast<size_t>(c->n_list) * sizeof(int); }
+    c->list = new_list;
+  }
+  c->n_list = n_list;
   uint8_t* t = c->cls;  c->cls = c->cls_alt;  c->cls_alt = t;
   c->n_solid = static_cast<long long>(h[1]);
   c->n_masked = static_cast<long long>(h[2]);
@@ -268,7 +345,8 @@ lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype) {
   std::memset(c, 0, sizeof(*c));
   c->Q = lattice;  c->nx = nx;  c->ny = ny;  c->nz = nz;  c->dtype = dtype;  c->N = N;
   c->phase = PHASE_NONE;
-  c->block_threads = 128;
+  c->block_threads = 64;
+  c->use_vector = 1;
   c->last = default_params();
   std::snprintf(c->err, sizeof(c->err), "no error");
   const size_t pop = static_cast<size_t>(lattice) * N * dtype;
@@ -280,9 +358,10 @@ lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype) {
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->flags_raw), N);
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->counters), 4 * sizeof(unsigned long long));
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->totals_dev), 5 * sizeof(double));
+  if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->list_count_dev), sizeof(int));
   if (rc == LBM_OK && cudaMemset(c->cls, 0, N) != cudaSuccess) rc = fail(c, LBM_ECUDA, "cudaMemset failed");
   if (rc != LBM_OK) {
-    std::snprintf(g_create_error, sizeof(g_create_error), "lbm_create: %s", c->err);
+    std::snprintf(g_create_error, sizeof(g_create_error), "lbm_create: %.480s", c->err);
     lbm_destroy(c);
     return nullptr;
   }
@@ -295,6 +374,7 @@ void lbm_destroy(lbm_ctx* c) {
   cudaFree(c->f[0]);  cudaFree(c->f[1]);  cudaFree(c->d);
   cudaFree(c->cls);  cudaFree(c->cls_alt);  cudaFree(c->flags_raw);
   cudaFree(c->counters);  cudaFree(c->totals_dev);  cudaFree(c->staging);
+  cudaFree(c->list);  cudaFree(c->cub_tmp);  cudaFree(c->list_count_dev);
   cudaGetLastError();
   delete c;
 }
@@ -466,6 +546,7 @@ long long lbm_query(const lbm_ctx* c, int what) {
     case 3: return c->n_solid;
     case 4: return static_cast<long long>(c->device_bytes);
     case 5: return c->n_masked;
+    case 6: return c->n_list;
     default: return -1;
   }
 }
@@ -480,6 +561,11 @@ int lbm_set_option(lbm_ctx* c, const char* key, long long value) {
   if (std::strcmp(key, "block_threads") == 0) {
     if (value != 64 && value != 128 && value != 256) return fail(c, LBM_EINVAL, "block_threads must be 64, 128 or 256");
     c->block_threads = static_cast<int>(value);
+    return LBM_OK;
+  }
+  if (std::strcmp(key, "vector") == 0) {
+    if (value != 0 && value != 1) return fail(c, LBM_EINVAL, "vector must be 0 or 1");
+    c->use_vector = static_cast<int>(value);
     return LBM_OK;
   }
   return fail(c, LBM_EINVAL, "unknown option '%s'", key);

@@ -18,7 +18,9 @@
 namespace lbm {
 
 enum : int { T_FLUID = 0, T_SOLID = 1, T_INLET = 2, T_OUTLET = 3, T_WM = 4 };
-// internal class byte: bits 0-2 type, bits 3-5 wall-normal code, bit 7 = cell takes the masked path
+// internal class byte: bits 0-2 type, bits 3-5 wall-normal code, bit 7 = MASKED: the cell is SOLID or
+// WALLMODEL or has a SOLID lattice neighbour (it needs the per-cell boundary path).  INLET / OUTLET cells
+// without a SOLID neighbour are not MASKED: the vector kernel handles them in line.
 constexpr uint8_t CLS_TYPE = 0x07;
 constexpr uint8_t CLS_MASKED = 0x80;
 constexpr int CLS_NORMAL_SHIFT = 3;
@@ -73,12 +75,28 @@ struct StepArgs {
   T u_in[3];
   int wm_enable;
   double wm_kappa, wm_E, nu;
+  // vector kernel only: cells of every vector that is not pure bulk, handled by the first list_z z-slices
+  const int* __restrict__ list;
+  int n_list;
+  int list_z;
 };
 
 // ---- math helpers ---------------------------------------------------------------------------------
-__device__ __forceinline__ float rcp_(float x) { return __frcp_rn(x); }
+// fp32: hardware approximations (MUFU) instead of the IEEE-rounded software sequences, which cost ~10
+// instructions and a slow-path stub each.  rho is always a normal number near 1, so no denormal care is
+// needed.  The reciprocal gets one Newton step (2 FMA) and is then within 1 ulp and unbiased, which keeps
+// the momentum of the collision free of a systematic drift; sqrt only feeds tau_eff.
+__device__ __forceinline__ float rcp_(float x) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return fmaf(fmaf(-x, r, 1.0f), r, r);
+}
 __device__ __forceinline__ double rcp_(double x) { return 1.0 / x; }
-__device__ __forceinline__ float sqrt_(float x) { return __fsqrt_rn(x); }
+__device__ __forceinline__ float sqrt_(float x) {
+  float r;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
 __device__ __forceinline__ double sqrt_(double x) { return sqrt(x); }
 
 // A2..A6 on one cell held in registers.  f[] in: S_t, out: post-collision F_t.
@@ -114,14 +132,16 @@ __device__ __forceinline__ void collide_cell(T (&f)[Q], T d, T ubx, T uby, T ubz
   T omega;
   if (smago_k > T(0)) {
     // second moment of f^eq(rho, u^) is rho (I/3 + u^ u^)
+    const T qx = rho * ux, qy = rho * uy, qz = rho * uz;
     const T third = rho * T(1.0 / 3.0);
-    const T pxx = mxx - third - rho * ux * ux;
-    const T pyy = myy - third - rho * uy * uy;
-    const T pzz = mzz - third - rho * uz * uz;
-    const T pxy = mxy - rho * ux * uy;
-    const T pxz = mxz - rho * ux * uz;
-    const T pyz = myz - rho * uy * uz;
-    const T npi = sqrt_(pxx * pxx + pyy * pyy + pzz * pzz + T(2) * (pxy * pxy + pxz * pxz + pyz * pyz));
+    const T pxx = (mxx - third) - qx * ux;
+    const T pyy = (myy - third) - qy * uy;
+    const T pzz = (mzz - third) - qz * uz;
+    const T pxy = mxy - qx * uy;
+    const T pxz = mxz - qx * uz;
+    const T pyz = myz - qy * uz;
+    const T off = pxy * pxy + pxz * pxz + pyz * pyz;
+    const T npi = sqrt_(pxx * pxx + pyy * pyy + pzz * pzz + (off + off));
     const T tau = T(0.5) * (tau0 + sqrt_(tau0 * tau0 + smago_k * npi * inv_rho));
     omega = rcp_(tau);
   } else {
@@ -129,16 +149,26 @@ __device__ __forceinline__ void collide_cell(T (&f)[Q], T d, T ubx, T uby, T ubz
   }
   const T base = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
   const T keepf = T(1) - omega;
-  f[0] = keepf * f[0] + omega * (weight<Q, T>(0) * rho * base);
+  const T ro = rho * omega;
+  // per weight class (|c|^2 = 1, 2, 3): A = w rho omega base, B = 4.5 w rho omega, C = 3 w rho omega
+  T A[4], B[4], C[4];
+#pragma unroll
+  for (int k = 1; k <= ((Q == 19) ? 2 : 3); ++k) {
+    const T wr = weight<Q, T>(k) * ro;
+    A[k] = wr * base;
+    B[k] = wr * T(4.5);
+    C[k] = wr * T(3);
+  }
+  f[0] = keepf * f[0] + (weight<Q, T>(0) * ro) * base;
 #pragma unroll
   for (int i = 1; i <= H; ++i) {
     T cu = T(0);
     if (L.c[i][0] == 1) cu += ux; else if (L.c[i][0] == -1) cu -= ux;
     if (L.c[i][1] == 1) cu += uy; else if (L.c[i][1] == -1) cu -= uy;
     if (L.c[i][2] == 1) cu += uz; else if (L.c[i][2] == -1) cu -= uz;
-    const T wr = weight<Q, T>(L.c2[i]) * rho * omega;
-    const T even = wr * (base + T(4.5) * cu * cu);
-    const T odd = wr * T(3) * cu;
+    const int k = L.c2[i];
+    const T even = (B[k] * cu) * cu + A[k];
+    const T odd = C[k] * cu;
     f[i] = keepf * f[i] + (even + odd);
     f[i + H] = keepf * f[i + H] + (even - odd);
   }
@@ -184,42 +214,57 @@ __device__ __forceinline__ void inlet_fixup(T (&g)[Q], T uwx, T uwy, T uwz) {
   }
 }
 
-// Spalding's law (Eq. 17) and the two Newton solves of reading R8, in double for both dtypes
-// (0.8 % of the cells of config 3 take this path).  Returns U1 / U2.
+// Spalding's law (Eq. 17) and the two root solves of reading R8, in double for both dtypes (only the
+// wall-model cells take this path).  Returns U1 / U2.
+//   unknown p = u2+ = U2 / u_tau:   p Sp(p) = Re,  Re = U2 y2 / nu      (Eq. 15-16: y2+ u2+ = U2 y2 / nu)
+//   then q = u1+:                   Sp(q) = y1+ = (y1 / y2) Re / p
+// Both left sides are increasing and convex, so Newton converges monotonically once it is on the
+// right of the root; the start values (viscous / log-law estimates) put it there or one step away.
+// The roots are the unique ones the definition fixes, converged to 1e-14 relative.
+__device__ __forceinline__ void spalding_eval(double up, double kappa, double invE, double& sp, double& dsp) {
+  const double k = kappa * up;
+  const double ek = exp(k);
+  const double k2 = 0.5 * k * k;
+  sp = up + invE * (ek - 1.0 - k - k2 - k2 * k * (1.0 / 3.0));
+  dsp = 1.0 + kappa * invE * (ek - 1.0 - k - k2);
+}
+
 __device__ __noinline__ double wallmodel_ratio(double U2, double nu, double kappa, double E) {
   const double y2 = 1.5, y1 = 0.5;
   const double invE = 1.0 / E;
-  double ut = sqrt(nu * U2 / y2);
-  for (int it = 0; it < 200; ++it) {
-    const double up = U2 / ut;
-    const double k = kappa * up;
-    const double ek = exp(k);
-    const double sp = up + invE * (ek - 1.0 - k - 0.5 * k * k - k * k * k * (1.0 / 6.0));
-    const double dsp = 1.0 + kappa * invE * (ek - 1.0 - k - 0.5 * k * k);
-    const double R = sp - y2 * ut / nu;
-    const double dR = -dsp * up / ut - y2 / nu;
-    double un = ut - R / dR;
-    if (!(un > 0.0)) un = 0.5 * ut;
-    const double delta = fabs(un - ut);
-    ut = un;
-    if (delta <= 1e-13 * ut) break;
+  const double Re = U2 * y2 / nu;
+  double p = sqrt(Re);                       // viscous sublayer: Sp(p) = p
+  if (p > 8.0) {                             // log region estimate: p = ln(E Re / p) / kappa
+    double q = 20.0;
+#pragma unroll 1
+    for (int it = 0; it < 3; ++it) q = log(E * Re / q) / kappa;
+    if (q > 1.0 && q < p) p = q;
   }
-  const double y1p = y1 * ut / nu;
-  double lg = log(E * y1p) / kappa;
-  if (!(lg > 0.0)) lg = 0.0;
-  double up = fmin(y1p, lg + 1.0);
-  for (int it = 0; it < 200; ++it) {
-    const double k = kappa * up;
-    const double ek = exp(k);
-    const double sp = up + invE * (ek - 1.0 - k - 0.5 * k * k - k * k * k * (1.0 / 6.0));
-    const double dsp = 1.0 + kappa * invE * (ek - 1.0 - k - 0.5 * k * k);
-    double un = up - (sp - y1p) / dsp;
-    if (un < 0.0) un = 0.5 * up;
-    const double delta = fabs(un - up);
-    up = un;
-    if (delta <= 1e-13 * fabs(up)) break;
+#pragma unroll 1
+  for (int it = 0; it < 100; ++it) {
+    double sp, dsp;
+    spalding_eval(p, kappa, invE, sp, dsp);
+    const double G = p * sp - Re;
+    const double dG = sp + p * dsp;
+    double pn = p - G / dG;
+    if (!(pn > 0.0)) pn = 0.5 * p;
+    const double delta = fabs(pn - p);
+    p = pn;
+    if (delta <= 1e-14 * p) break;
   }
-  return up * ut / U2;
+  const double y1p = (y1 / y2) * Re / p;
+  double q = fmin(y1p, p);                   // Sp(q) >= y1+ at both candidates: right of the root
+#pragma unroll 1
+  for (int it = 0; it < 100; ++it) {
+    double sp, dsp;
+    spalding_eval(q, kappa, invE, sp, dsp);
+    double qn = q - (sp - y1p) / dsp;
+    if (qn < 0.0) qn = 0.5 * q;
+    const double delta = fabs(qn - q);
+    q = qn;
+    if (delta <= 1e-14 * fabs(q)) break;
+  }
+  return q / p;                              // U1 / U2 = u1+ u_tau / (u2+ u_tau)
 }
 
 struct Coord {
@@ -281,7 +326,7 @@ __device__ __forceinline__ void load_state(const StepArgs<T>& a, int x, int y, i
     const long long self = cell_index(x, y, z, a.nx, a.ny);
 #pragma unroll
     for (int i = 0; i < Q; ++i) f[i] = __ldg(a.fin + i * a.N + self);
-  } else if (cls & CLS_MASKED) {
+  } else if ((cls & CLS_MASKED) || type != T_FLUID) {
     pull_masked<Q, T>(a, x, y, z, type, f);
   } else {
     pull_bulk<Q, T>(a.fin, a.N, x, y, z, a.nx, a.ny, a.nz, f);
@@ -328,7 +373,7 @@ __device__ __forceinline__ void wallmodel_ub(const StepArgs<T>& a, int x, int y,
 // The masked path (A7 + A8): cells that are INLET / OUTLET / WALLMODEL or have a SOLID neighbour.
 // Kept out of line so that the bulk path keeps its populations in registers.
 template <int Q, typename T, int MODE>
-__device__ __noinline__ void step_masked_cell(const StepArgs<T>& a, int x, int y, int z, uint8_t cls) {
+__device__ __forceinline__ void step_cell_any(const StepArgs<T>& a, int x, int y, int z, uint8_t cls) {
   constexpr bool PULL = (MODE != MODE_COLLIDE);
   const long long self = cell_index(x, y, z, a.nx, a.ny);
   const int type = cls & CLS_TYPE;
@@ -344,6 +389,11 @@ __device__ __noinline__ void step_masked_cell(const StepArgs<T>& a, int x, int y
   for (int i = 0; i < Q; ++i) a.fout[i * a.N + self] = f[i];
 }
 
+template <int Q, typename T, int MODE>
+__device__ __noinline__ void step_masked_cell(const StepArgs<T>& a, int x, int y, int z, uint8_t cls) {
+  step_cell_any<Q, T, MODE>(a, x, y, z, cls);
+}
+
 // grid (ceil(nx/bx), ceil(ny/by), nz), block (bx, by): thread <-> cell, x fastest (coalesced rows).
 template <int Q, typename T, int MODE>
 __global__ void __launch_bounds__(256) k_step(const __grid_constant__ StepArgs<T> a) {
@@ -354,7 +404,7 @@ __global__ void __launch_bounds__(256) k_step(const __grid_constant__ StepArgs<T
   const long long self = cell_index(x, y, z, a.nx, a.ny);
   const uint8_t cls = a.cls[self];
   if ((cls & CLS_TYPE) == T_SOLID) return;   // SOLID cells are inert: nothing read, nothing written (R5)
-  if (cls & CLS_MASKED) {
+  if ((cls & CLS_MASKED) || (cls & CLS_TYPE) != T_FLUID) {
     step_masked_cell<Q, T, MODE>(a, x, y, z, cls);
     return;
   }
@@ -371,6 +421,214 @@ __global__ void __launch_bounds__(256) k_step(const __grid_constant__ StepArgs<T
   if (MODE != MODE_STREAM) collide_cell<Q, T>(f, d, T(0), T(0), T(0), a.tau0, a.smago_k);
 #pragma unroll
   for (int i = 0; i < Q; ++i) a.fout[i * a.N + self] = f[i];
+}
+
+// ---- the vectorised step kernel (the hot one) ------------------------------------------------------
+// One thread owns V = 16/sizeof(T) consecutive cells of a row (4 floats / 2 doubles): every population
+// is moved with one aligned 128-bit load and one aligned 128-bit store per thread.  The populations
+// with c_x = +-1 need the row shifted by one element: the thread loads its own aligned vector and takes
+// the one missing element from the neighbouring lane with a warp shuffle (row ends: one scalar load).
+// Vectors whose V cells are all plain bulk FLUID take this path; a vector that contains a SOLID,
+// INLET, OUTLET, WALLMODEL or solid-adjacent cell is processed cell by cell out of line (A7/A8).
+template <typename T> struct VecOf;
+template <> struct VecOf<float> { static constexpr int V = 4; };
+template <> struct VecOf<double> { static constexpr int V = 2; };
+
+__device__ __forceinline__ void ld_vec(const float* p, float (&v)[4]) {
+  const float4 t = __ldcs(reinterpret_cast<const float4*>(p));
+  v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+}
+__device__ __forceinline__ void ld_vec(const double* p, double (&v)[2]) {
+  const double2 t = __ldcs(reinterpret_cast<const double2*>(p));
+  v[0] = t.x; v[1] = t.y;
+}
+__device__ __forceinline__ void ld_vec_keep(const float* p, float (&v)[4]) {
+  const float4 t = __ldg(reinterpret_cast<const float4*>(p));
+  v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+}
+__device__ __forceinline__ void ld_vec_keep(const double* p, double (&v)[2]) {
+  const double2 t = __ldg(reinterpret_cast<const double2*>(p));
+  v[0] = t.x; v[1] = t.y;
+}
+__device__ __forceinline__ void st_vec(float* p, const float (&v)[4]) {
+  __stcs(reinterpret_cast<float4*>(p), make_float4(v[0], v[1], v[2], v[3]));
+}
+__device__ __forceinline__ void st_vec(double* p, const double (&v)[2]) {
+  __stcs(reinterpret_cast<double2*>(p), make_double2(v[0], v[1]));
+}
+// class bytes of one 32-byte sector of a population row (8 floats / 4 doubles = 2 vectors), one aligned load
+__device__ __forceinline__ unsigned long long ld_cls_sector(const uint8_t* p, float) { return *reinterpret_cast<const unsigned long long*>(p); }
+__device__ __forceinline__ unsigned long long ld_cls_sector(const uint8_t* p, double) { return *reinterpret_cast<const uint32_t*>(p); }
+
+// grid (ceil(nx/V/bx), ceil(ny/by), list_z + nz), block (bx, by), bx a power of two <= 32.
+// The first list_z z-slices of the grid do not own a lattice slab: their threads walk the compact list
+// of cells that belong to non-bulk vectors (the masked boundary kernel, A7/A8, as a block role of the
+// same launch: it is scheduled first and overlaps with the bulk blocks).
+template <int Q, typename T, int MODE>
+__global__ void __launch_bounds__(256) k_step_vec(const __grid_constant__ StepArgs<T> a) {
+  constexpr Stencil<Q> L{};
+  constexpr int V = VecOf<T>::V;
+  constexpr unsigned FULL = 0xffffffffu;
+  const int tx = threadIdx.x;
+  if (static_cast<int>(blockIdx.z) < a.list_z) {
+    const long long blk = (static_cast<long long>(blockIdx.z) * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+    const long long k = blk * (blockDim.x * blockDim.y) + threadIdx.y * blockDim.x + tx;
+    if (k < a.n_list) {
+      const int cell = a.list[k];
+      const int plane = a.nx * a.ny;
+      const int cz = cell / plane, rem = cell - cz * plane;
+      const int cy = rem / a.nx, cx = rem - cy * a.nx;
+      const uint8_t c = a.cls[cell];
+      if ((c & CLS_TYPE) == T_SOLID) {
+        // a SOLID cell that shares a 32-byte sector with cells of the list: copy it through, so that every
+        // store instruction of the warp covers whole sectors (partial-sector writes cost an L2 read-fill)
+#pragma unroll
+        for (int i = 0; i < Q; ++i) a.fout[i * a.N + cell] = __ldg(a.fin + i * a.N + cell);
+      } else {
+        step_cell_any<Q, T, MODE>(a, cx, cy, cz, c);
+      }
+    }
+    return;
+  }
+  const int lane = (threadIdx.y * blockDim.x + tx) & 31;
+  const int nvec = a.nx / V;
+  const int qx = blockIdx.x * blockDim.x + tx;
+  const int y = blockIdx.y * blockDim.y + threadIdx.y;
+  const int z = blockIdx.z - a.list_z;
+  const bool active = (qx < nvec) && (y < a.ny);
+  const int x0 = qx * V;
+  const int nx = a.nx, ny = a.ny, nz = a.nz;
+  const long long N = a.N;
+  const long long row = active ? (static_cast<long long>(z) * ny + y) * nx : 0;
+  const long long self = row + (active ? x0 : 0);
+  // class bytes of the vector's 32-byte sector (2 vectors): the vector takes the bulk path only if no
+  // cell of its sector is MASKED, so that bulk and list stores never split a sector
+  unsigned long long secw = ~0ull;
+  if (active) secw = ld_cls_sector(a.cls + row + (x0 & ~(2 * V - 1)), T(0));
+  constexpr unsigned long long MASKED_ALL = (V == 4) ? 0x8080808080808080ull : 0x80808080ull;
+  constexpr uint32_t TYPE_ALL = (V == 4) ? 0x07070707u : 0x0707u;
+  constexpr uint32_t SOLID_ALL = (V == 4) ? 0x01010101u : 0x0101u;
+  const uint32_t clsw = static_cast<uint32_t>(secw >> ((qx & 1) ? 8 * V : 0)) & ((V == 4) ? 0xffffffffu : 0xffffu);
+  const bool all_solid = !active || ((clsw & TYPE_ALL) == SOLID_ALL);
+  const bool bulk = active && ((secw & MASKED_ALL) == 0);
+  const bool doload = active && !all_solid;
+  // INLET (only ever at x = 0) / OUTLET (only ever at x = nx-1) cells of a bulk vector
+  const bool inlet0 = bulk && (x0 == 0) && ((clsw & CLS_TYPE) == T_INLET);
+  const bool outletN = bulk && (qx == nvec - 1) && (((clsw >> (8 * (V - 1))) & CLS_TYPE) == T_OUTLET);
+
+  T f[Q][V];
+  T d[V];
+#pragma unroll
+  for (int v = 0; v < V; ++v) d[v] = T(0);
+  if (MODE != MODE_STREAM && bulk && a.d != nullptr) {
+    T dv[V];
+    ld_vec_keep(a.d + self, dv);
+#pragma unroll
+    for (int v = 0; v < V; ++v) d[v] = dv[v];
+  }
+  if (MODE == MODE_COLLIDE) {
+    if (bulk) {
+#pragma unroll
+      for (int i = 0; i < Q; ++i) ld_vec(a.fin + i * N + self, f[i]);
+    }
+  } else {
+    const int ym = (y == 0) ? ny - 1 : y - 1, yp = (y >= ny - 1) ? 0 : y + 1;
+    const int zm = (z == 0) ? nz - 1 : z - 1, zp = (z == nz - 1) ? 0 : z + 1;
+    const int xl = (x0 == 0) ? nx - 1 : x0 - 1;            // element left of the vector (periodic)
+    const int xr = (x0 + V >= nx) ? 0 : x0 + V;            // element right of the vector
+    const bool edge_l = doload && ((lane == 0) || (tx == 0));
+    const bool edge_r = doload && ((lane == 31) || (tx == static_cast<int>(blockDim.x) - 1) || (qx == nvec - 1));
+    // phase 1: issue every load before anything consumes one (in-order issue: a shuffle placed right
+    // after its load would serialise the 19 loads).  Addresses: one running pointer per population
+    // (+N each) plus one of 9 (dy,dz) row offsets; all deltas fit 32 bits because N < 2^31.
+    const int dym = (ym - y) * nx, dyp = (yp - y) * nx;
+    const int plane = nx * ny;
+    const int dzm = (zm - z) * plane, dzp = (zp - z) * plane;
+    const int exl = xl - x0, exr = xr - x0;                  // edge element, relative to the vector start
+    const T* pself = a.fin + self;
+    T e[Q];   // the one element a shifted row needs from outside the warp / row (edge lanes only)
+#pragma unroll
+    for (int i = 0; i < Q; ++i) {
+      const long long off = static_cast<long long>((L.c[i][1] == 0) ? 0 : ((L.c[i][1] == 1) ? dym : dyp)) +
+                            static_cast<long long>((L.c[i][2] == 0) ? 0 : ((L.c[i][2] == 1) ? dzm : dzp));
+      const T* src = pself + off;                            // source row, at the vector's x
+      pself += N;
+#pragma unroll
+      for (int v = 0; v < V; ++v) f[i][v] = T(0);
+      e[i] = T(0);
+      if (doload) ld_vec(src, f[i]);
+      if (L.c[i][0] == 1 && edge_l) e[i] = __ldg(src + exl);
+      if (L.c[i][0] == -1 && edge_r) e[i] = __ldg(src + exr);
+    }
+    // phase 2: realign the rows with c_x = +-1 by one element through the neighbouring lane
+#pragma unroll
+    for (int i = 0; i < Q; ++i) {
+      if (L.c[i][0] == 1) {                                  // source x - 1: shift right by one
+        T nb = __shfl_up_sync(FULL, f[i][V - 1], 1);
+        if (edge_l) nb = e[i];
+#pragma unroll
+        for (int v = V - 1; v > 0; --v) f[i][v] = f[i][v - 1];
+        f[i][0] = nb;
+      } else if (L.c[i][0] == -1) {                          // source x + 1: shift left by one
+        T nb = __shfl_down_sync(FULL, f[i][0], 1);
+        if (edge_r) nb = e[i];
+        if (outletN) nb = f[i][V - 1];                       // R7: ghost plane nx := plane nx-1
+#pragma unroll
+        for (int v = 0; v < V - 1; ++v) f[i][v] = f[i][v + 1];
+        f[i][V - 1] = nb;
+      }
+    }
+  }
+
+  if (bulk) {
+    if (MODE != MODE_COLLIDE && inlet0) {                    // R6 on the x = 0 cell of the row
+      T fc[Q];
+#pragma unroll
+      for (int i = 0; i < Q; ++i) fc[i] = f[i][0];
+      inlet_fixup<Q, T>(fc, a.u_in[0], a.u_in[1], a.u_in[2]);
+#pragma unroll
+      for (int i = 0; i < Q; ++i) f[i][0] = fc[i];
+    }
+    if (MODE != MODE_STREAM) {
+#pragma unroll
+      for (int v = 0; v < V; ++v) {
+        T fc[Q];
+#pragma unroll
+        for (int i = 0; i < Q; ++i) fc[i] = f[i][v];
+        collide_cell<Q, T>(fc, d[v], T(0), T(0), T(0), a.tau0, a.smago_k);
+#pragma unroll
+        for (int i = 0; i < Q; ++i) f[i][v] = fc[i];
+      }
+    }
+    T* pout = a.fout + self;
+#pragma unroll
+    for (int i = 0; i < Q; ++i) {
+      st_vec(pout, f[i]);
+      pout += N;
+    }
+  }
+  // non-bulk vectors: their cells are in the compact list and were handled by the list blocks
+}
+
+// marks the cells that the list blocks of k_step_vec must process: EVERY cell (SOLID ones included, they
+// are copied through) of a 32-byte sector (SV = 8 floats / 4 doubles, aligned) that holds at least one
+// MASKED cell and is not SOLID throughout.  mark[] feeds a stream compaction.
+template <int SV>
+__global__ void __launch_bounds__(256) k_mark_list(const uint8_t* __restrict__ cls, uint8_t* __restrict__ mark,
+                                                   long long nsec_total, unsigned long long* __restrict__ counters) {
+  const long long q = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (q >= nsec_total) return;
+  bool any_masked = false, all_solid = true;
+#pragma unroll
+  for (int v = 0; v < SV; ++v) {
+    const uint8_t c = cls[q * SV + v];
+    any_masked = any_masked || (c & CLS_MASKED);
+    all_solid = all_solid && ((c & CLS_TYPE) == T_SOLID);
+  }
+  const bool m = any_masked && !all_solid;
+#pragma unroll
+  for (int v = 0; v < SV; ++v) mark[q * SV + v] = m ? 1 : 0;
+  if (m) atomicAdd(counters + 3, static_cast<unsigned long long>(SV));
 }
 
 // ---- A9: moments of S_t -----------------------------------------------------------------------------
@@ -487,7 +745,8 @@ __global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ fl
   if (type == T_INLET && x != 0) bad = true;
   if (type == T_OUTLET && x != nx - 1) bad = true;
   if (bad) { atomicAdd(counters, 1ull); return; }
-  bool masked = type != T_FLUID;
+  bool masked = (type == T_SOLID) || (type == T_WM);
+  bool special = type != T_FLUID;
   if (type != T_SOLID) {
 #pragma unroll
     for (int i = 1; i < Q; ++i) {
@@ -500,7 +759,7 @@ __global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ fl
   }
   cls[self] = static_cast<uint8_t>(type | ((type == T_WM ? hi : 0) << CLS_NORMAL_SHIFT) | (masked ? CLS_MASKED : 0));
   if (type == T_SOLID) atomicAdd(counters + 1, 1ull);
-  else if (masked) atomicAdd(counters + 2, 1ull);
+  else if (masked || special) atomicAdd(counters + 2, 1ull);
 }
 
 }  // namespace lbm

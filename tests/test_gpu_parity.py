@@ -14,7 +14,7 @@ pytestmark = pytest.mark.gpu
 TORCH_DTYPE = {"f32": torch.float32, "f64": torch.float64}
 
 
-def gpu_run(cfg, f, d, nsteps, dtype, host=False, split=None, block_threads=None):
+def gpu_run(cfg, f, d, nsteps, dtype, host=False, split=None, block_threads=None, vector=None):
     """Run nsteps through the C ABI; returns (populations, rho, u, totals) as numpy."""
     nz, ny, nx = cfg["shape"]
     Q = cfg["Q"]
@@ -22,6 +22,8 @@ def gpu_run(cfg, f, d, nsteps, dtype, host=False, split=None, block_threads=None
     with P.LBM(Q, nx, ny, nz, dtype) as sim:
         if block_threads:
             sim.set_option("block_threads", block_threads)
+        if vector is not None:
+            sim.set_option("vector", vector)
         if host:
             sim.set_fields(f, d, cfg["flags"])
         else:
@@ -140,9 +142,27 @@ def test_all_solid_and_no_flags():
 
 
 @pytest.mark.parametrize("block_threads", [64, 256])
-def test_other_block_sizes(block_threads):
+@pytest.mark.parametrize("vector", [0, 1])
+def test_other_block_sizes_and_scalar_kernel(block_threads, vector):
     cfg = I.make_config(3, shape=(24, 20, 72))
-    check_parity(cfg, "f32", block_threads=block_threads)
+    check_parity(cfg, "f32", block_threads=block_threads, vector=vector)
+    check_parity(cfg, "f64", block_threads=block_threads, vector=vector)
+
+
+@pytest.mark.parametrize("nx", [4, 8, 36, 132, 260])
+def test_vector_kernel_row_ends(nx):
+    """Rows shorter / longer than a warp of vectors, and not a multiple of the block width."""
+    shape = (5, 6, nx)
+    rng = np.random.default_rng(nx)
+    rho = 1.0 + 0.02 * rng.uniform(-1, 1, size=shape)
+    u = 0.04 * rng.uniform(-1, 1, size=(3,) + shape)
+    flags = (rng.uniform(size=shape) < 0.05).astype(np.uint8) * I.SOLID
+    cfg = dict(Q=19, shape=shape, rho=rho, u=u, d=None, flags=flags, dtype="f64", params=dict(tau0=0.55, cs_smago=0.1))
+    check_parity(cfg, "f64")
+    check_parity(cfg, "f32")
+    cfg["flags"] = None
+    cfg["Q"] = 27
+    check_parity(cfg, "f32")
 
 
 def test_channel_with_every_wall_normal_and_inlet_components():
@@ -188,12 +208,13 @@ def test_roundtrip_is_bit_exact_and_phase_independent():
         got, rho, u, tot = gpu_run(cfg, f, d, 0, dtype)
         assert np.array_equal(got, f)
         rr, ru = O.moments(f.astype(np.float64))
-        assert field_error(rho, rr) <= (1e-6 if dtype == "f32" else 1e-15)
+        assert field_error(rho, rr) <= (1e-6 if dtype == "f32" else 2e-15)
         # splitting the run, or reading the state in between, changes nothing (bit-identical)
         a = gpu_run(cfg, f, d, 10, dtype)
         b = gpu_run(cfg, f, d, 10, dtype, split=[1, 2, 7])
-        for x, y in zip(a, b):
+        for x, y in zip(a[:3], b[:3]):
             assert np.array_equal(x, y)
+        assert np.allclose(a[3], b[3], rtol=1e-13, atol=0)      # totals: atomic accumulation order is free
 
 
 def test_reading_state_midrun_does_not_perturb_it():
@@ -222,8 +243,9 @@ def test_host_pointers_equal_device_pointers():
     f, d = oracle_inputs(cfg, "f32")
     a = gpu_run(cfg, f, d, 6, "f32", host=False)
     b = gpu_run(cfg, f, d, 6, "f32", host=True)
-    for x, y in zip(a, b):
+    for x, y in zip(a[:3], b[:3]):
         assert np.array_equal(x, y)
+    assert np.allclose(a[3], b[3], rtol=1e-13, atol=0)
 
 
 @pytest.mark.parametrize("Q", [19, 27])
@@ -261,7 +283,7 @@ def test_error_codes():
         bad[3, 3, 3] = I.INLET                      # INLET off the x = 0 plane
         with pytest.raises(P.LbmError):
             sim.set_fields(f, None, bad)
-        bad[3, 3, 3] = 0x14                         # high nibble on a non-WALLMODEL type
+        bad[3, 3, 3] = 0x10                         # high nibble on a non-WALLMODEL type
         with pytest.raises(P.LbmError):
             sim.set_fields(f, None, bad)
         bad[3, 3, 3] = 0x64                         # normal code 6
