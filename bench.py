@@ -53,6 +53,18 @@ def measured_peak():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def ncu_traffic(workload):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/ncu_traffic.csv)."""
+    import csv
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    if not os.path.exists(p):
+        return None
+    for row in csv.DictReader(open(p)):
+        if row["workload"] == workload:
+            return int(row["dram_read_bytes_per_launch"]) + int(row["dram_write_bytes_per_launch"])
+    return None
+
+
 def algorithmic_bytes_per_step(cfg, dtype, n_solid):
     """2*Q*sizeof(T) + sizeof(T) (porosity, when use_hlbm) + 1 (flag) per non-SOLID cell,
     1 byte per SOLID cell."""
@@ -144,8 +156,8 @@ def run_reference(args, rank, world):
     f = O.step(f, nsteps=args.steps, **kw)
     dt = time.perf_counter() - t0
     value = nonsolid * args.steps / dt / 1e6
-    sample_txt = "oracle (fp64, %d OpenMP threads) on U%s generated like the workload, %d steps" % (
-        str(tuple(reversed(sample))), cores, args.steps)
+    sample_txt = "oracle (fp64, %d OpenMP threads) on the workload generator at (nz,ny,nx)=%s, %d steps" % (
+        cores, str(tuple(sample)), args.steps)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dt / max(args.steps, 1) * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -306,8 +318,8 @@ def main():
                        "finite": finite, "mass_drift_rel": (tot1[0] - tot0[0]) / tot0[0],
                        "bytes_per_update": per_cell},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": None, "peak_source": peak_src, "frac_of_8000_datasheet": achieved / 8000.0,
-                         "algorithmic_bytes_per_launch": step_bytes, "kernel": "lbm::k_step<%d,%s,STREAM_COLLIDE>" % (Q, "float" if dtype == "f32" else "double")},
+                         "traffic": ncu_traffic(args.workload), "peak_source": peak_src, "frac_of_8000_datasheet": achieved / 8000.0,
+                         "algorithmic_bytes_per_launch": step_bytes, "kernel": "lbm::k_step_vec<%d,%s,MODE_STREAM_COLLIDE>" % (Q, "float" if dtype == "f32" else "double")},
             "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         }
         print(json.dumps(line), flush=True)
