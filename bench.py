@@ -74,6 +74,22 @@ def algorithmic_bytes_per_step(cfg, dtype, n_solid):
     return (N - n_solid) * per_cell + n_solid * 1, per_cell
 
 
+def max_over_ranks(x, world, device="cuda"):
+    """Replicas-only multi-GPU: the job time is the max over ranks (all_reduce MAX; a no-op for one rank)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_mlups(world, units_per_rank, steps, seconds):
+    """Whole-job throughput: every rank processed units_per_rank * steps cell updates in `seconds` (max over ranks)."""
+    return world * units_per_rank * steps / seconds / 1e6
+
+
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
 
@@ -249,13 +265,10 @@ def main():
     clocks = sampler.stop()
     launches = sim.query("launches") - l0
     ms = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, world)
     tot1 = sim.totals()
     finite = bool(np.isfinite(tot1).all())
-    value = world * n_fluid * args.steps / (ms * 1e-3) / 1e6
+    value = job_mlups(world, n_fluid, args.steps, ms * 1e-3)
     step_bytes, per_cell = algorithmic_bytes_per_step(cfg, dtype, n_solid)
     peak, peak_src = measured_peak()
     achieved = step_bytes / (ms * 1e-3 / max(launches, 1)) / 1e9      # GB/s, per launch = per step
@@ -278,14 +291,11 @@ def main():
         sim.moments(h_rho, h_u)                        # D2H: rho, u
         sim.synchronize()
         dt = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = max_over_ranks(dt, world)
         h2d = h_f.numel() * h_f.element_size() + (0 if h_d is None else h_d.numel() * h_d.element_size()) + \
             (0 if h_fl is None else h_fl.numel())
         d2h = 4 * N * h_rho.element_size()
-        e2e = {"value": world * n_fluid * args.steps / dt / 1e6, "unit": UNIT,
+        e2e = {"value": job_mlups(world, n_fluid, args.steps, dt), "unit": UNIT,
                "h2d_bytes_per_step": h2d / args.steps, "d2h_bytes_per_step": d2h / args.steps,
                "what": "lbm_set_fields(host populations, porosity, flags) + lbm_step(K) + lbm_moments(host rho,u), wall clock"}
 

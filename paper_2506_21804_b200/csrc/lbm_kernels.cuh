@@ -150,16 +150,27 @@ __device__ __forceinline__ void collide_cell(T (&f)[Q], T d, T ubx, T uby, T ubz
   const T base = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
   const T keepf = T(1) - omega;
   const T ro = rho * omega;
-  // per weight class (|c|^2 = 1, 2, 3): A = w rho omega base, B = 4.5 w rho omega, C = 3 w rho omega
+  // per weight class (|c|^2 = 1, 2, 3): A = w rho omega base, B = 4.5 w rho omega, C = 3 w rho omega.
+  // Conservation in fp32: the lattice weights are not exactly representable, so sum_i w_i != 1 and
+  // sum_i 3 w_i c_ix^2 != 1 in floating point -- a systematic (not random) drift of mass and momentum of a few
+  // 1e-8 per step.  Two remedies that cost (almost) nothing:
+  //  * the odd-part constants c3[k] = 3 w_k are chosen so that 2 c3[1] + 8 c3[2] (+ 8 c3[3]) == 1 exactly
+  //    (c3[1] takes the remainder), which makes sum_i c_i f^eq_i = rho u^ free of weight rounding;
+  //  * the rest population takes what is left of the mass: f0' = (1-omega) f0 + (rho omega - 2 sum_pairs even),
+  //    so sum_i f_i' = rho up to unbiased rounding of the individual operations.
+  constexpr double c3_2 = static_cast<double>(static_cast<T>(3.0 * static_cast<double>(weight<Q, double>(2))));
+  constexpr double c3_3 = (Q == 27) ? static_cast<double>(static_cast<T>(3.0 * static_cast<double>(weight<Q, double>(3)))) : 0.0;
+  constexpr double c3_1 = (1.0 - 8.0 * c3_2 - 8.0 * c3_3) / 2.0;
+  constexpr T c3[4] = {T(0), static_cast<T>(c3_1), static_cast<T>(c3_2), static_cast<T>(c3_3)};
   T A[4], B[4], C[4];
 #pragma unroll
   for (int k = 1; k <= ((Q == 19) ? 2 : 3); ++k) {
     const T wr = weight<Q, T>(k) * ro;
     A[k] = wr * base;
     B[k] = wr * T(4.5);
-    C[k] = wr * T(3);
+    C[k] = c3[k] * ro;
   }
-  f[0] = keepf * f[0] + (weight<Q, T>(0) * ro) * base;
+  T esum = T(0);
 #pragma unroll
   for (int i = 1; i <= H; ++i) {
     T cu = T(0);
@@ -169,9 +180,11 @@ __device__ __forceinline__ void collide_cell(T (&f)[Q], T d, T ubx, T uby, T ubz
     const int k = L.c2[i];
     const T even = (B[k] * cu) * cu + A[k];
     const T odd = C[k] * cu;
+    esum += even;
     f[i] = keepf * f[i] + (even + odd);
     f[i + H] = keepf * f[i + H] + (even - odd);
   }
+  f[0] = keepf * f[0] + (ro - (esum + esum));
 }
 
 // O4 / reading R6: regularised velocity inlet on a cell of the plane x = 0 (inward normal +x).

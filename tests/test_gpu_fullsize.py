@@ -1,0 +1,167 @@
+"""T1 at BASELINE.json's FULL sizes, in the launch configuration bench.py times (library defaults), and T2 invariants.
+
+The oracle cannot hold these sizes, so parity is checked on light-cone windows (pin P11b, DESIGN.md / SURVEY 8(c)):
+information moves <= 1 cell per step (a wall-model cell reaches 1 more along its normal), so the oracle run on a crop of
+the INPUTS with margin m = 2 s + 2 around a window reproduces the window exactly after s = 10 steps.  Crops that touch
+the inlet / outlet planes or the solid floor / top are flush with them.  >= 8 windows per config.
+"""
+import numpy as np
+import pytest
+import torch
+
+import lbm_inputs as I
+import paper_2506_21804_b200 as P
+from oracle import oracle as O
+from parity_util import NP_DTYPE, TOL, field_error
+
+pytestmark = pytest.mark.gpu
+S = 10
+M = 2 * S + 2
+W = 8
+
+
+def _axis_crop(lo, n, closed):
+    """Index arrays (crop indices, position of the window inside the crop) for a window [lo, lo+W) on an axis of size n.
+    closed: the axis is bounded by special planes (inlet/outlet or solid layers): clip the crop flush instead of wrapping."""
+    a, b = lo - M, lo + W + M
+    if closed:
+        a, b = max(a, 0), min(b, n)
+        idx = np.arange(a, b)
+    else:
+        if b - a >= n:
+            idx = np.arange(n)
+            a = 0
+        else:
+            idx = np.arange(a, b) % n
+    return idx, lo - a
+
+
+def _check_windows(cfg, dtype, windows, closed_axes):
+    nz, ny, nx = cfg["shape"]
+    Q = cfg["Q"]
+    npdt = NP_DTYPE[dtype]
+    # the same populations for both sides: the oracle's equilibrium rounded to the run's dtype
+    f = O.init_equilibrium(Q, cfg["rho"], cfg["u"]).astype(npdt)
+    d = None if cfg["d"] is None else cfg["d"].astype(npdt)
+    par = P.LbmParams(**cfg["params"])
+    with P.LBM(Q, nx, ny, nz, dtype) as sim:
+        sim.set_fields(f, d, cfg["flags"])                  # host pointers, library defaults = bench configuration
+        sim.step(S, par)
+        out = torch.empty((Q, nz, ny, nx), dtype=torch.float32 if dtype == "f32" else torch.float64, device="cuda")
+        sim.get_populations(out)
+        rho = torch.empty((nz, ny, nx), dtype=out.dtype, device="cuda")
+        u = torch.empty((3, nz, ny, nx), dtype=out.dtype, device="cuda")
+        sim.moments(rho, u)
+        sim.synchronize()
+    worst = 0.0
+    for (z0, y0, x0) in windows:
+        iz, wz = _axis_crop(z0, nz, closed_axes[0])
+        iy, wy = _axis_crop(y0, ny, closed_axes[1])
+        ix, wx = _axis_crop(x0, nx, closed_axes[2])
+        sel = np.ix_(iz, iy, ix)
+        fc = np.ascontiguousarray(f[(slice(None),) + sel]).astype(np.float64)
+        dc = None if d is None else np.ascontiguousarray(d[sel]).astype(np.float64)
+        flc = None if cfg["flags"] is None else np.ascontiguousarray(cfg["flags"][sel])
+        ref = O.step(fc, d=dc, flags=flc, nsteps=S, nthreads=min(O.max_threads(), 8), **cfg["params"])
+        inner = (slice(None), slice(wz, wz + W), slice(wy, wy + W), slice(wx, wx + W))
+        refw = ref[inner]
+        gz, gy, gx = iz[wz:wz + W], iy[wy:wy + W], ix[wx:wx + W]
+        gsel = np.ix_(gz, gy, gx)
+        tz, ty, tx = (torch.as_tensor(v, device="cuda") for v in (gz, gy, gx))
+        gotw = out[:, tz][:, :, ty][:, :, :, tx].cpu().numpy().astype(np.float64)
+        mask = None
+        if flc is not None:
+            mask = (cfg["flags"][gsel] & 15) != I.SOLID
+            if not mask.any():
+                continue
+            solid = ~mask
+            assert np.array_equal(gotw[:, solid], f[(slice(None),) + gsel][:, solid].astype(np.float64))
+        err = field_error(gotw, refw, mask)
+        rr, ru = O.moments(ref)
+        rw = rr[inner[1:]]
+        uw = ru[(slice(None),) + inner[1:]]
+        e_rho = field_error(rho[tz][:, ty][:, :, tx].cpu().numpy(), rw, mask)
+        e_u = field_error(u[:, tz][:, :, ty][:, :, :, tx].cpu().numpy(), uw, mask)
+        worst = max(worst, err, e_rho, e_u)
+        assert err <= TOL[dtype], ("populations", (z0, y0, x0), err)
+        assert e_rho <= TOL[dtype], ("rho", (z0, y0, x0), e_rho)
+        assert e_u <= TOL[dtype], ("u", (z0, y0, x0), e_u)
+    return worst
+
+
+def test_config2_full_size_windows():
+    cfg = I.make_config(2)
+    rng = np.random.default_rng(2)
+    wins = [(0, 0, 0), (248, 248, 248), (124, 0, 252)] + [tuple(int(v) for v in rng.integers(0, 248, 3)) for _ in range(5)]
+    _check_windows(cfg, "f32", wins, (False, False, False))
+
+
+def test_config3_full_size_windows():
+    cfg = I.make_config(3)
+    nz, ny, nx = cfg["shape"]
+    d, fl = cfg["d"], cfg["flags"]
+    # floor + inlet, floor + outlet, top, a building, a tree, wall-model floor mid-domain, bulk, y-wrap
+    bz, by, bx = np.argwhere((d == 1.0) & (fl == 0))[len(np.argwhere((d == 1.0) & (fl == 0))) // 2]
+    tz, ty, tx = np.argwhere((d > 0) & (d < 1))[len(np.argwhere((d > 0) & (d < 1))) // 3]
+    wins = [(1, 10, 0), (1, 100, nx - W), (nz - 1 - W, 50, 200), (max(int(bz) - 3, 1), int(by), min(int(bx), nx - W)),
+            (max(int(tz) - 3, 1), int(ty), min(int(tx), nx - W)), (1, 60, 150), (60, 90, 190), (30, ny - 4, 100),
+            (40, 0, 0), (40, 20, nx - W)]
+    _check_windows(cfg, "f32", wins, (True, False, True))
+
+
+def test_config3_full_size_windows_fp64():
+    cfg = I.make_config(3)
+    nz, ny, nx = cfg["shape"]
+    wins = [(1, 10, 0), (1, 100, nx - W), (nz - 1 - W, 50, 200), (1, 60, 150), (60, 90, 190), (30, ny - 4, 100),
+            (20, 40, 120), (5, 130, 250)]
+    _check_windows(cfg, "f64", wins, (True, False, True))
+
+
+def test_config4_full_size_windows():
+    cfg = I.make_config(4)
+    fl = cfg["flags"]
+    rng = np.random.default_rng(4)
+    solid = np.argwhere(fl == I.SOLID)
+    wins = [tuple(int(v) for v in solid[k] - 2) for k in rng.integers(0, len(solid), 5)]      # windows cutting spheres
+    wins = [tuple(min(max(v, 0), 512 - W) for v in w) for w in wins]
+    wins += [(0, 0, 0), (504, 504, 504), (250, 0, 504)]
+    _check_windows(cfg, "f32", wins, (False, False, False))
+
+
+# ---- T2: invariants after the configs' full step counts ------------------------------------------
+def _full_run(number, dtype, shape=None):
+    cfg = I.make_config(number, shape=shape)
+    nz, ny, nx = cfg["shape"]
+    npdt = NP_DTYPE[dtype]
+    par = P.LbmParams(**cfg["params"])
+    with P.LBM(cfg["Q"], nx, ny, nz, dtype) as sim:
+        sim.set_geometry(None if cfg["d"] is None else cfg["d"].astype(npdt), cfg["flags"])
+        sim.init_equilibrium(cfg["rho"].astype(npdt), cfg["u"].astype(npdt))
+        t0 = sim.totals()
+        sim.step(cfg["steps"], par)
+        t1 = sim.totals()
+        u = torch.empty((3, nz, ny, nx), dtype=torch.float32 if dtype == "f32" else torch.float64, device="cuda")
+        sim.moments(None, u)
+        sim.synchronize()
+        umax = float(u.abs().max())
+    return cfg, np.array(t0), np.array(t1), umax
+
+
+def test_config2_full_run_invariants():
+    cfg, t0, t1, umax = _full_run(2, "f32")
+    assert np.isfinite(t1).all()
+    assert abs(t1[0] / t0[0] - 1.0) < 2e-6              # periodic box: mass conserved (unbiased fp32 rounding only)
+    assert np.abs(t1[1:4] - t0[1:4]).max() < 2e-6 * t0[0]
+    assert t1[4] < t0[4] and umax < 0.3                 # energy decays, velocity bounded
+
+
+def test_config3_full_run_invariants():
+    cfg, t0, t1, umax = _full_run(3, "f32")
+    assert np.isfinite(t1).all() and umax < 0.4
+    assert abs(t1[0] / t0[0] - 1.0) < 0.02              # open boundaries: density level may drift (DESIGN.md / SURVEY 7-9)
+
+
+def test_config4_full_run_invariants():
+    cfg, t0, t1, umax = _full_run(4, "f32")
+    assert np.isfinite(t1).all() and umax < 0.4
+    assert abs(t1[0] / t0[0] - 1.0) < 2e-6              # closed (periodic + bounce-back): mass conserved
