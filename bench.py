@@ -35,11 +35,13 @@ WORKLOADS = {
     "config2_les_periodic_256_f32": (2, None, "f32"),
     "config4_d3q27_spheres_512_f32": (4, None, "f32"),
     "config3_urban_channel_384x192x128_f64": (3, None, "f64"),
-    "config5_urban_cube_128_f32": (5, (128, 128, 128), "f32"),
-    "config5_urban_cube_256_f32": (5, (256, 256, 256), "f32"),
-    "config5_urban_cube_512_f32": (5, (512, 512, 512), "f32"),
     "config1_tgv_32_f64": (1, None, "f64"),
 }
+# config 5, the single-GPU capacity sweep: cubes 128^3 .. 896^3 (fp32) and 128^3 .. 640^3 (fp64)
+for _n in (128, 256, 384, 512, 640, 768, 896):
+    WORKLOADS["config5_urban_cube_%d_f32" % _n] = (5, (_n, _n, _n), "f32")
+    if _n <= 640:
+        WORKLOADS["config5_urban_cube_%d_f64" % _n] = (5, (_n, _n, _n), "f64")
 DEFAULT_WORKLOAD = "config3_urban_channel_384x192x128_f32"
 
 
@@ -305,12 +307,12 @@ def main():
         from oracle import oracle as O
         cores = O.max_threads()
         if number == 1:
-            sample_shape, ns = None, 20
+            sample_shape, ns = None, 2000
         else:
             base = np.array(cfg["shape"], dtype=float)
             scale = min(1.0, (1.5e6 / base.prod()) ** (1.0 / 3.0))
             sample_shape = tuple(max(16, int(round(b * scale / 8)) * 8) for b in base)
-            ns = 4
+            ns = 100   # ~1.5e8 cell updates: about 10 s of host work at the oracle's ~15 MLUPs
         v, dt_cpu, shp = cpu_oracle_time(number, sample_shape, ns, cores)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": "fp64 oracle, %d OpenMP threads, workload generator at (nz,ny,nx)=%s, %d steps after 1 warm-up, %.1f s"

@@ -21,10 +21,22 @@
 //                          zero-gradient outlet (G16/R7)
 //   O4 inlet fix-up        l.155 "regularized local velocity boundary condition" (G15/R6)
 //   O6 moments             l.97 "fluid velocity moment u" (G19)
+//   O2h collide, HRR form  (params.collision = 1; the paper's own collision)
+//                          Eq. 6 (l.70) with f~(1) of Eq. 7 (l.74); Eq. 8-9 (l.81-86) regularised
+//                          f(1), third-order coefficient by the recursion the method's name and
+//                          refs [30,31] fix (G29); Eq. 10 (l.90) FD part with the sign and weight of
+//                          reading G10; Eq. 11 (l.94) in full, third-order term = projection on the
+//                          third-order Hermite polynomials the lattice supports (G9); sigma = 0 on
+//                          wall-model cells (l.131); FD velocity = u^ of the same time level (G30-G32)
 //
 // Pins (tests/test_oracle_*.py, all run with -m "not gpu"): P1 isotropy identities, P2
 // equilibrium fixed point, P3 conservation, P4 Cs=0 == separately written BGK, P5 porous
 // decay closed form, P6 tau_eff self-consistency, P7 Taylor-Green decay vs exp(-4 nu k^2 t),
+// HRR pins (tests/test_oracle_hrr.py): H1 Hermite moments of the third-order equilibrium up to order
+// 3, H2 fixed point, H3 conservation, H4 projection idempotence, H5 u = 0 reduction to the pinned
+// BGK collide, H6 FD strain of a sine shear + closed-form post-collision stress at sigma = 0, H7
+// Taylor-Green decay at sigma = 1, 0.5, 0 (fixes sign and factor of Eq. 10), H8 brute force via a
+// numerically inverted Gram matrix, H9 lattice symmetry.
 // P8 Poiseuille profile, P9 Spalding residual + viscous/log limits, P10 inlet moments /
 // idempotence, P11a long-double brute force on 4^3, P12 bounce-back pulse + mass, P13 second
 // order convergence, P14 lattice symmetry, P15 D3Q27.
@@ -117,6 +129,8 @@ struct Params {           // the oracle's own copy of the step parameters (not s
   int wm_enable;
   double wm_kappa;
   double wm_E;
+  int collision;          // 0: BGK form of Eq. 6 (G1); 1: hybrid recursive-regularised (Eq. 6-11)
+  double sigma;           // Eq. 7 hybridisation factor, in [0,1]
 };
 
 inline int cell_type(uint8_t flag) { return flag & 0x0F; }
@@ -163,6 +177,106 @@ void collide_cell(const Lattice& L, const double* fc, double d, const double ub[
     tau = 0.5 * (tau0 + std::sqrt(tau0 * tau0 + 18.0 * std::sqrt(2.0) * cs_smago * cs_smago * nPi / rho));
   }
   for (int i = 0; i < L.Q; ++i) fs[i] = fc[i] - (fc[i] - feq[i]) / tau;  // A6, Eq. 6
+  if (tau_out) *tau_out = tau;
+}
+
+// ---- HRR form: Eq. 6-11 in full -----------------------------------------------------
+// Third-order Hermite polynomial H(3)_abg of direction i:  c_a c_b c_g - c_s^2 (d_ab c_g + d_ag c_b + d_bg c_a).
+inline double herm3(const Lattice& L, int i, int a, int b, int g) {
+  const double ca = L.c[i][a], cb = L.c[i][b], cg = L.c[i][g];
+  return ca * cb * cg - (1.0 / 3.0) * ((a == b ? cg : 0.0) + (a == g ? cb : 0.0) + (b == g ? ca : 0.0));
+}
+
+// Third-order coefficients carried by the lattices: index 0..6 = xxy, xxz, xyy, xzz, yyz, yzz, xyz.
+constexpr int N3 = 7;
+constexpr int IDX3[N3][3] = {{0, 0, 1}, {0, 0, 2}, {0, 1, 1}, {0, 2, 2}, {1, 1, 2}, {1, 2, 2}, {0, 1, 2}};
+
+// The order-3 term of a Hermite series (Eq. 8 / Eq. 11) for direction i, WITHOUT the weight w_i: the
+// orthogonal projection on the third-order polynomials the lattice supports (reading G9).
+//  D3Q27: sum over the six aab-type components of H_aab a_aab / (2 c_s^6)  [1/3! times 3 index
+//         permutations = the printed 1/(2 c_s^6)]  +  H_xyz a_xyz / c_s^6   [6 permutations].
+//  D3Q19: H_xyz vanishes on the stencil and H_xxy, H_yzz (likewise H_xzz, H_xyy and H_yyz, H_xxz) are not
+//         orthogonal; their sum and difference are (squared norms 2 c_s^6 and 6 c_s^6), which gives
+//         [3 (H_xxy+H_yzz)(a_xxy+a_yzz) + (H_xxy-H_yzz)(a_xxy-a_yzz) + ...] / (6 c_s^6)   (refs [30,31]).
+inline double order3_term(const Lattice& L, int i, const double a3[N3]) {
+  double H[N3];
+  for (int k = 0; k < N3; ++k) H[k] = herm3(L, i, IDX3[k][0], IDX3[k][1], IDX3[k][2]);
+  const double cs6 = 1.0 / 27.0;
+  if (L.Q == 27) {
+    double s = 0.0;
+    for (int k = 0; k < 6; ++k) s += H[k] * a3[k];
+    return s / (2.0 * cs6) + H[6] * a3[6] / cs6;
+  }
+  // pairs (xxy, yzz) = (0,5), (xzz, xyy) = (3,2), (yyz, xxz) = (4,1)
+  const int P[3][2] = {{0, 5}, {3, 2}, {4, 1}};
+  double s = 0.0;
+  for (int k = 0; k < 3; ++k) {
+    const int p = P[k][0], q = P[k][1];
+    s += 3.0 * (H[p] + H[q]) * (a3[p] + a3[q]) + (H[p] - H[q]) * (a3[p] - a3[q]);
+  }
+  return s / (6.0 * cs6);
+}
+
+// Eq. 11 (l.94) in full: a^_0^(0) = rho, a^_0^(n) = a^_0^(n-1) u^.
+inline double feq3_i(const Lattice& L, int i, double rho, const double u[3]) {
+  double a3[N3];
+  for (int k = 0; k < N3; ++k) a3[k] = rho * u[IDX3[k][0]] * u[IDX3[k][1]] * u[IDX3[k][2]];
+  return feq_i(L, i, rho, u) + L.w[i] * order3_term(L, i, a3);
+}
+
+// O2h for one cell.  S = S^FD(x,t) (symmetric 3x3), sigma = the cell's hybridisation factor.
+void collide_cell_hrr(const Lattice& L, const double* fc, double d, const double ub[3], double tau0,
+                      double cs_smago, double sigma, const double S[3][3], double* fs, double* tau_out) {
+  double rho, u[3];
+  raw_moments(L, fc, rho, u);                                            // A2
+  double uh[3];
+  for (int a = 0; a < 3; ++a) uh[a] = (1.0 - d) * u[a] + d * ub[a];      // A3, Eq. 12
+  double feq[QMAX], f1[QMAX];
+  for (int i = 0; i < L.Q; ++i) feq[i] = feq3_i(L, i, rho, uh);          // Eq. 11
+  for (int i = 0; i < L.Q; ++i) f1[i] = fc[i] - feq[i];                  // raw non-equilibrium
+  // Eq. 9: a_1^(n) = sum_i H_i^(n) f_i^(1), n = 0, 1, 2
+  double a0 = 0.0, a1[3] = {0, 0, 0}, a2[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}}, Pi[3][3];
+  for (int i = 0; i < L.Q; ++i) {
+    a0 += f1[i];
+    for (int a = 0; a < 3; ++a) {
+      a1[a] += L.c[i][a] * f1[i];
+      for (int b = 0; b < 3; ++b) a2[a][b] += (L.c[i][a] * L.c[i][b] - ((a == b) ? 1.0 / 3.0 : 0.0)) * f1[i];
+    }
+  }
+  double tau = tau0;
+  if (cs_smago > 0.0) {                                                  // A5 as in the BGK form: Pi = sum c c f1
+    for (int a = 0; a < 3; ++a)
+      for (int b = 0; b < 3; ++b) {
+        Pi[a][b] = 0.0;
+        for (int i = 0; i < L.Q; ++i) Pi[a][b] += L.c[i][a] * L.c[i][b] * f1[i];
+      }
+    const double nPi = std::sqrt(Pi[0][0] * Pi[0][0] + Pi[1][1] * Pi[1][1] + Pi[2][2] * Pi[2][2] +
+                                 2.0 * (Pi[0][1] * Pi[0][1] + Pi[0][2] * Pi[0][2] + Pi[1][2] * Pi[1][2]));
+    tau = 0.5 * (tau0 + std::sqrt(tau0 * tau0 + 18.0 * std::sqrt(2.0) * cs_smago * cs_smago * nPi / rho));
+  }
+  // recursion for the third-order coefficient (G29): a_1,abg = u^_a a_1,bg + u^_b a_1,ag + u^_g a_1,ab
+  double a3[N3];
+  for (int k = 0; k < N3; ++k) {
+    const int a = IDX3[k][0], b = IDX3[k][1], g = IDX3[k][2];
+    a3[k] = uh[a] * a2[b][g] + uh[b] * a2[a][g] + uh[g] * a2[a][b];
+  }
+  for (int i = 0; i < L.Q; ++i) {
+    // Eq. 8: f(1)_i = w_i sum_n H^(n) : a_1^(n) / (c_s^2n n!)
+    double h1 = 0.0, h2 = 0.0, hS = 0.0;
+    for (int a = 0; a < 3; ++a) {
+      h1 += L.c[i][a] * a1[a];
+      for (int b = 0; b < 3; ++b) {
+        const double H2 = L.c[i][a] * L.c[i][b] - ((a == b) ? 1.0 / 3.0 : 0.0);
+        h2 += H2 * a2[a][b];
+        hS += H2 * S[a][b];
+      }
+    }
+    const double freg = L.w[i] * (a0 + 3.0 * h1 + 4.5 * h2 + order3_term(L, i, a3));
+    // Eq. 10 with the sign and the weight of reading G10: -w_i rho tau / c_s^2  H(2) : S^FD  (tau = tau_eff, G31)
+    const double ffd = -L.w[i] * rho * tau * 3.0 * hS;
+    const double ft = sigma * freg + (1.0 - sigma) * ffd;                // Eq. 7 (G10)
+    fs[i] = feq[i] + (1.0 - 1.0 / tau) * ft;                             // Eq. 6
+  }
   if (tau_out) *tau_out = tau;
 }
 
@@ -282,6 +396,26 @@ int orc_collide_cell(int Q, const double* fc, double d, const double* ub, double
   return 0;
 }
 
+// Eq. 11 in full (third-order equilibrium)
+int orc_feq3(int Q, double rho, const double* u, double* out) {
+  Lattice L;
+  if (!make_lattice(Q, L)) return -1;
+  for (int i = 0; i < Q; ++i) out[i] = feq3_i(L, i, rho, u);
+  return 0;
+}
+
+// O2h on one cell; S = S^FD row-major [9]
+int orc_collide_cell_hrr(int Q, const double* fc, double d, const double* ub, double tau0, double cs_smago,
+                         double sigma, const double* S, double* fs, double* tau_out) {
+  Lattice L;
+  if (!make_lattice(Q, L)) return -1;
+  double S33[3][3];
+  for (int a = 0; a < 3; ++a)
+    for (int b = 0; b < 3; ++b) S33[a][b] = S[3 * a + b];
+  collide_cell_hrr(L, fc, d, ub, tau0, cs_smago, sigma, S33, fs, tau_out);
+  return 0;
+}
+
 int orc_inlet_fixup_cell(int Q, double* g, const double* uw) {
   Lattice L;
   if (!make_lattice(Q, L)) return -1;
@@ -313,7 +447,7 @@ int orc_init_equilibrium(int Q, int64_t N, const double* rho, const double* u, d
 // nthreads <= 1: serial.  nthreads > 1: the same loop nests with "omp parallel for" over z.
 // Returns 0, or -1 on bad arguments.
 int orc_step(int Q, int nx, int ny, int nz, double* f, const double* d, const uint8_t* flags,
-             const double* par /* tau0, cs, use_hlbm, uin0, uin1, uin2, wm_enable, kappa, E */,
+             const double* par /* tau0, cs, use_hlbm, uin0, uin1, uin2, wm_enable, kappa, E, collision, sigma */,
              int nsteps, int nthreads) {
   Lattice L;
   if (!make_lattice(Q, L)) return -1;
@@ -322,7 +456,10 @@ int orc_step(int Q, int nx, int ny, int nz, double* f, const double* d, const ui
   p.tau0 = par[0];  p.cs_smago = par[1];  p.use_hlbm = (par[2] != 0.0);
   p.u_in[0] = par[3];  p.u_in[1] = par[4];  p.u_in[2] = par[5];
   p.wm_enable = (par[6] != 0.0);  p.wm_kappa = par[7];  p.wm_E = par[8];
+  p.collision = static_cast<int>(par[9]);  p.sigma = par[10];
   if (!(p.tau0 > 0.5) || p.cs_smago < 0.0) return -1;
+  if (p.collision != 0 && p.collision != 1) return -1;
+  if (p.collision == 1 && !(p.sigma >= 0.0 && p.sigma <= 1.0)) return -1;
 #ifdef _OPENMP
   const int nth = (nthreads > 1) ? nthreads : 1;
 #else
@@ -343,6 +480,8 @@ int orc_step(int Q, int nx, int ny, int nz, double* f, const double* d, const ui
     }
   }
   std::vector<double> uB(3 * wm_cells.size(), 0.0);
+  std::vector<double> uhat;                                // u^(x,t), [3][N], HRR form only
+  if (p.collision == 1) uhat.assign(3 * static_cast<size_t>(N), 0.0);
   double* cur = f;
   double* nxt = g.data();
 
@@ -372,6 +511,29 @@ int orc_step(int Q, int nx, int ny, int nz, double* f, const double* d, const ui
       for (int a = 0; a < 3; ++a) ub[a] = (U1 / U2) * ut[a];               // step 7
     }
 
+    // ---- O1b (HRR form): u^(x,t) of every cell, the field the FD strain is taken of (G30) ------
+    // SOLID cells: u^ = 0 (a resting wall).
+    if (p.collision == 1) {
+#pragma omp parallel for num_threads(nth) if (nth > 1)
+      for (int64_t x = 0; x < N; ++x) {
+        const int type = flags ? cell_type(flags[x]) : FLUID;
+        double uh[3] = {0.0, 0.0, 0.0};
+        if (type != SOLID) {
+          double fc[QMAX], rho, u[3];
+          for (int i = 0; i < Q; ++i) fc[i] = cur[i * N + x];
+          raw_moments(L, fc, rho, u);
+          const double dd = (p.use_hlbm && d) ? d[x] : 0.0;
+          double ub[3] = {0.0, 0.0, 0.0};
+          if (type == WALLMODEL && p.wm_enable && !wm_slot.empty()) {
+            const int32_t k = wm_slot[x];
+            ub[0] = uB[3 * k];  ub[1] = uB[3 * k + 1];  ub[2] = uB[3 * k + 2];
+          }
+          for (int a = 0; a < 3; ++a) uh[a] = (1.0 - dd) * u[a] + dd * ub[a];
+        }
+        for (int a = 0; a < 3; ++a) uhat[a * N + x] = uh[a];
+      }
+    }
+
     // ---- O2: collide ------------------------------------------------------------------------
 #pragma omp parallel for num_threads(nth) if (nth > 1)
     for (int z = 0; z < nz; ++z)
@@ -391,7 +553,29 @@ int orc_step(int Q, int nx, int ny, int nz, double* f, const double* d, const ui
             const int32_t k = wm_slot[x];
             ub[0] = uB[3 * k];  ub[1] = uB[3 * k + 1];  ub[2] = uB[3 * k + 2];
           }
-          collide_cell(L, fc, dd, ub, p.tau0, p.cs_smago, fs, nullptr);
+          if (p.collision == 1) {
+            // S^FD_ab = (D_a u^_b + D_b u^_a) / 2, D_a g = (g(x+e_a) - g(x-e_a)) / 2; periodic wrap, except
+            // that the ghost planes beyond the INLET / OUTLET planes copy those planes (G32)
+            const int pos[3] = {xx, y, z}, dim[3] = {nx, ny, nz};
+            double D[3][3];   // D[a][b] = D_a u^_b
+            for (int a = 0; a < 3; ++a) {
+              int qp[3] = {xx, y, z}, qm[3] = {xx, y, z};
+              qp[a] = wrap(pos[a] + 1, dim[a]);
+              qm[a] = wrap(pos[a] - 1, dim[a]);
+              if (a == 0 && type == OUTLET) qp[0] = xx;
+              if (a == 0 && type == INLET) qm[0] = xx;
+              const int64_t sp = (static_cast<int64_t>(qp[2]) * ny + qp[1]) * nx + qp[0];
+              const int64_t sm = (static_cast<int64_t>(qm[2]) * ny + qm[1]) * nx + qm[0];
+              for (int b = 0; b < 3; ++b) D[a][b] = 0.5 * (uhat[b * N + sp] - uhat[b * N + sm]);
+            }
+            double S[3][3];
+            for (int a = 0; a < 3; ++a)
+              for (int b = 0; b < 3; ++b) S[a][b] = 0.5 * (D[a][b] + D[b][a]);
+            const double sig = (type == WALLMODEL && p.wm_enable) ? 0.0 : p.sigma;   // l.131
+            collide_cell_hrr(L, fc, dd, ub, p.tau0, p.cs_smago, sig, S, fs, nullptr);
+          } else {
+            collide_cell(L, fc, dd, ub, p.tau0, p.cs_smago, fs, nullptr);
+          }
           for (int i = 0; i < Q; ++i) fstar[i * N + x] = fs[i];
         }
 
