@@ -43,6 +43,9 @@ def lib():
         L.orc_collide_cell.argtypes = [ctypes.c_int, _c_dp, ctypes.c_double, _c_dp, ctypes.c_double,
                                        ctypes.c_double, _c_dp, _c_dp]
         L.orc_inlet_fixup_cell.argtypes = [ctypes.c_int, _c_dp, _c_dp]
+        L.orc_feq3.argtypes = [ctypes.c_int, ctypes.c_double, _c_dp, _c_dp]
+        L.orc_collide_cell_hrr.argtypes = [ctypes.c_int, _c_dp, ctypes.c_double, _c_dp, ctypes.c_double,
+                                           ctypes.c_double, ctypes.c_double, _c_dp, _c_dp, _c_dp]
         L.orc_spalding.argtypes = [ctypes.c_double] * 3
         L.orc_spalding.restype = ctypes.c_double
         L.orc_wallmodel_speed.argtypes = [ctypes.c_double] * 6 + [_c_dp, _c_ip, _c_ip]
@@ -93,6 +96,26 @@ def collide_cell(Q, fc, d=0.0, ub=(0.0, 0.0, 0.0), tau0=0.6, cs_smago=0.0):
     return fs, tau.value
 
 
+def feq3(Q, rho, u):
+    """Eq. 11 in full (third-order equilibrium)."""
+    out = np.zeros(Q)
+    u = _f64(u)
+    assert lib().orc_feq3(Q, float(rho), _dp(u), _dp(out)) == 0
+    return out
+
+
+def collide_cell_hrr(Q, fc, d=0.0, ub=(0.0, 0.0, 0.0), tau0=0.6, cs_smago=0.0, sigma=1.0, S=None):
+    """O2h on one cell (S = S^FD, 3x3) -> (fstar[Q], tau_eff)."""
+    fc = _f64(fc)
+    ub = _f64(ub)
+    S = _f64(np.zeros((3, 3)) if S is None else S)
+    fs = np.zeros(Q)
+    tau = ctypes.c_double(0.0)
+    assert lib().orc_collide_cell_hrr(Q, _dp(fc), float(d), _dp(ub), float(tau0), float(cs_smago), float(sigma),
+                                      _dp(S), _dp(fs), ctypes.byref(tau)) == 0
+    return fs, tau.value
+
+
 def inlet_fixup_cell(Q, g, uw):
     g = _f64(g).copy()
     uw = _f64(uw)
@@ -123,9 +146,11 @@ def init_equilibrium(Q, rho, u):
     return f
 
 
-def pack_params(tau0, cs_smago=0.0, use_hlbm=0, u_in=(0.0, 0.0, 0.0), wm_enable=0, wm_kappa=0.41, wm_E=9.8):
+def pack_params(tau0, cs_smago=0.0, use_hlbm=0, u_in=(0.0, 0.0, 0.0), wm_enable=0, wm_kappa=0.41, wm_E=9.8,
+                collision=0, sigma=1.0):
+    """collision: 0 = BGK form (G1), 1 = HRR (Eq. 6-11); sigma = Eq. 7 hybridisation factor."""
     return np.array([tau0, cs_smago, float(use_hlbm), u_in[0], u_in[1], u_in[2], float(wm_enable),
-                     wm_kappa, wm_E], dtype=np.float64)
+                     wm_kappa, wm_E, float(collision), sigma], dtype=np.float64)
 
 
 def step(f, d=None, flags=None, nsteps=1, nthreads=1, **params):
