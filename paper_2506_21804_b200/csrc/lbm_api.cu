@@ -34,6 +34,10 @@ struct lbm_ctx {
   uint8_t* cls;          // class byte per cell (see lbm_kernels.cuh)
   uint8_t* cls_alt;      // classification target before it is accepted
   uint8_t* flags_raw;    // device copy of the caller's flag bytes; afterwards the list marks
+  uint32_t* nbmask;      // per cell: which lattice neighbours are SOLID (ghost-slot bounce-back)
+  int* solid_list;       // SOLID cells, ascending
+  void* solid_vals;      // their own populations [Q][n_solid] (their lattice storage doubles as ghost slots)
+  long long n_solid_list;
   int* list;             // cells of the non-bulk vectors (vector kernel), ascending
   long long n_list;
   void* cub_tmp;
@@ -128,6 +132,7 @@ lbm::StepArgs<T> make_args(const lbm_ctx* c, const lbm_params* p, int in, int ou
   a.fout = static_cast<T*>(c->f[out]);
   a.d = (p && p->use_hlbm && c->has_d) ? static_cast<const T*>(c->d) : nullptr;
   a.cls = c->cls;
+  a.nbmask = c->nbmask;
   a.nx = c->nx;  a.ny = c->ny;  a.nz = c->nz;
   a.N = c->N;
   a.list = c->list;
@@ -149,9 +154,9 @@ lbm::StepArgs<T> make_args(const lbm_ctx* c, const lbm_params* p, int in, int ou
 }
 
 // vector kernel: thread <-> V consecutive cells; block (bx quads, by rows)
-template <typename T>
+template <int Q, typename T>
 void launch_dims_vec(const lbm_ctx* c, dim3& grid, dim3& block) {
-  const int V = lbm::VecOf<T>::V;
+  const int V = lbm::VecOf<Q, T>::V;
   const int nvec = c->nx / V;
   int bx = 1;
   while (bx < nvec && bx < 32) bx <<= 1;
@@ -169,9 +174,9 @@ int launch_step_t(lbm_ctx* c, const lbm_params* p, int mode) {
   dim3 grid, block;
   const int in = c->cur, out = 1 - c->cur;
   lbm::StepArgs<T> a = make_args<T>(c, p, in, out);
-  const bool vec = c->use_vector && (c->nx % (2 * lbm::VecOf<T>::V) == 0);   // whole 32-byte sectors per row
+  const bool vec = c->use_vector && (c->nx % (32 / static_cast<int>(sizeof(T))) == 0);   // whole 32-byte sectors per row
   if (vec) {
-    launch_dims_vec<T>(c, grid, block);
+    launch_dims_vec<Q, T>(c, grid, block);
     const long long per_slice = static_cast<long long>(grid.x) * grid.y * block.x * block.y;
     a.list_z = static_cast<int>((c->n_list + per_slice - 1) / per_slice);
     grid.z += a.list_z;
@@ -204,10 +209,7 @@ int launch_moments_t(lbm_ctx* c, const lbm_params* p, void* rho, void* u) {
   dim3 grid, block;
   launch_dims(c, grid, block);
   lbm::StepArgs<T> a = make_args<T>(c, p, c->cur, 1 - c->cur);
-  if (c->phase == PHASE_POST)
-    lbm::k_moments<Q, T, true><<<grid, block, 0, c->stream>>>(a, static_cast<T*>(rho), static_cast<T*>(u));
-  else
-    lbm::k_moments<Q, T, false><<<grid, block, 0, c->stream>>>(a, static_cast<T*>(rho), static_cast<T*>(u));
+  lbm::k_moments<Q, T><<<grid, block, 0, c->stream>>>(a, static_cast<T*>(rho), static_cast<T*>(u));
   LBM_CUDA(c, cudaGetLastError());
   c->launches++;
   return LBM_OK;
@@ -218,10 +220,7 @@ int launch_totals_t(lbm_ctx* c, const lbm_params* p) {
   dim3 grid, block;
   launch_dims(c, grid, block);
   lbm::StepArgs<T> a = make_args<T>(c, p, c->cur, 1 - c->cur);
-  if (c->phase == PHASE_POST)
-    lbm::k_totals<Q, T, true><<<grid, block, 0, c->stream>>>(a, c->totals_dev);
-  else
-    lbm::k_totals<Q, T, false><<<grid, block, 0, c->stream>>>(a, c->totals_dev);
+  lbm::k_totals<Q, T><<<grid, block, 0, c->stream>>>(a, c->totals_dev);
   LBM_CUDA(c, cudaGetLastError());
   c->launches++;
   return LBM_OK;
@@ -232,7 +231,7 @@ int launch_init_t(lbm_ctx* c, const void* rho, const void* u) {
   const int threads = 256;
   const long long blocks = (c->N + threads - 1) / threads;
   lbm::k_init_equilibrium<Q, T><<<static_cast<unsigned>(blocks), threads, 0, c->stream>>>(
-      static_cast<const T*>(rho), static_cast<const T*>(u), static_cast<T*>(c->f[0]), static_cast<T*>(c->f[1]), c->N);
+      static_cast<const T*>(rho), static_cast<const T*>(u), static_cast<T*>(c->f[0]), c->N);
   LBM_CUDA(c, cudaGetLastError());
   c->launches++;
   return LBM_OK;
@@ -258,6 +257,48 @@ int check_params(lbm_ctx* c, const lbm_params* p) {
   if (p->wm_enable && (!(p->wm_kappa > 0.0) || !(p->wm_E > 0.0)))
     return fail(c, LBM_EINVAL, "lbm_step: wm_enable needs wm_kappa > 0 and wm_E > 0");
   if (!(p->u_in[0] < 1.0)) return fail(c, LBM_EINVAL, "lbm_step: u_in[0] = %g must be < 1", p->u_in[0]);
+  return LBM_OK;
+}
+
+// stream compaction of the cell indices n with flags_raw[n] != 0 (count known) into a new device array
+int compact_marks(lbm_ctx* c, long long count, int** out) {
+  *out = nullptr;
+  if (count <= 0) return LBM_OK;
+  int* arr = nullptr;
+  int rc = dev_alloc(c, reinterpret_cast<void**>(&arr), static_cast<size_t>(count) * sizeof(int));
+  if (rc != LBM_OK) return rc;
+  cub::CountingInputIterator<int> it(0);
+  size_t need = 0;
+  LBM_CUDA(c, cub::DeviceSelect::Flagged(nullptr, need, it, c->flags_raw, arr, c->list_count_dev, static_cast<int>(c->N), c->stream));
+  if (need > c->cub_tmp_bytes) {
+    if (c->cub_tmp) { cudaFree(c->cub_tmp); c->device_bytes -= c->cub_tmp_bytes; c->cub_tmp = nullptr; c->cub_tmp_bytes = 0; }
+    rc = dev_alloc(c, &c->cub_tmp, need);
+    if (rc != LBM_OK) { cudaFree(arr); return rc; }
+    c->cub_tmp_bytes = need;
+  }
+  LBM_CUDA(c, cub::DeviceSelect::Flagged(c->cub_tmp, need, it, c->flags_raw, arr, c->list_count_dev, static_cast<int>(c->N), c->stream));
+  LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  *out = arr;
+  return LBM_OK;
+}
+
+// SOLID cells' own values: lattice c->cur -> side buffer (save) or back (restore)
+int solid_values(lbm_ctx* c, bool save) {
+  if (c->n_solid_list <= 0) return LBM_OK;
+  const unsigned blocks = static_cast<unsigned>((c->n_solid_list + 255) / 256);
+  if (c->dtype == LBM_F32) {
+    float* f = static_cast<float*>(c->f[c->cur]);
+    float* sv = static_cast<float*>(c->solid_vals);
+    if (save) lbm::k_solid_values<float, true><<<blocks, 256, 0, c->stream>>>(f, sv, c->solid_list, c->n_solid_list, c->N, c->Q);
+    else      lbm::k_solid_values<float, false><<<blocks, 256, 0, c->stream>>>(f, sv, c->solid_list, c->n_solid_list, c->N, c->Q);
+  } else {
+    double* f = static_cast<double*>(c->f[c->cur]);
+    double* sv = static_cast<double*>(c->solid_vals);
+    if (save) lbm::k_solid_values<double, true><<<blocks, 256, 0, c->stream>>>(f, sv, c->solid_list, c->n_solid_list, c->N, c->Q);
+    else      lbm::k_solid_values<double, false><<<blocks, 256, 0, c->stream>>>(f, sv, c->solid_list, c->n_solid_list, c->N, c->Q);
+  }
+  LBM_CUDA(c, cudaGetLastError());
+  c->launches++;
   return LBM_OK;
 }
 
@@ -294,28 +335,39 @@ int classify(lbm_ctx* c, const uint8_t* cell_flags) {
     LBM_CUDA(c, cudaStreamSynchronize(c->stream));
     n_list = static_cast<long long>(h[3]);
     int* new_list = nullptr;
-    if (n_list > 0) {
-      int rc = dev_alloc(c, reinterpret_cast<void**>(&new_list), static_cast<size_t>(n_list) * sizeof(int));
-      if (rc != LBM_OK) return rc;
-      cub::CountingInputIterator<int> it(0);
-      size_t need = 0;
-      LBM_CUDA(c, cub::DeviceSelect::Flagged(nullptr, need, it, c->flags_raw, new_list, c->list_count_dev,
-                                             static_cast<int>(c->N), c->stream));
-      if (need > c->cub_tmp_bytes) {
-        if (c->cub_tmp) { cudaFree(c->cub_tmp); c->device_bytes -= c->cub_tmp_bytes; c->cub_tmp = nullptr; c->cub_tmp_bytes = 0; }
-        rc = dev_alloc(c, &c->cub_tmp, need);
-        if (rc != LBM_OK) { cudaFree(new_list); return rc; }
-        c->cub_tmp_bytes = need;
-      }
-      LBM_CUDA(c, cub::DeviceSelect::Flagged(c->cub_tmp, need, it, c->flags_raw, new_list, c->list_count_dev,
-                                             static_cast<int>(c->N), c->stream));
-      LBM_CUDA(c, cudaStreamSynchronize(c->stream));
-    }
+    int rc = compact_marks(c, n_list, &new_list);
+    if (rc != LBM_OK) return rc;
     if (c->list) { cudaFree(c->list); c->device_bytes -= static_cast<size_t>(c->n_list) * sizeof(int); }
     c->list = new_list;
   }
+  // SOLID cells: list + side buffer for their own values
+  {
+    const long long n_solid = static_cast<long long>(h[1]);
+    const unsigned blocks = static_cast<unsigned>((c->N + 255) / 256);
+    lbm::k_mark_solid<<<blocks, 256, 0, c->stream>>>(c->cls_alt, c->flags_raw, c->N);
+    LBM_CUDA(c, cudaGetLastError());
+    c->launches++;
+    int* new_list = nullptr;
+    int rc = compact_marks(c, n_solid, &new_list);
+    if (rc != LBM_OK) return rc;
+    void* new_vals = nullptr;
+    const size_t vbytes = static_cast<size_t>(n_solid) * c->Q * c->dtype;
+    if (n_solid > 0) {
+      rc = dev_alloc(c, &new_vals, vbytes);
+      if (rc != LBM_OK) { cudaFree(new_list); return rc; }
+    }
+    if (c->solid_list) { cudaFree(c->solid_list); c->device_bytes -= static_cast<size_t>(c->n_solid_list) * sizeof(int); }
+    if (c->solid_vals) { cudaFree(c->solid_vals); c->device_bytes -= static_cast<size_t>(c->n_solid_list) * c->Q * c->dtype; }
+    c->solid_list = new_list;
+    c->solid_vals = new_vals;
+    c->n_solid_list = n_solid;
+  }
   c->n_list = n_list;
   uint8_t* t = c->cls;  c->cls = c->cls_alt;  c->cls_alt = t;
+  if (c->Q == 19) lbm::k_nbmask<19><<<grid, block, 0, c->stream>>>(c->cls, c->nbmask, c->nx, c->ny, c->nz);
+  else            lbm::k_nbmask<27><<<grid, block, 0, c->stream>>>(c->cls, c->nbmask, c->nx, c->ny, c->nz);
+  LBM_CUDA(c, cudaGetLastError());
+  c->launches++;
   c->n_solid = static_cast<long long>(h[1]);
   c->n_masked = static_cast<long long>(h[2]);
   return LBM_OK;
@@ -356,10 +408,12 @@ lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype) {
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->cls), N);
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->cls_alt), N);
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->flags_raw), N);
+  if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->nbmask), static_cast<size_t>(N) * sizeof(uint32_t));
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->counters), 4 * sizeof(unsigned long long));
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->totals_dev), 5 * sizeof(double));
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->list_count_dev), sizeof(int));
   if (rc == LBM_OK && cudaMemset(c->cls, 0, N) != cudaSuccess) rc = fail(c, LBM_ECUDA, "cudaMemset failed");
+  if (rc == LBM_OK && cudaMemset(c->nbmask, 0, static_cast<size_t>(N) * sizeof(uint32_t)) != cudaSuccess) rc = fail(c, LBM_ECUDA, "cudaMemset failed");
   if (rc != LBM_OK) {
     std::snprintf(g_create_error, sizeof(g_create_error), "lbm_create: %.480s", c->err);
     lbm_destroy(c);
@@ -375,6 +429,7 @@ void lbm_destroy(lbm_ctx* c) {
   cudaFree(c->cls);  cudaFree(c->cls_alt);  cudaFree(c->flags_raw);
   cudaFree(c->counters);  cudaFree(c->totals_dev);  cudaFree(c->staging);
   cudaFree(c->list);  cudaFree(c->cub_tmp);  cudaFree(c->list_count_dev);
+  cudaFree(c->nbmask);  cudaFree(c->solid_list);  cudaFree(c->solid_vals);
   cudaGetLastError();
   delete c;
 }
@@ -412,13 +467,11 @@ int lbm_set_fields(lbm_ctx* c, const void* populations, const void* porosity, co
   if (rc != LBM_OK) return rc;
   const size_t pop = static_cast<size_t>(c->Q) * c->N * c->dtype;
   LBM_CUDA(c, cudaMemcpyAsync(c->f[0], populations, pop, cudaMemcpyDefault, c->stream));
-  // SOLID cells are never written by the step kernel: both lattices must hold their values
-  LBM_CUDA(c, cudaMemcpyAsync(c->f[1], c->f[0], pop, cudaMemcpyDeviceToDevice, c->stream));
   if (!is_device_pointer(populations)) LBM_CUDA(c, cudaStreamSynchronize(c->stream));
   c->cur = 0;
   c->phase = PHASE_PRE;
   c->steps = 0;
-  return LBM_OK;
+  return solid_values(c, true);      // SOLID cells' own values -> side buffer (their storage becomes ghost slots)
 }
 
 int lbm_init_equilibrium(lbm_ctx* c, const void* rho, const void* u) {
@@ -441,7 +494,7 @@ int lbm_init_equilibrium(lbm_ctx* c, const void* rho, const void* u) {
   c->cur = 0;
   c->phase = PHASE_PRE;
   c->steps = 0;
-  return LBM_OK;
+  return solid_values(c, true);
 }
 
 // POST -> PRE: write S_t = stream(F_{t-1}) into the other lattice and make it current
@@ -451,7 +504,7 @@ static int materialise(lbm_ctx* c) {
   int rc = launch_step(c, &p, lbm::MODE_STREAM);
   if (rc != LBM_OK) return rc;
   c->phase = PHASE_PRE;
-  return LBM_OK;
+  return solid_values(c, false);     // the stream pass does not write SOLID cells: put their own values back
 }
 
 int lbm_set_geometry(lbm_ctx* c, const void* porosity, const uint8_t* cell_flags) {
@@ -461,10 +514,7 @@ int lbm_set_geometry(lbm_ctx* c, const void* porosity, const uint8_t* cell_flags
   if (rc != LBM_OK) return rc;
   rc = set_geometry_fields(c, porosity, cell_flags);
   if (rc != LBM_OK) return rc;
-  if (c->phase == PHASE_PRE) {
-    const size_t pop = static_cast<size_t>(c->Q) * c->N * c->dtype;
-    LBM_CUDA(c, cudaMemcpyAsync(c->f[1 - c->cur], c->f[c->cur], pop, cudaMemcpyDeviceToDevice, c->stream));
-  }
+  if (c->phase == PHASE_PRE) return solid_values(c, true);   // the SOLID set changed: save the new set's values
   return LBM_OK;
 }
 
@@ -504,7 +554,9 @@ int lbm_moments(lbm_ctx* c, void* rho, void* u) {
     if (hu) du = s + cell_bytes;
   }
   lbm_params p = c->last;
-  int rc = LBM_DISPATCH(c, launch_moments_t, c, &p, drho, du);
+  int rc = materialise(c);           // S_t in the cell's own storage (one extra pass when the storage held F_{t-1})
+  if (rc != LBM_OK) return rc;
+  rc = LBM_DISPATCH(c, launch_moments_t, c, &p, drho, du);
   if (rc != LBM_OK) return rc;
   if (hr) LBM_CUDA(c, cudaMemcpyAsync(rho, drho, cell_bytes, cudaMemcpyDefault, c->stream));
   if (hu) LBM_CUDA(c, cudaMemcpyAsync(u, du, 3 * cell_bytes, cudaMemcpyDefault, c->stream));
@@ -530,7 +582,9 @@ int lbm_totals(lbm_ctx* c, double out[5]) {
   if (c->phase == PHASE_NONE) return fail(c, LBM_ESTATE, "lbm_totals: no state");
   LBM_CUDA(c, cudaMemsetAsync(c->totals_dev, 0, 5 * sizeof(double), c->stream));
   lbm_params p = c->last;
-  int rc = LBM_DISPATCH(c, launch_totals_t, c, &p);
+  int rc = materialise(c);
+  if (rc != LBM_OK) return rc;
+  rc = LBM_DISPATCH(c, launch_totals_t, c, &p);
   if (rc != LBM_OK) return rc;
   LBM_CUDA(c, cudaMemcpyAsync(out, c->totals_dev, 5 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
   LBM_CUDA(c, cudaStreamSynchronize(c->stream));

@@ -18,11 +18,19 @@
 namespace lbm {
 
 enum : int { T_FLUID = 0, T_SOLID = 1, T_INLET = 2, T_OUTLET = 3, T_WM = 4 };
-// internal class byte: bits 0-2 type, bits 3-5 wall-normal code, bit 7 = MASKED: the cell is SOLID or
-// WALLMODEL or has a SOLID lattice neighbour (it needs the per-cell boundary path).  INLET / OUTLET cells
-// without a SOLID neighbour are not MASKED: the vector kernel handles them in line.
+// internal class byte: bits 0-2 type, bits 3-5 wall-normal code,
+//   bit 6 = ADJ:     the (non-SOLID) cell has at least one SOLID lattice neighbour: it writes ghost slots (below);
+//   bit 7 = SPECIAL: the cell needs the per-cell path (list blocks): WALLMODEL cells (A8) and OUTLET cells with a
+//                    SOLID neighbour (their clamped pull does not fit the ghost-slot rule).
+// Halfway bounce-back through GHOST SLOTS (A7, reading R5): a non-SOLID cell x whose neighbour s = x + c_j is SOLID
+// stores its post-collision F_j(x) a second time into the slot (opp(j), s) of the SOLID cell.  The next step's pull
+// of direction opp(j) at x reads exactly that slot: g_opp(j)(x) = A[opp(j)][x - c_opp(j)] = A[opp(j)][s] = F_j(x).
+// The pull therefore never tests a flag.  Slot (i, s) has the single writer s + c_i, so there is no race; SOLID
+// cells' own values are kept in a side buffer by the host side (they are inert, R5) and patched back whenever the
+// state is materialised.
 constexpr uint8_t CLS_TYPE = 0x07;
-constexpr uint8_t CLS_MASKED = 0x80;
+constexpr uint8_t CLS_ADJ = 0x40;
+constexpr uint8_t CLS_SPECIAL = 0x80;
 constexpr int CLS_NORMAL_SHIFT = 3;
 
 // kernel modes
@@ -68,6 +76,7 @@ struct StepArgs {
   T* __restrict__ fout;           // [Q][N]
   const T* __restrict__ d;        // [N] or nullptr (=> d = 0)
   const uint8_t* __restrict__ cls;  // [N]
+  const uint32_t* __restrict__ nbmask;  // [N] bit j: neighbour x + c_j is SOLID (non-zero only on ADJ cells)
   int nx, ny, nz;
   long long N;                    // cells = population stride
   T tau0;
@@ -288,34 +297,18 @@ __device__ __forceinline__ long long cell_index(int x, int y, int z, int nx, int
   return (static_cast<long long>(z) * ny + y) * nx + x;
 }
 
-// Fast pull: every neighbour is a regular cell (no SOLID neighbour, cell is plain FLUID).
+// Pull of one cell (A1 + the pull half of A7): g_i(x) = A[i][x - c_i], periodic wrap; SOLID neighbours need no
+// test because their ghost slots hold the bounced-back value.  OUTLET cells clamp the source of the c_x < 0
+// populations to their own plane (R7: ghost plane nx := plane nx-1); if that clamped source is SOLID the ghost
+// slot belongs to another cell, so the bounce-back is taken explicitly from the cell's own opposite population.
+// INLET cells get the fix-up R6.  `type` is the cell's own type (not SOLID).
 template <int Q, typename T>
-__device__ __forceinline__ void pull_bulk(const T* __restrict__ fin, long long N, int x, int y, int z, int nx, int ny,
-                                          int nz, T (&f)[Q]) {
-  constexpr Stencil<Q> L{};
-  const int xm = (x == 0) ? nx - 1 : x - 1, xp = (x == nx - 1) ? 0 : x + 1;
-  const int ym = (y == 0) ? ny - 1 : y - 1, yp = (y == ny - 1) ? 0 : y + 1;
-  const int zm = (z == 0) ? nz - 1 : z - 1, zp = (z == nz - 1) ? 0 : z + 1;
-#pragma unroll
-  for (int i = 0; i < Q; ++i) {
-    // source = x - c_i
-    const int sx = (L.c[i][0] == 0) ? x : ((L.c[i][0] == 1) ? xm : xp);
-    const int sy = (L.c[i][1] == 0) ? y : ((L.c[i][1] == 1) ? ym : yp);
-    const int sz = (L.c[i][2] == 0) ? z : ((L.c[i][2] == 1) ? zm : zp);
-    f[i] = __ldg(fin + i * N + cell_index(sx, sy, sz, nx, ny));
-  }
-}
-
-// Masked pull (A7): halfway bounce-back at SOLID neighbours, zero-gradient outlet clamp, then the
-// inlet fix-up if the cell is an INLET cell.  `type` is the cell's own type (not SOLID).
-template <int Q, typename T>
-__device__ __forceinline__ void pull_masked(const StepArgs<T>& a, int x, int y, int z, int type, T (&f)[Q]) {
+__device__ __forceinline__ void pull_cell(const StepArgs<T>& a, int x, int y, int z, int type, T (&f)[Q]) {
   constexpr Stencil<Q> L{};
   const int nx = a.nx, ny = a.ny, nz = a.nz;
   const long long N = a.N;
   const long long self = cell_index(x, y, z, nx, ny);
   const int xm = (x == 0) ? nx - 1 : x - 1;
-  // outlet: the ghost plane beyond x = nx-1 is a copy of plane nx-1 (no wrap)
   const int xp = (type == T_OUTLET) ? x : ((x == nx - 1) ? 0 : x + 1);
   const int ym = (y == 0) ? ny - 1 : y - 1, yp = (y == ny - 1) ? 0 : y + 1;
   const int zm = (z == 0) ? nz - 1 : z - 1, zp = (z == nz - 1) ? 0 : z + 1;
@@ -325,24 +318,45 @@ __device__ __forceinline__ void pull_masked(const StepArgs<T>& a, int x, int y, 
     const int sy = (L.c[i][1] == 0) ? y : ((L.c[i][1] == 1) ? ym : yp);
     const int sz = (L.c[i][2] == 0) ? z : ((L.c[i][2] == 1) ? zm : zp);
     const long long s = cell_index(sx, sy, sz, nx, ny);
-    const bool solid = (i != 0) && ((a.cls[s] & CLS_TYPE) == T_SOLID);
-    f[i] = solid ? __ldg(a.fin + L.opp[i] * N + self) : __ldg(a.fin + i * N + s);
+    bool own = false;
+    if (L.c[i][0] == -1 && type == T_OUTLET) own = (a.cls[s] & CLS_TYPE) == T_SOLID;
+    f[i] = own ? __ldg(a.fin + L.opp[i] * N + self) : __ldg(a.fin + i * N + s);
   }
   if (type == T_INLET) inlet_fixup<Q, T>(f, a.u_in[0], a.u_in[1], a.u_in[2]);
 }
 
-// S_t of one cell, whatever the storage phase.  PULL = input holds F_{t-1}.
+// S_t of one non-SOLID cell, whatever the storage phase.  PULL = input holds F_{t-1}.
 template <int Q, typename T, bool PULL>
 __device__ __forceinline__ void load_state(const StepArgs<T>& a, int x, int y, int z, uint8_t cls, T (&f)[Q]) {
-  const int type = cls & CLS_TYPE;
-  if (!PULL || type == T_SOLID) {
+  if (!PULL) {
     const long long self = cell_index(x, y, z, a.nx, a.ny);
 #pragma unroll
     for (int i = 0; i < Q; ++i) f[i] = __ldg(a.fin + i * a.N + self);
-  } else if ((cls & CLS_MASKED) || type != T_FLUID) {
-    pull_masked<Q, T>(a, x, y, z, type, f);
   } else {
-    pull_bulk<Q, T>(a.fin, a.N, x, y, z, a.nx, a.ny, a.nz, f);
+    pull_cell<Q, T>(a, x, y, z, cls & CLS_TYPE, f);
+  }
+}
+
+// Store of one non-SOLID cell (the store half of A7): its Q values, plus the ghost slots of its SOLID neighbours.
+template <int Q, typename T, bool GHOST>
+__device__ __forceinline__ void store_cell(const StepArgs<T>& a, int x, int y, int z, uint8_t cls, const T (&f)[Q]) {
+  constexpr Stencil<Q> L{};
+  const long long self = cell_index(x, y, z, a.nx, a.ny);
+#pragma unroll
+  for (int i = 0; i < Q; ++i) a.fout[i * a.N + self] = f[i];
+  if (GHOST && (cls & CLS_ADJ)) {
+    const uint32_t m = a.nbmask[self];
+    const int nx = a.nx, ny = a.ny, nz = a.nz;
+#pragma unroll
+    for (int j = 1; j < Q; ++j) {
+      if (m & (1u << j)) {
+        int sx = x + L.c[j][0], sy = y + L.c[j][1], sz = z + L.c[j][2];
+        sx = (sx < 0) ? sx + nx : ((sx >= nx) ? sx - nx : sx);
+        sy = (sy < 0) ? sy + ny : ((sy >= ny) ? sy - ny : sy);
+        sz = (sz < 0) ? sz + nz : ((sz >= nz) ? sz - nz : sz);
+        a.fout[L.opp[j] * a.N + cell_index(sx, sy, sz, nx, ny)] = f[j];
+      }
+    }
   }
 }
 
@@ -382,9 +396,8 @@ __device__ __forceinline__ void wallmodel_ub(const StepArgs<T>& a, int x, int y,
   ubz = static_cast<T>(r * t2);
 }
 
-// ---- the step kernel --------------------------------------------------------------------------------
-// The masked path (A7 + A8): cells that are INLET / OUTLET / WALLMODEL or have a SOLID neighbour.
-// Kept out of line so that the bulk path keeps its populations in registers.
+// ---- the per-cell step (scalar kernel; list blocks of the vector kernel) ------------------------------
+// One non-SOLID cell of any type: pull (MODE != COLLIDE), wall model, collide (MODE != STREAM), store + ghost slots.
 template <int Q, typename T, int MODE>
 __device__ __forceinline__ void step_cell_any(const StepArgs<T>& a, int x, int y, int z, uint8_t cls) {
   constexpr bool PULL = (MODE != MODE_COLLIDE);
@@ -398,42 +411,20 @@ __device__ __forceinline__ void step_cell_any(const StepArgs<T>& a, int x, int y
   T f[Q];
   load_state<Q, T, PULL>(a, x, y, z, cls, f);
   if (MODE != MODE_STREAM) collide_cell<Q, T>(f, d, ubx, uby, ubz, a.tau0, a.smago_k);
-#pragma unroll
-  for (int i = 0; i < Q; ++i) a.fout[i * a.N + self] = f[i];
-}
-
-template <int Q, typename T, int MODE>
-__device__ __noinline__ void step_masked_cell(const StepArgs<T>& a, int x, int y, int z, uint8_t cls) {
-  step_cell_any<Q, T, MODE>(a, x, y, z, cls);
+  store_cell<Q, T, MODE != MODE_STREAM>(a, x, y, z, cls, f);
 }
 
 // grid (ceil(nx/bx), ceil(ny/by), nz), block (bx, by): thread <-> cell, x fastest (coalesced rows).
+// Fallback for row lengths the vector kernel does not take.
 template <int Q, typename T, int MODE>
 __global__ void __launch_bounds__(256) k_step(const __grid_constant__ StepArgs<T> a) {
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
   const int z = blockIdx.z;
   if (x >= a.nx || y >= a.ny) return;
-  const long long self = cell_index(x, y, z, a.nx, a.ny);
-  const uint8_t cls = a.cls[self];
-  if ((cls & CLS_TYPE) == T_SOLID) return;   // SOLID cells are inert: nothing read, nothing written (R5)
-  if ((cls & CLS_MASKED) || (cls & CLS_TYPE) != T_FLUID) {
-    step_masked_cell<Q, T, MODE>(a, x, y, z, cls);
-    return;
-  }
-  // bulk path: plain FLUID cell, no SOLID neighbour
-  T f[Q];
-  T d = T(0);
-  if (MODE != MODE_STREAM && a.d != nullptr) d = __ldg(a.d + self);
-  if (MODE == MODE_COLLIDE) {
-#pragma unroll
-    for (int i = 0; i < Q; ++i) f[i] = __ldg(a.fin + i * a.N + self);
-  } else {
-    pull_bulk<Q, T>(a.fin, a.N, x, y, z, a.nx, a.ny, a.nz, f);
-  }
-  if (MODE != MODE_STREAM) collide_cell<Q, T>(f, d, T(0), T(0), T(0), a.tau0, a.smago_k);
-#pragma unroll
-  for (int i = 0; i < Q; ++i) a.fout[i * a.N + self] = f[i];
+  const uint8_t cls = a.cls[cell_index(x, y, z, a.nx, a.ny)];
+  if ((cls & CLS_TYPE) == T_SOLID) return;   // SOLID cells are inert (R5)
+  step_cell_any<Q, T, MODE>(a, x, y, z, cls);
 }
 
 // ---- the vectorised step kernel (the hot one) ------------------------------------------------------
@@ -443,44 +434,68 @@ __global__ void __launch_bounds__(256) k_step(const __grid_constant__ StepArgs<T
 // the one missing element from the neighbouring lane with a warp shuffle (row ends: one scalar load).
 // Vectors whose V cells are all plain bulk FLUID take this path; a vector that contains a SOLID,
 // INLET, OUTLET, WALLMODEL or solid-adjacent cell is processed cell by cell out of line (A7/A8).
-template <typename T> struct VecOf;
-template <> struct VecOf<float> { static constexpr int V = 4; };
-template <> struct VecOf<double> { static constexpr int V = 2; };
+// cells per thread: 128-bit access for D3Q19 (4 floats / 2 doubles); D3Q27 takes half of that (64-bit access, still
+// whole 32-byte sectors per warp instruction) because 27 x 4 live values leave room for only 8 warps per SM and the
+// kernel then stalls on its own latency (ncu, profiles/: 12.5 % occupancy, 0.27 issue slots per cycle).
+template <int Q, typename T> struct VecOf;
+template <> struct VecOf<19, float> { static constexpr int V = 4; };
+template <> struct VecOf<19, double> { static constexpr int V = 2; };
+template <> struct VecOf<27, float> { static constexpr int V = 2; };
+template <> struct VecOf<27, double> { static constexpr int V = 1; };
 
-__device__ __forceinline__ void ld_vec(const float* p, float (&v)[4]) {
-  const float4 t = __ldcs(reinterpret_cast<const float4*>(p));
+template <bool STREAMING>
+__device__ __forceinline__ void ld_vec_t(const float* p, float (&v)[4]) {
+  const float4 t = STREAMING ? __ldcs(reinterpret_cast<const float4*>(p)) : __ldg(reinterpret_cast<const float4*>(p));
   v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
 }
-__device__ __forceinline__ void ld_vec(const double* p, double (&v)[2]) {
-  const double2 t = __ldcs(reinterpret_cast<const double2*>(p));
+template <bool STREAMING>
+__device__ __forceinline__ void ld_vec_t(const float* p, float (&v)[2]) {
+  const float2 t = STREAMING ? __ldcs(reinterpret_cast<const float2*>(p)) : __ldg(reinterpret_cast<const float2*>(p));
   v[0] = t.x; v[1] = t.y;
 }
-__device__ __forceinline__ void ld_vec_keep(const float* p, float (&v)[4]) {
-  const float4 t = __ldg(reinterpret_cast<const float4*>(p));
-  v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
-}
-__device__ __forceinline__ void ld_vec_keep(const double* p, double (&v)[2]) {
-  const double2 t = __ldg(reinterpret_cast<const double2*>(p));
+template <bool STREAMING>
+__device__ __forceinline__ void ld_vec_t(const double* p, double (&v)[2]) {
+  const double2 t = STREAMING ? __ldcs(reinterpret_cast<const double2*>(p)) : __ldg(reinterpret_cast<const double2*>(p));
   v[0] = t.x; v[1] = t.y;
 }
+template <bool STREAMING>
+__device__ __forceinline__ void ld_vec_t(const double* p, double (&v)[1]) {
+  v[0] = STREAMING ? __ldcs(p) : __ldg(p);
+}
+template <typename T, int V> __device__ __forceinline__ void ld_vec(const T* p, T (&v)[V]) { ld_vec_t<true>(p, v); }
+template <typename T, int V> __device__ __forceinline__ void ld_vec_keep(const T* p, T (&v)[V]) { ld_vec_t<false>(p, v); }
 __device__ __forceinline__ void st_vec(float* p, const float (&v)[4]) {
   __stcs(reinterpret_cast<float4*>(p), make_float4(v[0], v[1], v[2], v[3]));
 }
+__device__ __forceinline__ void st_vec(float* p, const float (&v)[2]) { __stcs(reinterpret_cast<float2*>(p), make_float2(v[0], v[1])); }
 __device__ __forceinline__ void st_vec(double* p, const double (&v)[2]) {
   __stcs(reinterpret_cast<double2*>(p), make_double2(v[0], v[1]));
 }
-// class bytes of one 32-byte sector of a population row (8 floats / 4 doubles = 2 vectors), one aligned load
+__device__ __forceinline__ void st_vec(double* p, const double (&v)[1]) { __stcs(p, v[0]); }
+// class bytes of one 32-byte sector of a population row (8 floats / 4 doubles), one aligned load
 __device__ __forceinline__ unsigned long long ld_cls_sector(const uint8_t* p, float) { return *reinterpret_cast<const unsigned long long*>(p); }
 __device__ __forceinline__ unsigned long long ld_cls_sector(const uint8_t* p, double) { return *reinterpret_cast<const uint32_t*>(p); }
+__device__ __forceinline__ void ld_nbmask(const uint32_t* p, uint32_t (&m)[4]) {
+  const uint4 t = __ldg(reinterpret_cast<const uint4*>(p));
+  m[0] = t.x; m[1] = t.y; m[2] = t.z; m[3] = t.w;
+}
+__device__ __forceinline__ void ld_nbmask(const uint32_t* p, uint32_t (&m)[2]) {
+  const uint2 t = __ldg(reinterpret_cast<const uint2*>(p));
+  m[0] = t.x; m[1] = t.y;
+}
+__device__ __forceinline__ void ld_nbmask(const uint32_t* p, uint32_t (&m)[1]) { m[0] = __ldg(p); }
+__host__ __device__ constexpr uint32_t rep_byte(uint32_t b, int n) { return n <= 0 ? 0u : (b | (rep_byte(b, n - 1) << 8)); }
 
 // grid (ceil(nx/V/bx), ceil(ny/by), list_z + nz), block (bx, by), bx a power of two <= 32.
 // The first list_z z-slices of the grid do not own a lattice slab: their threads walk the compact list
-// of cells that belong to non-bulk vectors (the masked boundary kernel, A7/A8, as a block role of the
-// same launch: it is scheduled first and overlaps with the bulk blocks).
+// of the cells of SPECIAL sectors (A8 wall model; OUTLET cells next to a wall), one cell per thread: the masked
+// boundary kernel as a block role of the same launch (scheduled first, overlaps with the row blocks).
+// Everything else -- bulk, solid-adjacent (ghost slots), INLET and OUTLET cells -- runs in the vector path.
 template <int Q, typename T, int MODE>
-__global__ void __launch_bounds__(256) k_step_vec(const __grid_constant__ StepArgs<T> a) {
+__global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ StepArgs<T> a) {
   constexpr Stencil<Q> L{};
-  constexpr int V = VecOf<T>::V;
+  constexpr int V = VecOf<Q, T>::V;
+  constexpr int SV = 32 / static_cast<int>(sizeof(T));      // cells per 32-byte sector
   constexpr unsigned FULL = 0xffffffffu;
   const int tx = threadIdx.x;
   if (static_cast<int>(blockIdx.z) < a.list_z) {
@@ -488,16 +503,11 @@ __global__ void __launch_bounds__(256) k_step_vec(const __grid_constant__ StepAr
     const long long k = blk * (blockDim.x * blockDim.y) + threadIdx.y * blockDim.x + tx;
     if (k < a.n_list) {
       const int cell = a.list[k];
-      const int plane = a.nx * a.ny;
-      const int cz = cell / plane, rem = cell - cz * plane;
-      const int cy = rem / a.nx, cx = rem - cy * a.nx;
       const uint8_t c = a.cls[cell];
-      if ((c & CLS_TYPE) == T_SOLID) {
-        // a SOLID cell that shares a 32-byte sector with cells of the list: copy it through, so that every
-        // store instruction of the warp covers whole sectors (partial-sector writes cost an L2 read-fill)
-#pragma unroll
-        for (int i = 0; i < Q; ++i) a.fout[i * a.N + cell] = __ldg(a.fin + i * a.N + cell);
-      } else {
+      if ((c & CLS_TYPE) != T_SOLID) {     // SOLID sector-mates hold ghost slots written by others: never touched
+        const int plane = a.nx * a.ny;
+        const int cz = cell / plane, rem = cell - cz * plane;
+        const int cy = rem / a.nx, cx = rem - cy * a.nx;
         step_cell_any<Q, T, MODE>(a, cx, cy, cz, c);
       }
     }
@@ -514,50 +524,65 @@ __global__ void __launch_bounds__(256) k_step_vec(const __grid_constant__ StepAr
   const long long N = a.N;
   const long long row = active ? (static_cast<long long>(z) * ny + y) * nx : 0;
   const long long self = row + (active ? x0 : 0);
-  // class bytes of the vector's 32-byte sector (2 vectors): the vector takes the bulk path only if no
-  // cell of its sector is MASKED, so that bulk and list stores never split a sector
+  // class bytes of the vector's 32-byte sector (2 vectors): a sector with a SPECIAL cell belongs to the list blocks
   unsigned long long secw = ~0ull;
-  if (active) secw = ld_cls_sector(a.cls + row + (x0 & ~(2 * V - 1)), T(0));
-  constexpr unsigned long long MASKED_ALL = (V == 4) ? 0x8080808080808080ull : 0x80808080ull;
-  constexpr uint32_t TYPE_ALL = (V == 4) ? 0x07070707u : 0x0707u;
-  constexpr uint32_t SOLID_ALL = (V == 4) ? 0x01010101u : 0x0101u;
-  const uint32_t clsw = static_cast<uint32_t>(secw >> ((qx & 1) ? 8 * V : 0)) & ((V == 4) ? 0xffffffffu : 0xffffu);
+  if (active) secw = ld_cls_sector(a.cls + row + (x0 & ~(SV - 1)), T(0));
+  constexpr unsigned long long SPECIAL_ALL = (SV == 8) ? 0x8080808080808080ull : 0x80808080ull;
+  constexpr uint32_t VMASK = rep_byte(0xffu, V);
+  constexpr uint32_t TYPE_ALL = rep_byte(0x07u, V);
+  constexpr uint32_t SOLID_ALL = rep_byte(0x01u, V);
+  constexpr uint32_t ADJ_ALL = rep_byte(0x40u, V);
+  const uint32_t clsw = static_cast<uint32_t>(secw >> (8 * (x0 & (SV - 1)))) & VMASK;
   const bool all_solid = !active || ((clsw & TYPE_ALL) == SOLID_ALL);
-  const bool bulk = active && ((secw & MASKED_ALL) == 0);
-  const bool doload = active && !all_solid;
-  // INLET (only ever at x = 0) / OUTLET (only ever at x = nx-1) cells of a bulk vector
-  const bool inlet0 = bulk && (x0 == 0) && ((clsw & CLS_TYPE) == T_INLET);
-  const bool outletN = bulk && (qx == nvec - 1) && (((clsw >> (8 * (V - 1))) & CLS_TYPE) == T_OUTLET);
+  const bool mine = active && !all_solid && ((secw & SPECIAL_ALL) == 0);   // this thread computes and stores the vector
+  const bool doload = active && !all_solid;                                 // neighbours may need its lanes' values
+  // which cells of the vector are SOLID (bit v)
+  unsigned solid_bits = 0;
+#pragma unroll
+  for (int v = 0; v < V; ++v) solid_bits |= (((clsw >> (8 * v)) & CLS_TYPE) == T_SOLID) ? (1u << v) : 0u;
+  const bool adj = mine && (MODE != MODE_STREAM) && ((clsw & ADJ_ALL) != 0);
+  // INLET (only ever at x = 0) / OUTLET (only ever at x = nx-1; SPECIAL if next to a wall) cells
+  const bool inlet0 = mine && (x0 == 0) && ((clsw & CLS_TYPE) == T_INLET);
+  const bool outletN = mine && (qx == nvec - 1) && (((clsw >> (8 * (V - 1))) & CLS_TYPE) == T_OUTLET);
 
   T f[Q][V];
   T d[V];
 #pragma unroll
   for (int v = 0; v < V; ++v) d[v] = T(0);
-  if (MODE != MODE_STREAM && bulk && a.d != nullptr) {
+  if (MODE != MODE_STREAM && mine && a.d != nullptr) {
     T dv[V];
     ld_vec_keep(a.d + self, dv);
 #pragma unroll
     for (int v = 0; v < V; ++v) d[v] = dv[v];
   }
+  // per-cell SOLID-neighbour masks of a solid-adjacent vector (one aligned 128 / 64-bit load)
+  uint32_t nbm[V];
+#pragma unroll
+  for (int v = 0; v < V; ++v) nbm[v] = 0u;
+  if (adj) ld_nbmask(a.nbmask + self, nbm);
+  // row offsets of the (dy, dz) neighbour rows; all deltas fit 32 bits because N < 2^31
+  const int ym = (y == 0) ? ny - 1 : y - 1, yp = (y >= ny - 1) ? 0 : y + 1;
+  const int zm = (z == 0) ? nz - 1 : z - 1, zp = (z == nz - 1) ? 0 : z + 1;
+  const int dym = (ym - y) * nx, dyp = (yp - y) * nx;
+  const int plane = nx * ny;
+  const int dzm = (zm - z) * plane, dzp = (zp - z) * plane;
+  const int xl = (x0 == 0) ? nx - 1 : x0 - 1;            // element left of the vector (periodic)
+  const int xr = (x0 + V >= nx) ? 0 : x0 + V;            // element right of the vector
+  const int exl = xl - x0, exr = xr - x0;                // relative to the vector start
   if (MODE == MODE_COLLIDE) {
-    if (bulk) {
+    if (mine) {
 #pragma unroll
       for (int i = 0; i < Q; ++i) ld_vec(a.fin + i * N + self, f[i]);
     }
   } else {
-    const int ym = (y == 0) ? ny - 1 : y - 1, yp = (y >= ny - 1) ? 0 : y + 1;
-    const int zm = (z == 0) ? nz - 1 : z - 1, zp = (z == nz - 1) ? 0 : z + 1;
-    const int xl = (x0 == 0) ? nx - 1 : x0 - 1;            // element left of the vector (periodic)
-    const int xr = (x0 + V >= nx) ? 0 : x0 + V;            // element right of the vector
-    const bool edge_l = doload && ((lane == 0) || (tx == 0));
-    const bool edge_r = doload && ((lane == 31) || (tx == static_cast<int>(blockDim.x) - 1) || (qx == nvec - 1));
+    // a vector that is SOLID throughout loads nothing, but its end cells may hold ghost slots the neighbouring
+    // vector pulls: that neighbour fetches the one element itself, like a lane at the edge of the warp
+    const bool solid_l = __shfl_up_sync(FULL, all_solid ? 1 : 0, 1) != 0;
+    const bool solid_r = __shfl_down_sync(FULL, all_solid ? 1 : 0, 1) != 0;
+    const bool edge_l = doload && ((lane == 0) || (tx == 0) || solid_l);
+    const bool edge_r = doload && ((lane == 31) || (tx == static_cast<int>(blockDim.x) - 1) || (qx == nvec - 1) || solid_r);
     // phase 1: issue every load before anything consumes one (in-order issue: a shuffle placed right
-    // after its load would serialise the 19 loads).  Addresses: one running pointer per population
-    // (+N each) plus one of 9 (dy,dz) row offsets; all deltas fit 32 bits because N < 2^31.
-    const int dym = (ym - y) * nx, dyp = (yp - y) * nx;
-    const int plane = nx * ny;
-    const int dzm = (zm - z) * plane, dzp = (zp - z) * plane;
-    const int exl = xl - x0, exr = xr - x0;                  // edge element, relative to the vector start
+    // after its load would serialise the loads).  One running pointer per population (+N each).
     const T* pself = a.fin + self;
     T e[Q];   // the one element a shifted row needs from outside the warp / row (edge lanes only)
 #pragma unroll
@@ -592,60 +617,91 @@ __global__ void __launch_bounds__(256) k_step_vec(const __grid_constant__ StepAr
       }
     }
   }
+  if (!mine) return;   // SOLID throughout, or a SPECIAL sector (list blocks)
 
-  if (bulk) {
-    if (MODE != MODE_COLLIDE && inlet0) {                    // R6 on the x = 0 cell of the row
+  if (MODE != MODE_COLLIDE && inlet0) {                      // R6 on the x = 0 cell of the row
+    T fc[Q];
+#pragma unroll
+    for (int i = 0; i < Q; ++i) fc[i] = f[i][0];
+    inlet_fixup<Q, T>(fc, a.u_in[0], a.u_in[1], a.u_in[2]);
+#pragma unroll
+    for (int i = 0; i < Q; ++i) f[i][0] = fc[i];
+  }
+  if (MODE != MODE_STREAM) {
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
       T fc[Q];
 #pragma unroll
-      for (int i = 0; i < Q; ++i) fc[i] = f[i][0];
-      inlet_fixup<Q, T>(fc, a.u_in[0], a.u_in[1], a.u_in[2]);
+      for (int i = 0; i < Q; ++i) fc[i] = f[i][v];
+      collide_cell<Q, T>(fc, d[v], T(0), T(0), T(0), a.tau0, a.smago_k);
 #pragma unroll
-      for (int i = 0; i < Q; ++i) f[i][0] = fc[i];
+      for (int i = 0; i < Q; ++i) f[i][v] = fc[i];
     }
-    if (MODE != MODE_STREAM) {
-#pragma unroll
-      for (int v = 0; v < V; ++v) {
-        T fc[Q];
-#pragma unroll
-        for (int i = 0; i < Q; ++i) fc[i] = f[i][v];
-        collide_cell<Q, T>(fc, d[v], T(0), T(0), T(0), a.tau0, a.smago_k);
-#pragma unroll
-        for (int i = 0; i < Q; ++i) f[i][v] = fc[i];
-      }
-    }
-    T* pout = a.fout + self;
+  }
+  T* pout = a.fout + self;
+  if (solid_bits == 0) {
 #pragma unroll
     for (int i = 0; i < Q; ++i) {
       st_vec(pout, f[i]);
       pout += N;
     }
+  } else {
+    // a vector that holds SOLID cells: element stores of the others only (the SOLID cells' slots are ghost slots
+    // that other threads write in this very launch)
+#pragma unroll
+    for (int i = 0; i < Q; ++i) {
+#pragma unroll
+      for (int v = 0; v < V; ++v)
+        if (!(solid_bits & (1u << v))) pout[v] = f[i][v];
+      pout += N;
+    }
   }
-  // non-bulk vectors: their cells are in the compact list and were handled by the list blocks
+  if (adj) {
+    // ghost slots: F_j(x) -> slot (opp(j), x + c_j) for every SOLID neighbour x + c_j (row offset = the pull row of
+    // opp(j); the x neighbour of an end-of-row cell wraps)
+    uint32_t any = 0u;
+#pragma unroll
+    for (int v = 0; v < V; ++v) any |= (solid_bits & (1u << v)) ? 0u : nbm[v];
+    T* pg = a.fout + self;
+#pragma unroll
+    for (int j = 1; j < Q; ++j) {
+      if (any & (1u << j)) {
+        // the row of x + c_j (c_opp(j) = -c_j, written out so that the table index stays a compile-time constant)
+        const long long off = static_cast<long long>((L.c[j][1] == 0) ? 0 : ((L.c[j][1] == 1) ? dyp : dym)) +
+                              static_cast<long long>((L.c[j][2] == 0) ? 0 : ((L.c[j][2] == 1) ? dzp : dzm));
+        T* dst = pg + static_cast<long long>(L.opp[j]) * N + off;
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+          if (!(solid_bits & (1u << v)) && (nbm[v] & (1u << j))) {
+            int ex = v + L.c[j][0];
+            if (L.c[j][0] == -1 && v == 0) ex = exl;
+            if (L.c[j][0] == 1 && v == V - 1) ex = exr;
+            dst[ex] = f[j][v];
+          }
+        }
+      }
+    }
+  }
 }
 
-// marks the cells that the list blocks of k_step_vec must process: EVERY cell (SOLID ones included, they
-// are copied through) of a 32-byte sector (SV = 8 floats / 4 doubles, aligned) that holds at least one
-// MASKED cell and is not SOLID throughout.  mark[] feeds a stream compaction.
+// marks the cells that the list blocks of k_step_vec must process: every cell of a 32-byte sector (SV = 8 floats /
+// 4 doubles, aligned) that holds at least one SPECIAL cell.  mark[] feeds a stream compaction.
 template <int SV>
 __global__ void __launch_bounds__(256) k_mark_list(const uint8_t* __restrict__ cls, uint8_t* __restrict__ mark,
                                                    long long nsec_total, unsigned long long* __restrict__ counters) {
   const long long q = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
   if (q >= nsec_total) return;
-  bool any_masked = false, all_solid = true;
+  bool m = false;
 #pragma unroll
-  for (int v = 0; v < SV; ++v) {
-    const uint8_t c = cls[q * SV + v];
-    any_masked = any_masked || (c & CLS_MASKED);
-    all_solid = all_solid && ((c & CLS_TYPE) == T_SOLID);
-  }
-  const bool m = any_masked && !all_solid;
+  for (int v = 0; v < SV; ++v) m = m || (cls[q * SV + v] & CLS_SPECIAL);
 #pragma unroll
   for (int v = 0; v < SV; ++v) mark[q * SV + v] = m ? 1 : 0;
   if (m) atomicAdd(counters + 3, static_cast<unsigned long long>(SV));
 }
 
 // ---- A9: moments of S_t -----------------------------------------------------------------------------
-template <int Q, typename T, bool PULL>
+// (the host side materialises S_t first when the storage holds F_{t-1}: plain loads of the cell's own values)
+template <int Q, typename T>
 __global__ void __launch_bounds__(256) k_moments(const __grid_constant__ StepArgs<T> a, T* __restrict__ rho_out, T* __restrict__ u_out) {
   constexpr Stencil<Q> L{};
   constexpr int H = (Q - 1) / 2;
@@ -654,9 +710,9 @@ __global__ void __launch_bounds__(256) k_moments(const __grid_constant__ StepArg
   const int z = blockIdx.z;
   if (x >= a.nx || y >= a.ny) return;
   const long long self = cell_index(x, y, z, a.nx, a.ny);
-  const uint8_t cls = a.cls[self];
   T f[Q];
-  load_state<Q, T, PULL>(a, x, y, z, cls, f);
+#pragma unroll
+  for (int i = 0; i < Q; ++i) f[i] = __ldg(a.fin + i * a.N + self);
   T rho = f[0], jx = T(0), jy = T(0), jz = T(0);
 #pragma unroll
   for (int i = 1; i <= H; ++i) {
@@ -676,7 +732,7 @@ __global__ void __launch_bounds__(256) k_moments(const __grid_constant__ StepArg
 
 // ---- A9: totals over non-SOLID cells (mass, momentum, kinetic energy), fp64 accumulation --------------
 // warp shuffle tree -> one shared-memory partial per warp -> one atomicAdd(double) per block and quantity
-template <int Q, typename T, bool PULL>
+template <int Q, typename T>
 __global__ void __launch_bounds__(256) k_totals(const __grid_constant__ StepArgs<T> a, double* __restrict__ out /*[5]*/) {
   constexpr Stencil<Q> L{};
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
@@ -688,7 +744,8 @@ __global__ void __launch_bounds__(256) k_totals(const __grid_constant__ StepArgs
     const uint8_t cls = a.cls[self];
     if ((cls & CLS_TYPE) != T_SOLID) {
       T f[Q];
-      load_state<Q, T, PULL>(a, x, y, z, cls, f);
+#pragma unroll
+      for (int i = 0; i < Q; ++i) f[i] = __ldg(a.fin + i * a.N + self);
       double rho = 0.0, jx = 0.0, jy = 0.0, jz = 0.0;
 #pragma unroll
       for (int i = 0; i < Q; ++i) {
@@ -724,7 +781,7 @@ __global__ void __launch_bounds__(256) k_totals(const __grid_constant__ StepArgs
 // ---- A4 as an initialiser: f = f^eq(rho, u) ----------------------------------------------------------
 template <int Q, typename T>
 __global__ void __launch_bounds__(256) k_init_equilibrium(const T* __restrict__ rho_in, const T* __restrict__ u_in,
-                                                          T* __restrict__ fa, T* __restrict__ fb, long long N) {
+                                                          T* __restrict__ fa, long long N) {
   constexpr Stencil<Q> L{};
   const long long n = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
   if (n >= N) return;
@@ -735,16 +792,15 @@ __global__ void __launch_bounds__(256) k_init_equilibrium(const T* __restrict__ 
     const T cu = T(L.c[i][0]) * ux + T(L.c[i][1]) * uy + T(L.c[i][2]) * uz;
     const T v = weight<Q, T>(L.c2[i]) * rho * (base + T(3) * cu + T(4.5) * cu * cu);
     fa[i * N + n] = v;
-    fb[i * N + n] = v;   // SOLID cells must hold the same values in both lattices
   }
 }
 
 // ---- flag validation + classification ------------------------------------------------------------
-// cls = type | normal<<3 | MASKED if the cell is not plain FLUID or any lattice neighbour is SOLID.
-// counters[0] = invalid flag bytes, [1] = SOLID cells, [2] = masked cells.
+// cls = type | normal<<3 | ADJ | SPECIAL (see the top of this file).
+// counters[0] = invalid flag bytes, [1] = SOLID cells, [2] = masked cells (non-SOLID, not plain bulk FLUID).
 template <int Q>
-__global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ flags, uint8_t* __restrict__ cls, int nx,
-                                                  int ny, int nz, unsigned long long* __restrict__ counters) {
+__global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ flags, uint8_t* __restrict__ cls,
+                                                  int nx, int ny, int nz, unsigned long long* __restrict__ counters) {
   constexpr Stencil<Q> L{};
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
@@ -758,21 +814,66 @@ __global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ fl
   if (type == T_INLET && x != 0) bad = true;
   if (type == T_OUTLET && x != nx - 1) bad = true;
   if (bad) { atomicAdd(counters, 1ull); return; }
-  bool masked = (type == T_SOLID) || (type == T_WM);
-  bool special = type != T_FLUID;
+  uint32_t m = 0u;
   if (type != T_SOLID) {
 #pragma unroll
-    for (int i = 1; i < Q; ++i) {
-      int sx = x - L.c[i][0], sy = y - L.c[i][1], sz = z - L.c[i][2];
+    for (int j = 1; j < Q; ++j) {
+      int sx = x + L.c[j][0], sy = y + L.c[j][1], sz = z + L.c[j][2];
       sx = (sx < 0) ? sx + nx : ((sx >= nx) ? sx - nx : sx);
       sy = (sy < 0) ? sy + ny : ((sy >= ny) ? sy - ny : sy);
       sz = (sz < 0) ? sz + nz : ((sz >= nz) ? sz - nz : sz);
-      masked = masked || ((flags[cell_index(sx, sy, sz, nx, ny)] & 0x0F) == T_SOLID);
+      if ((flags[cell_index(sx, sy, sz, nx, ny)] & 0x0F) == T_SOLID) m |= (1u << j);
     }
   }
-  cls[self] = static_cast<uint8_t>(type | ((type == T_WM ? hi : 0) << CLS_NORMAL_SHIFT) | (masked ? CLS_MASKED : 0));
+  const bool adj = (m != 0u);
+  const bool special = (type == T_WM) || (type == T_OUTLET && adj);
+  cls[self] = static_cast<uint8_t>(type | ((type == T_WM ? hi : 0) << CLS_NORMAL_SHIFT) | (adj ? CLS_ADJ : 0) |
+                                   (special ? CLS_SPECIAL : 0));
   if (type == T_SOLID) atomicAdd(counters + 1, 1ull);
-  else if (masked || special) atomicAdd(counters + 2, 1ull);
+  else if (adj || type != T_FLUID) atomicAdd(counters + 2, 1ull);
+}
+
+// nbmask of an accepted classification (a rejected flag array must leave the old geometry intact)
+template <int Q>
+__global__ void __launch_bounds__(256) k_nbmask(const uint8_t* __restrict__ cls, uint32_t* __restrict__ nbmask, int nx, int ny, int nz) {
+  constexpr Stencil<Q> L{};
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  const int y = blockIdx.y * blockDim.y + threadIdx.y;
+  const int z = blockIdx.z;
+  if (x >= nx || y >= ny) return;
+  const long long self = cell_index(x, y, z, nx, ny);
+  uint32_t m = 0u;
+  if (cls[self] & CLS_ADJ) {
+#pragma unroll
+    for (int j = 1; j < Q; ++j) {
+      int sx = x + L.c[j][0], sy = y + L.c[j][1], sz = z + L.c[j][2];
+      sx = (sx < 0) ? sx + nx : ((sx >= nx) ? sx - nx : sx);
+      sy = (sy < 0) ? sy + ny : ((sy >= ny) ? sy - ny : sy);
+      sz = (sz < 0) ? sz + nz : ((sz >= nz) ? sz - nz : sz);
+      if ((cls[cell_index(sx, sy, sz, nx, ny)] & CLS_TYPE) == T_SOLID) m |= (1u << j);
+    }
+  }
+  nbmask[self] = m;
+}
+
+// mark[n] = 1 on SOLID cells (feeds the compaction of the SOLID-cell list)
+__global__ void __launch_bounds__(256) k_mark_solid(const uint8_t* __restrict__ cls, uint8_t* __restrict__ mark, long long N) {
+  const long long n = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (n < N) mark[n] = ((cls[n] & CLS_TYPE) == T_SOLID) ? 1 : 0;
+}
+
+// SOLID cells are inert (R5) but their storage doubles as ghost slots: their own Q values live in a side buffer
+// side[Q][n_solid].  SAVE: lattice -> side;  !SAVE: side -> lattice (after a materialisation).
+template <typename T, bool SAVE>
+__global__ void __launch_bounds__(256) k_solid_values(T* __restrict__ f, T* __restrict__ side, const int* __restrict__ solid_list,
+                                                      long long n_solid, long long N, int Q) {
+  const long long k = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (k >= n_solid) return;
+  const long long cell = solid_list[k];
+  for (int i = 0; i < Q; ++i) {
+    if (SAVE) side[i * n_solid + k] = f[i * N + cell];
+    else f[i * N + cell] = side[i * n_solid + k];
+  }
 }
 
 }  // namespace lbm
