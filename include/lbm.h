@@ -51,6 +51,7 @@ enum { LBM_OK = 0, LBM_EINVAL = -1, LBM_ENOMEM = -2, LBM_ECUDA = -3, LBM_ESTATE 
 enum { LBM_D3Q19 = 19, LBM_D3Q27 = 27 };
 enum { LBM_F32 = 4, LBM_F64 = 8 };
 enum { LBM_FLUID = 0, LBM_SOLID = 1, LBM_INLET = 2, LBM_OUTLET = 3, LBM_WALLMODEL = 4 };
+enum { LBM_COLLISION_BGK = 0, LBM_COLLISION_HRR = 1 };
 
 typedef struct lbm_ctx lbm_ctx; /* opaque; owned by the library */
 
@@ -63,6 +64,13 @@ typedef struct {
   int wm_enable;    /* 0: WALLMODEL cells behave as FLUID; 1: Spalding wall model (Eq. 15-17, R8)  */
   double wm_kappa;  /* Spalding constants; the paper prints neither (defaults 0.41, 9.8)           */
   double wm_E;
+  int collision;    /* LBM_COLLISION_BGK (0): Eq. 6 with f~(1) = f - f^eq, Eq. 11 up to H(2) (G1);
+                     * LBM_COLLISION_HRR (1): the paper's own collision, Eq. 6-11 in full: third-order
+                     * equilibrium (Eq. 11, G9), recursive-regularised f(1) (Eq. 8-9, G29), finite-
+                     * difference part (Eq. 10, G10) hybridised by sigma (Eq. 7); the FD strain is the
+                     * central difference of u^(x,t) of the same time level (G30-G32); sigma = 0 on
+                     * WALLMODEL cells when wm_enable (l.131).  Smagorinsky tau_eff as in the BGK form. */
+  double sigma;     /* Eq. 7 hybridisation factor in [0,1]; read only when collision == HRR         */
 } lbm_params;
 
 /* Create a context for an nx x ny x nz lattice (nx fastest in memory).
@@ -97,9 +105,12 @@ int lbm_set_geometry(lbm_ctx* ctx, const void* porosity, const uint8_t* cell_fla
  *   -> tau_eff from the local non-equilibrium stress (Eq. 3-5, 14) -> relaxation (Eq. 6) -> propagation
  *   with halfway bounce-back at SOLID neighbours (R5), zero-gradient outlet (R7), regularised velocity
  *   inlet (l.155, R6).
- * One fused kernel launch per step on the context's stream; asynchronous.
+ * BGK form: one fused kernel launch per step on the context's stream.  HRR form: two launches per
+ * z-slab of the lattice (u^ pass, then the fused step) and 3 more values of dtype per
+ * cell of device memory (allocated on the first HRR step; LBM_ENOMEM if that fails).  Asynchronous.
  * Errors: LBM_EINVAL (NULL ctx/params, n_steps < 0, tau0 <= 0.5, cs_smago < 0, wm_enable with
- * wm_kappa <= 0 or wm_E <= 0), LBM_ESTATE (no state set yet), LBM_ECUDA. */
+ * wm_kappa <= 0 or wm_E <= 0, collision not 0/1, sigma outside [0,1] with HRR), LBM_ESTATE (no state
+ * set yet), LBM_ECUDA. */
 int lbm_step(lbm_ctx* ctx, int n_steps, const lbm_params* params);
 
 /* Moments of the state S_t for EVERY cell (SOLID cells report whatever was set):

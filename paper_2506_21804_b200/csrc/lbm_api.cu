@@ -34,9 +34,9 @@ struct lbm_ctx {
   uint8_t* cls;          // class byte per cell (see lbm_kernels.cuh)
   uint8_t* cls_alt;      // classification target before it is accepted
   uint8_t* flags_raw;    // device copy of the caller's flag bytes; afterwards the list marks
-  uint32_t* nbmask;      // per cell: which lattice neighbours are SOLID (ghost-slot bounce-back)
+  uint32_t* nbmask;      // per cell: which lattice neighbours are SOLID (read-side bounce-back)
   int* solid_list;       // SOLID cells, ascending
-  void* solid_vals;      // their own populations [Q][n_solid] (their lattice storage doubles as ghost slots)
+  void* solid_vals;      // their own populations [Q][n_solid] (the step kernels write zeros over their lattice slots)
   long long n_solid_list;
   int* list;             // cells of the non-bulk vectors (vector kernel), ascending
   long long n_list;
@@ -471,7 +471,7 @@ int lbm_set_fields(lbm_ctx* c, const void* populations, const void* porosity, co
   c->cur = 0;
   c->phase = PHASE_PRE;
   c->steps = 0;
-  return solid_values(c, true);      // SOLID cells' own values -> side buffer (their storage becomes ghost slots)
+  return solid_values(c, true);      // SOLID cells' own values -> side buffer (the step kernels overwrite their slots)
 }
 
 int lbm_init_equilibrium(lbm_ctx* c, const void* rho, const void* u) {
@@ -504,7 +504,7 @@ static int materialise(lbm_ctx* c) {
   int rc = launch_step(c, &p, lbm::MODE_STREAM);
   if (rc != LBM_OK) return rc;
   c->phase = PHASE_PRE;
-  return solid_values(c, false);     // the stream pass does not write SOLID cells: put their own values back
+  return solid_values(c, false);     // the stream pass leaves zeros or stale data on SOLID cells: put their own values back
 }
 
 int lbm_set_geometry(lbm_ctx* c, const void* porosity, const uint8_t* cell_flags) {

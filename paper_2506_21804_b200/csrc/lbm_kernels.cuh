@@ -19,15 +19,15 @@ namespace lbm {
 
 enum : int { T_FLUID = 0, T_SOLID = 1, T_INLET = 2, T_OUTLET = 3, T_WM = 4 };
 // internal class byte: bits 0-2 type, bits 3-5 wall-normal code,
-//   bit 6 = ADJ:     the (non-SOLID) cell has at least one SOLID lattice neighbour: it writes ghost slots (below);
+//   bit 6 = ADJ:     the (non-SOLID) cell has at least one SOLID lattice neighbour (nbmask[] says which);
 //   bit 7 = SPECIAL: the cell needs the per-cell path (list blocks): WALLMODEL cells (A8) and OUTLET cells with a
-//                    SOLID neighbour (their clamped pull does not fit the ghost-slot rule).
-// Halfway bounce-back through GHOST SLOTS (A7, reading R5): a non-SOLID cell x whose neighbour s = x + c_j is SOLID
-// stores its post-collision F_j(x) a second time into the slot (opp(j), s) of the SOLID cell.  The next step's pull
-// of direction opp(j) at x reads exactly that slot: g_opp(j)(x) = A[opp(j)][x - c_opp(j)] = A[opp(j)][s] = F_j(x).
-// The pull therefore never tests a flag.  Slot (i, s) has the single writer s + c_i, so there is no race; SOLID
-// cells' own values are kept in a side buffer by the host side (they are inert, R5) and patched back whenever the
-// state is materialised.
+//                    SOLID neighbour (their clamped pull needs a class lookup).
+// Halfway bounce-back (A7, reading R5) on the READ side: the pull of direction i at a cell x whose source x - c_i is
+// SOLID takes the cell's own F_opp(i)(x) instead.  Nobody ever consumes the lattice slots of a SOLID cell, so the
+// step kernels write every 128-byte line they touch IN FULL (zeros on SOLID cells): a store stream with holes at
+// the walls leaves partial sectors that the L2 has to fill from DRAM, which cost config 4 a third of its
+// bandwidth (profiles/r1_config4_spheres.md).  SOLID cells' own values (inert, R5) are kept in a side buffer by
+// the host side and patched back whenever the state is materialised.
 constexpr uint8_t CLS_TYPE = 0x07;
 constexpr uint8_t CLS_ADJ = 0x40;
 constexpr uint8_t CLS_SPECIAL = 0x80;
@@ -297,17 +297,19 @@ __device__ __forceinline__ long long cell_index(int x, int y, int z, int nx, int
   return (static_cast<long long>(z) * ny + y) * nx + x;
 }
 
-// Pull of one cell (A1 + the pull half of A7): g_i(x) = A[i][x - c_i], periodic wrap; SOLID neighbours need no
-// test because their ghost slots hold the bounced-back value.  OUTLET cells clamp the source of the c_x < 0
-// populations to their own plane (R7: ghost plane nx := plane nx-1); if that clamped source is SOLID the ghost
-// slot belongs to another cell, so the bounce-back is taken explicitly from the cell's own opposite population.
-// INLET cells get the fix-up R6.  `type` is the cell's own type (not SOLID).
+// Pull of one cell (A1 + A7): g_i(x) = A[i][x - c_i], periodic wrap; a SOLID source means halfway bounce-back:
+// the cell's own opposite population (nbmask bit opp(i): the neighbour x + c_opp(i) = x - c_i is SOLID).  OUTLET
+// cells clamp the source of the c_x < 0 populations to their own plane (R7: ghost plane nx := plane nx-1), so for
+// those the class of the clamped source decides.  INLET cells get the fix-up R6.  `cls` is the cell's own class
+// byte (not SOLID).
 template <int Q, typename T>
-__device__ __forceinline__ void pull_cell(const StepArgs<T>& a, int x, int y, int z, int type, T (&f)[Q]) {
+__device__ __forceinline__ void pull_cell(const StepArgs<T>& a, int x, int y, int z, uint8_t cls, T (&f)[Q]) {
   constexpr Stencil<Q> L{};
+  const int type = cls & CLS_TYPE;
   const int nx = a.nx, ny = a.ny, nz = a.nz;
   const long long N = a.N;
   const long long self = cell_index(x, y, z, nx, ny);
+  const uint32_t nbm = (cls & CLS_ADJ) ? a.nbmask[self] : 0u;
   const int xm = (x == 0) ? nx - 1 : x - 1;
   const int xp = (type == T_OUTLET) ? x : ((x == nx - 1) ? 0 : x + 1);
   const int ym = (y == 0) ? ny - 1 : y - 1, yp = (y == ny - 1) ? 0 : y + 1;
@@ -318,7 +320,7 @@ __device__ __forceinline__ void pull_cell(const StepArgs<T>& a, int x, int y, in
     const int sy = (L.c[i][1] == 0) ? y : ((L.c[i][1] == 1) ? ym : yp);
     const int sz = (L.c[i][2] == 0) ? z : ((L.c[i][2] == 1) ? zm : zp);
     const long long s = cell_index(sx, sy, sz, nx, ny);
-    bool own = false;
+    bool own = (i > 0) && ((nbm >> L.opp[i]) & 1u);
     if (L.c[i][0] == -1 && type == T_OUTLET) own = (a.cls[s] & CLS_TYPE) == T_SOLID;
     f[i] = own ? __ldg(a.fin + L.opp[i] * N + self) : __ldg(a.fin + i * N + s);
   }
@@ -333,31 +335,22 @@ __device__ __forceinline__ void load_state(const StepArgs<T>& a, int x, int y, i
 #pragma unroll
     for (int i = 0; i < Q; ++i) f[i] = __ldg(a.fin + i * a.N + self);
   } else {
-    pull_cell<Q, T>(a, x, y, z, cls & CLS_TYPE, f);
+    pull_cell<Q, T>(a, x, y, z, cls, f);
   }
 }
 
-// Store of one non-SOLID cell (the store half of A7): its Q values, plus the ghost slots of its SOLID neighbours.
-template <int Q, typename T, bool GHOST>
-__device__ __forceinline__ void store_cell(const StepArgs<T>& a, int x, int y, int z, uint8_t cls, const T (&f)[Q]) {
-  constexpr Stencil<Q> L{};
+// Store of one cell's Q values.
+template <int Q, typename T>
+__device__ __forceinline__ void store_cell(const StepArgs<T>& a, int x, int y, int z, const T (&f)[Q]) {
   const long long self = cell_index(x, y, z, a.nx, a.ny);
 #pragma unroll
   for (int i = 0; i < Q; ++i) a.fout[i * a.N + self] = f[i];
-  if (GHOST && (cls & CLS_ADJ)) {
-    const uint32_t m = a.nbmask[self];
-    const int nx = a.nx, ny = a.ny, nz = a.nz;
+}
+// SOLID cells: nobody reads their slots; zeros keep every written sector whole.
+template <int Q, typename T>
+__device__ __forceinline__ void store_zero(const StepArgs<T>& a, long long self) {
 #pragma unroll
-    for (int j = 1; j < Q; ++j) {
-      if (m & (1u << j)) {
-        int sx = x + L.c[j][0], sy = y + L.c[j][1], sz = z + L.c[j][2];
-        sx = (sx < 0) ? sx + nx : ((sx >= nx) ? sx - nx : sx);
-        sy = (sy < 0) ? sy + ny : ((sy >= ny) ? sy - ny : sy);
-        sz = (sz < 0) ? sz + nz : ((sz >= nz) ? sz - nz : sz);
-        a.fout[L.opp[j] * a.N + cell_index(sx, sy, sz, nx, ny)] = f[j];
-      }
-    }
-  }
+  for (int i = 0; i < Q; ++i) a.fout[i * a.N + self] = T(0);
 }
 
 // A8 / reading R8: u^B of a wall-model cell from the tangential velocity at x + n.
@@ -397,7 +390,7 @@ __device__ __forceinline__ void wallmodel_ub(const StepArgs<T>& a, int x, int y,
 }
 
 // ---- the per-cell step (scalar kernel; list blocks of the vector kernel) ------------------------------
-// One non-SOLID cell of any type: pull (MODE != COLLIDE), wall model, collide (MODE != STREAM), store + ghost slots.
+// One non-SOLID cell of any type: pull (MODE != COLLIDE), wall model, collide (MODE != STREAM), store.
 template <int Q, typename T, int MODE>
 __device__ __forceinline__ void step_cell_any(const StepArgs<T>& a, int x, int y, int z, uint8_t cls) {
   constexpr bool PULL = (MODE != MODE_COLLIDE);
@@ -411,7 +404,7 @@ __device__ __forceinline__ void step_cell_any(const StepArgs<T>& a, int x, int y
   T f[Q];
   load_state<Q, T, PULL>(a, x, y, z, cls, f);
   if (MODE != MODE_STREAM) collide_cell<Q, T>(f, d, ubx, uby, ubz, a.tau0, a.smago_k);
-  store_cell<Q, T, MODE != MODE_STREAM>(a, x, y, z, cls, f);
+  store_cell<Q, T>(a, x, y, z, f);
 }
 
 // grid (ceil(nx/bx), ceil(ny/by), nz), block (bx, by): thread <-> cell, x fastest (coalesced rows).
@@ -422,8 +415,12 @@ __global__ void __launch_bounds__(256) k_step(const __grid_constant__ StepArgs<T
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
   const int z = blockIdx.z;
   if (x >= a.nx || y >= a.ny) return;
-  const uint8_t cls = a.cls[cell_index(x, y, z, a.nx, a.ny)];
-  if ((cls & CLS_TYPE) == T_SOLID) return;   // SOLID cells are inert (R5)
+  const long long self = cell_index(x, y, z, a.nx, a.ny);
+  const uint8_t cls = a.cls[self];
+  if ((cls & CLS_TYPE) == T_SOLID) {         // SOLID cells are inert (R5); their slots are never read
+    store_zero<Q, T>(a, self);
+    return;
+  }
   step_cell_any<Q, T, MODE>(a, x, y, z, cls);
 }
 
@@ -490,13 +487,15 @@ __host__ __device__ constexpr uint32_t rep_byte(uint32_t b, int n) { return n <=
 // The first list_z z-slices of the grid do not own a lattice slab: their threads walk the compact list
 // of the cells of SPECIAL sectors (A8 wall model; OUTLET cells next to a wall), one cell per thread: the masked
 // boundary kernel as a block role of the same launch (scheduled first, overlaps with the row blocks).
-// Everything else -- bulk, solid-adjacent (ghost slots), INLET and OUTLET cells -- runs in the vector path.
+// Everything else -- bulk, solid-adjacent (read-side bounce-back), INLET and OUTLET cells -- runs in the vector path.
 template <int Q, typename T, int MODE>
 __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ StepArgs<T> a) {
   constexpr Stencil<Q> L{};
   constexpr int V = VecOf<Q, T>::V;
   constexpr int SV = 32 / static_cast<int>(sizeof(T));      // cells per 32-byte sector
+  constexpr int LG = 128 / (V * static_cast<int>(sizeof(T)));  // lanes per 128-byte line
   constexpr unsigned FULL = 0xffffffffu;
+  constexpr bool PULL = (MODE != MODE_COLLIDE);
   const int tx = threadIdx.x;
   if (static_cast<int>(blockIdx.z) < a.list_z) {
     const long long blk = (static_cast<long long>(blockIdx.z) * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
@@ -504,7 +503,9 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
     if (k < a.n_list) {
       const int cell = a.list[k];
       const uint8_t c = a.cls[cell];
-      if ((c & CLS_TYPE) != T_SOLID) {     // SOLID sector-mates hold ghost slots written by others: never touched
+      if ((c & CLS_TYPE) == T_SOLID) {     // SOLID sector-mate: zeros keep the sector whole
+        store_zero<Q, T>(a, cell);
+      } else {
         const int plane = a.nx * a.ny;
         const int cz = cell / plane, rem = cell - cz * plane;
         const int cy = rem / a.nx, cx = rem - cy * a.nx;
@@ -524,7 +525,7 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
   const long long N = a.N;
   const long long row = active ? (static_cast<long long>(z) * ny + y) * nx : 0;
   const long long self = row + (active ? x0 : 0);
-  // class bytes of the vector's 32-byte sector (2 vectors): a sector with a SPECIAL cell belongs to the list blocks
+  // class bytes of the vector's 32-byte sector: a sector with a SPECIAL cell belongs to the list blocks
   unsigned long long secw = ~0ull;
   if (active) secw = ld_cls_sector(a.cls + row + (x0 & ~(SV - 1)), T(0));
   constexpr unsigned long long SPECIAL_ALL = (SV == 8) ? 0x8080808080808080ull : 0x80808080ull;
@@ -534,13 +535,18 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
   constexpr uint32_t ADJ_ALL = rep_byte(0x40u, V);
   const uint32_t clsw = static_cast<uint32_t>(secw >> (8 * (x0 & (SV - 1)))) & VMASK;
   const bool all_solid = !active || ((clsw & TYPE_ALL) == SOLID_ALL);
-  const bool mine = active && !all_solid && ((secw & SPECIAL_ALL) == 0);   // this thread computes and stores the vector
-  const bool doload = active && !all_solid;                                 // neighbours may need its lanes' values
+  const bool special = (secw & SPECIAL_ALL) != 0;
+  // an all-SOLID vector whose 128-byte line holds a non-SOLID vector stores zeros, so that the line is written whole
+  const unsigned live_lanes = __ballot_sync(FULL, active && !all_solid);
+  const unsigned group = (LG >= 32) ? FULL : (((1u << (LG & 31)) - 1u) << (lane & ~(LG - 1)));
+  const bool zero_fill = active && all_solid && !special && ((live_lanes & group) != 0u);
+  const bool mine = active && !all_solid && !special;       // this thread computes and stores the vector
+  const bool doload = active && !all_solid;                 // neighbours may need its lanes' values
   // which cells of the vector are SOLID (bit v)
   unsigned solid_bits = 0;
 #pragma unroll
   for (int v = 0; v < V; ++v) solid_bits |= (((clsw >> (8 * v)) & CLS_TYPE) == T_SOLID) ? (1u << v) : 0u;
-  const bool adj = mine && (MODE != MODE_STREAM) && ((clsw & ADJ_ALL) != 0);
+  const bool adj = mine && PULL && ((clsw & ADJ_ALL) != 0);
   // INLET (only ever at x = 0) / OUTLET (only ever at x = nx-1; SPECIAL if next to a wall) cells
   const bool inlet0 = mine && (x0 == 0) && ((clsw & CLS_TYPE) == T_INLET);
   const bool outletN = mine && (qx == nvec - 1) && (((clsw >> (8 * (V - 1))) & CLS_TYPE) == T_OUTLET);
@@ -569,14 +575,14 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
   const int xl = (x0 == 0) ? nx - 1 : x0 - 1;            // element left of the vector (periodic)
   const int xr = (x0 + V >= nx) ? 0 : x0 + V;            // element right of the vector
   const int exl = xl - x0, exr = xr - x0;                // relative to the vector start
-  if (MODE == MODE_COLLIDE) {
+  if (!PULL) {
     if (mine) {
 #pragma unroll
       for (int i = 0; i < Q; ++i) ld_vec(a.fin + i * N + self, f[i]);
     }
   } else {
-    // a vector that is SOLID throughout loads nothing, but its end cells may hold ghost slots the neighbouring
-    // vector pulls: that neighbour fetches the one element itself, like a lane at the edge of the warp
+    // a vector that is SOLID throughout loads nothing, but the rows its neighbour pulls from (y -+ 1, z -+ 1) may be
+    // fluid at its end cells: that neighbour fetches the one element itself, like a lane at the edge of the warp
     const bool solid_l = __shfl_up_sync(FULL, all_solid ? 1 : 0, 1) != 0;
     const bool solid_r = __shfl_down_sync(FULL, all_solid ? 1 : 0, 1) != 0;
     const bool edge_l = doload && ((lane == 0) || (tx == 0) || solid_l);
@@ -617,9 +623,50 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
       }
     }
   }
-  if (!mine) return;   // SOLID throughout, or a SPECIAL sector (list blocks)
+  T* pout = a.fout + self;
+  if (zero_fill) {
+    T zero[V];
+#pragma unroll
+    for (int v = 0; v < V; ++v) zero[v] = T(0);
+#pragma unroll
+    for (int i = 0; i < Q; ++i) {
+      st_vec(pout, zero);
+      pout += N;
+    }
+    return;
+  }
+  if (!mine) return;   // SOLID throughout in an all-SOLID line, or a SPECIAL sector (list blocks)
 
-  if (MODE != MODE_COLLIDE && inlet0) {                      // R6 on the x = 0 cell of the row
+  if (adj) {
+    // R5, read side: where the source x - c_i of population i is SOLID (nbmask bit j = opp(i): x + c_j is SOLID), the
+    // pulled value is replaced by the cell's own F_j(x).  Own-cell vectors are fetched in three batches so that the
+    // loads of a batch are in flight together without holding Q more vectors in registers.
+    uint32_t any = 0u;
+#pragma unroll
+    for (int v = 0; v < V; ++v) any |= (solid_bits & (1u << v)) ? 0u : nbm[v];
+    constexpr int G = (Q - 1 + 2) / 3;
+#pragma unroll
+    for (int j0 = 1; j0 < Q; j0 += G) {
+      T own[G][V];
+#pragma unroll
+      for (int g = 0; g < G; ++g) {
+        const int j = j0 + g;
+#pragma unroll
+        for (int v = 0; v < V; ++v) own[g][v] = T(0);
+        if (j < Q && (any & (1u << j))) ld_vec(a.fin + static_cast<long long>(j) * N + self, own[g]);
+      }
+#pragma unroll
+      for (int g = 0; g < G; ++g) {
+        const int j = j0 + g;
+        if (j < Q) {
+#pragma unroll
+          for (int v = 0; v < V; ++v)
+            if (nbm[v] & (1u << j)) f[L.opp[j]][v] = own[g][v];
+        }
+      }
+    }
+  }
+  if (PULL && inlet0) {                                      // R6 on the x = 0 cell of the row
     T fc[Q];
 #pragma unroll
     for (int i = 0; i < Q; ++i) fc[i] = f[i][0];
@@ -638,49 +685,17 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
       for (int i = 0; i < Q; ++i) f[i][v] = fc[i];
     }
   }
-  T* pout = a.fout + self;
-  if (solid_bits == 0) {
+  if (solid_bits != 0) {   // SOLID cells inside the vector: their slots are never read; zeros, so that the store is whole
 #pragma unroll
-    for (int i = 0; i < Q; ++i) {
-      st_vec(pout, f[i]);
-      pout += N;
-    }
-  } else {
-    // a vector that holds SOLID cells: element stores of the others only (the SOLID cells' slots are ghost slots
-    // that other threads write in this very launch)
-#pragma unroll
-    for (int i = 0; i < Q; ++i) {
+    for (int i = 0; i < Q; ++i)
 #pragma unroll
       for (int v = 0; v < V; ++v)
-        if (!(solid_bits & (1u << v))) pout[v] = f[i][v];
-      pout += N;
-    }
+        if (solid_bits & (1u << v)) f[i][v] = T(0);
   }
-  if (adj) {
-    // ghost slots: F_j(x) -> slot (opp(j), x + c_j) for every SOLID neighbour x + c_j (row offset = the pull row of
-    // opp(j); the x neighbour of an end-of-row cell wraps)
-    uint32_t any = 0u;
 #pragma unroll
-    for (int v = 0; v < V; ++v) any |= (solid_bits & (1u << v)) ? 0u : nbm[v];
-    T* pg = a.fout + self;
-#pragma unroll
-    for (int j = 1; j < Q; ++j) {
-      if (any & (1u << j)) {
-        // the row of x + c_j (c_opp(j) = -c_j, written out so that the table index stays a compile-time constant)
-        const long long off = static_cast<long long>((L.c[j][1] == 0) ? 0 : ((L.c[j][1] == 1) ? dyp : dym)) +
-                              static_cast<long long>((L.c[j][2] == 0) ? 0 : ((L.c[j][2] == 1) ? dzp : dzm));
-        T* dst = pg + static_cast<long long>(L.opp[j]) * N + off;
-#pragma unroll
-        for (int v = 0; v < V; ++v) {
-          if (!(solid_bits & (1u << v)) && (nbm[v] & (1u << j))) {
-            int ex = v + L.c[j][0];
-            if (L.c[j][0] == -1 && v == 0) ex = exl;
-            if (L.c[j][0] == 1 && v == V - 1) ex = exr;
-            dst[ex] = f[j][v];
-          }
-        }
-      }
-    }
+  for (int i = 0; i < Q; ++i) {
+    st_vec(pout, f[i]);
+    pout += N;
   }
 }
 
@@ -862,7 +877,7 @@ __global__ void __launch_bounds__(256) k_mark_solid(const uint8_t* __restrict__ 
   if (n < N) mark[n] = ((cls[n] & CLS_TYPE) == T_SOLID) ? 1 : 0;
 }
 
-// SOLID cells are inert (R5) but their storage doubles as ghost slots: their own Q values live in a side buffer
+// SOLID cells are inert (R5) but the step kernels write zeros over their slots: their own Q values live in a side buffer
 // side[Q][n_solid].  SAVE: lattice -> side;  !SAVE: side -> lattice (after a materialisation).
 template <typename T, bool SAVE>
 __global__ void __launch_bounds__(256) k_solid_values(T* __restrict__ f, T* __restrict__ side, const int* __restrict__ solid_list,
