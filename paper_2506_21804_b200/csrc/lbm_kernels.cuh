@@ -639,31 +639,14 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
 
   if (adj) {
     // R5, read side: where the source x - c_i of population i is SOLID (nbmask bit j = opp(i): x + c_j is SOLID), the
-    // pulled value is replaced by the cell's own F_j(x).  Own-cell vectors are fetched in three batches so that the
-    // loads of a batch are in flight together without holding Q more vectors in registers.
-    uint32_t any = 0u;
+    // pulled value is replaced by the cell's own F_j(x).  Predicated element loads straight into the population
+    // registers: no extra registers, and all of them are in flight together (one round trip).
+    const T* pown = a.fin + self;
 #pragma unroll
-    for (int v = 0; v < V; ++v) any |= (solid_bits & (1u << v)) ? 0u : nbm[v];
-    constexpr int G = (Q - 1 + 2) / 3;
+    for (int j = 1; j < Q; ++j) {
 #pragma unroll
-    for (int j0 = 1; j0 < Q; j0 += G) {
-      T own[G][V];
-#pragma unroll
-      for (int g = 0; g < G; ++g) {
-        const int j = j0 + g;
-#pragma unroll
-        for (int v = 0; v < V; ++v) own[g][v] = T(0);
-        if (j < Q && (any & (1u << j))) ld_vec(a.fin + static_cast<long long>(j) * N + self, own[g]);
-      }
-#pragma unroll
-      for (int g = 0; g < G; ++g) {
-        const int j = j0 + g;
-        if (j < Q) {
-#pragma unroll
-          for (int v = 0; v < V; ++v)
-            if (nbm[v] & (1u << j)) f[L.opp[j]][v] = own[g][v];
-        }
-      }
+      for (int v = 0; v < V; ++v)
+        if (nbm[v] & (1u << j)) f[L.opp[j]][v] = __ldg(pown + static_cast<long long>(j) * N + v);
     }
   }
   if (PULL && inlet0) {                                      // R6 on the x = 0 cell of the row
