@@ -55,6 +55,8 @@ struct lbm_ctx {
   int block_threads;
   int use_vector;        // 1: 128-bit vector kernel when nx % (32/dtype) == 0 (default); 0: scalar kernel
   int use_graph;
+  void* uhat;            // HRR form: u^(x,t) [3][N], allocated on the first HRR step
+  int hrr_slab;          // HRR form: z-slices per slab of the two-pass step (0 = whole lattice)
   lbm_params last;       // parameters of the last lbm_step: the inlet rule is part of how S_t is formed from F_{t-1}
   char err[512];
 };
@@ -138,6 +140,9 @@ lbm::StepArgs<T> make_args(const lbm_ctx* c, const lbm_params* p, int in, int ou
   a.list = c->list;
   a.n_list = static_cast<int>(c->n_list);
   a.list_z = 0;
+  a.z0 = 0;
+  a.uhat = static_cast<T*>(c->uhat);
+  a.sigma = p ? static_cast<T>(p->sigma) : T(1);
   if (p) {
     a.tau0 = static_cast<T>(p->tau0);
     a.smago_k = static_cast<T>(18.0 * 1.4142135623730951 * p->cs_smago * p->cs_smago);
@@ -154,9 +159,9 @@ lbm::StepArgs<T> make_args(const lbm_ctx* c, const lbm_params* p, int in, int ou
 }
 
 // vector kernel: thread <-> V consecutive cells; block (bx quads, by rows)
-template <int Q, typename T>
+template <int Q, typename T, int COLL>
 void launch_dims_vec(const lbm_ctx* c, dim3& grid, dim3& block) {
-  const int V = lbm::VecOf<Q, T>::V;
+  const int V = lbm::VecOf<Q, T, COLL>::V;
   const int nvec = c->nx / V;
   int bx = 1;
   while (bx < nvec && bx < 32) bx <<= 1;
@@ -169,32 +174,85 @@ void launch_dims_vec(const lbm_ctx* c, dim3& grid, dim3& block) {
   grid = dim3((nvec + bx - 1) / bx, (c->ny + by - 1) / by, c->nz);
 }
 
-template <int Q, typename T>
-int launch_step_t(lbm_ctx* c, const lbm_params* p, int mode) {
+// One launch of a step kernel over the z-slices [z0, z0 + nzs) (+ the list blocks when with_list), lattice `in` -> `out`.
+template <int Q, typename T, int MODE, int COLL>
+int launch_one(lbm_ctx* c, const lbm_params* p, int in, int out, int z0, int nzs, bool with_list) {
   dim3 grid, block;
-  const int in = c->cur, out = 1 - c->cur;
   lbm::StepArgs<T> a = make_args<T>(c, p, in, out);
+  a.z0 = z0;
   const bool vec = c->use_vector && (c->nx % (32 / static_cast<int>(sizeof(T))) == 0);   // whole 32-byte sectors per row
   if (vec) {
-    launch_dims_vec<Q, T>(c, grid, block);
-    const long long per_slice = static_cast<long long>(grid.x) * grid.y * block.x * block.y;
-    a.list_z = static_cast<int>((c->n_list + per_slice - 1) / per_slice);
-    grid.z += a.list_z;
-    switch (mode) {
-      case lbm::MODE_COLLIDE: lbm::k_step_vec<Q, T, lbm::MODE_COLLIDE><<<grid, block, 0, c->stream>>>(a); break;
-      case lbm::MODE_STREAM_COLLIDE: lbm::k_step_vec<Q, T, lbm::MODE_STREAM_COLLIDE><<<grid, block, 0, c->stream>>>(a); break;
-      default: lbm::k_step_vec<Q, T, lbm::MODE_STREAM><<<grid, block, 0, c->stream>>>(a); break;
+    launch_dims_vec<Q, T, COLL>(c, grid, block);
+    a.list_z = 0;
+    if (with_list) {
+      const long long per_slice = static_cast<long long>(grid.x) * grid.y * block.x * block.y;
+      a.list_z = static_cast<int>((c->n_list + per_slice - 1) / per_slice);
     }
+    grid.z = nzs + a.list_z;
+    if (grid.z == 0) return LBM_OK;
+    lbm::k_step_vec<Q, T, MODE, COLL><<<grid, block, 0, c->stream>>>(a);
   } else {
+    if (nzs == 0) return LBM_OK;
     launch_dims(c, grid, block);
-    switch (mode) {
-      case lbm::MODE_COLLIDE: lbm::k_step<Q, T, lbm::MODE_COLLIDE><<<grid, block, 0, c->stream>>>(a); break;
-      case lbm::MODE_STREAM_COLLIDE: lbm::k_step<Q, T, lbm::MODE_STREAM_COLLIDE><<<grid, block, 0, c->stream>>>(a); break;
-      default: lbm::k_step<Q, T, lbm::MODE_STREAM><<<grid, block, 0, c->stream>>>(a); break;
-    }
+    grid.z = nzs;
+    lbm::k_step<Q, T, MODE, COLL><<<grid, block, 0, c->stream>>>(a);
   }
   LBM_CUDA(c, cudaGetLastError());
   c->launches++;
+  return LBM_OK;
+}
+
+// HRR form (Eq. 7-11): the FD strain (Eq. 10) needs u^(x,t) of the six neighbours, i.e. their streamed populations, so
+// a step is two passes: UHAT (pull, moments, Eq. 12 -> u^ field) and the fused step that reads it.  The passes are
+// interleaved slab by slab in z, the UHAT pass one slice ahead, so that the populations the UHAT pass pulled are still
+// in the 126 MB L2 when the step pass pulls them again.  The list cells (wall model, ...) go with the
+// first UHAT launch and the last step launch.
+template <int Q, typename T, int MODE_U, int MODE_S>
+int launch_hrr_t(lbm_ctx* c, const lbm_params* p, int in, int out) {
+  const int nz = c->nz;
+  int slab = (c->hrr_slab > 0) ? c->hrr_slab : nz;
+  if (slab >= nz - 1) {
+    int rc = launch_one<Q, T, MODE_U, lbm::COLL_BGK>(c, p, in, out, 0, nz, true);
+    if (rc != LBM_OK) return rc;
+    return launch_one<Q, T, MODE_S, lbm::COLL_HRR>(c, p, in, out, 0, nz, true);
+  }
+  // UHAT: slice nz-1 first (the periodic neighbour of slice 0), then [0, slab], [slab+1, 2 slab], ... up to nz-2
+  int rc = launch_one<Q, T, MODE_U, lbm::COLL_BGK>(c, p, in, out, nz - 1, 1, true);
+  if (rc != LBM_OK) return rc;
+  int udone = 0;                       // slices [0, udone) have their u^
+  for (int z0 = 0; z0 < nz; z0 += slab) {
+    const int zend = (z0 + slab < nz) ? z0 + slab : nz;          // step pass covers [z0, zend)
+    int uneed = (zend + 1 < nz - 1) ? zend + 1 : nz - 1;         // needs u^ on [z0 - 1, zend]; nz-1 is done
+    if (uneed > udone) {
+      rc = launch_one<Q, T, MODE_U, lbm::COLL_BGK>(c, p, in, out, udone, uneed - udone, false);
+      if (rc != LBM_OK) return rc;
+      udone = uneed;
+    }
+    rc = launch_one<Q, T, MODE_S, lbm::COLL_HRR>(c, p, in, out, z0, zend - z0, zend == nz);
+    if (rc != LBM_OK) return rc;
+  }
+  return LBM_OK;
+}
+
+template <int Q, typename T>
+int launch_step_t(lbm_ctx* c, const lbm_params* p, int mode) {
+  const int in = c->cur, out = 1 - c->cur;
+  const bool hrr = p && p->collision == LBM_COLLISION_HRR;
+  int rc;
+  switch (mode) {
+    case lbm::MODE_COLLIDE:
+      rc = hrr ? launch_hrr_t<Q, T, lbm::MODE_UHAT_PRE, lbm::MODE_COLLIDE>(c, p, in, out)
+               : launch_one<Q, T, lbm::MODE_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 0, c->nz, true);
+      break;
+    case lbm::MODE_STREAM_COLLIDE:
+      rc = hrr ? launch_hrr_t<Q, T, lbm::MODE_UHAT_PULL, lbm::MODE_STREAM_COLLIDE>(c, p, in, out)
+               : launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 0, c->nz, true);
+      break;
+    default:
+      rc = launch_one<Q, T, lbm::MODE_STREAM, lbm::COLL_BGK>(c, p, in, out, 0, c->nz, true);
+      break;
+  }
+  if (rc != LBM_OK) return rc;
   c->cur = out;
   return LBM_OK;
 }
@@ -257,6 +315,10 @@ int check_params(lbm_ctx* c, const lbm_params* p) {
   if (p->wm_enable && (!(p->wm_kappa > 0.0) || !(p->wm_E > 0.0)))
     return fail(c, LBM_EINVAL, "lbm_step: wm_enable needs wm_kappa > 0 and wm_E > 0");
   if (!(p->u_in[0] < 1.0)) return fail(c, LBM_EINVAL, "lbm_step: u_in[0] = %g must be < 1", p->u_in[0]);
+  if (p->collision != LBM_COLLISION_BGK && p->collision != LBM_COLLISION_HRR)
+    return fail(c, LBM_EINVAL, "lbm_step: collision = %d must be 0 (BGK) or 1 (HRR)", p->collision);
+  if (p->collision == LBM_COLLISION_HRR && !(p->sigma >= 0.0 && p->sigma <= 1.0))
+    return fail(c, LBM_EINVAL, "lbm_step: sigma = %g must be in [0,1]", p->sigma);
   return LBM_OK;
 }
 
@@ -425,7 +487,7 @@ lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype) {
 void lbm_destroy(lbm_ctx* c) {
   if (!c) return;
   cudaStreamSynchronize(c->stream);
-  cudaFree(c->f[0]);  cudaFree(c->f[1]);  cudaFree(c->d);
+  cudaFree(c->f[0]);  cudaFree(c->f[1]);  cudaFree(c->d);  cudaFree(c->uhat);
   cudaFree(c->cls);  cudaFree(c->cls_alt);  cudaFree(c->flags_raw);
   cudaFree(c->counters);  cudaFree(c->totals_dev);  cudaFree(c->staging);
   cudaFree(c->list);  cudaFree(c->cub_tmp);  cudaFree(c->list_count_dev);
@@ -451,6 +513,8 @@ int lbm_synchronize(lbm_ctx* c) {
 static int set_geometry_fields(lbm_ctx* c, const void* porosity, const uint8_t* cell_flags) {
   int rc = classify(c, cell_flags);
   if (rc != LBM_OK) return rc;
+  if (c->uhat)   // cells that turned SOLID must read u^ = 0 (the UHAT pass does not visit all-SOLID lines)
+    LBM_CUDA(c, cudaMemsetAsync(c->uhat, 0, 3 * static_cast<size_t>(c->N) * c->dtype, c->stream));
   if (porosity) {
     LBM_CUDA(c, cudaMemcpyAsync(c->d, porosity, static_cast<size_t>(c->N) * c->dtype, cudaMemcpyDefault, c->stream));
     c->has_d = true;
@@ -525,6 +589,13 @@ int lbm_step(lbm_ctx* c, int n_steps, const lbm_params* params) {
   if (n_steps < 0) return fail(c, LBM_EINVAL, "lbm_step: n_steps = %d must be >= 0", n_steps);
   if (c->phase == PHASE_NONE) return fail(c, LBM_ESTATE, "lbm_step: no state; call lbm_set_fields or lbm_init_equilibrium first");
   c->last = *params;
+  if (params->collision == LBM_COLLISION_HRR && !c->uhat && n_steps > 0) {
+    const size_t bytes = 3 * static_cast<size_t>(c->N) * c->dtype;
+    rc = dev_alloc(c, &c->uhat, bytes);
+    if (rc != LBM_OK) return rc;
+    // SOLID cells of all-SOLID lines are never written by the UHAT pass: u^ = 0 there (resting wall) from here on
+    LBM_CUDA(c, cudaMemsetAsync(c->uhat, 0, bytes, c->stream));
+  }
   for (int s = 0; s < n_steps; ++s) {
     if (c->phase == PHASE_PRE) {
       rc = launch_step(c, params, lbm::MODE_COLLIDE);          // S_t -> F_t
@@ -615,6 +686,11 @@ int lbm_set_option(lbm_ctx* c, const char* key, long long value) {
   if (std::strcmp(key, "block_threads") == 0) {
     if (value != 64 && value != 128 && value != 256) return fail(c, LBM_EINVAL, "block_threads must be 64, 128 or 256");
     c->block_threads = static_cast<int>(value);
+    return LBM_OK;
+  }
+  if (std::strcmp(key, "hrr_slab") == 0) {
+    if (value < 0) return fail(c, LBM_EINVAL, "hrr_slab must be >= 0");
+    c->hrr_slab = static_cast<int>(value);
     return LBM_OK;
   }
   if (std::strcmp(key, "vector") == 0) {

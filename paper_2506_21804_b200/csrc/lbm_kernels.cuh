@@ -36,7 +36,14 @@ constexpr int CLS_NORMAL_SHIFT = 3;
 // kernel modes
 enum : int { MODE_COLLIDE = 0,        // input holds S_t (fresh state): collide only           -> F_t
              MODE_STREAM_COLLIDE = 1, // input holds F_{t-1}: pull to S_t, collide             -> F_t
-             MODE_STREAM = 2 };       // input holds F_{t-1}: pull to S_t, store S_t (materialise)
+             MODE_STREAM = 2,         // input holds F_{t-1}: pull to S_t, store S_t (materialise)
+             MODE_UHAT_PULL = 3,      // input holds F_{t-1}: pull to S_t, store u^(x,t) (HRR form, first pass)
+             MODE_UHAT_PRE = 4 };     // input holds S_t: store u^(x,t)
+// collision forms (lbm_params.collision)
+enum : int { COLL_BGK = 0, COLL_HRR = 1 };
+__host__ __device__ constexpr bool mode_pulls(int mode) { return mode == MODE_STREAM_COLLIDE || mode == MODE_STREAM || mode == MODE_UHAT_PULL; }
+__host__ __device__ constexpr bool mode_collides(int mode) { return mode == MODE_COLLIDE || mode == MODE_STREAM_COLLIDE; }
+__host__ __device__ constexpr bool mode_uhat(int mode) { return mode == MODE_UHAT_PULL || mode == MODE_UHAT_PRE; }
 
 // ---- velocity set by rule R1 (G13), generated at compile time -------------------------
 template <int Q>
@@ -88,6 +95,10 @@ struct StepArgs {
   const int* __restrict__ list;
   int n_list;
   int list_z;
+  int z0;                         // first lattice z-slice of this launch (the grid covers a slab z0 .. z0 + gridDim.z - list_z - 1)
+  // HRR form (Eq. 7-11): u^(x,t) of every cell [3][N] (written by the MODE_UHAT_* pass, SOLID cells 0), Eq. 7 factor
+  T* __restrict__ uhat;
+  T sigma;
 };
 
 // ---- math helpers ---------------------------------------------------------------------------------
@@ -194,6 +205,142 @@ __device__ __forceinline__ void collide_cell(T (&f)[Q], T d, T ubx, T uby, T ubz
     f[i + H] = keepf * f[i + H] + (even - odd);
   }
   f[0] = keepf * f[0] + (ro - (esum + esum));
+}
+
+// ---- HRR form: the paper's own collision, Eq. 6-11 in full ------------------------------------
+// Third-order Hermite coefficients carried by the lattices: k = 0..6 <-> xxy, xxz, xyy, xzz, yyz, yzz, xyz.
+// h3<Q>(i, k) = the factor of coefficient A3[k] in the order-3 term of a Hermite series at direction i (without w_i):
+//   D3Q27: H(3)_k(c_i) / (2 c_s^6) for the six aab components (Eq. 11 as printed), H(3)_xyz / c_s^6;
+//   D3Q19: projection on the orthogonal combinations H_xxy +- H_yzz, H_xzz +- H_xyy, H_yyz +- H_xxz (reading G9):
+//          [3 (Hp+Hq)(ap+aq) + (Hp-Hq)(ap-aq)] / (6 c_s^6)  =>  factor of ap: 18 Hp + 9 Hq, of aq: 9 Hp + 18 Hq.
+__host__ __device__ constexpr double herm3_raw(int cx, int cy, int cz, int k) {
+  // H(3)_abg = c_a c_b c_g - c_s^2 (d_ab c_g + d_ag c_b + d_bg c_a)
+  return k == 0 ? cy * (cx * cx - 1.0 / 3.0)
+       : k == 1 ? cz * (cx * cx - 1.0 / 3.0)
+       : k == 2 ? cx * (cy * cy - 1.0 / 3.0)
+       : k == 3 ? cx * (cz * cz - 1.0 / 3.0)
+       : k == 4 ? cz * (cy * cy - 1.0 / 3.0)
+       : k == 5 ? cy * (cz * cz - 1.0 / 3.0)
+                : static_cast<double>(cx * cy * cz);
+}
+template <int Q>
+__host__ __device__ constexpr double h3(int cx, int cy, int cz, int k) {
+  if (Q == 27) return (k < 6 ? 13.5 : 27.0) * herm3_raw(cx, cy, cz, k);
+  if (k == 6) return 0.0;
+  // partner of k in the pairs (xxy,yzz) = (0,5), (xzz,xyy) = (3,2), (yyz,xxz) = (4,1)
+  const int q = (k == 0) ? 5 : (k == 5) ? 0 : (k == 3) ? 2 : (k == 2) ? 3 : (k == 4) ? 1 : 4;
+  return 18.0 * herm3_raw(cx, cy, cz, k) + 9.0 * herm3_raw(cx, cy, cz, q);
+}
+
+// A2..A6 in the HRR form on one cell held in registers.  f[] in: S_t, out: post-collision F_t.
+//   f*_i = f^eq_i + (1 - 1/tau) [sigma f(1)_i + (1 - sigma) f(1,FD)_i]                          (Eq. 6, 7)
+//   f^eq = w (rho + 3 c.rho u^ + 4.5 H2:rho u^u^ + order3(rho u^u^u^))                           (Eq. 11)
+//   f(1) = w (a0 + 3 c.a1 + 4.5 H2:a2 + order3(a3)),  a_n = sum_i H(n)_i (f_i - f^eq_i),         (Eq. 8-9)
+//          a3_abg = u^_a a2_bg + u^_b a2_ag + u^_g a2_ab                                          (G29)
+//   f(1,FD) = -w rho tau / c_s^2 H2:S                                                            (Eq. 10, G10)
+// Every part is a Hermite series with the same basis, so the coefficients are combined first (k = 1 - 1/tau):
+//   A1 = rho u^ + k sigma a1,  A2 = rho u^u^ + k (sigma a2 - (1-sigma)(2/3) rho tau S),  A3 = rho u^u^u^ + k sigma a3
+// and the series is evaluated once.  a0 = 0, a1 = rho (u - u^), a2 = M2 - rho (I/3 + u^u^) follow from the moments
+// of Eq. 11 (its order-3 term has no moments below order 3).  tau = tau_eff from |a2| as in the BGK form (A5).
+// S[6] = S^FD_xx, yy, zz, xy, xz, yz.
+template <int Q, typename T>
+__device__ __forceinline__ void collide_cell_hrr(T (&f)[Q], T d, T ubx, T uby, T ubz, T tau0, T smago_k, T sigma,
+                                                 const T (&S)[6]) {
+  constexpr Stencil<Q> L{};
+  constexpr int H = (Q - 1) / 2;
+  T rho = f[0], jx = T(0), jy = T(0), jz = T(0);
+  T mxx = T(0), myy = T(0), mzz = T(0), mxy = T(0), mxz = T(0), myz = T(0);
+#pragma unroll
+  for (int i = 1; i <= H; ++i) {
+    const T s = f[i] + f[i + H];
+    const T a = f[i] - f[i + H];
+    rho += s;
+    if (L.c[i][0] == 1) jx += a; else if (L.c[i][0] == -1) jx -= a;
+    if (L.c[i][1] == 1) jy += a; else if (L.c[i][1] == -1) jy -= a;
+    if (L.c[i][2] == 1) jz += a; else if (L.c[i][2] == -1) jz -= a;
+    if (L.c[i][0] != 0) mxx += s;
+    if (L.c[i][1] != 0) myy += s;
+    if (L.c[i][2] != 0) mzz += s;
+    if (L.c[i][0] * L.c[i][1] == 1) mxy += s; else if (L.c[i][0] * L.c[i][1] == -1) mxy -= s;
+    if (L.c[i][0] * L.c[i][2] == 1) mxz += s; else if (L.c[i][0] * L.c[i][2] == -1) mxz -= s;
+    if (L.c[i][1] * L.c[i][2] == 1) myz += s; else if (L.c[i][1] * L.c[i][2] == -1) myz -= s;
+  }
+  const T inv_rho = rcp_(rho);
+  const T keep = T(1) - d;                                  // Eq. 12
+  const T ux = keep * (jx * inv_rho) + d * ubx;
+  const T uy = keep * (jy * inv_rho) + d * uby;
+  const T uz = keep * (jz * inv_rho) + d * ubz;
+  const T qx = rho * ux, qy = rho * uy, qz = rho * uz;
+  const T third = rho * T(1.0 / 3.0);
+  // a2 (= Pi of the BGK form, now against the third-order equilibrium: same second moment)
+  const T pxx = (mxx - third) - qx * ux;
+  const T pyy = (myy - third) - qy * uy;
+  const T pzz = (mzz - third) - qz * uz;
+  const T pxy = mxy - qx * uy;
+  const T pxz = mxz - qx * uz;
+  const T pyz = myz - qy * uz;
+  T tau = tau0, omega;
+  if (smago_k > T(0)) {
+    const T off = pxy * pxy + pxz * pxz + pyz * pyz;
+    const T npi = sqrt_(pxx * pxx + pyy * pyy + pzz * pzz + (off + off));
+    tau = T(0.5) * (tau0 + sqrt_(tau0 * tau0 + smago_k * npi * inv_rho));
+  }
+  omega = rcp_(tau);
+  const T k = T(1) - omega;
+  const T ks = k * sigma;
+  const T kf = -(k - ks) * T(2.0 / 3.0) * rho * tau;        // k (1 - sigma) * (-(2/3) rho tau)
+  const T A1x = qx + ks * (jx - qx), A1y = qy + ks * (jy - qy), A1z = qz + ks * (jz - qz);
+  const T Axx = qx * ux + (ks * pxx + kf * S[0]);
+  const T Ayy = qy * uy + (ks * pyy + kf * S[1]);
+  const T Azz = qz * uz + (ks * pzz + kf * S[2]);
+  const T Axy = qx * uy + (ks * pxy + kf * S[3]);
+  const T Axz = qx * uz + (ks * pxz + kf * S[4]);
+  const T Ayz = qy * uz + (ks * pyz + kf * S[5]);
+  T A3[7];
+  A3[0] = qx * ux * uy + ks * (T(2) * ux * pxy + uy * pxx);          // xxy
+  A3[1] = qx * ux * uz + ks * (T(2) * ux * pxz + uz * pxx);          // xxz
+  A3[2] = qx * uy * uy + ks * (ux * pyy + T(2) * uy * pxy);          // xyy
+  A3[3] = qx * uz * uz + ks * (ux * pzz + T(2) * uz * pxz);          // xzz
+  A3[4] = qy * uy * uz + ks * (T(2) * uy * pyz + uz * pyy);          // yyz
+  A3[5] = qy * uz * uz + ks * (uy * pzz + T(2) * uz * pyz);          // yzz
+  A3[6] = qx * uy * uz + ks * (ux * pyz + uy * pxz + uz * pxy);      // xyz
+  // even part of direction i: w (rho - 1.5 tr A2 + 4.5 cc:A2); odd part: 3 w c.A1 + w sum_k h3 A3[k].
+  // Conservation in fp32 as in collide_cell: c3[] sums to exactly 1 over the stencil, the rest population takes what
+  // is left of rho.
+  constexpr double c3_2 = static_cast<double>(static_cast<T>(3.0 * static_cast<double>(weight<Q, double>(2))));
+  constexpr double c3_3 = (Q == 27) ? static_cast<double>(static_cast<T>(3.0 * static_cast<double>(weight<Q, double>(3)))) : 0.0;
+  constexpr double c3_1 = (1.0 - 8.0 * c3_2 - 8.0 * c3_3) / 2.0;
+  constexpr T c3[4] = {T(0), static_cast<T>(c3_1), static_cast<T>(c3_2), static_cast<T>(c3_3)};
+  const T e0 = rho - T(1.5) * (Axx + Ayy + Azz);
+  T esum = T(0);
+#pragma unroll
+  for (int i = 1; i <= H; ++i) {
+    const int cx = L.c[i][0], cy = L.c[i][1], cz = L.c[i][2];
+    const T w = weight<Q, T>(L.c2[i]);
+    T cA = T(0), cc = T(0), o3 = T(0);
+    if (cx == 1) cA += A1x; else if (cx == -1) cA -= A1x;
+    if (cy == 1) cA += A1y; else if (cy == -1) cA -= A1y;
+    if (cz == 1) cA += A1z; else if (cz == -1) cA -= A1z;
+    if (cx != 0) cc += Axx;
+    if (cy != 0) cc += Ayy;
+    if (cz != 0) cc += Azz;
+    T cross = T(0);
+    if (cx * cy == 1) cross += Axy; else if (cx * cy == -1) cross -= Axy;
+    if (cx * cz == 1) cross += Axz; else if (cx * cz == -1) cross -= Axz;
+    if (cy * cz == 1) cross += Ayz; else if (cy * cz == -1) cross -= Ayz;
+    cc += cross + cross;
+#pragma unroll
+    for (int kk = 0; kk < 7; ++kk) {
+      const double hk = h3<Q>(cx, cy, cz, kk) * static_cast<double>(weight<Q, double>(L.c2[i]));
+      if (hk != 0.0) o3 += static_cast<T>(hk) * A3[kk];
+    }
+    const T even = w * (e0 + T(4.5) * cc);
+    const T odd = c3[L.c2[i]] * cA + o3;
+    esum += even;
+    f[i] = even + odd;
+    f[i + H] = even - odd;
+  }
+  f[0] = rho - (esum + esum);
 }
 
 // O4 / reading R6: regularised velocity inlet on a cell of the plane x = 0 (inward normal +x).
@@ -389,39 +536,115 @@ __device__ __forceinline__ void wallmodel_ub(const StepArgs<T>& a, int x, int y,
   ubz = static_cast<T>(r * t2);
 }
 
+// S^FD(x,t) of one cell (Eq. 10): S_ab = (D_a u^_b + D_b u^_a)/2 with central differences of the stored u^ field,
+// periodic wrap; the ghost planes beyond the INLET / OUTLET planes copy those planes (G32).  S = xx, yy, zz, xy, xz, yz.
+template <typename T>
+__device__ __forceinline__ void fd_strain_cell(const StepArgs<T>& a, int x, int y, int z, int type, T (&S)[6]) {
+  const int nx = a.nx, ny = a.ny, nz = a.nz;
+  const int xm = (type == T_INLET) ? x : ((x == 0) ? nx - 1 : x - 1);
+  const int xp = (type == T_OUTLET) ? x : ((x == nx - 1) ? 0 : x + 1);
+  const int ym = (y == 0) ? ny - 1 : y - 1, yp = (y == ny - 1) ? 0 : y + 1;
+  const int zm = (z == 0) ? nz - 1 : z - 1, zp = (z == nz - 1) ? 0 : z + 1;
+  T D[3][3];   // D[a][b] = u^_b(x + e_a) - u^_b(x - e_a)
+#pragma unroll
+  for (int b = 0; b < 3; ++b) {
+    const T* u = a.uhat + b * a.N;
+    D[0][b] = u[cell_index(xp, y, z, nx, ny)] - u[cell_index(xm, y, z, nx, ny)];
+    D[1][b] = u[cell_index(x, yp, z, nx, ny)] - u[cell_index(x, ym, z, nx, ny)];
+    D[2][b] = u[cell_index(x, y, zp, nx, ny)] - u[cell_index(x, y, zm, nx, ny)];
+  }
+  S[0] = T(0.5) * D[0][0];
+  S[1] = T(0.5) * D[1][1];
+  S[2] = T(0.5) * D[2][2];
+  S[3] = T(0.25) * (D[0][1] + D[1][0]);
+  S[4] = T(0.25) * (D[0][2] + D[2][0]);
+  S[5] = T(0.25) * (D[1][2] + D[2][1]);
+}
+
+// u^ = (1-d) sum c f / sum f + d u^B of one cell (Eq. 12), the field the FD strain is taken of (G30).
+template <int Q, typename T>
+__device__ __forceinline__ void uhat_of(const T (&f)[Q], T d, T ubx, T uby, T ubz, T& ux, T& uy, T& uz) {
+  constexpr Stencil<Q> L{};
+  constexpr int H = (Q - 1) / 2;
+  T rho = f[0], jx = T(0), jy = T(0), jz = T(0);
+#pragma unroll
+  for (int i = 1; i <= H; ++i) {
+    rho += f[i] + f[i + H];
+    const T df = f[i] - f[i + H];
+    if (L.c[i][0] == 1) jx += df; else if (L.c[i][0] == -1) jx -= df;
+    if (L.c[i][1] == 1) jy += df; else if (L.c[i][1] == -1) jy -= df;
+    if (L.c[i][2] == 1) jz += df; else if (L.c[i][2] == -1) jz -= df;
+  }
+  const T inv_rho = rcp_(rho);
+  const T keep = T(1) - d;
+  ux = keep * (jx * inv_rho) + d * ubx;
+  uy = keep * (jy * inv_rho) + d * uby;
+  uz = keep * (jz * inv_rho) + d * ubz;
+}
+
 // ---- the per-cell step (scalar kernel; list blocks of the vector kernel) ------------------------------
-// One non-SOLID cell of any type: pull (MODE != COLLIDE), wall model, collide (MODE != STREAM), store.
-template <int Q, typename T, int MODE>
+// One non-SOLID cell of any type: pull (modes that pull), wall model, then collide + store (collide modes), store S_t
+// (MODE_STREAM) or store u^ (MODE_UHAT_*).
+template <int Q, typename T, int MODE, int COLL>
 __device__ __forceinline__ void step_cell_any(const StepArgs<T>& a, int x, int y, int z, uint8_t cls) {
-  constexpr bool PULL = (MODE != MODE_COLLIDE);
+  constexpr bool PULL = mode_pulls(MODE);
   const long long self = cell_index(x, y, z, a.nx, a.ny);
   const int type = cls & CLS_TYPE;
   T d = T(0), ubx = T(0), uby = T(0), ubz = T(0);
+  const bool wm = (type == T_WM) && a.wm_enable;
   if (MODE != MODE_STREAM) {
     if (a.d != nullptr) d = __ldg(a.d + self);
-    if (type == T_WM && a.wm_enable) wallmodel_ub<Q, T, PULL>(a, x, y, z, cls, ubx, uby, ubz);
+    if (wm) wallmodel_ub<Q, T, PULL>(a, x, y, z, cls, ubx, uby, ubz);
   }
   T f[Q];
   load_state<Q, T, PULL>(a, x, y, z, cls, f);
-  if (MODE != MODE_STREAM) collide_cell<Q, T>(f, d, ubx, uby, ubz, a.tau0, a.smago_k);
+  if (mode_uhat(MODE)) {
+    T ux, uy, uz;
+    uhat_of<Q, T>(f, d, ubx, uby, ubz, ux, uy, uz);
+    a.uhat[self] = ux;
+    a.uhat[a.N + self] = uy;
+    a.uhat[2 * a.N + self] = uz;
+    return;
+  }
+  if (mode_collides(MODE)) {
+    if (COLL == COLL_HRR) {
+      T S[6];
+      fd_strain_cell<T>(a, x, y, z, type, S);
+      collide_cell_hrr<Q, T>(f, d, ubx, uby, ubz, a.tau0, a.smago_k, wm ? T(0) : a.sigma, S);   // sigma = 0: l.131
+    } else {
+      collide_cell<Q, T>(f, d, ubx, uby, ubz, a.tau0, a.smago_k);
+    }
+  }
   store_cell<Q, T>(a, x, y, z, f);
 }
 
-// grid (ceil(nx/bx), ceil(ny/by), nz), block (bx, by): thread <-> cell, x fastest (coalesced rows).
-// Fallback for row lengths the vector kernel does not take.
+// SOLID cell in the per-cell paths: zeros over its lattice slots (never read; keeps sectors whole) / u^ = 0 (resting wall)
 template <int Q, typename T, int MODE>
+__device__ __forceinline__ void solid_cell_any(const StepArgs<T>& a, long long self) {
+  if (mode_uhat(MODE)) {
+    a.uhat[self] = T(0);
+    a.uhat[a.N + self] = T(0);
+    a.uhat[2 * a.N + self] = T(0);
+  } else {
+    store_zero<Q, T>(a, self);
+  }
+}
+
+// grid (ceil(nx/bx), ceil(ny/by), slab), block (bx, by): thread <-> cell, x fastest (coalesced rows).
+// Fallback for row lengths the vector kernel does not take.
+template <int Q, typename T, int MODE, int COLL>
 __global__ void __launch_bounds__(256) k_step(const __grid_constant__ StepArgs<T> a) {
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
-  const int z = blockIdx.z;
+  const int z = a.z0 + blockIdx.z;
   if (x >= a.nx || y >= a.ny) return;
   const long long self = cell_index(x, y, z, a.nx, a.ny);
   const uint8_t cls = a.cls[self];
   if ((cls & CLS_TYPE) == T_SOLID) {         // SOLID cells are inert (R5); their slots are never read
-    store_zero<Q, T>(a, self);
+    solid_cell_any<Q, T, MODE>(a, self);
     return;
   }
-  step_cell_any<Q, T, MODE>(a, x, y, z, cls);
+  step_cell_any<Q, T, MODE, COLL>(a, x, y, z, cls);
 }
 
 // ---- the vectorised step kernel (the hot one) ------------------------------------------------------
@@ -434,11 +657,16 @@ __global__ void __launch_bounds__(256) k_step(const __grid_constant__ StepArgs<T
 // cells per thread: 128-bit access for D3Q19 (4 floats / 2 doubles); D3Q27 takes half of that (64-bit access, still
 // whole 32-byte sectors per warp instruction) because 27 x 4 live values leave room for only 8 warps per SM and the
 // kernel then stalls on its own latency (ncu, profiles/: 12.5 % occupancy, 0.27 issue slots per cycle).
-template <int Q, typename T> struct VecOf;
-template <> struct VecOf<19, float> { static constexpr int V = 4; };
-template <> struct VecOf<19, double> { static constexpr int V = 2; };
-template <> struct VecOf<27, float> { static constexpr int V = 2; };
-template <> struct VecOf<27, double> { static constexpr int V = 1; };
+// The HRR form carries 15 more vectors (u^ of the six neighbours) and a longer collision: half the width again.
+template <int Q, typename T, int COLL = COLL_BGK> struct VecOf;
+template <> struct VecOf<19, float, COLL_BGK> { static constexpr int V = 4; };
+template <> struct VecOf<19, double, COLL_BGK> { static constexpr int V = 2; };
+template <> struct VecOf<27, float, COLL_BGK> { static constexpr int V = 2; };
+template <> struct VecOf<27, double, COLL_BGK> { static constexpr int V = 1; };
+template <> struct VecOf<19, float, COLL_HRR> { static constexpr int V = 2; };
+template <> struct VecOf<19, double, COLL_HRR> { static constexpr int V = 1; };
+template <> struct VecOf<27, float, COLL_HRR> { static constexpr int V = 2; };
+template <> struct VecOf<27, double, COLL_HRR> { static constexpr int V = 1; };
 
 template <bool STREAMING>
 __device__ __forceinline__ void ld_vec_t(const float* p, float (&v)[4]) {
@@ -483,19 +711,39 @@ __device__ __forceinline__ void ld_nbmask(const uint32_t* p, uint32_t (&m)[2]) {
 __device__ __forceinline__ void ld_nbmask(const uint32_t* p, uint32_t (&m)[1]) { m[0] = __ldg(p); }
 __host__ __device__ constexpr uint32_t rep_byte(uint32_t b, int n) { return n <= 0 ? 0u : (b | (rep_byte(b, n - 1) << 8)); }
 
+// HRR form, vector path: u^ of the six neighbours of the V cells of a vector.  gu[5 b + {0,1,2,3,4}] = component b at
+// rows y+1, y-1, z+1, z-1 and the own row; gl / gr = the elements left / right of the vector (L1 hits: the
+// neighbouring lanes load those lines).
+template <typename T, int V>
+__device__ __forceinline__ void ld_uhat_nb(const T* pu, long long N, int dyp, int dym, int dzp, int dzm, int exl, int exr,
+                                           T (&gu)[15][V], T (&gl)[3], T (&gr)[3]) {
+#pragma unroll
+  for (int b = 0; b < 3; ++b) {
+    ld_vec_keep(pu + dyp, gu[5 * b + 0]);
+    ld_vec_keep(pu + dym, gu[5 * b + 1]);
+    ld_vec_keep(pu + dzp, gu[5 * b + 2]);
+    ld_vec_keep(pu + dzm, gu[5 * b + 3]);
+    ld_vec_keep(pu, gu[5 * b + 4]);
+    gl[b] = __ldg(pu + exl);
+    gr[b] = __ldg(pu + exr);
+    pu += N;
+  }
+}
+
 // grid (ceil(nx/V/bx), ceil(ny/by), list_z + nz), block (bx, by), bx a power of two <= 32.
 // The first list_z z-slices of the grid do not own a lattice slab: their threads walk the compact list
 // of the cells of SPECIAL sectors (A8 wall model; OUTLET cells next to a wall), one cell per thread: the masked
 // boundary kernel as a block role of the same launch (scheduled first, overlaps with the row blocks).
 // Everything else -- bulk, solid-adjacent (read-side bounce-back), INLET and OUTLET cells -- runs in the vector path.
-template <int Q, typename T, int MODE>
+template <int Q, typename T, int MODE, int COLL>
 __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ StepArgs<T> a) {
   constexpr Stencil<Q> L{};
-  constexpr int V = VecOf<Q, T>::V;
+  constexpr int V = VecOf<Q, T, COLL>::V;
+  constexpr bool HRR = (COLL == COLL_HRR) && mode_collides(MODE);
   constexpr int SV = 32 / static_cast<int>(sizeof(T));      // cells per 32-byte sector
   constexpr int LG = 128 / (V * static_cast<int>(sizeof(T)));  // lanes per 128-byte line
   constexpr unsigned FULL = 0xffffffffu;
-  constexpr bool PULL = (MODE != MODE_COLLIDE);
+  constexpr bool PULL = mode_pulls(MODE);
   const int tx = threadIdx.x;
   if (static_cast<int>(blockIdx.z) < a.list_z) {
     const long long blk = (static_cast<long long>(blockIdx.z) * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
@@ -504,12 +752,12 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
       const int cell = a.list[k];
       const uint8_t c = a.cls[cell];
       if ((c & CLS_TYPE) == T_SOLID) {     // SOLID sector-mate: zeros keep the sector whole
-        store_zero<Q, T>(a, cell);
+        solid_cell_any<Q, T, MODE>(a, cell);
       } else {
         const int plane = a.nx * a.ny;
         const int cz = cell / plane, rem = cell - cz * plane;
         const int cy = rem / a.nx, cx = rem - cy * a.nx;
-        step_cell_any<Q, T, MODE>(a, cx, cy, cz, c);
+        step_cell_any<Q, T, MODE, COLL>(a, cx, cy, cz, c);
       }
     }
     return;
@@ -518,7 +766,7 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
   const int nvec = a.nx / V;
   const int qx = blockIdx.x * blockDim.x + tx;
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
-  const int z = blockIdx.z - a.list_z;
+  const int z = a.z0 + static_cast<int>(blockIdx.z) - a.list_z;
   const bool active = (qx < nvec) && (y < a.ny);
   const int x0 = qx * V;
   const int nx = a.nx, ny = a.ny, nz = a.nz;
@@ -575,10 +823,14 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
   const int xl = (x0 == 0) ? nx - 1 : x0 - 1;            // element left of the vector (periodic)
   const int xr = (x0 + V >= nx) ? 0 : x0 + V;            // element right of the vector
   const int exl = xl - x0, exr = xr - x0;                // relative to the vector start
+  T gu[HRR ? 15 : 1][V], gl[3], gr[3];      // HRR form: u^ of the neighbours (FD strain, Eq. 10)
   if (!PULL) {
     if (mine) {
 #pragma unroll
       for (int i = 0; i < Q; ++i) ld_vec(a.fin + i * N + self, f[i]);
+    }
+    if constexpr (HRR) {
+      if (mine) ld_uhat_nb<T, V>(a.uhat + self, N, dyp, dym, dzp, dzm, exl, exr, gu, gl, gr);
     }
   } else {
     // a vector that is SOLID throughout loads nothing, but the rows its neighbour pulls from (y -+ 1, z -+ 1) may be
@@ -604,6 +856,9 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
       if (L.c[i][0] == 1 && edge_l) e[i] = __ldg(src + exl);
       if (L.c[i][0] == -1 && edge_r) e[i] = __ldg(src + exr);
     }
+    if constexpr (HRR) {
+      if (mine) ld_uhat_nb<T, V>(a.uhat + self, N, dyp, dym, dzp, dzm, exl, exr, gu, gl, gr);
+    }
     // phase 2: realign the rows with c_x = +-1 by one element through the neighbouring lane
 #pragma unroll
     for (int i = 0; i < Q; ++i) {
@@ -623,13 +878,13 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
       }
     }
   }
-  T* pout = a.fout + self;
+  T* pout = mode_uhat(MODE) ? a.uhat + self : a.fout + self;
   if (zero_fill) {
     T zero[V];
 #pragma unroll
     for (int v = 0; v < V; ++v) zero[v] = T(0);
 #pragma unroll
-    for (int i = 0; i < Q; ++i) {
+    for (int i = 0; i < (mode_uhat(MODE) ? 3 : Q); ++i) {
       st_vec(pout, zero);
       pout += N;
     }
@@ -657,13 +912,47 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
 #pragma unroll
     for (int i = 0; i < Q; ++i) f[i][0] = fc[i];
   }
-  if (MODE != MODE_STREAM) {
+  if constexpr (mode_uhat(MODE)) {                            // first pass of the HRR form: u^(x,t) (Eq. 12), SOLID cells 0
+    T uo[3][V];
 #pragma unroll
     for (int v = 0; v < V; ++v) {
       T fc[Q];
 #pragma unroll
       for (int i = 0; i < Q; ++i) fc[i] = f[i][v];
-      collide_cell<Q, T>(fc, d[v], T(0), T(0), T(0), a.tau0, a.smago_k);
+      uhat_of<Q, T>(fc, d[v], T(0), T(0), T(0), uo[0][v], uo[1][v], uo[2][v]);
+      if (solid_bits & (1u << v)) uo[0][v] = uo[1][v] = uo[2][v] = T(0);
+    }
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+      st_vec(pout, uo[b]);
+      pout += N;
+    }
+    return;
+  }
+  if constexpr (mode_collides(MODE)) {
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      T fc[Q];
+#pragma unroll
+      for (int i = 0; i < Q; ++i) fc[i] = f[i][v];
+      if constexpr (HRR) {
+        T D[3][3];   // D[a][b] = u^_b(x + e_a) - u^_b(x - e_a); G32: the planes beyond INLET / OUTLET copy those planes
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+          T left = (v > 0) ? gu[5 * b + 4][v > 0 ? v - 1 : 0] : gl[b];
+          T right = (v < V - 1) ? gu[5 * b + 4][v < V - 1 ? v + 1 : 0] : gr[b];
+          if (v == 0 && inlet0) left = gu[5 * b + 4][0];
+          if (v == V - 1 && outletN) right = gu[5 * b + 4][V - 1];
+          D[0][b] = right - left;
+          D[1][b] = gu[5 * b + 0][v] - gu[5 * b + 1][v];
+          D[2][b] = gu[5 * b + 2][v] - gu[5 * b + 3][v];
+        }
+        const T S[6] = {T(0.5) * D[0][0], T(0.5) * D[1][1], T(0.5) * D[2][2], T(0.25) * (D[0][1] + D[1][0]),
+                        T(0.25) * (D[0][2] + D[2][0]), T(0.25) * (D[1][2] + D[2][1])};
+        collide_cell_hrr<Q, T>(fc, d[v], T(0), T(0), T(0), a.tau0, a.smago_k, a.sigma, S);
+      } else {
+        collide_cell<Q, T>(fc, d[v], T(0), T(0), T(0), a.tau0, a.smago_k);
+      }
 #pragma unroll
       for (int i = 0; i < Q; ++i) f[i][v] = fc[i];
     }
