@@ -1,6 +1,6 @@
 /* =====================================================================================
  * lbm.h -- C ABI of the B200-native lattice Boltzmann hot path of arxiv 2506.21804
- * (BGK + Smagorinsky LES + homogenised-LBM porosity; D3Q19 / D3Q27; fp32 / fp64).
+ * (BGK or HRR collision + Smagorinsky LES + homogenised-LBM porosity; D3Q19 / D3Q27; fp32 / fp64).
  *
  * Library: paper_2506_21804_b200/liblbm_b200.so (CUDA, sm_100a).  Every step of the path runs
  * in the library's own kernels; there is no CPU fallback: every call fails with LBM_ECUDA when no

@@ -679,6 +679,10 @@ __device__ __forceinline__ void ld_vec_t(const float* p, float (&v)[2]) {
   v[0] = t.x; v[1] = t.y;
 }
 template <bool STREAMING>
+__device__ __forceinline__ void ld_vec_t(const float* p, float (&v)[1]) {
+  v[0] = STREAMING ? __ldcs(p) : __ldg(p);
+}
+template <bool STREAMING>
 __device__ __forceinline__ void ld_vec_t(const double* p, double (&v)[2]) {
   const double2 t = STREAMING ? __ldcs(reinterpret_cast<const double2*>(p)) : __ldg(reinterpret_cast<const double2*>(p));
   v[0] = t.x; v[1] = t.y;
@@ -693,6 +697,7 @@ __device__ __forceinline__ void st_vec(float* p, const float (&v)[4]) {
   __stcs(reinterpret_cast<float4*>(p), make_float4(v[0], v[1], v[2], v[3]));
 }
 __device__ __forceinline__ void st_vec(float* p, const float (&v)[2]) { __stcs(reinterpret_cast<float2*>(p), make_float2(v[0], v[1])); }
+__device__ __forceinline__ void st_vec(float* p, const float (&v)[1]) { __stcs(p, v[0]); }
 __device__ __forceinline__ void st_vec(double* p, const double (&v)[2]) {
   __stcs(reinterpret_cast<double2*>(p), make_double2(v[0], v[1]));
 }

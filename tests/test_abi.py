@@ -33,11 +33,20 @@ def test_library_exports_every_declared_symbol(lib):
         assert hasattr(lib, name), name
 
 
-def test_params_struct_layout_matches_header():
-    # typedef struct { double tau0; double cs_smago; int use_hlbm; double u_in[3]; int wm_enable; double wm_kappa; double wm_E; }
+def test_params_struct_layout_matches_header(tmp_path):
+    """the ctypes mirror against the C compiler's view of include/lbm.h (offsetof / sizeof printed by a gcc-built probe)"""
+    import subprocess
     S = P.LbmParams
-    assert ctypes.sizeof(S) == 72
-    assert [getattr(S, f).offset for f, _ in S._fields_] == [0, 8, 16, 24, 48, 56, 64]
+    names = [f for f, _ in S._fields_]
+    assert names == ["tau0", "cs_smago", "use_hlbm", "u_in", "wm_enable", "wm_kappa", "wm_E", "collision", "sigma"]
+    src = tmp_path / "probe.c"
+    src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "lbm.h"\nint main(void){printf("%zu", sizeof(lbm_params));'
+                   + "".join('printf(" %%zu", offsetof(lbm_params, %s));' % n for n in names) + "return 0;}\n")
+    exe = tmp_path / "probe"
+    subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
+    out = [int(t) for t in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()]
+    assert ctypes.sizeof(S) == out[0] == 88
+    assert [getattr(S, f).offset for f in names] == out[1:] == [0, 8, 16, 24, 48, 56, 64, 72, 80]
 
 
 def test_bad_arguments_are_rejected_without_touching_the_gpu(lib):
