@@ -36,7 +36,7 @@ def _axis_crop(lo, n, closed):
     return idx, lo - a
 
 
-def _check_windows(cfg, dtype, windows, closed_axes):
+def _check_windows(cfg, dtype, windows, closed_axes, steps=S):
     nz, ny, nx = cfg["shape"]
     Q = cfg["Q"]
     npdt = NP_DTYPE[dtype]
@@ -46,7 +46,7 @@ def _check_windows(cfg, dtype, windows, closed_axes):
     par = P.LbmParams(**cfg["params"])
     with P.LBM(Q, nx, ny, nz, dtype) as sim:
         sim.set_fields(f, d, cfg["flags"])                  # host pointers, library defaults = bench configuration
-        sim.step(S, par)
+        sim.step(steps, par)
         out = torch.empty((Q, nz, ny, nx), dtype=torch.float32 if dtype == "f32" else torch.float64, device="cuda")
         sim.get_populations(out)
         rho = torch.empty((nz, ny, nx), dtype=out.dtype, device="cuda")
@@ -62,7 +62,7 @@ def _check_windows(cfg, dtype, windows, closed_axes):
         fc = np.ascontiguousarray(f[(slice(None),) + sel]).astype(np.float64)
         dc = None if d is None else np.ascontiguousarray(d[sel]).astype(np.float64)
         flc = None if cfg["flags"] is None else np.ascontiguousarray(cfg["flags"][sel])
-        ref = O.step(fc, d=dc, flags=flc, nsteps=S, nthreads=min(O.max_threads(), 8), **cfg["params"])
+        ref = O.step(fc, d=dc, flags=flc, nsteps=steps, nthreads=min(O.max_threads(), 8), **cfg["params"])
         inner = (slice(None), slice(wz, wz + W), slice(wy, wy + W), slice(wx, wx + W))
         refw = ref[inner]
         gz, gy, gx = iz[wz:wz + W], iy[wy:wy + W], ix[wx:wx + W]
@@ -126,6 +126,32 @@ def test_config4_full_size_windows():
     wins = [tuple(min(max(v, 0), 512 - W) for v in w) for w in wins]
     wins += [(0, 0, 0), (504, 504, 504), (250, 0, 504)]
     _check_windows(cfg, "f32", wins, (False, False, False))
+
+
+# HRR form at the sizes bench.py's *_hrr workloads time.  The FD strain reads u^ of the neighbours, whose pull reaches
+# one cell further: information moves <= 2 cells per step (3 along a wall-model normal), so 6 steps stay inside the margin 22.
+HRR = dict(collision=1, sigma=0.7)      # = bench.py's HRR workloads
+
+
+def test_config3_hrr_full_size_windows():
+    cfg = I.make_config(3)
+    cfg["params"] = dict(cfg["params"], **HRR)
+    nz, ny, nx = cfg["shape"]
+    wins = [(1, 10, 0), (1, 100, nx - W), (nz - 1 - W, 50, 200), (1, 60, 150), (60, 90, 190), (30, ny - 4, 100),
+            (20, 40, 120), (5, 130, 250)]
+    _check_windows(cfg, "f32", wins, (True, False, True), steps=6)
+
+
+def test_config4_hrr_full_size_windows():
+    cfg = I.make_config(4)
+    cfg["params"] = dict(cfg["params"], **HRR)
+    fl = cfg["flags"]
+    rng = np.random.default_rng(44)
+    solid = np.argwhere(fl == I.SOLID)
+    wins = [tuple(int(v) for v in solid[k] - 2) for k in rng.integers(0, len(solid), 5)]
+    wins = [tuple(min(max(v, 0), 512 - W) for v in w) for w in wins]
+    wins += [(0, 0, 0), (504, 504, 504), (250, 0, 504)]
+    _check_windows(cfg, "f32", wins, (False, False, False), steps=6)
 
 
 # ---- T2: invariants after the configs' full step counts ------------------------------------------
