@@ -9,12 +9,12 @@ these generators take their structure and stand in for them (DESIGN.md "Input re
 
 All randomness: numpy.random.Generator(numpy.random.PCG64(seed)), seed = 1000 + config number.
 Array layouts: rho[nz,ny,nx], u[3,nz,ny,nx], d[nz,ny,nx] float64; flags[nz,ny,nx] uint8.
-Flag byte: low nibble {0 FLUID, 1 SOLID, 2 INLET, 3 OUTLET, 4 WALLMODEL}; WALLMODEL carries the
+Flag byte: low nibble {0 FLUID, 1 SOLID, 2 INLET, 3 OUTLET, 4 WALLMODEL, 5 MOVINGWALL}; WALLMODEL carries the
 wall-normal code in the high nibble {0:+x,1:-x,2:+y,3:-y,4:+z,5:-z}.
 """
 import numpy as np
 
-FLUID, SOLID, INLET, OUTLET, WALLMODEL = 0, 1, 2, 3, 4
+FLUID, SOLID, INLET, OUTLET, WALLMODEL, MOVINGWALL = 0, 1, 2, 3, 4, 5
 WM_FLOOR = 0x44  # WALLMODEL with normal +z
 
 
@@ -220,4 +220,30 @@ def make_config(number, shape=None, k_max=None, n_modes=None):
         u[:, (flags & 0x0F) == SOLID] = 0.0
         return dict(number=4, Q=27, dtype="f32", shape=tuple(shape), steps=200, rho=np.ones(shape), u=u, d=None,
                     flags=flags, params=dict(tau0=tau_les, cs_smago=0.12, use_hlbm=0))
+    if number == 6:
+        # lid-driven cavity (the paper's scaling benchmark; not a BASELINE.json config):
+        # closed box, five resting walls, the z = nz-1 plane moves with u_wall = (0.05, 0, 0); fluid at rest, rho = 1;
+        # fp32 as in the paper ("base arithmetic type ... single-precision"); tau0 / Cs are this build's choice.
+        shape = tuple(shape or (512, 512, 512))
+        return dict(number=6, Q=19, dtype="f32", shape=shape, steps=200, rho=np.ones(shape), u=np.zeros((3,) + shape),
+                    d=None, flags=cavity_flags(shape),
+                    params=dict(tau0=0.52, cs_smago=0.1, use_hlbm=0, u_wall=(0.05, 0.0, 0.0)))
     raise ValueError("unknown config %r" % number)
+
+
+def cavity_flags(shape):
+    """closed box: SOLID on x = 0, nx-1, y = 0, ny-1, z = 0; MOVINGWALL on the whole plane z = nz-1 (the lid)"""
+    flags = np.zeros(shape, dtype=np.uint8)
+    flags[0] = SOLID
+    flags[:, 0] = SOLID
+    flags[:, -1] = SOLID
+    flags[:, :, 0] = SOLID
+    flags[:, :, -1] = SOLID
+    flags[-1] = MOVINGWALL
+    return flags
+
+
+def is_wall(flags):
+    """cells that are walls (resting SOLID or MOVINGWALL): inert, excluded from every comparison of fluid values"""
+    t = flags & 0x0F
+    return (t == SOLID) | (t == MOVINGWALL)

@@ -20,6 +20,10 @@
 //   O3 stream              Eq. 6 left-hand side (l.70); halfway bounce-back (G14/R5);
 //                          zero-gradient outlet (G16/R7)
 //   O4 inlet fix-up        l.155 "regularized local velocity boundary condition" (G15/R6)
+//   O3m moving wall       lid of the "established lid-driven cavity benchmark" (l.214): halfway bounce-back
+//                          off a wall moving with u_w: + 2 w_i rho_w (c_i.u_w)/c_s^2 on the returned population, rho_w = 1
+//                          (reading G33; the paper does not say how its lid is imposed -> PARITY UNPINNED against the
+//                          paper, pinned as the textbook rule by M1-M4 in tests/test_oracle_cavity.py)
 //   O6 moments             l.97 "fluid velocity moment u" (G19)
 //   O2h collide, HRR form  (params.collision = 1; the paper's own collision)
 //                          Eq. 6 (l.70) with f~(1) of Eq. 7 (l.74); Eq. 8-9 (l.81-86) regularised
@@ -46,7 +50,7 @@
 //
 // Layouts (all row-major, x fastest): f[Q][nz][ny][nx] double, d[nz][ny][nx] double,
 // flag[nz][ny][nx] uint8.  Cell index = (z*ny + y)*nx + x.
-// Flag byte: low nibble type {0 FLUID,1 SOLID,2 INLET,3 OUTLET,4 WALLMODEL}; for WALLMODEL the
+// Flag byte: low nibble type {0 FLUID,1 SOLID,2 INLET,3 OUTLET,4 WALLMODEL,5 MOVINGWALL}; for WALLMODEL the
 // high nibble is the wall-normal code {0:+x,1:-x,2:+y,3:-y,4:+z,5:-z} (wall -> fluid).
 // =====================================================================================
 #include <cmath>
@@ -61,7 +65,7 @@
 namespace {
 
 constexpr int QMAX = 27;
-enum CellType : int { FLUID = 0, SOLID = 1, INLET = 2, OUTLET = 3, WALLMODEL = 4 };
+enum CellType : int { FLUID = 0, SOLID = 1, INLET = 2, OUTLET = 3, WALLMODEL = 4, MOVINGWALL = 5 };
 
 struct Lattice {
   int Q = 0;
@@ -131,9 +135,12 @@ struct Params {           // the oracle's own copy of the step parameters (not s
   double wm_E;
   int collision;          // 0: BGK form of Eq. 6 (G1); 1: hybrid recursive-regularised (Eq. 6-11)
   double sigma;           // Eq. 7 hybridisation factor, in [0,1]
+  double u_wall[3];       // velocity of the MOVINGWALL cells (lid of the lid-driven cavity, l.214; reading G33)
 };
 
 inline int cell_type(uint8_t flag) { return flag & 0x0F; }
+// a wall cell (resting SOLID or MOVINGWALL): inert, never collided, bounces populations back (R5, G33)
+inline bool is_wall(int type) { return type == SOLID || type == MOVINGWALL; }
 
 // A4.  Eq. 11 (l.94) truncated after the H(2) term, c_s^2 = 1/3:
 // f_i^eq = w_i rho (1 + 3 c.u + 4.5 (c.u)^2 - 1.5 u.u)
@@ -447,7 +454,7 @@ int orc_init_equilibrium(int Q, int64_t N, const double* rho, const double* u, d
 // nthreads <= 1: serial.  nthreads > 1: the same loop nests with "omp parallel for" over z.
 // Returns 0, or -1 on bad arguments.
 int orc_step(int Q, int nx, int ny, int nz, double* f, const double* d, const uint8_t* flags,
-             const double* par /* tau0, cs, use_hlbm, uin0, uin1, uin2, wm_enable, kappa, E, collision, sigma */,
+             const double* par /* tau0, cs, use_hlbm, uin0, uin1, uin2, wm_enable, kappa, E, collision, sigma, uwall0, uwall1, uwall2 */,
              int nsteps, int nthreads) {
   Lattice L;
   if (!make_lattice(Q, L)) return -1;
@@ -457,6 +464,7 @@ int orc_step(int Q, int nx, int ny, int nz, double* f, const double* d, const ui
   p.u_in[0] = par[3];  p.u_in[1] = par[4];  p.u_in[2] = par[5];
   p.wm_enable = (par[6] != 0.0);  p.wm_kappa = par[7];  p.wm_E = par[8];
   p.collision = static_cast<int>(par[9]);  p.sigma = par[10];
+  p.u_wall[0] = par[11];  p.u_wall[1] = par[12];  p.u_wall[2] = par[13];
   if (!(p.tau0 > 0.5) || p.cs_smago < 0.0) return -1;
   if (p.collision != 0 && p.collision != 1) return -1;
   if (p.collision == 1 && !(p.sigma >= 0.0 && p.sigma <= 1.0)) return -1;
@@ -498,7 +506,7 @@ int orc_step(int Q, int nx, int ny, int nz, double* f, const double* d, const ui
       const int64_t s = (static_cast<int64_t>(z2) * ny + y2c) * nx + x2;
       double* ub = &uB[3 * k];
       ub[0] = ub[1] = ub[2] = 0.0;
-      if (cell_type(flags[s]) == SOLID) continue;                          // step 1
+      if (is_wall(cell_type(flags[s]))) continue;                          // step 1
       double fc[QMAX], rho2, u2[3];
       for (int i = 0; i < Q; ++i) fc[i] = cur[i * N + s];
       raw_moments(L, fc, rho2, u2);                                        // step 2
@@ -518,7 +526,9 @@ int orc_step(int Q, int nx, int ny, int nz, double* f, const double* d, const ui
       for (int64_t x = 0; x < N; ++x) {
         const int type = flags ? cell_type(flags[x]) : FLUID;
         double uh[3] = {0.0, 0.0, 0.0};
-        if (type != SOLID) {
+        if (type == MOVINGWALL) {
+          for (int a = 0; a < 3; ++a) uh[a] = p.u_wall[a];                 // the wall's own velocity (G33)
+        } else if (type != SOLID) {
           double fc[QMAX], rho, u[3];
           for (int i = 0; i < Q; ++i) fc[i] = cur[i * N + x];
           raw_moments(L, fc, rho, u);
@@ -541,7 +551,7 @@ int orc_step(int Q, int nx, int ny, int nz, double* f, const double* d, const ui
         for (int xx = 0; xx < nx; ++xx) {
           const int64_t x = (static_cast<int64_t>(z) * ny + y) * nx + xx;
           const int type = flags ? cell_type(flags[x]) : FLUID;
-          if (type == SOLID) {
+          if (is_wall(type)) {
             for (int i = 0; i < Q; ++i) fstar[i * N + x] = cur[i * N + x];
             continue;
           }
@@ -586,7 +596,7 @@ int orc_step(int Q, int nx, int ny, int nz, double* f, const double* d, const ui
         for (int xx = 0; xx < nx; ++xx) {
           const int64_t x = (static_cast<int64_t>(z) * ny + y) * nx + xx;
           const int type = flags ? cell_type(flags[x]) : FLUID;
-          if (type == SOLID) {
+          if (is_wall(type)) {
             for (int i = 0; i < Q; ++i) nxt[i * N + x] = cur[i * N + x];
             continue;
           }
@@ -597,8 +607,11 @@ int orc_step(int Q, int nx, int ny, int nz, double* f, const double* d, const ui
             const int sy = wrap(y - L.c[i][1], ny);
             const int sz = wrap(z - L.c[i][2], nz);
             const int64_t s = (static_cast<int64_t>(sz) * ny + sy) * nx + sx;
-            const bool solid = flags && cell_type(flags[s]) == SOLID;
-            nxt[i * N + x] = solid ? fstar[L.opp[i] * N + x] : fstar[i * N + s];
+            const int stype = flags ? cell_type(flags[s]) : FLUID;
+            double v = is_wall(stype) ? fstar[L.opp[i] * N + x] : fstar[i * N + s];
+            if (stype == MOVINGWALL)   // moving-wall bounce-back (G33): + 2 w_i rho_w (c_i . u_w) / c_s^2, rho_w = 1, c_i = wall -> fluid
+              v += 6.0 * L.w[i] * (L.c[i][0] * p.u_wall[0] + L.c[i][1] * p.u_wall[1] + L.c[i][2] * p.u_wall[2]);
+            nxt[i * N + x] = v;
           }
         }
 
@@ -643,7 +656,7 @@ int orc_totals(int Q, int64_t N, const double* f, const uint8_t* flags, double* 
   if (!make_lattice(Q, L)) return -1;
   for (int k = 0; k < 5; ++k) out[k] = 0.0;
   for (int64_t x = 0; x < N; ++x) {
-    if (flags && cell_type(flags[x]) == SOLID) continue;
+    if (flags && is_wall(cell_type(flags[x]))) continue;
     double fc[QMAX], r, uc[3];
     for (int i = 0; i < Q; ++i) fc[i] = f[i * N + x];
     raw_moments(L, fc, r, uc);

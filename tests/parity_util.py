@@ -36,7 +36,7 @@ def field_error(got, ref, mask=None):
 def nonsolid(cfg):
     if cfg["flags"] is None:
         return None
-    return (cfg["flags"] & 0x0F) != I.SOLID
+    return ~I.is_wall(cfg["flags"])
 
 
 def crop_config(cfg, f, d, z0, y0, x0, sz, sy, sx):
