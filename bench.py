@@ -50,6 +50,10 @@ WORKLOADS["config3_urban_channel_384x192x128_f64_hrr"] = (3, None, "f64", HRR)
 WORKLOADS["config2_les_periodic_256_f32_hrr"] = (2, None, "f32", HRR)
 WORKLOADS["config4_d3q27_spheres_512_f32_hrr"] = (4, None, "f32", HRR)
 WORKLOADS["config5_urban_cube_512_f32_hrr"] = (5, (512, 512, 512), "f32", HRR)
+# lid-driven cavity, the paper's own scaling benchmark (fp32): closed box, moving lid
+for _n in (256, 512, 640):
+    WORKLOADS["cavity_%d_f32" % _n] = (6, (_n, _n, _n), "f32")
+WORKLOADS["cavity_512_f32_hrr"] = (6, (512, 512, 512), "f32", HRR)
 DEFAULT_WORKLOAD = "config3_urban_channel_384x192x128_f32"
 
 
@@ -161,7 +165,7 @@ def cpu_oracle_time(cfg_number, sample_shape, nsteps, nthreads, extra):
     from oracle import oracle as O
     cfg = make_cfg(cfg_number, sample_shape, extra)
     f = O.init_equilibrium(cfg["Q"], cfg["rho"], cfg["u"])
-    nonsolid = f[0].size if cfg["flags"] is None else int(((cfg["flags"] & 15) != I.SOLID).sum())
+    nonsolid = f[0].size if cfg["flags"] is None else int((~I.is_wall(cfg["flags"])).sum())
     O.step(f, d=cfg["d"], flags=cfg["flags"], nsteps=1, nthreads=nthreads, **cfg["params"])     # warm-up
     t0 = time.perf_counter()
     O.step(f, d=cfg["d"], flags=cfg["flags"], nsteps=nsteps, nthreads=nthreads, **cfg["params"])
@@ -182,12 +186,12 @@ def run_reference(args, rank, world):
     if number == 1:
         sample = (32, 32, 32)
     else:
-        base = {2: (256, 256, 256), 3: (128, 192, 384), 4: (512, 512, 512), 5: shape}[number]
+        base = {2: (256, 256, 256), 3: (128, 192, 384), 4: (512, 512, 512), 5: shape, 6: shape}[number]
         scale = min(1.0, (cells_budget / float(np.prod(base))) ** (1.0 / 3.0))
         sample = tuple(max(16, int(round(b * scale / 8)) * 8) for b in base)
     cfg = make_cfg(number, sample, extra)
     f = O.init_equilibrium(cfg["Q"], cfg["rho"], cfg["u"])
-    nonsolid = f[0].size if cfg["flags"] is None else int(((cfg["flags"] & 15) != I.SOLID).sum())
+    nonsolid = f[0].size if cfg["flags"] is None else int((~I.is_wall(cfg["flags"])).sum())
     kw = dict(d=cfg["d"], flags=cfg["flags"], nthreads=cores, **cfg["params"])
     f = O.step(f, nsteps=args.warmup, **kw)
     t0 = time.perf_counter()

@@ -43,7 +43,8 @@ struct lbm_ctx {
   void* cub_tmp;
   size_t cub_tmp_bytes;
   int* list_count_dev;
-  unsigned long long* counters;  // device [4]
+  unsigned long long* counters;  // device [5]
+  long long n_moving;            // MOVINGWALL cells of the accepted geometry
   double* totals_dev;            // device [5]
   void* staging;         // host<->device bounce buffer, grown on demand
   size_t staging_bytes;
@@ -143,6 +144,7 @@ lbm::StepArgs<T> make_args(const lbm_ctx* c, const lbm_params* p, int in, int ou
   a.z0 = 0;
   a.uhat = static_cast<T*>(c->uhat);
   a.sigma = p ? static_cast<T>(p->sigma) : T(1);
+  for (int k = 0; k < 3; ++k) a.u_wall[k] = p ? static_cast<T>(p->u_wall[k]) : T(0);
   if (p) {
     a.tau0 = static_cast<T>(p->tau0);
     a.smago_k = static_cast<T>(18.0 * 1.4142135623730951 * p->cs_smago * p->cs_smago);
@@ -176,7 +178,7 @@ void launch_dims_vec(const lbm_ctx* c, dim3& grid, dim3& block) {
 
 // One launch of a step kernel over the z-slices [z0, z0 + nzs) (+ the list blocks when with_list), lattice `in` -> `out`.
 template <int Q, typename T, int MODE, int COLL>
-int launch_one(lbm_ctx* c, const lbm_params* p, int in, int out, int z0, int nzs, bool with_list) {
+int launch_one(lbm_ctx* c, const lbm_params* p, int in, int out, int z0, int nzs, bool with_list, bool may_meet_lid = true) {
   dim3 grid, block;
   lbm::StepArgs<T> a = make_args<T>(c, p, in, out);
   a.z0 = z0;
@@ -190,7 +192,8 @@ int launch_one(lbm_ctx* c, const lbm_params* p, int in, int out, int z0, int nzs
     }
     grid.z = nzs + a.list_z;
     if (grid.z == 0) return LBM_OK;
-    lbm::k_step_vec<Q, T, MODE, COLL><<<grid, block, 0, c->stream>>>(a);
+    if (c->n_moving > 0 && may_meet_lid && lbm::mode_pulls(MODE)) lbm::k_step_vec<Q, T, MODE, COLL, true><<<grid, block, 0, c->stream>>>(a);
+    else                                          lbm::k_step_vec<Q, T, MODE, COLL, false><<<grid, block, 0, c->stream>>>(a);
   } else {
     if (nzs == 0) return LBM_OK;
     launch_dims(c, grid, block);
@@ -234,6 +237,20 @@ int launch_hrr_t(lbm_ctx* c, const lbm_params* p, int in, int out) {
   return LBM_OK;
 }
 
+// The timed BGK step.  With a moving lid (MOVINGWALL cells live on the plane z = nz-1 only) the slices that can meet it
+// (z = nz-2, nz-1 and, through the periodic wrap, 0) take the kernel variant that looks the neighbour's class up; the bulk
+// runs the plain variant: three launches instead of one.
+template <int Q, typename T>
+int launch_bgk_pull_t(lbm_ctx* c, const lbm_params* p, int in, int out) {
+  const int nz = c->nz;
+  if (c->n_moving == 0 || nz < 8)
+    return launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 0, nz, true);
+  int rc = launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 1, nz - 3, true, false);
+  if (rc == LBM_OK) rc = launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, nz - 2, 2, false);
+  if (rc == LBM_OK) rc = launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 0, 1, false);
+  return rc;
+}
+
 template <int Q, typename T>
 int launch_step_t(lbm_ctx* c, const lbm_params* p, int mode) {
   const int in = c->cur, out = 1 - c->cur;
@@ -246,7 +263,7 @@ int launch_step_t(lbm_ctx* c, const lbm_params* p, int mode) {
       break;
     case lbm::MODE_STREAM_COLLIDE:
       rc = hrr ? launch_hrr_t<Q, T, lbm::MODE_UHAT_PULL, lbm::MODE_STREAM_COLLIDE>(c, p, in, out)
-               : launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 0, c->nz, true);
+               : launch_bgk_pull_t<Q, T>(c, p, in, out);
       break;
     default:
       rc = launch_one<Q, T, lbm::MODE_STREAM, lbm::COLL_BGK>(c, p, in, out, 0, c->nz, true);
@@ -371,18 +388,18 @@ int classify(lbm_ctx* c, const uint8_t* cell_flags) {
   } else {
     LBM_CUDA(c, cudaMemsetAsync(c->flags_raw, 0, c->N, c->stream));
   }
-  LBM_CUDA(c, cudaMemsetAsync(c->counters, 0, 4 * sizeof(unsigned long long), c->stream));
+  LBM_CUDA(c, cudaMemsetAsync(c->counters, 0, 5 * sizeof(unsigned long long), c->stream));
   dim3 grid, block;
   launch_dims(c, grid, block);
   if (c->Q == 19) lbm::k_classify<19><<<grid, block, 0, c->stream>>>(c->flags_raw, c->cls_alt, c->nx, c->ny, c->nz, c->counters);
   else            lbm::k_classify<27><<<grid, block, 0, c->stream>>>(c->flags_raw, c->cls_alt, c->nx, c->ny, c->nz, c->counters);
   LBM_CUDA(c, cudaGetLastError());
   c->launches++;
-  unsigned long long h[4];
+  unsigned long long h[5];
   LBM_CUDA(c, cudaMemcpyAsync(h, c->counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
   LBM_CUDA(c, cudaStreamSynchronize(c->stream));
   if (h[0] != 0)
-    return fail(c, LBM_EINVAL, "cell_flags: %llu invalid flag byte(s) (type > 4, bad high nibble, INLET off x=0 or OUTLET off x=nx-1)", h[0]);
+    return fail(c, LBM_EINVAL, "cell_flags: %llu invalid flag byte(s) (type > 5, bad high nibble, INLET off x=0, OUTLET off x=nx-1 or MOVINGWALL off z=nz-1)", h[0]);
   // compact list of the cells the vector kernel leaves to its list blocks
   const int SV = 32 / c->dtype;        // cells per 32-byte sector of a population row
   long long n_list = 0;
@@ -432,6 +449,7 @@ int classify(lbm_ctx* c, const uint8_t* cell_flags) {
   c->launches++;
   c->n_solid = static_cast<long long>(h[1]);
   c->n_masked = static_cast<long long>(h[2]);
+  c->n_moving = static_cast<long long>(h[4]);
   return LBM_OK;
 }
 
@@ -471,7 +489,7 @@ lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype) {
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->cls_alt), N);
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->flags_raw), N);
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->nbmask), static_cast<size_t>(N) * sizeof(uint32_t));
-  if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->counters), 4 * sizeof(unsigned long long));
+  if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->counters), 5 * sizeof(unsigned long long));
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->totals_dev), 5 * sizeof(double));
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->list_count_dev), sizeof(int));
   if (rc == LBM_OK && cudaMemset(c->cls, 0, N) != cudaSuccess) rc = fail(c, LBM_ECUDA, "cudaMemset failed");

@@ -17,7 +17,9 @@
 
 namespace lbm {
 
-enum : int { T_FLUID = 0, T_SOLID = 1, T_INLET = 2, T_OUTLET = 3, T_WM = 4 };
+enum : int { T_FLUID = 0, T_SOLID = 1, T_INLET = 2, T_OUTLET = 3, T_WM = 4, T_MOVING = 5 };
+// wall cells: resting SOLID (1 = 001b) and MOVINGWALL (5 = 101b) -- the only types whose two low bits are 01
+__host__ __device__ constexpr bool is_wall(int cls_or_type) { return (cls_or_type & 3) == 1; }
 // internal class byte: bits 0-2 type, bits 3-5 wall-normal code,
 //   bit 6 = ADJ:     the (non-SOLID) cell has at least one SOLID lattice neighbour (nbmask[] says which);
 //   bit 7 = SPECIAL: the cell needs the per-cell path (list blocks): WALLMODEL cells (A8) and OUTLET cells with a
@@ -77,6 +79,14 @@ __host__ __device__ constexpr T weight(int c2) {
                    : (c2 == 0 ? T(8.0 / 27.0) : (c2 == 1 ? T(2.0 / 27.0) : (c2 == 2 ? T(1.0 / 54.0) : T(1.0 / 216.0))));
 }
 
+// Moving-wall bounce-back (reading G33; lid of the lid-driven cavity): the population i that returns
+// from a wall moving with u_w gains 2 w_i rho_w (c_i . u_w) / c_s^2 = 6 w_i (c_i . u_w), rho_w = 1, c_i = wall -> fluid.
+template <int Q, typename T>
+__device__ __forceinline__ T moving_wall_term(int i, const T (&uw)[3]) {
+  constexpr Stencil<Q> L{};
+  return T(6) * weight<Q, T>(L.c2[i]) * (T(L.c[i][0]) * uw[0] + T(L.c[i][1]) * uw[1] + T(L.c[i][2]) * uw[2]);
+}
+
 template <typename T>
 struct StepArgs {
   const T* __restrict__ fin;      // [Q][N]
@@ -99,6 +109,7 @@ struct StepArgs {
   // HRR form (Eq. 7-11): u^(x,t) of every cell [3][N] (written by the MODE_UHAT_* pass, SOLID cells 0), Eq. 7 factor
   T* __restrict__ uhat;
   T sigma;
+  T u_wall[3];                    // velocity of the MOVINGWALL cells (only ever on the plane z = nz-1), reading G33
 };
 
 // ---- math helpers ---------------------------------------------------------------------------------
@@ -468,8 +479,9 @@ __device__ __forceinline__ void pull_cell(const StepArgs<T>& a, int x, int y, in
     const int sz = (L.c[i][2] == 0) ? z : ((L.c[i][2] == 1) ? zm : zp);
     const long long s = cell_index(sx, sy, sz, nx, ny);
     bool own = (i > 0) && ((nbm >> L.opp[i]) & 1u);
-    if (L.c[i][0] == -1 && type == T_OUTLET) own = (a.cls[s] & CLS_TYPE) == T_SOLID;
+    if (L.c[i][0] == -1 && type == T_OUTLET) own = is_wall(a.cls[s]);
     f[i] = own ? __ldg(a.fin + L.opp[i] * N + self) : __ldg(a.fin + i * N + s);
+    if (own && sz == nz - 1 && (a.cls[s] & CLS_TYPE) == T_MOVING) f[i] += moving_wall_term<Q, T>(i, a.u_wall);
   }
   if (type == T_INLET) inlet_fixup<Q, T>(f, a.u_in[0], a.u_in[1], a.u_in[2]);
 }
@@ -513,7 +525,7 @@ __device__ __forceinline__ void wallmodel_ub(const StepArgs<T>& a, int x, int y,
   y2 = (y2 < 0) ? y2 + a.ny : ((y2 >= a.ny) ? y2 - a.ny : y2);
   z2 = (z2 < 0) ? z2 + a.nz : ((z2 >= a.nz) ? z2 - a.nz : z2);
   const uint8_t cls2 = a.cls[cell_index(x2, y2, z2, a.nx, a.ny)];
-  if ((cls2 & CLS_TYPE) == T_SOLID) return;
+  if (is_wall(cls2)) return;
   T f2[Q];
   load_state<Q, T, PULL>(a, x2, y2, z2, cls2, f2);
   double rho = 0.0, j[3] = {0.0, 0.0, 0.0};
@@ -618,13 +630,14 @@ __device__ __forceinline__ void step_cell_any(const StepArgs<T>& a, int x, int y
   store_cell<Q, T>(a, x, y, z, f);
 }
 
-// SOLID cell in the per-cell paths: zeros over its lattice slots (never read; keeps sectors whole) / u^ = 0 (resting wall)
+// wall cell in the per-cell paths: zeros over its lattice slots (never read; keeps sectors whole) / u^ = the wall's velocity
 template <int Q, typename T, int MODE>
 __device__ __forceinline__ void solid_cell_any(const StepArgs<T>& a, long long self) {
   if (mode_uhat(MODE)) {
-    a.uhat[self] = T(0);
-    a.uhat[a.N + self] = T(0);
-    a.uhat[2 * a.N + self] = T(0);
+    const bool mv = (a.cls[self] & CLS_TYPE) == T_MOVING;     // u^ of a wall cell = the wall's velocity (G30, G33)
+    a.uhat[self] = mv ? a.u_wall[0] : T(0);
+    a.uhat[a.N + self] = mv ? a.u_wall[1] : T(0);
+    a.uhat[2 * a.N + self] = mv ? a.u_wall[2] : T(0);
   } else {
     store_zero<Q, T>(a, self);
   }
@@ -640,7 +653,7 @@ __global__ void __launch_bounds__(256) k_step(const __grid_constant__ StepArgs<T
   if (x >= a.nx || y >= a.ny) return;
   const long long self = cell_index(x, y, z, a.nx, a.ny);
   const uint8_t cls = a.cls[self];
-  if ((cls & CLS_TYPE) == T_SOLID) {         // SOLID cells are inert (R5); their slots are never read
+  if (is_wall(cls)) {                        // wall cells are inert (R5); their slots are never read
     solid_cell_any<Q, T, MODE>(a, self);
     return;
   }
@@ -740,7 +753,8 @@ __device__ __forceinline__ void ld_uhat_nb(const T* pu, long long N, int dyp, in
 // of the cells of SPECIAL sectors (A8 wall model; OUTLET cells next to a wall), one cell per thread: the masked
 // boundary kernel as a block role of the same launch (scheduled first, overlaps with the row blocks).
 // Everything else -- bulk, solid-adjacent (read-side bounce-back), INLET and OUTLET cells -- runs in the vector path.
-template <int Q, typename T, int MODE, int COLL>
+// MW: the geometry holds MOVINGWALL cells (compiled out otherwise: the test costs the wall-adjacent warps registers).
+template <int Q, typename T, int MODE, int COLL, bool MW>
 __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ StepArgs<T> a) {
   constexpr Stencil<Q> L{};
   constexpr int V = VecOf<Q, T, COLL>::V;
@@ -756,7 +770,7 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
     if (k < a.n_list) {
       const int cell = a.list[k];
       const uint8_t c = a.cls[cell];
-      if ((c & CLS_TYPE) == T_SOLID) {     // SOLID sector-mate: zeros keep the sector whole
+      if (is_wall(c)) {                    // wall sector-mate: zeros keep the sector whole
         solid_cell_any<Q, T, MODE>(a, cell);
       } else {
         const int plane = a.nx * a.ny;
@@ -783,7 +797,7 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
   if (active) secw = ld_cls_sector(a.cls + row + (x0 & ~(SV - 1)), T(0));
   constexpr unsigned long long SPECIAL_ALL = (SV == 8) ? 0x8080808080808080ull : 0x80808080ull;
   constexpr uint32_t VMASK = rep_byte(0xffu, V);
-  constexpr uint32_t TYPE_ALL = rep_byte(0x07u, V);
+  constexpr uint32_t TYPE_ALL = rep_byte(0x03u, V);         // is_wall: the two low type bits are 01
   constexpr uint32_t SOLID_ALL = rep_byte(0x01u, V);
   constexpr uint32_t ADJ_ALL = rep_byte(0x40u, V);
   const uint32_t clsw = static_cast<uint32_t>(secw >> (8 * (x0 & (SV - 1)))) & VMASK;
@@ -792,13 +806,14 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
   // an all-SOLID vector whose 128-byte line holds a non-SOLID vector stores zeros, so that the line is written whole
   const unsigned live_lanes = __ballot_sync(FULL, active && !all_solid);
   const unsigned group = (LG >= 32) ? FULL : (((1u << (LG & 31)) - 1u) << (lane & ~(LG - 1)));
-  const bool zero_fill = active && all_solid && !special && ((live_lanes & group) != 0u);
+  // (the u^ pass writes every wall vector: 12 bytes per cell, and the FD stencil may read any of them)
+  const bool zero_fill = active && all_solid && !special && (mode_uhat(MODE) || ((live_lanes & group) != 0u));
   const bool mine = active && !all_solid && !special;       // this thread computes and stores the vector
   const bool doload = active && !all_solid;                 // neighbours may need its lanes' values
   // which cells of the vector are SOLID (bit v)
   unsigned solid_bits = 0;
 #pragma unroll
-  for (int v = 0; v < V; ++v) solid_bits |= (((clsw >> (8 * v)) & CLS_TYPE) == T_SOLID) ? (1u << v) : 0u;
+  for (int v = 0; v < V; ++v) solid_bits |= is_wall(static_cast<int>(clsw >> (8 * v))) ? (1u << v) : 0u;
   const bool adj = mine && PULL && ((clsw & ADJ_ALL) != 0);
   // INLET (only ever at x = 0) / OUTLET (only ever at x = nx-1; SPECIAL if next to a wall) cells
   const bool inlet0 = mine && (x0 == 0) && ((clsw & CLS_TYPE) == T_INLET);
@@ -888,10 +903,21 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
     T zero[V];
 #pragma unroll
     for (int v = 0; v < V; ++v) zero[v] = T(0);
+    if constexpr (mode_uhat(MODE)) {                         // u^ of wall cells: 0, or u_w on MOVINGWALL cells
 #pragma unroll
-    for (int i = 0; i < (mode_uhat(MODE) ? 3 : Q); ++i) {
-      st_vec(pout, zero);
-      pout += N;
+      for (int b = 0; b < 3; ++b) {
+        T uw[V];
+#pragma unroll
+        for (int v = 0; v < V; ++v) uw[v] = (((clsw >> (8 * v)) & CLS_TYPE) == T_MOVING) ? a.u_wall[b] : T(0);
+        st_vec(pout, uw);
+        pout += N;
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < Q; ++i) {
+        st_vec(pout, zero);
+        pout += N;
+      }
     }
     return;
   }
@@ -907,6 +933,27 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
 #pragma unroll
       for (int v = 0; v < V; ++v)
         if (nbm[v] & (1u << j)) f[L.opp[j]][v] = __ldg(pown + static_cast<long long>(j) * N + v);
+    }
+    // moving wall (G33): MOVINGWALL cells exist only on the plane z = nz-1, so only directions towards that plane can
+    // meet one (block-uniform test); the neighbour's class byte decides
+    if (MW && (z >= nz - 2 || z == 0)) {
+#pragma unroll
+      for (int j = 1; j < Q; ++j) {
+        const int zn = z + L.c[j][2];
+        if (((zn < 0) ? zn + nz : ((zn >= nz) ? zn - nz : zn)) != nz - 1) continue;
+        const long long off = static_cast<long long>((L.c[j][1] == 0) ? 0 : ((L.c[j][1] == 1) ? dyp : dym)) +
+                              static_cast<long long>((L.c[j][2] == 0) ? 0 : ((L.c[j][2] == 1) ? dzp : dzm));
+        const uint8_t* pc = a.cls + self + off;
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+          if (nbm[v] & (1u << j)) {
+            int ex = v + L.c[j][0];
+            if (L.c[j][0] == -1 && v == 0) ex = exl;
+            if (L.c[j][0] == 1 && v == V - 1) ex = exr;
+            if ((pc[ex] & CLS_TYPE) == T_MOVING) f[L.opp[j]][v] += moving_wall_term<Q, T>(L.opp[j], a.u_wall);
+          }
+        }
+      }
     }
   }
   if (PULL && inlet0) {                                      // R6 on the x = 0 cell of the row
@@ -925,7 +972,12 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
 #pragma unroll
       for (int i = 0; i < Q; ++i) fc[i] = f[i][v];
       uhat_of<Q, T>(fc, d[v], T(0), T(0), T(0), uo[0][v], uo[1][v], uo[2][v]);
-      if (solid_bits & (1u << v)) uo[0][v] = uo[1][v] = uo[2][v] = T(0);
+      if (solid_bits & (1u << v)) {
+        const bool mv = ((clsw >> (8 * v)) & CLS_TYPE) == T_MOVING;
+        uo[0][v] = mv ? a.u_wall[0] : T(0);
+        uo[1][v] = mv ? a.u_wall[1] : T(0);
+        uo[2][v] = mv ? a.u_wall[2] : T(0);
+      }
     }
 #pragma unroll
     for (int b = 0; b < 3; ++b) {
@@ -1034,7 +1086,7 @@ __global__ void __launch_bounds__(256) k_totals(const __grid_constant__ StepArgs
   if (x < a.nx && y < a.ny) {
     const long long self = cell_index(x, y, z, a.nx, a.ny);
     const uint8_t cls = a.cls[self];
-    if ((cls & CLS_TYPE) != T_SOLID) {
+    if (!is_wall(cls)) {
       T f[Q];
 #pragma unroll
       for (int i = 0; i < Q; ++i) f[i] = __ldg(a.fin + i * a.N + self);
@@ -1089,7 +1141,8 @@ __global__ void __launch_bounds__(256) k_init_equilibrium(const T* __restrict__ 
 
 // ---- flag validation + classification ------------------------------------------------------------
 // cls = type | normal<<3 | ADJ | SPECIAL (see the top of this file).
-// counters[0] = invalid flag bytes, [1] = SOLID cells, [2] = masked cells (non-SOLID, not plain bulk FLUID).
+// counters[0] = invalid flag bytes, [1] = wall cells (SOLID + MOVINGWALL), [2] = masked cells (non-wall, not plain bulk FLUID),
+// [4] = MOVINGWALL cells ([3] belongs to k_mark_list).
 template <int Q>
 __global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ flags, uint8_t* __restrict__ cls,
                                                   int nx, int ny, int nz, unsigned long long* __restrict__ counters) {
@@ -1101,27 +1154,29 @@ __global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ fl
   const long long self = cell_index(x, y, z, nx, ny);
   const uint8_t fl = flags[self];
   const int type = fl & 0x0F, hi = fl >> 4;
-  bool bad = type > T_WM;
+  bool bad = type > T_MOVING;
   if (type == T_WM) bad = bad || hi > 5; else bad = bad || hi != 0;
   if (type == T_INLET && x != 0) bad = true;
   if (type == T_OUTLET && x != nx - 1) bad = true;
+  if (type == T_MOVING && z != nz - 1) bad = true;
   if (bad) { atomicAdd(counters, 1ull); return; }
   uint32_t m = 0u;
-  if (type != T_SOLID) {
+  if (!is_wall(type)) {
 #pragma unroll
     for (int j = 1; j < Q; ++j) {
       int sx = x + L.c[j][0], sy = y + L.c[j][1], sz = z + L.c[j][2];
       sx = (sx < 0) ? sx + nx : ((sx >= nx) ? sx - nx : sx);
       sy = (sy < 0) ? sy + ny : ((sy >= ny) ? sy - ny : sy);
       sz = (sz < 0) ? sz + nz : ((sz >= nz) ? sz - nz : sz);
-      if ((flags[cell_index(sx, sy, sz, nx, ny)] & 0x0F) == T_SOLID) m |= (1u << j);
+      if (is_wall(flags[cell_index(sx, sy, sz, nx, ny)] & 0x0F)) m |= (1u << j);
     }
   }
   const bool adj = (m != 0u);
   const bool special = (type == T_WM) || (type == T_OUTLET && adj);
   cls[self] = static_cast<uint8_t>(type | ((type == T_WM ? hi : 0) << CLS_NORMAL_SHIFT) | (adj ? CLS_ADJ : 0) |
                                    (special ? CLS_SPECIAL : 0));
-  if (type == T_SOLID) atomicAdd(counters + 1, 1ull);
+  if (is_wall(type)) atomicAdd(counters + 1, 1ull);
+  if (type == T_MOVING) atomicAdd(counters + 4, 1ull);
   else if (adj || type != T_FLUID) atomicAdd(counters + 2, 1ull);
 }
 
@@ -1142,7 +1197,7 @@ __global__ void __launch_bounds__(256) k_nbmask(const uint8_t* __restrict__ cls,
       sx = (sx < 0) ? sx + nx : ((sx >= nx) ? sx - nx : sx);
       sy = (sy < 0) ? sy + ny : ((sy >= ny) ? sy - ny : sy);
       sz = (sz < 0) ? sz + nz : ((sz >= nz) ? sz - nz : sz);
-      if ((cls[cell_index(sx, sy, sz, nx, ny)] & CLS_TYPE) == T_SOLID) m |= (1u << j);
+      if (is_wall(cls[cell_index(sx, sy, sz, nx, ny)])) m |= (1u << j);
     }
   }
   nbmask[self] = m;
@@ -1151,7 +1206,7 @@ __global__ void __launch_bounds__(256) k_nbmask(const uint8_t* __restrict__ cls,
 // mark[n] = 1 on SOLID cells (feeds the compaction of the SOLID-cell list)
 __global__ void __launch_bounds__(256) k_mark_solid(const uint8_t* __restrict__ cls, uint8_t* __restrict__ mark, long long N) {
   const long long n = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
-  if (n < N) mark[n] = ((cls[n] & CLS_TYPE) == T_SOLID) ? 1 : 0;
+  if (n < N) mark[n] = is_wall(cls[n]) ? 1 : 0;
 }
 
 // SOLID cells are inert (R5) but the step kernels write zeros over their slots: their own Q values live in a side buffer

@@ -71,7 +71,7 @@ def _check_windows(cfg, dtype, windows, closed_axes, steps=S):
         gotw = out[:, tz][:, :, ty][:, :, :, tx].cpu().numpy().astype(np.float64)
         mask = None
         if flc is not None:
-            mask = (cfg["flags"][gsel] & 15) != I.SOLID
+            mask = ~I.is_wall(cfg["flags"][gsel])
             if not mask.any():
                 continue
             solid = ~mask
@@ -152,6 +152,16 @@ def test_config4_hrr_full_size_windows():
     wins = [tuple(min(max(v, 0), 512 - W) for v in w) for w in wins]
     wins += [(0, 0, 0), (504, 504, 504), (250, 0, 504)]
     _check_windows(cfg, "f32", wins, (False, False, False), steps=6)
+
+
+def test_cavity_full_size_windows():
+    """lid-driven cavity 512^3 (bench.py cavity_512_f32: three launches per step, lid slices on the MW kernel variant):
+    windows at the lid's corners and edges, under the lid, at the floor and in the bulk; the walls close every axis"""
+    cfg = I.make_config(6)
+    n = 512
+    wins = [(n - 1 - W, 1, 1), (n - 1 - W, n - 1 - W, n - 1 - W), (n - 1 - W, 250, 1), (n - 1 - W, 1, 300), (n - 1 - W, 200, 200),
+            (1, 1, 1), (1, 300, n - 1 - W), (250, 250, 250), (n - 2 - W, 100, n - 1 - W)]
+    _check_windows(cfg, "f32", wins, (True, True, True))
 
 
 # ---- T2: invariants after the configs' full step counts ------------------------------------------
