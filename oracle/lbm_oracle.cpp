@@ -20,6 +20,8 @@
 //   O3 stream              Eq. 6 left-hand side (l.70); halfway bounce-back (G14/R5);
 //                          zero-gradient outlet (G16/R7)
 //   O4 inlet fix-up        l.155 "regularized local velocity boundary condition" (G15/R6)
+//   O4v Vortex Method inlet l.133-155, Eq. 18-21: per step the inflow velocity of every INLET cell from seeded
+//                          vortices (readings G11, G34, G35); feeds O4.  Pinned by V1-V7 in tests/test_oracle_vm.py
 //   O3m moving wall       lid of the "established lid-driven cavity benchmark" (l.214): halfway bounce-back
 //                          off a wall moving with u_w: + 2 w_i rho_w (c_i.u_w)/c_s^2 on the returned population, rho_w = 1
 //                          (reading G33; the paper does not say how its lid is imposed -> PARITY UNPINNED against the
@@ -371,6 +373,81 @@ void inlet_fixup_cell(const Lattice& L, double* g, const double uw[3]) {
   }
 }
 
+// ---- Vortex Method inflow: Eq. 18-21 ------------------------------------------
+// The inflow plane is x = 0 with d_inlet = (1,0,0); fields are [3][nz][ny] (component, z, y); mask[z][y] = 1 on INLET cells.
+// Seeds p_i = (y_i, z_i) in cell coordinates and signs s_i are INPUTS (the random numbers the method draws).
+//   k_i     = 3/2 (|u_mean(p_i)| I)^2                                                  (Eq. 18; u_mean at the nearest cell,
+//                                                                                        0 if that cell is not an INLET cell)
+//   Gamma_i = 4 s_i sqrt( pi A k_i / (3 N (2 ln 3 - 3 ln 2)) )                         (Eq. 19, reading G34: the printed
+//             "sqrt(pi/(6 ln3 - 9 ln2)) k_i A/n" with the root over the whole quotient, as in ref. [12]; A = number of
+//             INLET cells)
+//   u_v(x)  = 1/(2 pi) sum_i Gamma_i ((p_i - x) x d) (1 - exp(-|x-p_i|^2 / (2 sigma^2))) / |x-p_i|^2   (Eq. 20, G11: exp(-..))
+//   u(x)    = u_mean + u_v - (u_v . g^) d,  g^ = grad(u_prev . d)/|grad(u_prev . d)|   (Eq. 21, reading G35: in-plane
+//             central differences, a neighbour that is not an INLET cell is replaced by the cell itself, y wraps; the
+//             term is dropped where the gradient vanishes)
+struct VortexInlet {
+  const double* u_mean;   // [3][nz][ny]
+  double* u_inflow;       // [3][nz][ny]: in = inflow of the previous step, out = inflow of the last step
+  int nv;
+  const double* pos;      // [nv][2] (y, z)
+  const double* sign;     // [nv]
+  double sigma_v, intensity;
+};
+
+void vm_inflow(int ny, int nz, const uint8_t* mask, const double* u_mean, const double* u_prev, int nv, const double* pos,
+               const double* sign, double sigma_v, double intensity, double* out) {
+  const int64_t P = static_cast<int64_t>(ny) * nz;
+  const double PI = 3.14159265358979323846;
+  int64_t A = 0;
+  for (int64_t c = 0; c < P; ++c) A += mask[c] ? 1 : 0;
+  std::vector<double> gamma(nv > 0 ? nv : 0);
+  for (int i = 0; i < nv; ++i) {
+    int yi = static_cast<int>(std::floor(pos[2 * i] + 0.5)), zi = static_cast<int>(std::floor(pos[2 * i + 1] + 0.5));
+    yi = ((yi % ny) + ny) % ny;
+    zi = (zi < 0) ? 0 : ((zi >= nz) ? nz - 1 : zi);
+    const int64_t c = static_cast<int64_t>(zi) * ny + yi;
+    double k = 0.0;
+    if (mask[c]) {
+      const double um = std::sqrt(u_mean[c] * u_mean[c] + u_mean[P + c] * u_mean[P + c] + u_mean[2 * P + c] * u_mean[2 * P + c]);
+      k = 1.5 * (um * intensity) * (um * intensity);                                        // Eq. 18
+    }
+    gamma[i] = 4.0 * sign[i] * std::sqrt(PI * static_cast<double>(A) * k /
+                                         (3.0 * nv * (2.0 * std::log(3.0) - 3.0 * std::log(2.0))));   // Eq. 19 (G34)
+  }
+  for (int z = 0; z < nz; ++z)
+    for (int y = 0; y < ny; ++y) {
+      const int64_t c = static_cast<int64_t>(z) * ny + y;
+      if (!mask[c]) {
+        for (int a = 0; a < 3; ++a) out[a * P + c] = u_mean[a * P + c];
+        continue;
+      }
+      double uv[3] = {0.0, 0.0, 0.0};
+      for (int i = 0; i < nv; ++i) {                                                         // Eq. 20
+        const double ry = pos[2 * i] - y, rz = pos[2 * i + 1] - z;                           // p_i - x (in-plane)
+        const double r2 = ry * ry + rz * rz;
+        if (r2 == 0.0) continue;                                                             // limit of the summand is 0
+        // (0, ry, rz) x (1, 0, 0) = (0, rz, -ry)
+        const double fac = gamma[i] * (1.0 - std::exp(-r2 / (2.0 * sigma_v * sigma_v))) / r2 / (2.0 * PI);
+        uv[1] += fac * rz;
+        uv[2] += -fac * ry;
+      }
+      // Eq. 21 (G35): streamwise fluctuation along the gradient of the previous inflow's streamwise component
+      const double* sp = u_prev;                                                             // component 0 = u_prev . d
+      const int yp = (y + 1) % ny, ym = (y + ny - 1) % ny;
+      const int64_t cyp = mask[static_cast<int64_t>(z) * ny + yp] ? static_cast<int64_t>(z) * ny + yp : c;
+      const int64_t cym = mask[static_cast<int64_t>(z) * ny + ym] ? static_cast<int64_t>(z) * ny + ym : c;
+      const int64_t czp = (z + 1 < nz && mask[c + ny]) ? c + ny : c;
+      const int64_t czm = (z - 1 >= 0 && mask[c - ny]) ? c - ny : c;
+      const double gy = 0.5 * (sp[cyp] - sp[cym]), gz = 0.5 * (sp[czp] - sp[czm]);
+      const double gn = std::sqrt(gy * gy + gz * gz);
+      double us = 0.0;
+      if (gn > 0.0) us = -(uv[1] * gy + uv[2] * gz) / gn;
+      out[c] = u_mean[c] + uv[0] + us;
+      out[P + c] = u_mean[P + c] + uv[1];
+      out[2 * P + c] = u_mean[2 * P + c] + uv[2];
+    }
+}
+
 }  // namespace
 
 extern "C" {
@@ -453,9 +530,11 @@ int orc_init_equilibrium(int Q, int64_t N, const double* rho, const double* u, d
 // f is updated in place (the second lattice is internal).  d and flags may be NULL.
 // nthreads <= 1: serial.  nthreads > 1: the same loop nests with "omp parallel for" over z.
 // Returns 0, or -1 on bad arguments.
-int orc_step(int Q, int nx, int ny, int nz, double* f, const double* d, const uint8_t* flags,
+}  // extern "C"
+namespace {
+int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const uint8_t* flags,
              const double* par /* tau0, cs, use_hlbm, uin0, uin1, uin2, wm_enable, kappa, E, collision, sigma, uwall0, uwall1, uwall2 */,
-             int nsteps, int nthreads) {
+             int nsteps, int nthreads, VortexInlet* vm) {
   Lattice L;
   if (!make_lattice(Q, L)) return -1;
   if (nx < 1 || ny < 1 || nz < 1 || nsteps < 0) return -1;
@@ -615,6 +694,18 @@ int orc_step(int Q, int nx, int ny, int nz, double* f, const double* d, const ui
           }
         }
 
+    // ---- O4v (Vortex Method inlet, Eq. 18-21): this step's inflow velocity field from the previous one ----------
+    if (vm && flags) {
+      const int64_t P = static_cast<int64_t>(ny) * nz;
+      std::vector<uint8_t> mask(P);
+      for (int z = 0; z < nz; ++z)
+        for (int y = 0; y < ny; ++y)
+          mask[static_cast<int64_t>(z) * ny + y] = cell_type(flags[(static_cast<int64_t>(z) * ny + y) * nx]) == INLET;
+      std::vector<double> unew(3 * P);
+      vm_inflow(ny, nz, mask.data(), vm->u_mean, vm->u_inflow, vm->nv, vm->pos, vm->sign, vm->sigma_v, vm->intensity, unew.data());
+      std::memcpy(vm->u_inflow, unew.data(), sizeof(double) * 3 * P);
+    }
+
     // ---- O4: inlet fix-up ----------------------------------------------------------------------
     if (flags) {
 #pragma omp parallel for num_threads(nth) if (nth > 1)
@@ -625,7 +716,12 @@ int orc_step(int Q, int nx, int ny, int nz, double* f, const double* d, const ui
             if (cell_type(flags[x]) != INLET) continue;
             double gc[QMAX];
             for (int i = 0; i < Q; ++i) gc[i] = nxt[i * N + x];
-            inlet_fixup_cell(L, gc, p.u_in);
+            double uw[3] = {p.u_in[0], p.u_in[1], p.u_in[2]};
+            if (vm) {
+              const int64_t P = static_cast<int64_t>(ny) * nz, c = static_cast<int64_t>(z) * ny + y;
+              for (int a = 0; a < 3; ++a) uw[a] = vm->u_inflow[a * P + c];
+            }
+            inlet_fixup_cell(L, gc, uw);
             for (int i = 0; i < Q; ++i) nxt[i * N + x] = gc[i];
           }
     }
@@ -634,6 +730,31 @@ int orc_step(int Q, int nx, int ny, int nz, double* f, const double* d, const ui
     double* t = cur; cur = nxt; nxt = t;
   }
   if (cur != f) std::memcpy(f, cur, sizeof(double) * static_cast<size_t>(Q) * N);
+  return 0;
+}
+}  // namespace
+
+extern "C" {
+
+int orc_step(int Q, int nx, int ny, int nz, double* f, const double* d, const uint8_t* flags, const double* par, int nsteps,
+             int nthreads) {
+  return step_impl(Q, nx, ny, nz, f, d, flags, par, nsteps, nthreads, nullptr);
+}
+
+// the step with the Vortex Method inlet: u_inflow [3][nz][ny] holds the inflow of the previous step on entry (u_mean
+// before the first step) and the inflow of the last step on return; seeds and signs stay fixed for the nsteps steps
+int orc_step_vm(int Q, int nx, int ny, int nz, double* f, const double* d, const uint8_t* flags, const double* par, int nsteps,
+                int nthreads, const double* u_mean, double* u_inflow, int nv, const double* pos, const double* sign,
+                double sigma_v, double intensity) {
+  if (!u_mean || !u_inflow || nv < 0 || (nv > 0 && (!pos || !sign)) || !(sigma_v > 0.0) || intensity < 0.0) return -1;
+  VortexInlet vm{u_mean, u_inflow, nv, pos, sign, sigma_v, intensity};
+  return step_impl(Q, nx, ny, nz, f, d, flags, par, nsteps, nthreads, &vm);
+}
+
+int orc_vm_inflow(int ny, int nz, const uint8_t* mask, const double* u_mean, const double* u_prev, int nv, const double* pos,
+                  const double* sign, double sigma_v, double intensity, double* out) {
+  if (ny < 1 || nz < 1 || !mask || !u_mean || !u_prev || !out || nv < 0 || !(sigma_v > 0.0)) return -1;
+  vm_inflow(ny, nz, mask, u_mean, u_prev, nv, pos, sign, sigma_v, intensity, out);
   return 0;
 }
 

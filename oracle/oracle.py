@@ -53,6 +53,10 @@ def lib():
         L.orc_init_equilibrium.argtypes = [ctypes.c_int, ctypes.c_int64, _c_dp, _c_dp, _c_dp]
         L.orc_step.argtypes = [ctypes.c_int] * 4 + [_c_dp, _c_dp, _c_u8p, _c_dp, ctypes.c_int, ctypes.c_int]
         L.orc_moments.argtypes = [ctypes.c_int, ctypes.c_int64, _c_dp, _c_dp, _c_dp]
+        L.orc_step_vm.argtypes = [ctypes.c_int] * 4 + [_c_dp, _c_dp, _c_u8p, _c_dp, ctypes.c_int, ctypes.c_int,
+                                  _c_dp, _c_dp, ctypes.c_int, _c_dp, _c_dp, ctypes.c_double, ctypes.c_double]
+        L.orc_vm_inflow.argtypes = [ctypes.c_int, ctypes.c_int, _c_u8p, _c_dp, _c_dp, ctypes.c_int, _c_dp, _c_dp,
+                                    ctypes.c_double, ctypes.c_double, _c_dp]
         L.orc_totals.argtypes = [ctypes.c_int, ctypes.c_int64, _c_dp, _c_u8p, _c_dp]
         L.orc_max_threads.restype = ctypes.c_int
         _lib = L
@@ -173,6 +177,45 @@ def step(f, d=None, flags=None, nsteps=1, nthreads=1, **params):
     if rc != 0:
         raise ValueError("orc_step rejected its arguments")
     return f
+
+
+def vm_inflow(mask, u_mean, u_prev, pos, sign, sigma_v, intensity):
+    """Vortex Method inflow field (Eq. 18-21) on the plane x = 0.  mask[nz,ny] (1 = INLET cell), u_mean / u_prev [3,nz,ny],
+    pos[nv,2] = seed positions (y, z) in cell coordinates, sign[nv] = +-1.  Returns u[3,nz,ny]."""
+    mask = np.ascontiguousarray(mask, dtype=np.uint8)
+    nz, ny = mask.shape
+    u_mean, u_prev = _f64(u_mean), _f64(u_prev)
+    pos = _f64(np.asarray(pos, dtype=np.float64).reshape(-1, 2))
+    sign = _f64(np.asarray(sign, dtype=np.float64).reshape(-1))
+    assert u_mean.shape == (3, nz, ny) and u_prev.shape == (3, nz, ny) and len(sign) == len(pos)
+    out = np.empty((3, nz, ny))
+    rc = lib().orc_vm_inflow(ny, nz, mask.ctypes.data_as(_c_u8p), _dp(u_mean), _dp(u_prev), len(pos), _dp(pos), _dp(sign),
+                             float(sigma_v), float(intensity), _dp(out))
+    if rc != 0:
+        raise ValueError("orc_vm_inflow rejected its arguments")
+    return out
+
+
+def step_vm(f, u_mean, u_inflow, pos, sign, sigma_v, intensity, d=None, flags=None, nsteps=1, nthreads=1, **params):
+    """orc_step with the Vortex Method inlet.  u_inflow[3,nz,ny] = inflow of the previous step (u_mean before the first).
+    Returns (f, u_inflow) after nsteps."""
+    f = _f64(f).copy()
+    Q, nz, ny, nx = f.shape
+    par = pack_params(**params)
+    dptr = None
+    if d is not None:
+        d = _f64(d)
+        dptr = _dp(d)
+    flags = np.ascontiguousarray(flags, dtype=np.uint8)
+    u_mean = _f64(u_mean)
+    u_inflow = _f64(u_inflow).copy()
+    pos = _f64(np.asarray(pos, dtype=np.float64).reshape(-1, 2))
+    sign = _f64(np.asarray(sign, dtype=np.float64).reshape(-1))
+    rc = lib().orc_step_vm(Q, nx, ny, nz, _dp(f), dptr, flags.ctypes.data_as(_c_u8p), _dp(par), int(nsteps), int(nthreads),
+                           _dp(u_mean), _dp(u_inflow), len(pos), _dp(pos), _dp(sign), float(sigma_v), float(intensity))
+    if rc != 0:
+        raise ValueError("orc_step_vm rejected its arguments")
+    return f, u_inflow
 
 
 def moments(f):
