@@ -105,6 +105,32 @@ int lbm_init_equilibrium(lbm_ctx* ctx, const void* rho, const void* u);
 /* Replace porosity and flags only (same rules as lbm_set_fields); the populations are kept. */
 int lbm_set_geometry(lbm_ctx* ctx, const void* porosity, const uint8_t* cell_flags);
 
+/* Inflow velocity field of the INLET cells (plane x = 0) and the Vortex Method that perturbs it (Eq. 18-21;
+ * SURVEY 8(f)-3; readings G11, G34, G35 of DESIGN.md).
+ *   u_mean : [3][nz][ny] dtype (component, z, y), host or device: the mean velocity profile u_mean(x) of Eq. 21; entries of
+ *            cells that are not INLET cells are ignored.  NULL switches back to the uniform lbm_params.u_in.
+ * Once set, every lbm_step forms the inflow velocity of the new time level before the inlet rule (l.155) is applied:
+ *   u(x) = u_mean(x) + u_vortex(x) - (u_vortex(x) . g^(x)) d_inlet,     d_inlet = (1,0,0),
+ *   u_vortex by Eq. 20 from the seeds set with lbm_set_vortices (none => u = u_mean), g^ = the normalised in-plane gradient of
+ *   the previous step's streamwise inflow (central differences; a neighbour that is not an INLET cell is replaced by the cell
+ *   itself; y wraps).  "Previous inflow" is u_mean before the first step after this call / lbm_set_fields / lbm_init_equilibrium.
+ * The inflow fields are kept and computed in fp64 for both dtypes (Eq. 21 normalises a difference of neighbouring values) and
+ * rounded to dtype where the inlet rule reads them.
+ * Errors: LBM_EINVAL (NULL ctx), LBM_ENOMEM, LBM_ECUDA. */
+int lbm_set_inflow(lbm_ctx* ctx, const void* u_mean);
+
+/* Seeds of the Vortex Method: n_vortices >= 0 positions pos[n][2] = (y, z) in cell coordinates on the inflow plane and signs
+ * sign[n] = +-1 (HOST arrays of double: the random numbers the method draws are inputs), vortex size sigma_v > 0 (cells) and
+ * turbulence intensity >= 0.  Circulations: k_i = 3/2 (|u_mean(p_i)| I)^2 (Eq. 18, u_mean at the nearest cell, 0 over a cell that
+ * is not an INLET cell), Gamma_i = 4 s_i sqrt(pi A k_i / (3 n (2 ln 3 - 3 ln 2))) (Eq. 19, G34), A = number of INLET cells.
+ * The seeds stay until the next call; needs lbm_set_inflow first to take effect.
+ * Errors: LBM_EINVAL (NULL ctx, n < 0, NULL arrays with n > 0, sigma_v <= 0, intensity < 0), LBM_ENOMEM, LBM_ECUDA. */
+int lbm_set_vortices(lbm_ctx* ctx, int n_vortices, const double* pos, const double* sign, double sigma_v, double intensity);
+
+/* The inflow velocity field that belongs to the state S_t (the one its INLET cells carry): u[3][nz][ny] dtype, host or
+ * device.  LBM_ESTATE if no inflow field is set. */
+int lbm_get_inflow(lbm_ctx* ctx, void* u);
+
 /* Advance S_t -> S_{t+n_steps}: per step, per non-SOLID cell (Eq. 6, l.70):
  *   wall model u^B (Eq. 15-17, l.131) -> moments (l.97) -> u^ = (1-d)u + d u^B (Eq. 12) -> f^eq (Eq. 11)
  *   -> tau_eff from the local non-equilibrium stress (Eq. 3-5, 14) -> relaxation (Eq. 6) -> propagation

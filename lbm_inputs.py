@@ -231,6 +231,20 @@ def make_config(number, shape=None, k_max=None, n_modes=None):
     raise ValueError("unknown config %r" % number)
 
 
+def vm_inlet(shape, seed, n_vortices=256, sigma_v=6.0, intensity=0.15, u_ref=0.05, alpha=0.25):
+    """Vortex Method inlet of the urban channel: an atmospheric power-law mean profile
+    u_mean = u_ref ((z - 1/2)/(nz - 2))^alpha e_x over the floor z = 1/2 (stand-in for the paper's profile [23], which is not
+    printed), seeded vortex positions (uniform over the inflow plane) and signs.  No method arithmetic: inputs only."""
+    nz, ny, nx = shape
+    rng = _rng(seed)
+    u_mean = np.zeros((3, nz, ny))
+    h = np.clip((np.arange(nz) - 0.5) / max(nz - 2, 1), 0.5 / max(nz - 2, 1), 1.0)
+    u_mean[0] = (u_ref * h ** alpha)[:, None]
+    pos = np.stack([rng.uniform(0.0, ny, n_vortices), rng.uniform(1.0, nz - 1.0, n_vortices)], axis=1)
+    sign = rng.choice([-1.0, 1.0], n_vortices)
+    return dict(u_mean=u_mean, pos=pos, sign=sign, sigma_v=float(sigma_v), intensity=float(intensity))
+
+
 def cavity_flags(shape):
     """closed box: SOLID on x = 0, nx-1, y = 0, ny-1, z = 0; MOVINGWALL on the whole plane z = nz-1 (the lid)"""
     flags = np.zeros(shape, dtype=np.uint8)

@@ -1,4 +1,4 @@
-"""B200-native lattice Boltzmann hot path of arxiv 2506.21804 (BGK + Smagorinsky LES + HLBM).
+"""B200-native lattice Boltzmann hot path of arxiv 2506.21804 (BGK / HRR + Smagorinsky LES + HLBM).
 
 Thin Python binding over the C ABI in include/lbm.h (library: liblbm_b200.so, CUDA sm_100a).
 The binding only marshals arguments; every step of the path runs in the library's kernels.
@@ -7,8 +7,10 @@ no CUDA device is usable.
 """
 from .binding import (LBM, LbmError, LbmParams, lbm_create, lbm_destroy, lbm_get_populations, lbm_init_equilibrium,
                       lbm_last_error, lbm_moments, lbm_query, lbm_set_fields, lbm_set_geometry, lbm_set_option,
-                      lbm_set_stream, lbm_step, lbm_synchronize, lbm_totals, library_path, load_library)
+                      lbm_set_stream, lbm_step, lbm_synchronize, lbm_totals, library_path, load_library, lbm_set_inflow,
+                      lbm_set_vortices, lbm_get_inflow)
 
 __all__ = ["LBM", "LbmError", "LbmParams", "lbm_create", "lbm_destroy", "lbm_get_populations", "lbm_init_equilibrium",
            "lbm_last_error", "lbm_moments", "lbm_query", "lbm_set_fields", "lbm_set_geometry", "lbm_set_option",
-           "lbm_set_stream", "lbm_step", "lbm_synchronize", "lbm_totals", "library_path", "load_library"]
+           "lbm_set_stream", "lbm_step", "lbm_synchronize", "lbm_totals", "library_path", "load_library", "lbm_set_inflow",
+           "lbm_set_vortices", "lbm_get_inflow"]

@@ -15,7 +15,7 @@ LBM_D3Q19, LBM_D3Q27 = 19, 27
 LBM_F32, LBM_F64 = 4, 8
 EXPORTS = ["lbm_create", "lbm_destroy", "lbm_set_fields", "lbm_init_equilibrium", "lbm_set_geometry", "lbm_step",
            "lbm_moments", "lbm_get_populations", "lbm_totals", "lbm_set_stream", "lbm_synchronize", "lbm_last_error",
-           "lbm_query", "lbm_set_option"]
+           "lbm_query", "lbm_set_option", "lbm_set_inflow", "lbm_set_vortices", "lbm_get_inflow"]
 
 
 class LbmError(RuntimeError):
@@ -64,6 +64,9 @@ def load_library():
     L.lbm_init_equilibrium.argtypes = [vp, vp, vp]
     L.lbm_set_geometry.argtypes = [vp, vp, vp]
     L.lbm_step.argtypes = [vp, ip, ctypes.POINTER(LbmParams)]
+    L.lbm_set_inflow.argtypes = [vp, vp]
+    L.lbm_set_vortices.argtypes = [vp, ip, vp, vp, ctypes.c_double, ctypes.c_double]
+    L.lbm_get_inflow.argtypes = [vp, vp]
     L.lbm_moments.argtypes = [vp, vp, vp]
     L.lbm_get_populations.argtypes = [vp, vp]
     L.lbm_totals.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
@@ -127,6 +130,25 @@ def lbm_init_equilibrium(ctx, rho, u):
 
 def lbm_set_geometry(ctx, porosity=None, cell_flags=None):
     return _check(ctx, load_library().lbm_set_geometry(ctx, _ptr(porosity), _ptr(cell_flags)))
+
+
+def lbm_set_inflow(ctx, u_mean):
+    return _check(ctx, load_library().lbm_set_inflow(ctx, _ptr(u_mean)))
+
+
+def lbm_set_vortices(ctx, pos, sign, sigma_v, intensity):
+    """pos[n][2] = (y, z), sign[n]: converted to contiguous host float64 arrays (argument marshalling only)"""
+    import numpy as np
+    pos = np.ascontiguousarray(np.asarray(pos, dtype=np.float64).reshape(-1, 2))
+    sign = np.ascontiguousarray(np.asarray(sign, dtype=np.float64).reshape(-1))
+    if len(pos) != len(sign):
+        raise ValueError("pos and sign must have the same length")
+    return _check(ctx, load_library().lbm_set_vortices(ctx, len(sign), _ptr(pos) if len(sign) else None,
+                                                       _ptr(sign) if len(sign) else None, float(sigma_v), float(intensity)))
+
+
+def lbm_get_inflow(ctx, u):
+    return _check(ctx, load_library().lbm_get_inflow(ctx, _ptr(u)))
 
 
 def lbm_step(ctx, n_steps, params):
@@ -199,6 +221,15 @@ class LBM:
 
     def init_equilibrium(self, rho, u):
         return lbm_init_equilibrium(self.ctx, rho, u)
+
+    def set_inflow(self, u_mean):
+        return lbm_set_inflow(self.ctx, u_mean)
+
+    def set_vortices(self, pos, sign, sigma_v, intensity):
+        return lbm_set_vortices(self.ctx, pos, sign, sigma_v, intensity)
+
+    def get_inflow(self, u):
+        return lbm_get_inflow(self.ctx, u)
 
     def step(self, n_steps, params):
         return lbm_step(self.ctx, n_steps, params)

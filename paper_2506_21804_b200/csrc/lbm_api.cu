@@ -56,6 +56,15 @@ struct lbm_ctx {
   int block_threads;
   int use_vector;        // 1: 128-bit vector kernel when nx % (32/dtype) == 0 (default); 0: scalar kernel
   int use_graph;
+  // Vortex Method inlet / per-cell inflow field (lbm_set_inflow, lbm_set_vortices)
+  double* uin_mean;      // [3][nz][ny] fp64 (whatever the dtype), nullptr = uniform params.u_in
+  double* uin_field[2];  // inflow of the current / the previous time level, fp64
+  int uin_cur;
+  long long inflow_index;   // the time level t the current inflow field belongs to (S_t carries it)
+  int nv;
+  double* vpos;  double* vsign;  double* vgamma;     // device [nv][2], [nv], [nv]
+  double vm_sigma, vm_intensity;
+  bool gamma_dirty;
   void* uhat;            // HRR form: u^(x,t) [3][N], allocated on the first HRR step
   int hrr_slab;          // HRR form: z-slices per slab of the two-pass step (0 = whole lattice)
   lbm_params last;       // parameters of the last lbm_step: the inlet rule is part of how S_t is formed from F_{t-1}
@@ -145,6 +154,7 @@ lbm::StepArgs<T> make_args(const lbm_ctx* c, const lbm_params* p, int in, int ou
   a.uhat = static_cast<T*>(c->uhat);
   a.sigma = p ? static_cast<T>(p->sigma) : T(1);
   for (int k = 0; k < 3; ++k) a.u_wall[k] = p ? static_cast<T>(p->u_wall[k]) : T(0);
+  a.uin_field = c->uin_mean ? c->uin_field[c->uin_cur] : nullptr;
   if (p) {
     a.tau0 = static_cast<T>(p->tau0);
     a.smago_k = static_cast<T>(18.0 * 1.4142135623730951 * p->cs_smago * p->cs_smago);
@@ -453,6 +463,45 @@ int classify(lbm_ctx* c, const uint8_t* cell_flags) {
   return LBM_OK;
 }
 
+// ---- Vortex Method inlet: host side (Eq. 18-21) ---------------------------------------------------------------------
+int vm_advance(lbm_ctx* c) {
+  const long long P = static_cast<long long>(c->ny) * c->nz;
+  if (c->gamma_dirty && c->nv > 0) {
+    lbm::k_vm_gamma<double><<<1, 256, 0, c->stream>>>(c->cls, c->nx, c->ny, c->nz, c->uin_mean, c->nv, c->vpos, c->vsign,
+                                                       c->vm_intensity, c->vgamma);
+    LBM_CUDA(c, cudaGetLastError());
+    c->launches++;
+  }
+  c->gamma_dirty = false;
+  const unsigned blocks = static_cast<unsigned>((P + 255) / 256);
+  lbm::k_vm_inflow<double><<<blocks, 256, 0, c->stream>>>(c->cls, c->nx, c->ny, c->nz, c->uin_mean, c->uin_field[c->uin_cur], c->nv,
+                                                          c->vpos, c->vgamma, c->vm_sigma, c->uin_field[1 - c->uin_cur]);
+  LBM_CUDA(c, cudaGetLastError());
+  c->launches++;
+  c->uin_cur = 1 - c->uin_cur;
+  return LBM_OK;
+}
+
+// the inflow field of time level t must be current before S_t is formed (pulled) for the first time
+int ensure_inflow(lbm_ctx* c, long long t) {
+  if (!c->uin_mean) return LBM_OK;
+  while (c->inflow_index < t) {
+    int rc = vm_advance(c);
+    if (rc != LBM_OK) return rc;
+    c->inflow_index++;
+  }
+  return LBM_OK;
+}
+
+// "previous inflow" := u_mean; the current time level is c->steps
+int reset_inflow(lbm_ctx* c) {
+  if (!c->uin_mean) return LBM_OK;
+  const size_t bytes = 3 * static_cast<size_t>(c->ny) * c->nz * sizeof(double);
+  LBM_CUDA(c, cudaMemcpyAsync(c->uin_field[c->uin_cur], c->uin_mean, bytes, cudaMemcpyDeviceToDevice, c->stream));
+  c->inflow_index = c->steps;
+  return LBM_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -506,6 +555,7 @@ void lbm_destroy(lbm_ctx* c) {
   if (!c) return;
   cudaStreamSynchronize(c->stream);
   cudaFree(c->f[0]);  cudaFree(c->f[1]);  cudaFree(c->d);  cudaFree(c->uhat);
+  cudaFree(c->uin_mean);  cudaFree(c->uin_field[0]);  cudaFree(c->uin_field[1]);  cudaFree(c->vpos);  cudaFree(c->vsign);  cudaFree(c->vgamma);
   cudaFree(c->cls);  cudaFree(c->cls_alt);  cudaFree(c->flags_raw);
   cudaFree(c->counters);  cudaFree(c->totals_dev);  cudaFree(c->staging);
   cudaFree(c->list);  cudaFree(c->cub_tmp);  cudaFree(c->list_count_dev);
@@ -531,6 +581,7 @@ int lbm_synchronize(lbm_ctx* c) {
 static int set_geometry_fields(lbm_ctx* c, const void* porosity, const uint8_t* cell_flags) {
   int rc = classify(c, cell_flags);
   if (rc != LBM_OK) return rc;
+  c->gamma_dirty = true;   // A and the seeds' cells depend on the flags
   if (c->uhat)   // cells that turned SOLID must read u^ = 0 (the UHAT pass does not visit all-SOLID lines)
     LBM_CUDA(c, cudaMemsetAsync(c->uhat, 0, 3 * static_cast<size_t>(c->N) * c->dtype, c->stream));
   if (porosity) {
@@ -553,6 +604,7 @@ int lbm_set_fields(lbm_ctx* c, const void* populations, const void* porosity, co
   c->cur = 0;
   c->phase = PHASE_PRE;
   c->steps = 0;
+  { int rci = reset_inflow(c); if (rci != LBM_OK) return rci; }
   return solid_values(c, true);      // SOLID cells' own values -> side buffer (the step kernels overwrite their slots)
 }
 
@@ -576,6 +628,7 @@ int lbm_init_equilibrium(lbm_ctx* c, const void* rho, const void* u) {
   c->cur = 0;
   c->phase = PHASE_PRE;
   c->steps = 0;
+  { int rci = reset_inflow(c); if (rci != LBM_OK) return rci; }
   return solid_values(c, true);
 }
 
@@ -583,6 +636,8 @@ int lbm_init_equilibrium(lbm_ctx* c, const void* rho, const void* u) {
 static int materialise(lbm_ctx* c) {
   if (c->phase != PHASE_POST) return LBM_OK;
   lbm_params p = c->last;
+  int rci = ensure_inflow(c, c->steps);
+  if (rci != LBM_OK) return rci;
   int rc = launch_step(c, &p, lbm::MODE_STREAM);
   if (rc != LBM_OK) return rc;
   c->phase = PHASE_PRE;
@@ -597,6 +652,89 @@ int lbm_set_geometry(lbm_ctx* c, const void* porosity, const uint8_t* cell_flags
   rc = set_geometry_fields(c, porosity, cell_flags);
   if (rc != LBM_OK) return rc;
   if (c->phase == PHASE_PRE) return solid_values(c, true);   // the SOLID set changed: save the new set's values
+  return LBM_OK;
+}
+
+int lbm_set_inflow(lbm_ctx* c, const void* u_mean) {
+  if (!c) return LBM_EINVAL;
+  const long long n = 3ll * c->ny * c->nz;
+  const size_t bytes = static_cast<size_t>(n) * sizeof(double);       // kept in fp64 whatever the dtype
+  // the state S_t keeps the inflow it was formed with
+  int rc = materialise(c);
+  if (rc != LBM_OK) return rc;
+  if (!u_mean) {
+    if (c->uin_mean) {
+      LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+      cudaFree(c->uin_mean);  cudaFree(c->uin_field[0]);  cudaFree(c->uin_field[1]);
+      c->uin_mean = c->uin_field[0] = c->uin_field[1] = nullptr;
+      c->device_bytes -= 3 * bytes;
+    }
+    return LBM_OK;
+  }
+  if (!c->uin_mean) {
+    rc = dev_alloc(c, reinterpret_cast<void**>(&c->uin_mean), bytes);
+    if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->uin_field[0]), bytes);
+    if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->uin_field[1]), bytes);
+    if (rc != LBM_OK) return rc;
+    c->uin_cur = 0;
+  }
+  if (c->dtype == LBM_F64) {
+    LBM_CUDA(c, cudaMemcpyAsync(c->uin_mean, u_mean, bytes, cudaMemcpyDefault, c->stream));
+  } else {                               // fp32 input -> staging (the other field buffer) -> fp64
+    float* tmp = reinterpret_cast<float*>(c->uin_field[1 - c->uin_cur]);
+    LBM_CUDA(c, cudaMemcpyAsync(tmp, u_mean, static_cast<size_t>(n) * sizeof(float), cudaMemcpyDefault, c->stream));
+    lbm::k_convert<float, double><<<static_cast<unsigned>((n + 255) / 256), 256, 0, c->stream>>>(tmp, c->uin_mean, n);
+    LBM_CUDA(c, cudaGetLastError());
+    c->launches++;
+  }
+  if (!is_device_pointer(u_mean)) LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  c->gamma_dirty = true;
+  return reset_inflow(c);
+}
+
+int lbm_set_vortices(lbm_ctx* c, int n, const double* pos, const double* sign, double sigma_v, double intensity) {
+  if (!c) return LBM_EINVAL;
+  if (n < 0 || (n > 0 && (!pos || !sign))) return fail(c, LBM_EINVAL, "lbm_set_vortices: n = %d, pos / sign must not be NULL", n);
+  if (!(sigma_v > 0.0) || !(intensity >= 0.0)) return fail(c, LBM_EINVAL, "lbm_set_vortices: sigma_v = %g must be > 0, intensity = %g >= 0", sigma_v, intensity);
+  int rc = materialise(c);             // S_t keeps the inflow it was formed with
+  if (rc != LBM_OK) return rc;
+  LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  if (c->vpos) { cudaFree(c->vpos); cudaFree(c->vsign); cudaFree(c->vgamma); c->device_bytes -= 4 * sizeof(double) * static_cast<size_t>(c->nv); }
+  c->vpos = c->vsign = c->vgamma = nullptr;
+  c->nv = 0;
+  if (n > 0) {
+    rc = dev_alloc(c, reinterpret_cast<void**>(&c->vpos), 2 * sizeof(double) * n);
+    if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->vsign), sizeof(double) * n);
+    if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->vgamma), sizeof(double) * n);
+    if (rc != LBM_OK) return rc;
+    LBM_CUDA(c, cudaMemcpyAsync(c->vpos, pos, 2 * sizeof(double) * n, cudaMemcpyHostToDevice, c->stream));
+    LBM_CUDA(c, cudaMemcpyAsync(c->vsign, sign, sizeof(double) * n, cudaMemcpyHostToDevice, c->stream));
+    LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->nv = n;
+  }
+  c->vm_sigma = sigma_v;
+  c->vm_intensity = intensity;
+  c->gamma_dirty = true;
+  return LBM_OK;
+}
+
+int lbm_get_inflow(lbm_ctx* c, void* u) {
+  if (!c) return LBM_EINVAL;
+  if (!u) return fail(c, LBM_EINVAL, "lbm_get_inflow: u is NULL");
+  if (!c->uin_mean) return fail(c, LBM_ESTATE, "lbm_get_inflow: no inflow field set (lbm_set_inflow)");
+  int rc = ensure_inflow(c, c->steps);
+  if (rc != LBM_OK) return rc;
+  const long long n = 3ll * c->ny * c->nz;
+  if (c->dtype == LBM_F64) {
+    LBM_CUDA(c, cudaMemcpyAsync(u, c->uin_field[c->uin_cur], static_cast<size_t>(n) * sizeof(double), cudaMemcpyDefault, c->stream));
+  } else {                               // fp64 -> fp32 through the idle field buffer
+    float* tmp = reinterpret_cast<float*>(c->uin_field[1 - c->uin_cur]);
+    lbm::k_convert<double, float><<<static_cast<unsigned>((n + 255) / 256), 256, 0, c->stream>>>(c->uin_field[c->uin_cur], tmp, n);
+    LBM_CUDA(c, cudaGetLastError());
+    c->launches++;
+    LBM_CUDA(c, cudaMemcpyAsync(u, tmp, static_cast<size_t>(n) * sizeof(float), cudaMemcpyDefault, c->stream));
+  }
+  if (!is_device_pointer(u)) LBM_CUDA(c, cudaStreamSynchronize(c->stream));
   return LBM_OK;
 }
 
@@ -619,6 +757,8 @@ int lbm_step(lbm_ctx* c, int n_steps, const lbm_params* params) {
       rc = launch_step(c, params, lbm::MODE_COLLIDE);          // S_t -> F_t
       c->phase = PHASE_POST;
     } else {
+      rc = ensure_inflow(c, c->steps + s);                     // Vortex Method inlet: the inflow S_t carries (Eq. 21)
+      if (rc != LBM_OK) return rc;
       rc = launch_step(c, params, lbm::MODE_STREAM_COLLIDE);   // F_{t-1} -> S_t -> F_t
     }
     if (rc != LBM_OK) return rc;

@@ -109,6 +109,8 @@ struct StepArgs {
   // HRR form (Eq. 7-11): u^(x,t) of every cell [3][N] (written by the MODE_UHAT_* pass, SOLID cells 0), Eq. 7 factor
   T* __restrict__ uhat;
   T sigma;
+  const double* __restrict__ uin_field;  // [3][nz][ny] per-cell inlet velocity (Vortex Method inlet / mean profile) or nullptr => u_in;
+                                         // fp64 for both dtypes: Eq. 21 normalises a gradient of this field (ill-conditioned in fp32)
   T u_wall[3];                    // velocity of the MOVINGWALL cells (only ever on the plane z = nz-1), reading G33
 };
 
@@ -455,6 +457,19 @@ __device__ __forceinline__ long long cell_index(int x, int y, int z, int nx, int
   return (static_cast<long long>(z) * ny + y) * nx + x;
 }
 
+// velocity imposed on the INLET cell (0, y, z): the per-cell inflow field when one is set (Eq. 21 / mean profile), else u_in
+template <typename T>
+__device__ __forceinline__ void inlet_velocity(const StepArgs<T>& a, int y, int z, T& ux, T& uy, T& uz) {
+  if (a.uin_field != nullptr) {
+    const long long P = static_cast<long long>(a.ny) * a.nz, c = static_cast<long long>(z) * a.ny + y;
+    ux = static_cast<T>(__ldg(a.uin_field + c));
+    uy = static_cast<T>(__ldg(a.uin_field + P + c));
+    uz = static_cast<T>(__ldg(a.uin_field + 2 * P + c));
+  } else {
+    ux = a.u_in[0];  uy = a.u_in[1];  uz = a.u_in[2];
+  }
+}
+
 // Pull of one cell (A1 + A7): g_i(x) = A[i][x - c_i], periodic wrap; a SOLID source means halfway bounce-back:
 // the cell's own opposite population (nbmask bit opp(i): the neighbour x + c_opp(i) = x - c_i is SOLID).  OUTLET
 // cells clamp the source of the c_x < 0 populations to their own plane (R7: ghost plane nx := plane nx-1), so for
@@ -483,7 +498,11 @@ __device__ __forceinline__ void pull_cell(const StepArgs<T>& a, int x, int y, in
     f[i] = own ? __ldg(a.fin + L.opp[i] * N + self) : __ldg(a.fin + i * N + s);
     if (own && sz == nz - 1 && (a.cls[s] & CLS_TYPE) == T_MOVING) f[i] += moving_wall_term<Q, T>(i, a.u_wall);
   }
-  if (type == T_INLET) inlet_fixup<Q, T>(f, a.u_in[0], a.u_in[1], a.u_in[2]);
+  if (type == T_INLET) {
+    T ux, uy, uz;
+    inlet_velocity<T>(a, y, z, ux, uy, uz);
+    inlet_fixup<Q, T>(f, ux, uy, uz);
+  }
 }
 
 // S_t of one non-SOLID cell, whatever the storage phase.  PULL = input holds F_{t-1}.
@@ -960,7 +979,9 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
     T fc[Q];
 #pragma unroll
     for (int i = 0; i < Q; ++i) fc[i] = f[i][0];
-    inlet_fixup<Q, T>(fc, a.u_in[0], a.u_in[1], a.u_in[2]);
+    T uwx, uwy, uwz;
+    inlet_velocity<T>(a, y, z, uwx, uwy, uwz);
+    inlet_fixup<Q, T>(fc, uwx, uwy, uwz);
 #pragma unroll
     for (int i = 0; i < Q; ++i) f[i][0] = fc[i];
   }
@@ -1141,6 +1162,107 @@ __global__ void __launch_bounds__(256) k_init_equilibrium(const T* __restrict__ 
 
 // ---- flag validation + classification ------------------------------------------------------------
 // cls = type | normal<<3 | ADJ | SPECIAL (see the top of this file).
+// ---- Vortex Method inflow (Eq. 18-21; readings G11, G34, G35) --------------------
+// Plane x = 0, d_inlet = (1,0,0); fields [3][nz][ny]; seeds (y_i, z_i) and signs are inputs.
+// k_vm_gamma (one block): A = number of INLET cells of the plane; Gamma_i = 4 s_i sqrt(pi A k_i / (3 N (2 ln 3 - 3 ln 2))),
+// k_i = 3/2 (|u_mean(p_i)| I)^2 with u_mean at the nearest cell (0 over a non-INLET cell).                    (Eq. 18-19)
+template <typename T>
+__global__ void __launch_bounds__(256) k_vm_gamma(const uint8_t* __restrict__ cls, int nx, int ny, int nz, const T* __restrict__ u_mean,
+                                                  int nv, const double* __restrict__ pos, const double* __restrict__ sign,
+                                                  double intensity, double* __restrict__ gamma) {
+  __shared__ long long part[256];
+  const long long P = static_cast<long long>(ny) * nz;
+  long long cnt = 0;
+  for (long long c = threadIdx.x; c < P; c += blockDim.x) cnt += ((cls[c * nx] & CLS_TYPE) == T_INLET) ? 1 : 0;
+  part[threadIdx.x] = cnt;
+  __syncthreads();
+  for (int s = 128; s > 0; s >>= 1) {
+    if (static_cast<int>(threadIdx.x) < s) part[threadIdx.x] += part[threadIdx.x + s];
+    __syncthreads();
+  }
+  const double A = static_cast<double>(part[0]);
+  const double PI = 3.14159265358979323846;
+  for (int i = threadIdx.x; i < nv; i += blockDim.x) {
+    int yi = static_cast<int>(floor(pos[2 * i] + 0.5)), zi = static_cast<int>(floor(pos[2 * i + 1] + 0.5));
+    yi = ((yi % ny) + ny) % ny;
+    zi = (zi < 0) ? 0 : ((zi >= nz) ? nz - 1 : zi);
+    const long long c = static_cast<long long>(zi) * ny + yi;
+    double k = 0.0;
+    if ((cls[c * nx] & CLS_TYPE) == T_INLET) {
+      const double a0 = static_cast<double>(u_mean[c]), a1 = static_cast<double>(u_mean[P + c]), a2 = static_cast<double>(u_mean[2 * P + c]);
+      const double um = sqrt(a0 * a0 + a1 * a1 + a2 * a2);
+      k = 1.5 * (um * intensity) * (um * intensity);
+    }
+    gamma[i] = 4.0 * sign[i] * sqrt(PI * A * k / (3.0 * nv * (2.0 * log(3.0) - 3.0 * log(2.0))));
+  }
+}
+
+// dtype <-> fp64 copies of the inflow plane (the inflow fields are kept in fp64 whatever the lattice dtype)
+template <typename A, typename B>
+__global__ void __launch_bounds__(256) k_convert(const A* __restrict__ in, B* __restrict__ out, long long n) {
+  const long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = static_cast<B>(in[i]);
+}
+
+// k_vm_inflow: one thread per cell of the inflow plane; the seeds are staged through shared memory 256 at a time.
+//   u_v(x) = 1/(2 pi) sum_i Gamma_i ((p_i - x) x d)(1 - exp(-r^2 / 2 sigma^2)) / r^2                           (Eq. 20)
+//   u(x)   = u_mean + u_v - (u_v . g^) d,  g^ = normalised in-plane central-difference gradient of u_prev . d   (Eq. 21)
+// A path bound by plain ALU arithmetic (ny nz nv summands of ~12 flops + one exp), off the bandwidth path.
+template <typename T>
+__global__ void __launch_bounds__(256) k_vm_inflow(const uint8_t* __restrict__ cls, int nx, int ny, int nz, const T* __restrict__ u_mean,
+                                                   const T* __restrict__ u_prev, int nv, const double* __restrict__ pos,
+                                                   const double* __restrict__ gamma, T sigma_v, T* __restrict__ out) {
+  __shared__ T sy[256], sz[256], sg[256];
+  const long long P = static_cast<long long>(ny) * nz;
+  const long long c = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  const bool in_plane = c < P;
+  const int z = in_plane ? static_cast<int>(c / ny) : 0, y = in_plane ? static_cast<int>(c - static_cast<long long>(z) * ny) : 0;
+  const bool inlet = in_plane && ((cls[c * nx] & CLS_TYPE) == T_INLET);
+  const T inv2s2 = T(1) / (T(2) * sigma_v * sigma_v);
+  T uvy = T(0), uvz = T(0);
+  for (int base = 0; base < nv; base += 256) {
+    const int i = base + threadIdx.x;
+    if (i < nv) {
+      sy[threadIdx.x] = static_cast<T>(pos[2 * i]);
+      sz[threadIdx.x] = static_cast<T>(pos[2 * i + 1]);
+      sg[threadIdx.x] = static_cast<T>(gamma[i] * (0.5 / 3.14159265358979323846));
+    }
+    __syncthreads();
+    const int m = (nv - base < 256) ? nv - base : 256;
+    if (inlet) {
+      for (int k = 0; k < m; ++k) {
+        const T ry = sy[k] - T(y), rz = sz[k] - T(z);
+        const T r2 = ry * ry + rz * rz;
+        if (r2 == T(0)) continue;
+        const T fac = sg[k] * (-expm1(-r2 * inv2s2)) / r2;
+        uvy += fac * rz;
+        uvz -= fac * ry;
+      }
+    }
+    __syncthreads();
+  }
+  if (!in_plane) return;
+  T o0 = u_mean[c], o1 = u_mean[P + c], o2 = u_mean[2 * P + c];
+  if (inlet) {
+    const int yp = (y + 1 == ny) ? 0 : y + 1, ym = (y == 0) ? ny - 1 : y - 1;
+    const long long row = static_cast<long long>(z) * ny;
+    const long long cyp = ((cls[(row + yp) * nx] & CLS_TYPE) == T_INLET) ? row + yp : c;
+    const long long cym = ((cls[(row + ym) * nx] & CLS_TYPE) == T_INLET) ? row + ym : c;
+    const long long czp = (z + 1 < nz && (cls[(c + ny) * nx] & CLS_TYPE) == T_INLET) ? c + ny : c;
+    const long long czm = (z >= 1 && (cls[(c - ny) * nx] & CLS_TYPE) == T_INLET) ? c - ny : c;
+    const T gy = T(0.5) * (u_prev[cyp] - u_prev[cym]), gz = T(0.5) * (u_prev[czp] - u_prev[czm]);
+    const T gn = sqrt(gy * gy + gz * gz);
+    T us = T(0);
+    if (gn > T(0)) us = -(uvy * gy + uvz * gz) / gn;
+    o0 += us;
+    o1 += uvy;
+    o2 += uvz;
+  }
+  out[c] = o0;
+  out[P + c] = o1;
+  out[2 * P + c] = o2;
+}
+
 // counters[0] = invalid flag bytes, [1] = wall cells (SOLID + MOVINGWALL), [2] = masked cells (non-wall, not plain bulk FLUID),
 // [4] = MOVINGWALL cells ([3] belongs to k_mark_list).
 template <int Q>

@@ -1,0 +1,110 @@
+"""T1 for the Vortex Method inlet (Eq. 18-21): the inflow field and the stepped state through the C
+ABI against orc_vm_inflow / orc_step_vm (pinned by tests/test_oracle_vm.py V1-V7), same seeded inputs, same tolerances."""
+import numpy as np
+import pytest
+
+import lbm_inputs as I
+import paper_2506_21804_b200 as P
+from oracle import oracle as O
+from parity_util import NP_DTYPE, TOL, field_error, nonsolid, oracle_inputs
+
+pytestmark = pytest.mark.gpu
+# Eq. 21 divides by the norm of a central difference of the previous inflow: rounding differences between the two sides (exp,
+# FMA contraction, summation order: ~1e-16) are amplified by |u_prev| / |grad u_prev| (1e2 .. 1e4 on these profiles) at every
+# step and fed back.  DESIGN.md (G35) derives 1e-9 for the fp64 path with the VM inlet; fp32 keeps 2e-5 (the inflow is fp64 inside).
+TOL_VM = {"f32": TOL["f32"], "f64": 1e-9}
+
+
+def _case(shape=(24, 32, 64), nv=40, sigma_v=3.0, extra=None):
+    cfg = I.make_config(3, shape=shape)
+    cfg["params"] = dict(cfg["params"], **(extra or {}))
+    vm = I.vm_inlet(shape, 1300, n_vortices=nv, sigma_v=sigma_v, intensity=0.2)
+    return cfg, vm
+
+
+def _gpu(cfg, vm, f, d, dtype, chunks):
+    nz, ny, nx = cfg["shape"]
+    npdt = NP_DTYPE[dtype]
+    par = P.LbmParams(**cfg["params"])
+    with P.LBM(cfg["Q"], nx, ny, nz, dtype) as sim:
+        sim.set_fields(f, d, cfg["flags"])
+        sim.set_inflow(vm["u_mean"].astype(npdt))
+        sim.set_vortices(vm["pos"], vm["sign"], vm["sigma_v"], vm["intensity"])
+        for n in chunks:
+            sim.step(n, par)
+        uin = np.empty((3, nz, ny), dtype=npdt)
+        sim.get_inflow(uin)
+        out = np.empty_like(f)
+        sim.get_populations(out)
+        return out, uin
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("coll", [0, 1])
+def test_vm_inlet_parity(dtype, coll):
+    cfg, vm = _case(extra=dict(collision=coll, sigma=0.7))
+    f, d = oracle_inputs(cfg, dtype)
+    um = vm["u_mean"].astype(NP_DTYPE[dtype]).astype(np.float64)
+    ref, uref = O.step_vm(f.astype(np.float64), um, um, vm["pos"], vm["sign"], vm["sigma_v"], vm["intensity"],
+                          d=d.astype(np.float64), flags=cfg["flags"], nsteps=10, nthreads=8, **cfg["params"])
+    got, uin = _gpu(cfg, vm, f, d, dtype, [10])
+    inl = (cfg["flags"][:, :, 0] & 15) == I.INLET
+    assert np.abs(uref[1:, inl]).max() > 1e-3                        # the vortices are there
+    assert field_error(uin[:, inl], uref[:, inl]) <= TOL_VM[dtype]
+    assert field_error(got, ref, nonsolid(cfg)) <= TOL_VM[dtype]
+    # chunked stepping with state reads in between (materialise path) forms every inflow field exactly once
+    got2, uin2 = _gpu(cfg, vm, f, d, dtype, [1, 3, 2, 4])
+    assert np.array_equal(got2, got) and np.array_equal(uin2, uin)
+
+
+def test_vm_inflow_field_alone_many_vortices_fp64():
+    """nv > 256 (several shared-memory batches), seeds on cell centres (r = 0 summand), walls in the plane"""
+    cfg, vm = _case(shape=(40, 48, 32), nv=700, sigma_v=5.0)
+    vm["pos"][:50] = np.floor(vm["pos"][:50])
+    f, d = oracle_inputs(cfg, "f64")
+    mask = ((cfg["flags"][:, :, 0] & 15) == I.INLET).astype(np.uint8)
+    u1 = O.vm_inflow(mask, vm["u_mean"], vm["u_mean"], vm["pos"], vm["sign"], vm["sigma_v"], vm["intensity"])
+    u2 = O.vm_inflow(mask, vm["u_mean"], u1, vm["pos"], vm["sign"], vm["sigma_v"], vm["intensity"])
+    nz, ny, nx = cfg["shape"]
+    with P.LBM(19, nx, ny, nz, "f64") as sim:
+        sim.set_fields(f, d, cfg["flags"])
+        sim.set_inflow(vm["u_mean"])
+        sim.set_vortices(vm["pos"], vm["sign"], vm["sigma_v"], vm["intensity"])
+        got = np.empty((3, nz, ny))
+        sim.get_inflow(got)
+        assert np.array_equal(got, vm["u_mean"])                       # before the first step: u_mean
+        sim.step(1, P.LbmParams(**cfg["params"]))
+        sim.get_inflow(got)
+        inl = mask.astype(bool)
+        assert field_error(got[:, inl], u1[:, inl]) <= 1e-13
+        sim.step(1, P.LbmParams(**cfg["params"]))
+        sim.get_inflow(got)
+        assert field_error(got[:, inl], u2[:, inl]) <= 1e-13
+        # the inlet plane of the state carries exactly that field
+        u = np.empty((3, nz, ny, nx))
+        sim.moments(None, u)
+        assert np.abs(u[:, :, :, 0][:, inl] - got[:, inl]).max() <= 1e-13
+
+
+def test_mean_profile_without_vortices_and_switching_back():
+    cfg, vm = _case()
+    f, d = oracle_inputs(cfg, "f64")
+    um = vm["u_mean"]
+    ref, _ = O.step_vm(f, um, um, np.zeros((0, 2)), np.zeros(0), 1.0, 0.0, d=d, flags=cfg["flags"], nsteps=5, **cfg["params"])
+    nz, ny, nx = cfg["shape"]
+    with P.LBM(19, nx, ny, nz, "f64") as sim:
+        sim.set_fields(f, d, cfg["flags"])
+        sim.set_inflow(um)
+        sim.step(5, P.LbmParams(**cfg["params"]))
+        out = np.empty_like(f)
+        sim.get_populations(out)
+        assert field_error(out, ref, nonsolid(cfg)) <= 1e-12
+        sim.set_inflow(None)                                             # back to the uniform params.u_in
+        sim.set_fields(f, d, cfg["flags"])
+        sim.step(5, P.LbmParams(**cfg["params"]))
+        sim.get_populations(out)
+        assert field_error(out, O.step(f, d=d, flags=cfg["flags"], nsteps=5, **cfg["params"]), nonsolid(cfg)) <= 1e-12
+        with pytest.raises(P.LbmError):
+            sim.get_inflow(np.empty((3, nz, ny)))
+        with pytest.raises(P.LbmError):
+            sim.set_vortices([[1.0, 1.0]], [1.0], 0.0, 0.1)
