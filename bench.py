@@ -54,6 +54,11 @@ WORKLOADS["config5_urban_cube_512_f32_hrr"] = (5, (512, 512, 512), "f32", HRR)
 for _n in (256, 512, 640):
     WORKLOADS["cavity_%d_f32" % _n] = (6, (_n, _n, _n), "f32")
 WORKLOADS["cavity_512_f32_hrr"] = (6, (512, 512, 512), "f32", HRR)
+# Vortex Method inlet (Eq. 18-21) on the config-3 channel: power-law mean profile, 256 seeded vortices of size 6 cells,
+# intensity 0.15; "_hrr_vm" = the paper's urban set-up as far as this build has it (HRR + Smagorinsky + HLBM + wall model + VM)
+VM = dict(n_vortices=256, sigma_v=6.0, intensity=0.15)
+WORKLOADS["config3_urban_channel_384x192x128_f32_vm"] = (3, None, "f32", {}, VM)
+WORKLOADS["config3_urban_channel_384x192x128_f32_hrr_vm"] = (3, None, "f32", HRR, VM)
 DEFAULT_WORKLOAD = "config3_urban_channel_384x192x128_f32"
 
 
@@ -61,6 +66,23 @@ def workload(name):
     """-> (config number, shape or None, dtype, extra lbm_params)"""
     w = WORKLOADS[name]
     return (w[0], w[1], w[2], dict(w[3]) if len(w) > 3 else {})
+
+
+def workload_vm(name, shape):
+    """Vortex Method inlet inputs of the workload (lbm_inputs.vm_inlet) or None"""
+    w = WORKLOADS[name]
+    if len(w) < 5:
+        return None
+    return I.vm_inlet(shape, 1300 + w[0], **w[4])
+
+
+def oracle_steps(O, f, cfg, vm, state, nsteps, nthreads):
+    """the oracle's step loop, with the VM inlet when the workload has one (state = the previous inflow, carried along)"""
+    kw = dict(d=cfg["d"], flags=cfg["flags"], nsteps=nsteps, nthreads=nthreads, **cfg["params"])
+    if vm is None:
+        return O.step(f, **kw), None
+    return O.step_vm(f, vm["u_mean"], vm["u_mean"] if state is None else state, vm["pos"], vm["sign"], vm["sigma_v"],
+                     vm["intensity"], **kw)
 
 
 def make_cfg(number, shape, extra):
@@ -160,15 +182,16 @@ class ClockSampler(threading.Thread):
         return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
-def cpu_oracle_time(cfg_number, sample_shape, nsteps, nthreads, extra):
+def cpu_oracle_time(cfg_number, sample_shape, nsteps, nthreads, extra, name):
     """Time the oracle, as it stands, on a bounded sample of the workload."""
     from oracle import oracle as O
     cfg = make_cfg(cfg_number, sample_shape, extra)
+    vm = workload_vm(name, cfg["shape"])
     f = O.init_equilibrium(cfg["Q"], cfg["rho"], cfg["u"])
     nonsolid = f[0].size if cfg["flags"] is None else int((~I.is_wall(cfg["flags"])).sum())
-    O.step(f, d=cfg["d"], flags=cfg["flags"], nsteps=1, nthreads=nthreads, **cfg["params"])     # warm-up
+    oracle_steps(O, f, cfg, vm, None, 1, nthreads)                                              # warm-up
     t0 = time.perf_counter()
-    O.step(f, d=cfg["d"], flags=cfg["flags"], nsteps=nsteps, nthreads=nthreads, **cfg["params"])
+    oracle_steps(O, f, cfg, vm, None, nsteps, nthreads)
     dt = time.perf_counter() - t0
     return nonsolid * nsteps / dt / 1e6, dt, cfg["shape"]
 
@@ -192,10 +215,10 @@ def run_reference(args, rank, world):
     cfg = make_cfg(number, sample, extra)
     f = O.init_equilibrium(cfg["Q"], cfg["rho"], cfg["u"])
     nonsolid = f[0].size if cfg["flags"] is None else int((~I.is_wall(cfg["flags"])).sum())
-    kw = dict(d=cfg["d"], flags=cfg["flags"], nthreads=cores, **cfg["params"])
-    f = O.step(f, nsteps=args.warmup, **kw)
+    vm = workload_vm(args.workload, cfg["shape"])
+    f, st = oracle_steps(O, f, cfg, vm, None, args.warmup, cores)
     t0 = time.perf_counter()
-    f = O.step(f, nsteps=args.steps, **kw)
+    f, st = oracle_steps(O, f, cfg, vm, st, args.steps, cores)
     dt = time.perf_counter() - t0
     value = nonsolid * args.steps / dt / 1e6
     sample_txt = "oracle (fp64, %d OpenMP threads) on the workload generator at (nz,ny,nx)=%s, %d steps" % (
@@ -269,6 +292,10 @@ def main():
     fl_d = None if cfg["flags"] is None else torch.from_numpy(cfg["flags"]).cuda()
     sim.set_geometry(d_d, fl_d)
     sim.init_equilibrium(rho_d, u_d)
+    vm = workload_vm(args.workload, cfg["shape"])
+    if vm is not None:
+        sim.set_inflow(torch.from_numpy(vm["u_mean"].astype(npdt)).cuda())
+        sim.set_vortices(vm["pos"], vm["sign"], vm["sigma_v"], vm["intensity"])
     n_solid = sim.query("solid_cells")
     n_fluid = N - n_solid
     tot0 = sim.totals()
@@ -340,7 +367,7 @@ def main():
             scale = min(1.0, (1.5e6 / base.prod()) ** (1.0 / 3.0))
             sample_shape = tuple(max(16, int(round(b * scale / 8)) * 8) for b in base)
             ns = 100   # ~1.5e8 cell updates: about 10 s of host work at the oracle's ~15 MLUPs
-        v, dt_cpu, shp = cpu_oracle_time(number, sample_shape, ns, cores, extra)
+        v, dt_cpu, shp = cpu_oracle_time(number, sample_shape, ns, cores, extra, args.workload)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": "fp64 oracle, %d OpenMP threads, workload generator at (nz,ny,nx)=%s, %d steps after 1 warm-up, %.1f s"
                          % (cores, str(tuple(shp)), ns, dt_cpu)}

@@ -65,6 +65,12 @@ struct lbm_ctx {
   double* vpos;  double* vsign;  double* vgamma;     // device [nv][2], [nv], [nv]
   double vm_sigma, vm_intensity;
   bool gamma_dirty;
+  // the inflow of level t+1 depends on the inflow of level t only, never on the lattice: it is formed on a side stream while
+  // step t runs (events order the two streams; two field buffers)
+  cudaStream_t vm_stream;
+  cudaEvent_t ev_vm, ev_step[2];
+  bool vm_pending;          // the newest field is still being written on vm_stream
+  long long ev_step_level[2];   // time level of the step after which ev_step[k] was recorded (-1: never)
   void* uhat;            // HRR form: u^(x,t) [3][N], allocated on the first HRR step
   int hrr_slab;          // HRR form: z-slices per slab of the two-pass step (0 = whole lattice)
   lbm_params last;       // parameters of the last lbm_step: the inlet rule is part of how S_t is formed from F_{t-1}
@@ -464,38 +470,79 @@ int classify(lbm_ctx* c, const uint8_t* cell_flags) {
 }
 
 // ---- Vortex Method inlet: host side (Eq. 18-21) ---------------------------------------------------------------------
-int vm_advance(lbm_ctx* c) {
+// main stream waits for a field that is still being formed on the side stream
+int vm_join(lbm_ctx* c) {
+  if (c->vm_pending) {
+    LBM_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_vm, 0));
+    c->vm_pending = false;
+  }
+  return LBM_OK;
+}
+
+// form the inflow of the next level from the current one, on stream st
+int vm_advance(lbm_ctx* c, cudaStream_t st) {
   const long long P = static_cast<long long>(c->ny) * c->nz;
   if (c->gamma_dirty && c->nv > 0) {
-    lbm::k_vm_gamma<double><<<1, 256, 0, c->stream>>>(c->cls, c->nx, c->ny, c->nz, c->uin_mean, c->nv, c->vpos, c->vsign,
-                                                       c->vm_intensity, c->vgamma);
+    lbm::k_vm_gamma<double><<<1, 256, 0, st>>>(c->cls, c->nx, c->ny, c->nz, c->uin_mean, c->nv, c->vpos, c->vsign,
+                                               c->vm_intensity, c->vgamma);
     LBM_CUDA(c, cudaGetLastError());
     c->launches++;
   }
   c->gamma_dirty = false;
-  const unsigned blocks = static_cast<unsigned>((P + 255) / 256);
-  lbm::k_vm_inflow<double><<<blocks, 256, 0, c->stream>>>(c->cls, c->nx, c->ny, c->nz, c->uin_mean, c->uin_field[c->uin_cur], c->nv,
-                                                          c->vpos, c->vgamma, c->vm_sigma, c->uin_field[1 - c->uin_cur]);
+  const unsigned blocks = static_cast<unsigned>((P + lbm::VM_CELLS - 1) / lbm::VM_CELLS);
+  lbm::k_vm_inflow<double><<<blocks, lbm::VM_CELLS * lbm::VM_SLICES, 0, st>>>(c->cls, c->nx, c->ny, c->nz, c->uin_mean, c->uin_field[c->uin_cur], c->nv,
+                                                   c->vpos, c->vgamma, c->vm_sigma, c->uin_field[1 - c->uin_cur]);
   LBM_CUDA(c, cudaGetLastError());
   c->launches++;
   c->uin_cur = 1 - c->uin_cur;
+  c->inflow_index++;
   return LBM_OK;
 }
 
 // the inflow field of time level t must be current before S_t is formed (pulled) for the first time
 int ensure_inflow(lbm_ctx* c, long long t) {
   if (!c->uin_mean) return LBM_OK;
+  int rc = vm_join(c);
+  if (rc != LBM_OK) return rc;
   while (c->inflow_index < t) {
-    int rc = vm_advance(c);
+    rc = vm_advance(c, c->stream);
     if (rc != LBM_OK) return rc;
-    c->inflow_index++;
   }
+  return LBM_OK;
+}
+
+// after the step of level t has been enqueued on the main stream: mark it, and form the inflow of level t+1 beside it
+int vm_prefetch(lbm_ctx* c, long long t) {
+  if (!c->uin_mean) return LBM_OK;
+  if (!c->vm_stream) {
+    int prio_lo = 0, prio_hi = 0;      // highest priority: its few blocks must not queue behind the step kernel's thousands
+    LBM_CUDA(c, cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+    LBM_CUDA(c, cudaStreamCreateWithPriority(&c->vm_stream, cudaStreamNonBlocking, prio_hi));
+    LBM_CUDA(c, cudaEventCreateWithFlags(&c->ev_vm, cudaEventDisableTiming));
+    LBM_CUDA(c, cudaEventCreateWithFlags(&c->ev_step[0], cudaEventDisableTiming));
+    LBM_CUDA(c, cudaEventCreateWithFlags(&c->ev_step[1], cudaEventDisableTiming));
+    c->ev_step_level[0] = c->ev_step_level[1] = -1;
+  }
+  const int k = static_cast<int>(t & 1);
+  LBM_CUDA(c, cudaEventRecord(c->ev_step[k], c->stream));
+  c->ev_step_level[k] = t;
+  if (c->inflow_index != t) return LBM_OK;
+  // the buffer about to be overwritten held level t-1: its last reader is the step of level t-1.  If that step's event is not
+  // on record (first step of a run, inputs just changed) wait for the step just enqueued instead (no overlap, once).
+  const int w = (c->ev_step_level[1 - k] == t - 1) ? 1 - k : k;
+  LBM_CUDA(c, cudaStreamWaitEvent(c->vm_stream, c->ev_step[w], 0));
+  int rc = vm_advance(c, c->vm_stream);
+  if (rc != LBM_OK) return rc;
+  LBM_CUDA(c, cudaEventRecord(c->ev_vm, c->vm_stream));
+  c->vm_pending = true;
   return LBM_OK;
 }
 
 // "previous inflow" := u_mean; the current time level is c->steps
 int reset_inflow(lbm_ctx* c) {
   if (!c->uin_mean) return LBM_OK;
+  { int rcj = vm_join(c); if (rcj != LBM_OK) return rcj; }
+  c->ev_step_level[0] = c->ev_step_level[1] = -1;      // inputs of the side stream change on the main stream: re-order once
   const size_t bytes = 3 * static_cast<size_t>(c->ny) * c->nz * sizeof(double);
   LBM_CUDA(c, cudaMemcpyAsync(c->uin_field[c->uin_cur], c->uin_mean, bytes, cudaMemcpyDeviceToDevice, c->stream));
   c->inflow_index = c->steps;
@@ -554,6 +601,11 @@ lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype) {
 void lbm_destroy(lbm_ctx* c) {
   if (!c) return;
   cudaStreamSynchronize(c->stream);
+  if (c->vm_stream) {
+    cudaStreamSynchronize(c->vm_stream);
+    cudaStreamDestroy(c->vm_stream);
+    cudaEventDestroy(c->ev_vm);  cudaEventDestroy(c->ev_step[0]);  cudaEventDestroy(c->ev_step[1]);
+  }
   cudaFree(c->f[0]);  cudaFree(c->f[1]);  cudaFree(c->d);  cudaFree(c->uhat);
   cudaFree(c->uin_mean);  cudaFree(c->uin_field[0]);  cudaFree(c->uin_field[1]);  cudaFree(c->vpos);  cudaFree(c->vsign);  cudaFree(c->vgamma);
   cudaFree(c->cls);  cudaFree(c->cls_alt);  cudaFree(c->flags_raw);
@@ -698,6 +750,9 @@ int lbm_set_vortices(lbm_ctx* c, int n, const double* pos, const double* sign, d
   if (!(sigma_v > 0.0) || !(intensity >= 0.0)) return fail(c, LBM_EINVAL, "lbm_set_vortices: sigma_v = %g must be > 0, intensity = %g >= 0", sigma_v, intensity);
   int rc = materialise(c);             // S_t keeps the inflow it was formed with
   if (rc != LBM_OK) return rc;
+  rc = vm_join(c);
+  if (rc != LBM_OK) return rc;
+  c->ev_step_level[0] = c->ev_step_level[1] = -1;
   LBM_CUDA(c, cudaStreamSynchronize(c->stream));
   if (c->vpos) { cudaFree(c->vpos); cudaFree(c->vsign); cudaFree(c->vgamma); c->device_bytes -= 4 * sizeof(double) * static_cast<size_t>(c->nv); }
   c->vpos = c->vsign = c->vgamma = nullptr;
@@ -761,6 +816,8 @@ int lbm_step(lbm_ctx* c, int n_steps, const lbm_params* params) {
       if (rc != LBM_OK) return rc;
       rc = launch_step(c, params, lbm::MODE_STREAM_COLLIDE);   // F_{t-1} -> S_t -> F_t
     }
+    if (rc != LBM_OK) return rc;
+    rc = vm_prefetch(c, c->steps + s);                         // inflow of the next level, beside this step
     if (rc != LBM_OK) return rc;
   }
   c->steps += n_steps;

@@ -1204,23 +1204,29 @@ __global__ void __launch_bounds__(256) k_convert(const A* __restrict__ in, B* __
   if (i < n) out[i] = static_cast<B>(in[i]);
 }
 
-// k_vm_inflow: one thread per cell of the inflow plane; the seeds are staged through shared memory 256 at a time.
+// k_vm_inflow: block = 64 cells of the inflow plane x 4 slices of the seeds (thread = one cell, every fourth seed); the seeds
+// are staged through shared memory 256 at a time, the four partial sums of a cell are combined through shared memory.
 //   u_v(x) = 1/(2 pi) sum_i Gamma_i ((p_i - x) x d)(1 - exp(-r^2 / 2 sigma^2)) / r^2                           (Eq. 20)
 //   u(x)   = u_mean + u_v - (u_v . g^) d,  g^ = normalised in-plane central-difference gradient of u_prev . d   (Eq. 21)
 // A path bound by plain ALU arithmetic (ny nz nv summands of ~12 flops + one exp), off the bandwidth path.
+constexpr int VM_CELLS = 64, VM_SLICES = 4;
 template <typename T>
-__global__ void __launch_bounds__(256) k_vm_inflow(const uint8_t* __restrict__ cls, int nx, int ny, int nz, const T* __restrict__ u_mean,
-                                                   const T* __restrict__ u_prev, int nv, const double* __restrict__ pos,
-                                                   const double* __restrict__ gamma, T sigma_v, T* __restrict__ out) {
-  __shared__ T sy[256], sz[256], sg[256];
+__global__ void __launch_bounds__(VM_CELLS * VM_SLICES) k_vm_inflow(const uint8_t* __restrict__ cls, int nx, int ny, int nz,
+                                                                    const T* __restrict__ u_mean, const T* __restrict__ u_prev, int nv,
+                                                                    const double* __restrict__ pos, const double* __restrict__ gamma,
+                                                                    T sigma_v, T* __restrict__ out) {
+  constexpr int NT = VM_CELLS * VM_SLICES;
+  __shared__ T sy[NT], sz[NT], sg[NT];
+  __shared__ T py[VM_SLICES][VM_CELLS], pz[VM_SLICES][VM_CELLS];
   const long long P = static_cast<long long>(ny) * nz;
-  const long long c = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  const int lc = threadIdx.x % VM_CELLS, slice = threadIdx.x / VM_CELLS;
+  const long long c = static_cast<long long>(blockIdx.x) * VM_CELLS + lc;
   const bool in_plane = c < P;
   const int z = in_plane ? static_cast<int>(c / ny) : 0, y = in_plane ? static_cast<int>(c - static_cast<long long>(z) * ny) : 0;
   const bool inlet = in_plane && ((cls[c * nx] & CLS_TYPE) == T_INLET);
   const T inv2s2 = T(1) / (T(2) * sigma_v * sigma_v);
   T uvy = T(0), uvz = T(0);
-  for (int base = 0; base < nv; base += 256) {
+  for (int base = 0; base < nv; base += NT) {
     const int i = base + threadIdx.x;
     if (i < nv) {
       sy[threadIdx.x] = static_cast<T>(pos[2 * i]);
@@ -1228,12 +1234,12 @@ __global__ void __launch_bounds__(256) k_vm_inflow(const uint8_t* __restrict__ c
       sg[threadIdx.x] = static_cast<T>(gamma[i] * (0.5 / 3.14159265358979323846));
     }
     __syncthreads();
-    const int m = (nv - base < 256) ? nv - base : 256;
+    const int m = (nv - base < NT) ? nv - base : NT;
     if (inlet) {
-      for (int k = 0; k < m; ++k) {
+      for (int k = slice; k < m; k += VM_SLICES) {
         const T ry = sy[k] - T(y), rz = sz[k] - T(z);
         const T r2 = ry * ry + rz * rz;
-        if (r2 == T(0)) continue;
+        if (r2 == T(0)) continue;                        // the summand tends to 0 at the seed itself
         const T fac = sg[k] * (-expm1(-r2 * inv2s2)) / r2;
         uvy += fac * rz;
         uvz -= fac * ry;
@@ -1241,7 +1247,12 @@ __global__ void __launch_bounds__(256) k_vm_inflow(const uint8_t* __restrict__ c
     }
     __syncthreads();
   }
-  if (!in_plane) return;
+  py[slice][lc] = uvy;
+  pz[slice][lc] = uvz;
+  __syncthreads();
+  if (slice != 0 || !in_plane) return;
+  uvy = (py[0][lc] + py[1][lc]) + (py[2][lc] + py[3][lc]);
+  uvz = (pz[0][lc] + pz[1][lc]) + (pz[2][lc] + pz[3][lc]);
   T o0 = u_mean[c], o1 = u_mean[P + c], o2 = u_mean[2 * P + c];
   if (inlet) {
     const int yp = (y + 1 == ny) ? 0 : y + 1, ym = (y == 0) ? ny - 1 : y - 1;
