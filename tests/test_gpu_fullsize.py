@@ -36,7 +36,7 @@ def _axis_crop(lo, n, closed):
     return idx, lo - a
 
 
-def _check_windows(cfg, dtype, windows, closed_axes, steps=S, u_scale=0.0):
+def _check_windows(cfg, dtype, windows, closed_axes, steps=S, u_scale=0.0, vm=None):
     """u_scale: velocity scale of the whole field (R12 normalises by the field's maximum; a window of fluid at rest has none)"""
     nz, ny, nx = cfg["shape"]
     Q = cfg["Q"]
@@ -47,6 +47,9 @@ def _check_windows(cfg, dtype, windows, closed_axes, steps=S, u_scale=0.0):
     par = P.LbmParams(**cfg["params"])
     with P.LBM(Q, nx, ny, nz, dtype) as sim:
         sim.set_fields(f, d, cfg["flags"])                  # host pointers, library defaults = bench configuration
+        if vm is not None:
+            sim.set_inflow(vm["u_mean"].astype(npdt))
+            sim.set_vortices(vm["pos"], vm["sign"], vm["sigma_v"], vm["intensity"])
         sim.step(steps, par)
         out = torch.empty((Q, nz, ny, nx), dtype=torch.float32 if dtype == "f32" else torch.float64, device="cuda")
         sim.get_populations(out)
@@ -54,6 +57,16 @@ def _check_windows(cfg, dtype, windows, closed_axes, steps=S, u_scale=0.0):
         u = torch.empty((3, nz, ny, nx), dtype=out.dtype, device="cuda")
         sim.moments(rho, u)
         sim.synchronize()
+    fields = None
+    if vm is not None:
+        # the inflow of every step on the WHOLE plane (it depends on all INLET cells and all seeds), from the oracle's Eq. 18-21;
+        # a crop then runs with that step's field as its "mean profile" and no vortices
+        mask = ((cfg["flags"][:, :, 0] & 15) == I.INLET).astype(np.uint8)
+        um = vm["u_mean"].astype(npdt).astype(np.float64)
+        fields, prev = [], um
+        for _ in range(steps):
+            prev = O.vm_inflow(mask, um, prev, vm["pos"], vm["sign"], vm["sigma_v"], vm["intensity"])
+            fields.append(prev)
     worst = 0.0
     for (z0, y0, x0) in windows:
         iz, wz = _axis_crop(z0, nz, closed_axes[0])
@@ -63,7 +76,14 @@ def _check_windows(cfg, dtype, windows, closed_axes, steps=S, u_scale=0.0):
         fc = np.ascontiguousarray(f[(slice(None),) + sel]).astype(np.float64)
         dc = None if d is None else np.ascontiguousarray(d[sel]).astype(np.float64)
         flc = None if cfg["flags"] is None else np.ascontiguousarray(cfg["flags"][sel])
-        ref = O.step(fc, d=dc, flags=flc, nsteps=steps, nthreads=min(O.max_threads(), 8), **cfg["params"])
+        if fields is None:
+            ref = O.step(fc, d=dc, flags=flc, nsteps=steps, nthreads=min(O.max_threads(), 8), **cfg["params"])
+        else:
+            ref = fc
+            for fld in fields:
+                uc = np.ascontiguousarray(fld[:, iz][:, :, iy])
+                ref, _ = O.step_vm(ref, uc, uc, np.zeros((0, 2)), np.zeros(0), 1.0, 0.0, d=dc, flags=flc, nsteps=1,
+                                   nthreads=min(O.max_threads(), 8), **cfg["params"])
         inner = (slice(None), slice(wz, wz + W), slice(wy, wy + W), slice(wx, wx + W))
         refw = ref[inner]
         gz, gy, gx = iz[wz:wz + W], iy[wy:wy + W], ix[wx:wx + W]
@@ -155,6 +175,15 @@ def test_config4_hrr_full_size_windows():
     wins = [tuple(min(max(v, 0), 512 - W) for v in w) for w in wins]
     wins += [(0, 0, 0), (504, 504, 504), (250, 0, 504)]
     _check_windows(cfg, "f32", wins, (False, False, False), steps=6)
+
+
+def test_config3_vm_inlet_full_size_windows():
+    """bench.py config3_urban_channel_384x192x128_f32_vm: Vortex Method inlet (256 seeds), windows on and behind the inflow plane"""
+    cfg = I.make_config(3)
+    nz, ny, nx = cfg["shape"]
+    vm = I.vm_inlet(cfg["shape"], 1303, n_vortices=256, sigma_v=6.0, intensity=0.15)
+    wins = [(1, 10, 0), (60, 100, 0), (nz - 1 - W, 50, 0), (30, ny - 4, 0), (90, 0, 0), (40, 150, 6), (1, 60, 150), (60, 90, 190)]
+    _check_windows(cfg, "f32", wins, (True, False, True), vm=vm)
 
 
 def test_cavity_full_size_windows():
