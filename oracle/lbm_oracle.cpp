@@ -22,6 +22,9 @@
 //   O4 inlet fix-up        l.155 "regularized local velocity boundary condition" (G15/R6)
 //   O4v Vortex Method inlet l.133-155, Eq. 18-21: per step the inflow velocity of every INLET cell from seeded
 //                          vortices (readings G11, G34, G35); feeds O4.  Pinned by V1-V7 in tests/test_oracle_vm.py
+//   O4p pressure outlet   l.255 "fixed local pressure condition" (reading G36): regularised local rule with rho
+//                          imposed and the normal velocity taken from the known populations.  PARITY UNPINNED against the
+//                          paper (not defined there); pinned as the mirror image of O4 + channel flow by B1-B4
 //   O3m moving wall       lid of the "established lid-driven cavity benchmark" (l.214): halfway bounce-back
 //                          off a wall moving with u_w: + 2 w_i rho_w (c_i.u_w)/c_s^2 on the returned population, rho_w = 1
 //                          (reading G33; the paper does not say how its lid is imposed -> PARITY UNPINNED against the
@@ -67,7 +70,7 @@
 namespace {
 
 constexpr int QMAX = 27;
-enum CellType : int { FLUID = 0, SOLID = 1, INLET = 2, OUTLET = 3, WALLMODEL = 4, MOVINGWALL = 5 };
+enum CellType : int { FLUID = 0, SOLID = 1, INLET = 2, OUTLET = 3, WALLMODEL = 4, MOVINGWALL = 5, POUTLET = 6 };
 
 struct Lattice {
   int Q = 0;
@@ -138,6 +141,7 @@ struct Params {           // the oracle's own copy of the step parameters (not s
   int collision;          // 0: BGK form of Eq. 6 (G1); 1: hybrid recursive-regularised (Eq. 6-11)
   double sigma;           // Eq. 7 hybridisation factor, in [0,1]
   double u_wall[3];       // velocity of the MOVINGWALL cells (lid of the lid-driven cavity, l.214; reading G33)
+  double rho_out;         // density (pressure / c_s^2) imposed on POUTLET cells (l.255 "fixed local pressure"; reading G36)
 };
 
 inline int cell_type(uint8_t flag) { return flag & 0x0F; }
@@ -373,6 +377,37 @@ void inlet_fixup_cell(const Lattice& L, double* g, const double uw[3]) {
   }
 }
 
+// O4p for one pressure-outlet cell on the plane x = nx-1 (outward normal +x, "fixed local
+// pressure condition"; reading G36: the regularised local boundary rule of O4 with the roles of density and normal velocity
+// exchanged).  Known after streaming: c_x >= 0; unknown: c_x < 0.  rho = rho_out is imposed, the normal velocity follows from
+// the known populations, u_x = (sum_{c_x=0} g + 2 sum_{c_x>0} g)/rho_out - 1, the tangential velocity is 0; then all
+// populations are replaced by f^eq + the second-order Hermite projection of the non-equilibrium stress, as in O4.
+void pressure_fixup_cell(const Lattice& L, double* g, double rho_out) {
+  double s0 = 0.0, sp = 0.0;
+  for (int i = 0; i < L.Q; ++i) {
+    if (L.c[i][0] == 0) s0 += g[i];
+    else if (L.c[i][0] > 0) sp += g[i];
+  }
+  const double uw[3] = {(s0 + 2.0 * sp) / rho_out - 1.0, 0.0, 0.0};
+  double feq[QMAX], n[QMAX];
+  for (int i = 0; i < L.Q; ++i) feq[i] = feq_i(L, i, rho_out, uw);
+  for (int i = 0; i < L.Q; ++i)
+    if (L.c[i][0] >= 0) n[i] = g[i] - feq[i];
+  for (int i = 0; i < L.Q; ++i)
+    if (L.c[i][0] < 0) n[i] = n[L.opp[i]];                 // bounce-back of the non-equilibrium part
+  double Pi[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+  for (int i = 0; i < L.Q; ++i)
+    for (int a = 0; a < 3; ++a)
+      for (int b = 0; b < 3; ++b) Pi[a][b] += L.c[i][a] * L.c[i][b] * n[i];
+  for (int i = 0; i < L.Q; ++i) {
+    double s = 0.0;
+    for (int a = 0; a < 3; ++a)
+      for (int b = 0; b < 3; ++b)
+        s += (L.c[i][a] * L.c[i][b] - ((a == b) ? 1.0 / 3.0 : 0.0)) * Pi[a][b];
+    g[i] = feq[i] + 4.5 * L.w[i] * s;
+  }
+}
+
 // ---- Vortex Method inflow: Eq. 18-21 ------------------------------------------
 // The inflow plane is x = 0 with d_inlet = (1,0,0); fields are [3][nz][ny] (component, z, y); mask[z][y] = 1 on INLET cells.
 // Seeds p_i = (y_i, z_i) in cell coordinates and signs s_i are INPUTS (the random numbers the method draws).
@@ -500,6 +535,13 @@ int orc_collide_cell_hrr(int Q, const double* fc, double d, const double* ub, do
   return 0;
 }
 
+int orc_pressure_fixup_cell(int Q, double* g, double rho_out) {
+  Lattice L;
+  if (!make_lattice(Q, L)) return -1;
+  pressure_fixup_cell(L, g, rho_out);
+  return 0;
+}
+
 int orc_inlet_fixup_cell(int Q, double* g, const double* uw) {
   Lattice L;
   if (!make_lattice(Q, L)) return -1;
@@ -533,7 +575,7 @@ int orc_init_equilibrium(int Q, int64_t N, const double* rho, const double* u, d
 }  // extern "C"
 namespace {
 int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const uint8_t* flags,
-             const double* par /* tau0, cs, use_hlbm, uin0, uin1, uin2, wm_enable, kappa, E, collision, sigma, uwall0, uwall1, uwall2 */,
+             const double* par /* tau0, cs, use_hlbm, uin0, uin1, uin2, wm_enable, kappa, E, collision, sigma, uwall0, uwall1, uwall2, rho_out */,
              int nsteps, int nthreads, VortexInlet* vm) {
   Lattice L;
   if (!make_lattice(Q, L)) return -1;
@@ -544,6 +586,7 @@ int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const u
   p.wm_enable = (par[6] != 0.0);  p.wm_kappa = par[7];  p.wm_E = par[8];
   p.collision = static_cast<int>(par[9]);  p.sigma = par[10];
   p.u_wall[0] = par[11];  p.u_wall[1] = par[12];  p.u_wall[2] = par[13];
+  p.rho_out = par[14];
   if (!(p.tau0 > 0.5) || p.cs_smago < 0.0) return -1;
   if (p.collision != 0 && p.collision != 1) return -1;
   if (p.collision == 1 && !(p.sigma >= 0.0 && p.sigma <= 1.0)) return -1;
@@ -651,7 +694,7 @@ int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const u
               int qp[3] = {xx, y, z}, qm[3] = {xx, y, z};
               qp[a] = wrap(pos[a] + 1, dim[a]);
               qm[a] = wrap(pos[a] - 1, dim[a]);
-              if (a == 0 && type == OUTLET) qp[0] = xx;
+              if (a == 0 && (type == OUTLET || type == POUTLET)) qp[0] = xx;
               if (a == 0 && type == INLET) qm[0] = xx;
               const int64_t sp = (static_cast<int64_t>(qp[2]) * ny + qp[1]) * nx + qp[0];
               const int64_t sm = (static_cast<int64_t>(qm[2]) * ny + qm[1]) * nx + qm[0];
@@ -713,6 +756,13 @@ int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const u
         for (int y = 0; y < ny; ++y)
           for (int xx = 0; xx < nx; ++xx) {
             const int64_t x = (static_cast<int64_t>(z) * ny + y) * nx + xx;
+            if (cell_type(flags[x]) == POUTLET) {                        // O4p
+              double gp[QMAX];
+              for (int i = 0; i < Q; ++i) gp[i] = nxt[i * N + x];
+              pressure_fixup_cell(L, gp, p.rho_out);
+              for (int i = 0; i < Q; ++i) nxt[i * N + x] = gp[i];
+              continue;
+            }
             if (cell_type(flags[x]) != INLET) continue;
             double gc[QMAX];
             for (int i = 0; i < Q; ++i) gc[i] = nxt[i * N + x];

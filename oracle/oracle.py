@@ -43,6 +43,7 @@ def lib():
         L.orc_collide_cell.argtypes = [ctypes.c_int, _c_dp, ctypes.c_double, _c_dp, ctypes.c_double,
                                        ctypes.c_double, _c_dp, _c_dp]
         L.orc_inlet_fixup_cell.argtypes = [ctypes.c_int, _c_dp, _c_dp]
+        L.orc_pressure_fixup_cell.argtypes = [ctypes.c_int, _c_dp, ctypes.c_double]
         L.orc_feq3.argtypes = [ctypes.c_int, ctypes.c_double, _c_dp, _c_dp]
         L.orc_collide_cell_hrr.argtypes = [ctypes.c_int, _c_dp, ctypes.c_double, _c_dp, ctypes.c_double,
                                            ctypes.c_double, ctypes.c_double, _c_dp, _c_dp, _c_dp]
@@ -127,6 +128,12 @@ def inlet_fixup_cell(Q, g, uw):
     return g
 
 
+def pressure_fixup_cell(Q, g, rho_out):
+    g = _f64(g).copy()
+    assert lib().orc_pressure_fixup_cell(Q, _dp(g), float(rho_out)) == 0
+    return g
+
+
 def spalding(up, kappa=0.41, E=9.8):
     return lib().orc_spalding(float(up), float(kappa), float(E))
 
@@ -151,11 +158,11 @@ def init_equilibrium(Q, rho, u):
 
 
 def pack_params(tau0, cs_smago=0.0, use_hlbm=0, u_in=(0.0, 0.0, 0.0), wm_enable=0, wm_kappa=0.41, wm_E=9.8,
-                collision=0, sigma=1.0, u_wall=(0.0, 0.0, 0.0)):
+                collision=0, sigma=1.0, u_wall=(0.0, 0.0, 0.0), rho_out=1.0):
     """collision: 0 = BGK form (G1), 1 = HRR (Eq. 6-11); sigma = Eq. 7 hybridisation factor; u_wall = velocity of the
     MOVINGWALL cells (G33)."""
     return np.array([tau0, cs_smago, float(use_hlbm), u_in[0], u_in[1], u_in[2], float(wm_enable),
-                     wm_kappa, wm_E, float(collision), sigma, u_wall[0], u_wall[1], u_wall[2]], dtype=np.float64)
+                     wm_kappa, wm_E, float(collision), sigma, u_wall[0], u_wall[1], u_wall[2], rho_out], dtype=np.float64)
 
 
 def step(f, d=None, flags=None, nsteps=1, nthreads=1, **params):
