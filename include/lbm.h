@@ -23,10 +23,10 @@
  *        porosity   [nz][ny][nx]      d in [0,1]; Eq. 12 convention: 0 = fluid, 1 = solid (G2)
  *        cell_flags [nz][ny][nx]      uint8
  *        rho        [nz][ny][nx],  u[3][nz][ny][nx]
- *  - FLAG BYTE: low nibble = type {0 FLUID, 1 SOLID, 2 INLET, 3 OUTLET, 4 WALLMODEL, 5 MOVINGWALL}.  For
+ *  - FLAG BYTE: low nibble = type {0 FLUID, 1 SOLID, 2 INLET, 3 OUTLET, 4 WALLMODEL, 5 MOVINGWALL, 6 POUTLET}.  For
  *    WALLMODEL the high nibble is the wall-normal code {0:+x, 1:-x, 2:+y, 3:-y, 4:+z, 5:-z}
  *    pointing from the wall into the fluid (config 3 floor cells: 0x44); otherwise it must be 0.
- *    INLET is accepted only on the plane x = 0, OUTLET only on x = nx-1, MOVINGWALL (a SOLID cell that moves with
+ *    INLET is accepted only on the plane x = 0, OUTLET (zero gradient) and POUTLET (fixed pressure) only on x = nx-1, MOVINGWALL (a SOLID cell that moves with
  *    lbm_params.u_wall; inert like SOLID) only on z = nz-1.
  *  - POPULATION ORDER (R1): i = 0 rest; 1..h (h = (Q-1)/2) the directions whose first non-zero
  *    component is +1 sorted by (|c|^2, -cx, -cy, -cz); h+1..Q-1 their negatives, opp(i) = i +- h.
@@ -51,7 +51,7 @@ extern "C" {
 enum { LBM_OK = 0, LBM_EINVAL = -1, LBM_ENOMEM = -2, LBM_ECUDA = -3, LBM_ESTATE = -4 };
 enum { LBM_D3Q19 = 19, LBM_D3Q27 = 27 };
 enum { LBM_F32 = 4, LBM_F64 = 8 };
-enum { LBM_FLUID = 0, LBM_SOLID = 1, LBM_INLET = 2, LBM_OUTLET = 3, LBM_WALLMODEL = 4, LBM_MOVINGWALL = 5 };
+enum { LBM_FLUID = 0, LBM_SOLID = 1, LBM_INLET = 2, LBM_OUTLET = 3, LBM_WALLMODEL = 4, LBM_MOVINGWALL = 5, LBM_POUTLET = 6 };
 enum { LBM_COLLISION_BGK = 0, LBM_COLLISION_HRR = 1 };
 
 typedef struct lbm_ctx lbm_ctx; /* opaque; owned by the library */
@@ -76,6 +76,9 @@ typedef struct {
                      * bounce-back off a moving wall (reading G33): the population i returning from the wall gains
                      * 2 w_i rho_w (c_i.u_w)/c_s^2 with rho_w = 1 and c_i pointing from the wall into the fluid;
                      * the HRR form's FD stencil sees u^ = u_wall on those cells                       */
+  double rho_out;   /* density (= pressure / c_s^2) imposed on POUTLET cells: the "fixed local pressure" outlet of the urban case
+                     * (l.255; reading G36: regularised local rule, normal velocity from the known populations, tangential
+                     * velocity 0).  0 means the default 1.                                                   */
 } lbm_params;
 
 /* Create a context for an nx x ny x nz lattice (nx fastest in memory).

@@ -160,6 +160,7 @@ lbm::StepArgs<T> make_args(const lbm_ctx* c, const lbm_params* p, int in, int ou
   a.uhat = static_cast<T*>(c->uhat);
   a.sigma = p ? static_cast<T>(p->sigma) : T(1);
   for (int k = 0; k < 3; ++k) a.u_wall[k] = p ? static_cast<T>(p->u_wall[k]) : T(0);
+  a.rho_out = (p && p->rho_out > 0.0) ? static_cast<T>(p->rho_out) : T(1);
   a.uin_field = c->uin_mean ? c->uin_field[c->uin_cur] : nullptr;
   if (p) {
     a.tau0 = static_cast<T>(p->tau0);
@@ -348,6 +349,7 @@ int check_params(lbm_ctx* c, const lbm_params* p) {
   if (p->wm_enable && (!(p->wm_kappa > 0.0) || !(p->wm_E > 0.0)))
     return fail(c, LBM_EINVAL, "lbm_step: wm_enable needs wm_kappa > 0 and wm_E > 0");
   if (!(p->u_in[0] < 1.0)) return fail(c, LBM_EINVAL, "lbm_step: u_in[0] = %g must be < 1", p->u_in[0]);
+  if (p->rho_out < 0.0) return fail(c, LBM_EINVAL, "lbm_step: rho_out = %g must be > 0 (0 = default 1)", p->rho_out);
   if (p->collision != LBM_COLLISION_BGK && p->collision != LBM_COLLISION_HRR)
     return fail(c, LBM_EINVAL, "lbm_step: collision = %d must be 0 (BGK) or 1 (HRR)", p->collision);
   if (p->collision == LBM_COLLISION_HRR && !(p->sigma >= 0.0 && p->sigma <= 1.0))
@@ -415,7 +417,7 @@ int classify(lbm_ctx* c, const uint8_t* cell_flags) {
   LBM_CUDA(c, cudaMemcpyAsync(h, c->counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
   LBM_CUDA(c, cudaStreamSynchronize(c->stream));
   if (h[0] != 0)
-    return fail(c, LBM_EINVAL, "cell_flags: %llu invalid flag byte(s) (type > 5, bad high nibble, INLET off x=0, OUTLET off x=nx-1 or MOVINGWALL off z=nz-1)", h[0]);
+    return fail(c, LBM_EINVAL, "cell_flags: %llu invalid flag byte(s) (type > 6, bad high nibble, INLET off x=0, OUTLET / POUTLET off x=nx-1 or MOVINGWALL off z=nz-1)", h[0]);
   // compact list of the cells the vector kernel leaves to its list blocks
   const int SV = 32 / c->dtype;        // cells per 32-byte sector of a population row
   long long n_list = 0;

@@ -17,7 +17,7 @@
 
 namespace lbm {
 
-enum : int { T_FLUID = 0, T_SOLID = 1, T_INLET = 2, T_OUTLET = 3, T_WM = 4, T_MOVING = 5 };
+enum : int { T_FLUID = 0, T_SOLID = 1, T_INLET = 2, T_OUTLET = 3, T_WM = 4, T_MOVING = 5, T_POUTLET = 6 };
 // wall cells: resting SOLID (1 = 001b) and MOVINGWALL (5 = 101b) -- the only types whose two low bits are 01
 __host__ __device__ constexpr bool is_wall(int cls_or_type) { return (cls_or_type & 3) == 1; }
 // internal class byte: bits 0-2 type, bits 3-5 wall-normal code,
@@ -111,6 +111,7 @@ struct StepArgs {
   T sigma;
   const double* __restrict__ uin_field;  // [3][nz][ny] per-cell inlet velocity (Vortex Method inlet / mean profile) or nullptr => u_in;
                                          // fp64 for both dtypes: Eq. 21 normalises a gradient of this field (ill-conditioned in fp32)
+  T rho_out;                      // density imposed on POUTLET cells (reading G36)
   T u_wall[3];                    // velocity of the MOVINGWALL cells (only ever on the plane z = nz-1), reading G33
 };
 
@@ -396,6 +397,46 @@ __device__ __forceinline__ void inlet_fixup(T (&g)[Q], T uwx, T uwy, T uwz) {
   }
 }
 
+// O4p / reading G36: regularised pressure outlet on a cell of the plane x = nx-1 (outward normal +x): rho_out is
+// imposed, the normal velocity follows from the known populations (c_x >= 0), tangential velocity 0 -- the mirror image of
+// inlet_fixup, which does the rest.
+template <int Q, typename T>
+__device__ __forceinline__ void pressure_fixup(T (&g)[Q], T rho_out) {
+  constexpr Stencil<Q> L{};
+  constexpr int H = (Q - 1) / 2;
+  T s0 = T(0), sp = T(0);
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    if (L.c[i][0] == 0) s0 += g[i];
+    else if (L.c[i][0] > 0) sp += g[i];
+  }
+  const T ux = (s0 + T(2) * sp) / rho_out - T(1);
+  // reflect in x (directions with c_x != 0 swap with their x-mirror), impose -u_x as on an inlet, reflect back
+  T m[Q];
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    int j = i;
+    if (L.c[i][0] != 0) {
+#pragma unroll
+      for (int k = 1; k < Q; ++k)
+        if (L.c[k][0] == -L.c[i][0] && L.c[k][1] == L.c[i][1] && L.c[k][2] == L.c[i][2]) j = k;
+    }
+    m[i] = g[j];
+  }
+  (void)H;
+  inlet_fixup<Q, T>(m, -ux, T(0), T(0));
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    int j = i;
+    if (L.c[i][0] != 0) {
+#pragma unroll
+      for (int k = 1; k < Q; ++k)
+        if (L.c[k][0] == -L.c[i][0] && L.c[k][1] == L.c[i][1] && L.c[k][2] == L.c[i][2]) j = k;
+    }
+    g[i] = m[j];
+  }
+}
+
 // Spalding's law (Eq. 17) and the two root solves of reading R8, in double for both dtypes (only the
 // wall-model cells take this path).  Returns U1 / U2.
 //   unknown p = u2+ = U2 / u_tau:   p Sp(p) = Re,  Re = U2 y2 / nu      (Eq. 15-16: y2+ u2+ = U2 y2 / nu)
@@ -503,6 +544,7 @@ __device__ __forceinline__ void pull_cell(const StepArgs<T>& a, int x, int y, in
     inlet_velocity<T>(a, y, z, ux, uy, uz);
     inlet_fixup<Q, T>(f, ux, uy, uz);
   }
+  if (type == T_POUTLET) pressure_fixup<Q, T>(f, a.rho_out);
 }
 
 // S_t of one non-SOLID cell, whatever the storage phase.  PULL = input holds F_{t-1}.
@@ -573,7 +615,7 @@ template <typename T>
 __device__ __forceinline__ void fd_strain_cell(const StepArgs<T>& a, int x, int y, int z, int type, T (&S)[6]) {
   const int nx = a.nx, ny = a.ny, nz = a.nz;
   const int xm = (type == T_INLET) ? x : ((x == 0) ? nx - 1 : x - 1);
-  const int xp = (type == T_OUTLET) ? x : ((x == nx - 1) ? 0 : x + 1);
+  const int xp = (type == T_OUTLET || type == T_POUTLET) ? x : ((x == nx - 1) ? 0 : x + 1);
   const int ym = (y == 0) ? ny - 1 : y - 1, yp = (y == ny - 1) ? 0 : y + 1;
   const int zm = (z == 0) ? nz - 1 : z - 1, zp = (z == nz - 1) ? 0 : z + 1;
   T D[3][3];   // D[a][b] = u^_b(x + e_a) - u^_b(x - e_a)
@@ -837,6 +879,7 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
   // INLET (only ever at x = 0) / OUTLET (only ever at x = nx-1; SPECIAL if next to a wall) cells
   const bool inlet0 = mine && (x0 == 0) && ((clsw & CLS_TYPE) == T_INLET);
   const bool outletN = mine && (qx == nvec - 1) && (((clsw >> (8 * (V - 1))) & CLS_TYPE) == T_OUTLET);
+  const bool poutN = mine && (qx == nvec - 1) && (((clsw >> (8 * (V - 1))) & CLS_TYPE) == T_POUTLET);
 
   T f[Q][V];
   T d[V];
@@ -985,6 +1028,14 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
 #pragma unroll
     for (int i = 0; i < Q; ++i) f[i][0] = fc[i];
   }
+  if (PULL && poutN) {                                       // G36 on the x = nx-1 cell of the row
+    T fc[Q];
+#pragma unroll
+    for (int i = 0; i < Q; ++i) fc[i] = f[i][V - 1];
+    pressure_fixup<Q, T>(fc, a.rho_out);
+#pragma unroll
+    for (int i = 0; i < Q; ++i) f[i][V - 1] = fc[i];
+  }
   if constexpr (mode_uhat(MODE)) {                            // first pass of the HRR form: u^(x,t) (Eq. 12), SOLID cells 0
     T uo[3][V];
 #pragma unroll
@@ -1020,7 +1071,7 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
           T left = (v > 0) ? gu[5 * b + 4][v > 0 ? v - 1 : 0] : gl[b];
           T right = (v < V - 1) ? gu[5 * b + 4][v < V - 1 ? v + 1 : 0] : gr[b];
           if (v == 0 && inlet0) left = gu[5 * b + 4][0];
-          if (v == V - 1 && outletN) right = gu[5 * b + 4][V - 1];
+          if (v == V - 1 && (outletN || poutN)) right = gu[5 * b + 4][V - 1];
           D[0][b] = right - left;
           D[1][b] = gu[5 * b + 0][v] - gu[5 * b + 1][v];
           D[2][b] = gu[5 * b + 2][v] - gu[5 * b + 3][v];
@@ -1287,10 +1338,10 @@ __global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ fl
   const long long self = cell_index(x, y, z, nx, ny);
   const uint8_t fl = flags[self];
   const int type = fl & 0x0F, hi = fl >> 4;
-  bool bad = type > T_MOVING;
+  bool bad = type > T_POUTLET;
   if (type == T_WM) bad = bad || hi > 5; else bad = bad || hi != 0;
   if (type == T_INLET && x != 0) bad = true;
-  if (type == T_OUTLET && x != nx - 1) bad = true;
+  if ((type == T_OUTLET || type == T_POUTLET) && x != nx - 1) bad = true;
   if (type == T_MOVING && z != nz - 1) bad = true;
   if (bad) { atomicAdd(counters, 1ull); return; }
   uint32_t m = 0u;
