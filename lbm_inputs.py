@@ -9,12 +9,12 @@ these generators take their structure and stand in for them (DESIGN.md "Input re
 
 All randomness: numpy.random.Generator(numpy.random.PCG64(seed)), seed = 1000 + config number.
 Array layouts: rho[nz,ny,nx], u[3,nz,ny,nx], d[nz,ny,nx] float64; flags[nz,ny,nx] uint8.
-Flag byte: low nibble {0 FLUID, 1 SOLID, 2 INLET, 3 OUTLET, 4 WALLMODEL, 5 MOVINGWALL, 6 POUTLET}; WALLMODEL carries the
+Flag byte: low nibble {0 FLUID, 1 SOLID, 2 INLET, 3 OUTLET, 4 WALLMODEL, 5 MOVINGWALL, 6 POUTLET, 7 SLIPWALL}; WALLMODEL carries the
 wall-normal code in the high nibble {0:+x,1:-x,2:+y,3:-y,4:+z,5:-z}.
 """
 import numpy as np
 
-FLUID, SOLID, INLET, OUTLET, WALLMODEL, MOVINGWALL, POUTLET = 0, 1, 2, 3, 4, 5, 6
+FLUID, SOLID, INLET, OUTLET, WALLMODEL, MOVINGWALL, POUTLET, SLIPWALL = 0, 1, 2, 3, 4, 5, 6, 7
 WM_FLOOR = 0x44  # WALLMODEL with normal +z
 
 
@@ -260,4 +260,4 @@ def cavity_flags(shape):
 def is_wall(flags):
     """cells that are walls (resting SOLID or MOVINGWALL): inert, excluded from every comparison of fluid values"""
     t = flags & 0x0F
-    return (t == SOLID) | (t == MOVINGWALL)
+    return (t == SOLID) | (t == MOVINGWALL) | (t == SLIPWALL)

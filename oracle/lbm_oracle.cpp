@@ -25,6 +25,9 @@
 //   O4p pressure outlet   l.255 "fixed local pressure condition" (reading G36): regularised local rule with rho
 //                          imposed and the normal velocity taken from the known populations.  PARITY UNPINNED against the
 //                          paper (not defined there); pinned as the mirror image of O4 + channel flow by B1-B4
+//   O3s full-slip wall    l.255 "outer walls using full slip boundaries" (reading G37): specular reflection at halfway
+//                          walls; wall-normal axes found from the single-axis neighbours.  Pinned by W1-W3 (a slip channel IS the mirror-extended
+//                          periodic domain, bit for bit; tangential momentum conserved; uniform flow is a fixed point)
 //   O3m moving wall       lid of the "established lid-driven cavity benchmark" (l.214): halfway bounce-back
 //                          off a wall moving with u_w: + 2 w_i rho_w (c_i.u_w)/c_s^2 on the returned population, rho_w = 1
 //                          (reading G33; the paper does not say how its lid is imposed -> PARITY UNPINNED against the
@@ -55,7 +58,7 @@
 //
 // Layouts (all row-major, x fastest): f[Q][nz][ny][nx] double, d[nz][ny][nx] double,
 // flag[nz][ny][nx] uint8.  Cell index = (z*ny + y)*nx + x.
-// Flag byte: low nibble type {0 FLUID,1 SOLID,2 INLET,3 OUTLET,4 WALLMODEL,5 MOVINGWALL}; for WALLMODEL the
+// Flag byte: low nibble type {0 FLUID,1 SOLID,2 INLET,3 OUTLET,4 WALLMODEL,5 MOVINGWALL,6 POUTLET,7 SLIPWALL}; for WALLMODEL the
 // high nibble is the wall-normal code {0:+x,1:-x,2:+y,3:-y,4:+z,5:-z} (wall -> fluid).
 // =====================================================================================
 #include <cmath>
@@ -70,7 +73,7 @@
 namespace {
 
 constexpr int QMAX = 27;
-enum CellType : int { FLUID = 0, SOLID = 1, INLET = 2, OUTLET = 3, WALLMODEL = 4, MOVINGWALL = 5, POUTLET = 6 };
+enum CellType : int { FLUID = 0, SOLID = 1, INLET = 2, OUTLET = 3, WALLMODEL = 4, MOVINGWALL = 5, POUTLET = 6, SLIPWALL = 7 };
 
 struct Lattice {
   int Q = 0;
@@ -146,7 +149,7 @@ struct Params {           // the oracle's own copy of the step parameters (not s
 
 inline int cell_type(uint8_t flag) { return flag & 0x0F; }
 // a wall cell (resting SOLID or MOVINGWALL): inert, never collided, bounces populations back (R5, G33)
-inline bool is_wall(int type) { return type == SOLID || type == MOVINGWALL; }
+inline bool is_wall(int type) { return type == SOLID || type == MOVINGWALL || type == SLIPWALL; }
 
 // A4.  Eq. 11 (l.94) truncated after the H(2) term, c_s^2 = 1/3:
 // f_i^eq = w_i rho (1 + 3 c.u + 4.5 (c.u)^2 - 1.5 u.u)
@@ -731,6 +734,36 @@ int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const u
             const int64_t s = (static_cast<int64_t>(sz) * ny + sy) * nx + sx;
             const int stype = flags ? cell_type(flags[s]) : FLUID;
             double v = is_wall(stype) ? fstar[L.opp[i] * N + x] : fstar[i * N + s];
+            if (stype == SLIPWALL) {
+              // full-slip wall (l.255 "outer walls using full slip boundaries", reading G37): specular reflection at
+              // the halfway wall.  The wall-normal axes are those along which the cell's own single-axis neighbour
+              // x - c_ia e_a is a slip wall cell: the population left the fluid cell x' = x - c_i + sum_a c_ia e_a with the
+              // velocity c_i' = c_i with those components reversed.  No such axis (a convex edge met diagonally), or a wall
+              // at x': plain bounce-back.
+              int cr[3] = {L.c[i][0], L.c[i][1], L.c[i][2]};
+              int pr[3] = {sx, sy, sz};
+              const int pos[3] = {xx, y, z}, dim[3] = {nx, ny, nz};
+              bool any = false;
+              for (int a = 0; a < 3; ++a) {
+                if (L.c[i][a] == 0) continue;
+                int q[3] = {xx, y, z};
+                q[a] = wrap(pos[a] - L.c[i][a], dim[a]);
+                if (cell_type(flags[(static_cast<int64_t>(q[2]) * ny + q[1]) * nx + q[0]]) == SLIPWALL) {
+                  cr[a] = -cr[a];
+                  pr[a] = pos[a];
+                  any = true;
+                }
+              }
+              if (any) {
+                const int64_t xr = (static_cast<int64_t>(pr[2]) * ny + pr[1]) * nx + pr[0];
+                if (!is_wall(cell_type(flags[xr]))) {
+                  int ir = -1;
+                  for (int k = 0; k < Q; ++k)
+                    if (L.c[k][0] == cr[0] && L.c[k][1] == cr[1] && L.c[k][2] == cr[2]) ir = k;
+                  v = fstar[ir * N + xr];
+                }
+              }
+            }
             if (stype == MOVINGWALL)   // moving-wall bounce-back (G33): + 2 w_i rho_w (c_i . u_w) / c_s^2, rho_w = 1, c_i = wall -> fluid
               v += 6.0 * L.w[i] * (L.c[i][0] * p.u_wall[0] + L.c[i][1] * p.u_wall[1] + L.c[i][2] * p.u_wall[2]);
             nxt[i * N + x] = v;
