@@ -23,11 +23,14 @@
  *        porosity   [nz][ny][nx]      d in [0,1]; Eq. 12 convention: 0 = fluid, 1 = solid (G2)
  *        cell_flags [nz][ny][nx]      uint8
  *        rho        [nz][ny][nx],  u[3][nz][ny][nx]
- *  - FLAG BYTE: low nibble = type {0 FLUID, 1 SOLID, 2 INLET, 3 OUTLET, 4 WALLMODEL, 5 MOVINGWALL, 6 POUTLET}.  For
+ *  - FLAG BYTE: low nibble = type {0 FLUID, 1 SOLID, 2 INLET, 3 OUTLET, 4 WALLMODEL, 5 MOVINGWALL, 6 POUTLET, 7 SLIPWALL}.  For
  *    WALLMODEL the high nibble is the wall-normal code {0:+x, 1:-x, 2:+y, 3:-y, 4:+z, 5:-z}
  *    pointing from the wall into the fluid (config 3 floor cells: 0x44); otherwise it must be 0.
  *    INLET is accepted only on the plane x = 0, OUTLET (zero gradient) and POUTLET (fixed pressure) only on x = nx-1, MOVINGWALL (a SOLID cell that moves with
  *    lbm_params.u_wall; inert like SOLID) only on z = nz-1.
+ *    SLIPWALL is a wall cell (inert like SOLID) with full slip (l.255; reading G37): a population pulled from it is the specular
+ *    image -- it comes from the fluid cell x - c_i + sum_a c_ia e_a with the components a of c_i reversed, a = the axes along
+ *    which the cell's single-axis neighbour x - c_ia e_a is a SLIPWALL cell; no such axis, or a wall at that cell: bounce-back.
  *  - POPULATION ORDER (R1): i = 0 rest; 1..h (h = (Q-1)/2) the directions whose first non-zero
  *    component is +1 sorted by (|c|^2, -cx, -cy, -cz); h+1..Q-1 their negatives, opp(i) = i +- h.
  *  - STATE (G12/R2): the state S_t is the set of PRE-collision populations f_i(x,t) of Eq. 6.
@@ -51,7 +54,7 @@ extern "C" {
 enum { LBM_OK = 0, LBM_EINVAL = -1, LBM_ENOMEM = -2, LBM_ECUDA = -3, LBM_ESTATE = -4 };
 enum { LBM_D3Q19 = 19, LBM_D3Q27 = 27 };
 enum { LBM_F32 = 4, LBM_F64 = 8 };
-enum { LBM_FLUID = 0, LBM_SOLID = 1, LBM_INLET = 2, LBM_OUTLET = 3, LBM_WALLMODEL = 4, LBM_MOVINGWALL = 5, LBM_POUTLET = 6 };
+enum { LBM_FLUID = 0, LBM_SOLID = 1, LBM_INLET = 2, LBM_OUTLET = 3, LBM_WALLMODEL = 4, LBM_MOVINGWALL = 5, LBM_POUTLET = 6, LBM_SLIPWALL = 7 };
 enum { LBM_COLLISION_BGK = 0, LBM_COLLISION_HRR = 1 };
 
 typedef struct lbm_ctx lbm_ctx; /* opaque; owned by the library */

@@ -43,8 +43,8 @@ struct lbm_ctx {
   void* cub_tmp;
   size_t cub_tmp_bytes;
   int* list_count_dev;
-  unsigned long long* counters;  // device [5]
-  long long n_moving;            // MOVINGWALL cells of the accepted geometry
+  unsigned long long* counters;  // device [6]
+  long long n_moving, n_slip;    // MOVINGWALL / SLIPWALL cells of the accepted geometry
   double* totals_dev;            // device [5]
   void* staging;         // host<->device bounce buffer, grown on demand
   size_t staging_bytes;
@@ -209,7 +209,7 @@ int launch_one(lbm_ctx* c, const lbm_params* p, int in, int out, int z0, int nzs
     }
     grid.z = nzs + a.list_z;
     if (grid.z == 0) return LBM_OK;
-    if (c->n_moving > 0 && may_meet_lid && lbm::mode_pulls(MODE)) lbm::k_step_vec<Q, T, MODE, COLL, true><<<grid, block, 0, c->stream>>>(a);
+    if (((c->n_moving > 0 && may_meet_lid) || c->n_slip > 0) && lbm::mode_pulls(MODE)) lbm::k_step_vec<Q, T, MODE, COLL, true><<<grid, block, 0, c->stream>>>(a);
     else                                          lbm::k_step_vec<Q, T, MODE, COLL, false><<<grid, block, 0, c->stream>>>(a);
   } else {
     if (nzs == 0) return LBM_OK;
@@ -260,7 +260,7 @@ int launch_hrr_t(lbm_ctx* c, const lbm_params* p, int in, int out) {
 template <int Q, typename T>
 int launch_bgk_pull_t(lbm_ctx* c, const lbm_params* p, int in, int out) {
   const int nz = c->nz;
-  if (c->n_moving == 0 || nz < 8)
+  if (c->n_moving == 0 || c->n_slip > 0 || nz < 8)
     return launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 0, nz, true);
   int rc = launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 1, nz - 3, true, false);
   if (rc == LBM_OK) rc = launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, nz - 2, 2, false);
@@ -406,18 +406,18 @@ int classify(lbm_ctx* c, const uint8_t* cell_flags) {
   } else {
     LBM_CUDA(c, cudaMemsetAsync(c->flags_raw, 0, c->N, c->stream));
   }
-  LBM_CUDA(c, cudaMemsetAsync(c->counters, 0, 5 * sizeof(unsigned long long), c->stream));
+  LBM_CUDA(c, cudaMemsetAsync(c->counters, 0, 6 * sizeof(unsigned long long), c->stream));
   dim3 grid, block;
   launch_dims(c, grid, block);
   if (c->Q == 19) lbm::k_classify<19><<<grid, block, 0, c->stream>>>(c->flags_raw, c->cls_alt, c->nx, c->ny, c->nz, c->counters);
   else            lbm::k_classify<27><<<grid, block, 0, c->stream>>>(c->flags_raw, c->cls_alt, c->nx, c->ny, c->nz, c->counters);
   LBM_CUDA(c, cudaGetLastError());
   c->launches++;
-  unsigned long long h[5];
+  unsigned long long h[6];
   LBM_CUDA(c, cudaMemcpyAsync(h, c->counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
   LBM_CUDA(c, cudaStreamSynchronize(c->stream));
   if (h[0] != 0)
-    return fail(c, LBM_EINVAL, "cell_flags: %llu invalid flag byte(s) (type > 6, bad high nibble, INLET off x=0, OUTLET / POUTLET off x=nx-1 or MOVINGWALL off z=nz-1)", h[0]);
+    return fail(c, LBM_EINVAL, "cell_flags: %llu invalid flag byte(s) (type > 7, bad high nibble, INLET off x=0, OUTLET / POUTLET off x=nx-1 or MOVINGWALL off z=nz-1)", h[0]);
   // compact list of the cells the vector kernel leaves to its list blocks
   const int SV = 32 / c->dtype;        // cells per 32-byte sector of a population row
   long long n_list = 0;
@@ -468,6 +468,7 @@ int classify(lbm_ctx* c, const uint8_t* cell_flags) {
   c->n_solid = static_cast<long long>(h[1]);
   c->n_masked = static_cast<long long>(h[2]);
   c->n_moving = static_cast<long long>(h[4]);
+  c->n_slip = static_cast<long long>(h[5]);
   return LBM_OK;
 }
 
@@ -587,7 +588,7 @@ lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype) {
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->cls_alt), N);
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->flags_raw), N);
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->nbmask), static_cast<size_t>(N) * sizeof(uint32_t));
-  if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->counters), 5 * sizeof(unsigned long long));
+  if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->counters), 6 * sizeof(unsigned long long));
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->totals_dev), 5 * sizeof(double));
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->list_count_dev), sizeof(int));
   if (rc == LBM_OK && cudaMemset(c->cls, 0, N) != cudaSuccess) rc = fail(c, LBM_ECUDA, "cudaMemset failed");

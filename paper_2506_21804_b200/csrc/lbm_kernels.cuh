@@ -17,9 +17,9 @@
 
 namespace lbm {
 
-enum : int { T_FLUID = 0, T_SOLID = 1, T_INLET = 2, T_OUTLET = 3, T_WM = 4, T_MOVING = 5, T_POUTLET = 6 };
-// wall cells: resting SOLID (1 = 001b) and MOVINGWALL (5 = 101b) -- the only types whose two low bits are 01
-__host__ __device__ constexpr bool is_wall(int cls_or_type) { return (cls_or_type & 3) == 1; }
+enum : int { T_FLUID = 0, T_SOLID = 1, T_INLET = 2, T_OUTLET = 3, T_WM = 4, T_MOVING = 5, T_POUTLET = 6, T_SLIP = 7 };
+// wall cells: resting SOLID (1), MOVINGWALL (5) and SLIPWALL (7): bits 1, 5, 7 of 0xA2
+__host__ __device__ constexpr bool is_wall(int cls_or_type) { return ((0xA2 >> (cls_or_type & 7)) & 1) != 0; }
 // internal class byte: bits 0-2 type, bits 3-5 wall-normal code,
 //   bit 6 = ADJ:     the (non-SOLID) cell has at least one SOLID lattice neighbour (nbmask[] says which);
 //   bit 7 = SPECIAL: the cell needs the per-cell path (list blocks): WALLMODEL cells (A8) and OUTLET cells with a
@@ -498,6 +498,46 @@ __device__ __forceinline__ long long cell_index(int x, int y, int z, int nx, int
   return (static_cast<long long>(z) * ny + y) * nx + x;
 }
 
+// Full-slip wall (reading G37): the population with velocity c = (cx,cy,cz) (wall -> fluid) that the cell (x,y,z)
+// pulls from a SLIPWALL source is the specular image: it left the fluid cell x' = x - c + sum_a c_a e_a with the velocity c with the
+// components a reversed, a = the axes along which the cell's single-axis neighbour x - c_a e_a is a slip wall.  No such axis, or a
+// wall at x': `fallback` (plain bounce-back).  sx0 = the x coordinate of the source as pulled (OUTLET cells clamp it).
+// Rare path (cells next to a slip wall only): kept out of line.
+template <int Q, typename T>
+__device__ __noinline__ T slip_pull(const StepArgs<T>& a, int x, int y, int z, int cx, int cy, int cz, int sx0, T fallback) {
+  constexpr Stencil<Q> L{};
+  const int pos[3] = {x, y, z}, dim[3] = {a.nx, a.ny, a.nz}, c[3] = {cx, cy, cz};
+  int cr[3] = {cx, cy, cz};
+  int pr[3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const int t = pos[k] - c[k];
+    pr[k] = (t < 0) ? t + dim[k] : ((t >= dim[k]) ? t - dim[k] : t);
+  }
+  const int wx = pr[0];
+  pr[0] = sx0;
+  bool any = false;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    if (c[k] == 0) continue;
+    int q[3] = {x, y, z};
+    q[k] = (k == 0) ? wx : pr[k];
+    if ((a.cls[cell_index(q[0], q[1], q[2], a.nx, a.ny)] & CLS_TYPE) == T_SLIP) {
+      cr[k] = -c[k];
+      pr[k] = pos[k];
+      any = true;
+    }
+  }
+  if (!any) return fallback;
+  const long long xr = cell_index(pr[0], pr[1], pr[2], a.nx, a.ny);
+  if (is_wall(a.cls[xr])) return fallback;
+  int ir = 0;
+#pragma unroll
+  for (int k = 1; k < Q; ++k)
+    if (L.c[k][0] == cr[0] && L.c[k][1] == cr[1] && L.c[k][2] == cr[2]) ir = k;
+  return __ldg(a.fin + static_cast<long long>(ir) * a.N + xr);
+}
+
 // velocity imposed on the INLET cell (0, y, z): the per-cell inflow field when one is set (Eq. 21 / mean profile), else u_in
 template <typename T>
 __device__ __forceinline__ void inlet_velocity(const StepArgs<T>& a, int y, int z, T& ux, T& uy, T& uz) {
@@ -537,7 +577,11 @@ __device__ __forceinline__ void pull_cell(const StepArgs<T>& a, int x, int y, in
     bool own = (i > 0) && ((nbm >> L.opp[i]) & 1u);
     if (L.c[i][0] == -1 && type == T_OUTLET) own = is_wall(a.cls[s]);
     f[i] = own ? __ldg(a.fin + L.opp[i] * N + self) : __ldg(a.fin + i * N + s);
-    if (own && sz == nz - 1 && (a.cls[s] & CLS_TYPE) == T_MOVING) f[i] += moving_wall_term<Q, T>(i, a.u_wall);
+    if (own) {
+      const int st = a.cls[s] & CLS_TYPE;
+      if (st == T_MOVING) f[i] += moving_wall_term<Q, T>(i, a.u_wall);
+      else if (st == T_SLIP) f[i] = slip_pull<Q, T>(a, x, y, z, L.c[i][0], L.c[i][1], L.c[i][2], sx, f[i]);
+    }
   }
   if (type == T_INLET) {
     T ux, uy, uz;
@@ -814,7 +858,7 @@ __device__ __forceinline__ void ld_uhat_nb(const T* pu, long long N, int dyp, in
 // of the cells of SPECIAL sectors (A8 wall model; OUTLET cells next to a wall), one cell per thread: the masked
 // boundary kernel as a block role of the same launch (scheduled first, overlaps with the row blocks).
 // Everything else -- bulk, solid-adjacent (read-side bounce-back), INLET and OUTLET cells -- runs in the vector path.
-// MW: the geometry holds MOVINGWALL cells (compiled out otherwise: the test costs the wall-adjacent warps registers).
+// MW: the launch may meet MOVINGWALL / SLIPWALL cells (compiled out otherwise: the test costs the wall-adjacent warps registers).
 template <int Q, typename T, int MODE, int COLL, bool MW>
 __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ StepArgs<T> a) {
   constexpr Stencil<Q> L{};
@@ -858,11 +902,12 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
   if (active) secw = ld_cls_sector(a.cls + row + (x0 & ~(SV - 1)), T(0));
   constexpr unsigned long long SPECIAL_ALL = (SV == 8) ? 0x8080808080808080ull : 0x80808080ull;
   constexpr uint32_t VMASK = rep_byte(0xffu, V);
-  constexpr uint32_t TYPE_ALL = rep_byte(0x03u, V);         // is_wall: the two low type bits are 01
-  constexpr uint32_t SOLID_ALL = rep_byte(0x01u, V);
   constexpr uint32_t ADJ_ALL = rep_byte(0x40u, V);
   const uint32_t clsw = static_cast<uint32_t>(secw >> (8 * (x0 & (SV - 1)))) & VMASK;
-  const bool all_solid = !active || ((clsw & TYPE_ALL) == SOLID_ALL);
+  unsigned wall_bits = 0;             // which cells of the vector are walls (bit v)
+#pragma unroll
+  for (int v = 0; v < V; ++v) wall_bits |= is_wall(static_cast<int>(clsw >> (8 * v))) ? (1u << v) : 0u;
+  const bool all_solid = !active || (wall_bits == ((1u << V) - 1u));
   const bool special = (secw & SPECIAL_ALL) != 0;
   // an all-SOLID vector whose 128-byte line holds a non-SOLID vector stores zeros, so that the line is written whole
   const unsigned live_lanes = __ballot_sync(FULL, active && !all_solid);
@@ -872,9 +917,7 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
   const bool mine = active && !all_solid && !special;       // this thread computes and stores the vector
   const bool doload = active && !all_solid;                 // neighbours may need its lanes' values
   // which cells of the vector are SOLID (bit v)
-  unsigned solid_bits = 0;
-#pragma unroll
-  for (int v = 0; v < V; ++v) solid_bits |= is_wall(static_cast<int>(clsw >> (8 * v))) ? (1u << v) : 0u;
+  const unsigned solid_bits = wall_bits;
   const bool adj = mine && PULL && ((clsw & ADJ_ALL) != 0);
   // INLET (only ever at x = 0) / OUTLET (only ever at x = nx-1; SPECIAL if next to a wall) cells
   const bool inlet0 = mine && (x0 == 0) && ((clsw & CLS_TYPE) == T_INLET);
@@ -996,13 +1039,11 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
       for (int v = 0; v < V; ++v)
         if (nbm[v] & (1u << j)) f[L.opp[j]][v] = __ldg(pown + static_cast<long long>(j) * N + v);
     }
-    // moving wall (G33): MOVINGWALL cells exist only on the plane z = nz-1, so only directions towards that plane can
-    // meet one (block-uniform test); the neighbour's class byte decides
-    if (MW && (z >= nz - 2 || z == 0)) {
+    // moving wall (G33) / slip wall (G37): the class byte of the wall the population bounced off decides (this kernel variant
+    // runs only where the geometry has such cells: the lid slices, or everywhere with slip walls)
+    if (MW) {
 #pragma unroll
       for (int j = 1; j < Q; ++j) {
-        const int zn = z + L.c[j][2];
-        if (((zn < 0) ? zn + nz : ((zn >= nz) ? zn - nz : zn)) != nz - 1) continue;
         const long long off = static_cast<long long>((L.c[j][1] == 0) ? 0 : ((L.c[j][1] == 1) ? dyp : dym)) +
                               static_cast<long long>((L.c[j][2] == 0) ? 0 : ((L.c[j][2] == 1) ? dzp : dzm));
         const uint8_t* pc = a.cls + self + off;
@@ -1012,7 +1053,14 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
             int ex = v + L.c[j][0];
             if (L.c[j][0] == -1 && v == 0) ex = exl;
             if (L.c[j][0] == 1 && v == V - 1) ex = exr;
-            if ((pc[ex] & CLS_TYPE) == T_MOVING) f[L.opp[j]][v] += moving_wall_term<Q, T>(L.opp[j], a.u_wall);
+            const int st = pc[ex] & CLS_TYPE;
+            if (st == T_MOVING) f[L.opp[j]][v] += moving_wall_term<Q, T>(L.opp[j], a.u_wall);
+            else if (st == T_SLIP) {
+              const int xg = x0 + v;
+              const int t = xg + L.c[j][0];
+              f[L.opp[j]][v] = slip_pull<Q, T>(a, xg, y, z, -L.c[j][0], -L.c[j][1], -L.c[j][2],
+                                               (t < 0) ? t + nx : ((t >= nx) ? t - nx : t), f[L.opp[j]][v]);
+            }
           }
         }
       }
@@ -1326,7 +1374,7 @@ __global__ void __launch_bounds__(VM_CELLS * VM_SLICES) k_vm_inflow(const uint8_
 }
 
 // counters[0] = invalid flag bytes, [1] = wall cells (SOLID + MOVINGWALL), [2] = masked cells (non-wall, not plain bulk FLUID),
-// [4] = MOVINGWALL cells ([3] belongs to k_mark_list).
+// [4] = MOVINGWALL cells, [5] = SLIPWALL cells ([3] belongs to k_mark_list).
 template <int Q>
 __global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ flags, uint8_t* __restrict__ cls,
                                                   int nx, int ny, int nz, unsigned long long* __restrict__ counters) {
@@ -1338,7 +1386,7 @@ __global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ fl
   const long long self = cell_index(x, y, z, nx, ny);
   const uint8_t fl = flags[self];
   const int type = fl & 0x0F, hi = fl >> 4;
-  bool bad = type > T_POUTLET;
+  bool bad = type > T_SLIP;
   if (type == T_WM) bad = bad || hi > 5; else bad = bad || hi != 0;
   if (type == T_INLET && x != 0) bad = true;
   if ((type == T_OUTLET || type == T_POUTLET) && x != nx - 1) bad = true;
@@ -1361,6 +1409,7 @@ __global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ fl
                                    (special ? CLS_SPECIAL : 0));
   if (is_wall(type)) atomicAdd(counters + 1, 1ull);
   if (type == T_MOVING) atomicAdd(counters + 4, 1ull);
+  if (type == T_SLIP) atomicAdd(counters + 5, 1ull);
   else if (adj || type != T_FLUID) atomicAdd(counters + 2, 1ull);
 }
 
