@@ -82,6 +82,10 @@ typedef struct {
   double rho_out;   /* density (= pressure / c_s^2) imposed on POUTLET cells: the "fixed local pressure" outlet of the urban case
                      * (l.255; reading G36: regularised local rule, normal velocity from the known populations, tangential
                      * velocity 0).  0 means the default 1.                                                   */
+  int fringe_len;   /* fringe zone in front of the outlet plane (l.255 "with fringe zone"; reading G38): over the last fringe_len
+                     * cells in x the molecular viscosity rises as nu_mo (1 + fringe_factor xi^2), xi = (x - (nx-1-fringe_len)) /
+                     * fringe_len in [0,1] (a sponge that damps what reaches the outlet).  0 = no fringe zone.              */
+  double fringe_factor;
 } lbm_params;
 
 /* Create a context for an nx x ny x nz lattice (nx fastest in memory).
@@ -146,7 +150,7 @@ int lbm_get_inflow(lbm_ctx* ctx, void* u);
  * z-slab of the lattice (u^ pass, then the fused step) and 3 more values of dtype per
  * cell of device memory (allocated on the first HRR step; LBM_ENOMEM if that fails).  Asynchronous.
  * Errors: LBM_EINVAL (NULL ctx/params, n_steps < 0, tau0 <= 0.5, cs_smago < 0, wm_enable with
- * wm_kappa <= 0 or wm_E <= 0, collision not 0/1, sigma outside [0,1] with HRR), LBM_ESTATE (no state
+ * wm_kappa <= 0 or wm_E <= 0, collision not 0/1, sigma outside [0,1] with HRR, rho_out < 0, fringe_len < 0, fringe_factor < 0), LBM_ESTATE (no state
  * set yet), LBM_ECUDA. */
 int lbm_step(lbm_ctx* ctx, int n_steps, const lbm_params* params);
 

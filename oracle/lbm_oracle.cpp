@@ -28,6 +28,9 @@
 //   O3s full-slip wall    l.255 "outer walls using full slip boundaries" (reading G37): specular reflection at halfway
 //                          walls; wall-normal axes found from the single-axis neighbours.  Pinned by W1-W3 (a slip channel IS the mirror-extended
 //                          periodic domain, bit for bit; tangential momentum conserved; uniform flow is a fixed point)
+//   O2f fringe zone       l.255 "outlet using a fixed local pressure condition with fringe zone" (reading G38): a sponge,
+//                          nu_mo(x) = nu_mo (1 + A xi^2) over the last L cells in x.  PARITY UNPINNED against the paper (neither
+//                          the kind of fringe nor its profile is printed); pinned as stated by Z1-Z3
 //   O3m moving wall       lid of the "established lid-driven cavity benchmark" (l.214): halfway bounce-back
 //                          off a wall moving with u_w: + 2 w_i rho_w (c_i.u_w)/c_s^2 on the returned population, rho_w = 1
 //                          (reading G33; the paper does not say how its lid is imposed -> PARITY UNPINNED against the
@@ -145,6 +148,8 @@ struct Params {           // the oracle's own copy of the step parameters (not s
   double sigma;           // Eq. 7 hybridisation factor, in [0,1]
   double u_wall[3];       // velocity of the MOVINGWALL cells (lid of the lid-driven cavity, l.214; reading G33)
   double rho_out;         // density (pressure / c_s^2) imposed on POUTLET cells (l.255 "fixed local pressure"; reading G36)
+  int fringe_len;         // fringe zone in front of the outlet plane (l.255; reading G38): the last fringe_len cells in x
+  double fringe_factor;   // nu_mo(x) = nu_mo (1 + fringe_factor xi^2), xi = (x - (nx-1-fringe_len)) / fringe_len in [0,1]
 };
 
 inline int cell_type(uint8_t flag) { return flag & 0x0F; }
@@ -578,7 +583,7 @@ int orc_init_equilibrium(int Q, int64_t N, const double* rho, const double* u, d
 }  // extern "C"
 namespace {
 int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const uint8_t* flags,
-             const double* par /* tau0, cs, use_hlbm, uin0, uin1, uin2, wm_enable, kappa, E, collision, sigma, uwall0, uwall1, uwall2, rho_out */,
+             const double* par /* tau0, cs, use_hlbm, uin0, uin1, uin2, wm_enable, kappa, E, collision, sigma, uwall0, uwall1, uwall2, rho_out, fringe_len, fringe_factor */,
              int nsteps, int nthreads, VortexInlet* vm) {
   Lattice L;
   if (!make_lattice(Q, L)) return -1;
@@ -590,6 +595,8 @@ int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const u
   p.collision = static_cast<int>(par[9]);  p.sigma = par[10];
   p.u_wall[0] = par[11];  p.u_wall[1] = par[12];  p.u_wall[2] = par[13];
   p.rho_out = par[14];
+  p.fringe_len = static_cast<int>(par[15]);  p.fringe_factor = par[16];
+  if (p.fringe_len < 0 || p.fringe_factor < 0.0) return -1;
   if (!(p.tau0 > 0.5) || p.cs_smago < 0.0) return -1;
   if (p.collision != 0 && p.collision != 1) return -1;
   if (p.collision == 1 && !(p.sigma >= 0.0 && p.sigma <= 1.0)) return -1;
@@ -688,6 +695,12 @@ int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const u
             const int32_t k = wm_slot[x];
             ub[0] = uB[3 * k];  ub[1] = uB[3 * k + 1];  ub[2] = uB[3 * k + 2];
           }
+          // fringe zone (G38): the molecular viscosity rises quadratically over the last fringe_len cells before the outlet
+          double tau0x = p.tau0;
+          if (p.fringe_len > 0 && xx > nx - 1 - p.fringe_len) {
+            const double xi = static_cast<double>(xx - (nx - 1 - p.fringe_len)) / p.fringe_len;
+            tau0x = 0.5 + (p.tau0 - 0.5) * (1.0 + p.fringe_factor * xi * xi);
+          }
           if (p.collision == 1) {
             // S^FD_ab = (D_a u^_b + D_b u^_a) / 2, D_a g = (g(x+e_a) - g(x-e_a)) / 2; periodic wrap, except
             // that the ghost planes beyond the INLET / OUTLET planes copy those planes (G32)
@@ -707,9 +720,9 @@ int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const u
             for (int a = 0; a < 3; ++a)
               for (int b = 0; b < 3; ++b) S[a][b] = 0.5 * (D[a][b] + D[b][a]);
             const double sig = (type == WALLMODEL && p.wm_enable) ? 0.0 : p.sigma;   // l.131
-            collide_cell_hrr(L, fc, dd, ub, p.tau0, p.cs_smago, sig, S, fs, nullptr);
+            collide_cell_hrr(L, fc, dd, ub, tau0x, p.cs_smago, sig, S, fs, nullptr);
           } else {
-            collide_cell(L, fc, dd, ub, p.tau0, p.cs_smago, fs, nullptr);
+            collide_cell(L, fc, dd, ub, tau0x, p.cs_smago, fs, nullptr);
           }
           for (int i = 0; i < Q; ++i) fstar[i * N + x] = fs[i];
         }

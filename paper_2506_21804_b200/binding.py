@@ -29,10 +29,11 @@ class LbmParams(ctypes.Structure):
     _fields_ = [("tau0", ctypes.c_double), ("cs_smago", ctypes.c_double), ("use_hlbm", ctypes.c_int),
                 ("u_in", ctypes.c_double * 3), ("wm_enable", ctypes.c_int), ("wm_kappa", ctypes.c_double),
                 ("wm_E", ctypes.c_double), ("collision", ctypes.c_int), ("sigma", ctypes.c_double),
-                ("u_wall", ctypes.c_double * 3), ("rho_out", ctypes.c_double)]
+                ("u_wall", ctypes.c_double * 3), ("rho_out", ctypes.c_double),
+                ("fringe_len", ctypes.c_int), ("fringe_factor", ctypes.c_double)]
 
     def __init__(self, tau0, cs_smago=0.0, use_hlbm=0, u_in=(0.0, 0.0, 0.0), wm_enable=0, wm_kappa=0.41, wm_E=9.8,
-                 collision=0, sigma=1.0, u_wall=(0.0, 0.0, 0.0), rho_out=1.0):
+                 collision=0, sigma=1.0, u_wall=(0.0, 0.0, 0.0), rho_out=1.0, fringe_len=0, fringe_factor=0.0):
         super().__init__()
         self.tau0, self.cs_smago, self.use_hlbm = tau0, cs_smago, int(use_hlbm)
         self.u_in[0], self.u_in[1], self.u_in[2] = u_in
@@ -40,6 +41,7 @@ class LbmParams(ctypes.Structure):
         self.collision, self.sigma = int(collision), float(sigma)
         self.u_wall[0], self.u_wall[1], self.u_wall[2] = u_wall
         self.rho_out = float(rho_out)
+        self.fringe_len, self.fringe_factor = int(fringe_len), float(fringe_factor)
 
 
 def library_path():

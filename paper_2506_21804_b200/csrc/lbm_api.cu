@@ -161,6 +161,12 @@ lbm::StepArgs<T> make_args(const lbm_ctx* c, const lbm_params* p, int in, int ou
   a.sigma = p ? static_cast<T>(p->sigma) : T(1);
   for (int k = 0; k < 3; ++k) a.u_wall[k] = p ? static_cast<T>(p->u_wall[k]) : T(0);
   a.rho_out = (p && p->rho_out > 0.0) ? static_cast<T>(p->rho_out) : T(1);
+  a.fringe_k = T(0);
+  a.fringe_x0 = c->nx;
+  if (p && p->fringe_len > 0 && p->fringe_factor > 0.0) {
+    a.fringe_k = static_cast<T>((p->tau0 - 0.5) * p->fringe_factor / (static_cast<double>(p->fringe_len) * p->fringe_len));
+    a.fringe_x0 = c->nx - 1 - p->fringe_len;
+  }
   a.uin_field = c->uin_mean ? c->uin_field[c->uin_cur] : nullptr;
   if (p) {
     a.tau0 = static_cast<T>(p->tau0);
@@ -350,6 +356,7 @@ int check_params(lbm_ctx* c, const lbm_params* p) {
     return fail(c, LBM_EINVAL, "lbm_step: wm_enable needs wm_kappa > 0 and wm_E > 0");
   if (!(p->u_in[0] < 1.0)) return fail(c, LBM_EINVAL, "lbm_step: u_in[0] = %g must be < 1", p->u_in[0]);
   if (p->rho_out < 0.0) return fail(c, LBM_EINVAL, "lbm_step: rho_out = %g must be > 0 (0 = default 1)", p->rho_out);
+  if (p->fringe_len < 0 || !(p->fringe_factor >= 0.0)) return fail(c, LBM_EINVAL, "lbm_step: fringe_len = %d, fringe_factor = %g must be >= 0", p->fringe_len, p->fringe_factor);
   if (p->collision != LBM_COLLISION_BGK && p->collision != LBM_COLLISION_HRR)
     return fail(c, LBM_EINVAL, "lbm_step: collision = %d must be 0 (BGK) or 1 (HRR)", p->collision);
   if (p->collision == LBM_COLLISION_HRR && !(p->sigma >= 0.0 && p->sigma <= 1.0))

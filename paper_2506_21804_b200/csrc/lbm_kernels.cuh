@@ -112,6 +112,8 @@ struct StepArgs {
   const double* __restrict__ uin_field;  // [3][nz][ny] per-cell inlet velocity (Vortex Method inlet / mean profile) or nullptr => u_in;
                                          // fp64 for both dtypes: Eq. 21 normalises a gradient of this field (ill-conditioned in fp32)
   T rho_out;                      // density imposed on POUTLET cells (reading G36)
+  T fringe_k;                     // fringe zone (reading G38): tau0(x) = tau0 + fringe_k max(0, x - fringe_x0)^2
+  int fringe_x0;
   T u_wall[3];                    // velocity of the MOVINGWALL cells (only ever on the plane z = nz-1), reading G33
 };
 
@@ -538,6 +540,14 @@ __device__ __noinline__ T slip_pull(const StepArgs<T>& a, int x, int y, int z, i
   return __ldg(a.fin + static_cast<long long>(ir) * a.N + xr);
 }
 
+// molecular relaxation time of the plane x: tau0, raised quadratically inside the fringe zone in front of the outlet
+// (l.255; reading G38: nu_mo(x) = nu_mo (1 + A xi^2), xi = (x - x0)/L; fringe_k = (tau0 - 1/2) A / L^2)
+template <typename T>
+__device__ __forceinline__ T tau0_at(const StepArgs<T>& a, int x) {
+  const int xd = (x > a.fringe_x0) ? x - a.fringe_x0 : 0;
+  return a.tau0 + a.fringe_k * static_cast<T>(xd * xd);
+}
+
 // velocity imposed on the INLET cell (0, y, z): the per-cell inflow field when one is set (Eq. 21 / mean profile), else u_in
 template <typename T>
 __device__ __forceinline__ void inlet_velocity(const StepArgs<T>& a, int y, int z, T& ux, T& uy, T& uz) {
@@ -727,9 +737,9 @@ __device__ __forceinline__ void step_cell_any(const StepArgs<T>& a, int x, int y
     if (COLL == COLL_HRR) {
       T S[6];
       fd_strain_cell<T>(a, x, y, z, type, S);
-      collide_cell_hrr<Q, T>(f, d, ubx, uby, ubz, a.tau0, a.smago_k, wm ? T(0) : a.sigma, S);   // sigma = 0: l.131
+      collide_cell_hrr<Q, T>(f, d, ubx, uby, ubz, tau0_at<T>(a, x), a.smago_k, wm ? T(0) : a.sigma, S);   // sigma = 0: l.131
     } else {
-      collide_cell<Q, T>(f, d, ubx, uby, ubz, a.tau0, a.smago_k);
+      collide_cell<Q, T>(f, d, ubx, uby, ubz, tau0_at<T>(a, x), a.smago_k);
     }
   }
   store_cell<Q, T>(a, x, y, z, f);
@@ -1126,9 +1136,9 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
         }
         const T S[6] = {T(0.5) * D[0][0], T(0.5) * D[1][1], T(0.5) * D[2][2], T(0.25) * (D[0][1] + D[1][0]),
                         T(0.25) * (D[0][2] + D[2][0]), T(0.25) * (D[1][2] + D[2][1])};
-        collide_cell_hrr<Q, T>(fc, d[v], T(0), T(0), T(0), a.tau0, a.smago_k, a.sigma, S);
+        collide_cell_hrr<Q, T>(fc, d[v], T(0), T(0), T(0), tau0_at<T>(a, x0 + v), a.smago_k, a.sigma, S);
       } else {
-        collide_cell<Q, T>(fc, d[v], T(0), T(0), T(0), a.tau0, a.smago_k);
+        collide_cell<Q, T>(fc, d[v], T(0), T(0), T(0), tau0_at<T>(a, x0 + v), a.smago_k);
       }
 #pragma unroll
       for (int i = 0; i < Q; ++i) f[i][v] = fc[i];

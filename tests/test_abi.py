@@ -38,15 +38,15 @@ def test_params_struct_layout_matches_header(tmp_path):
     import subprocess
     S = P.LbmParams
     names = [f for f, _ in S._fields_]
-    assert names == ["tau0", "cs_smago", "use_hlbm", "u_in", "wm_enable", "wm_kappa", "wm_E", "collision", "sigma", "u_wall", "rho_out"]
+    assert names == ["tau0", "cs_smago", "use_hlbm", "u_in", "wm_enable", "wm_kappa", "wm_E", "collision", "sigma", "u_wall", "rho_out", "fringe_len", "fringe_factor"]
     src = tmp_path / "probe.c"
     src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "lbm.h"\nint main(void){printf("%zu", sizeof(lbm_params));'
                    + "".join('printf(" %%zu", offsetof(lbm_params, %s));' % n for n in names) + "return 0;}\n")
     exe = tmp_path / "probe"
     subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
     out = [int(t) for t in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()]
-    assert ctypes.sizeof(S) == out[0] == 120
-    assert [getattr(S, f).offset for f in names] == out[1:] == [0, 8, 16, 24, 48, 56, 64, 72, 80, 88, 112]
+    assert ctypes.sizeof(S) == out[0] == 136
+    assert [getattr(S, f).offset for f in names] == out[1:] == [0, 8, 16, 24, 48, 56, 64, 72, 80, 88, 112, 120, 128]
 
 
 def test_bad_arguments_are_rejected_without_touching_the_gpu(lib):

@@ -50,3 +50,20 @@ def test_poutlet_flag_only_on_the_last_plane_and_rho_out_checked():
         sim.init_equilibrium(np.ones((6, 8, 8), np.float32), np.zeros((3, 6, 8, 8), np.float32))
         with pytest.raises(P.LbmError):
             sim.step(1, P.LbmParams(0.6, rho_out=-1.0))
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("coll", [0, 1])
+def test_fringe_zone_in_front_of_the_pressure_outlet(dtype, coll):
+    """reading G38: nu_mo(x) = nu_mo (1 + A xi^2) over the last L cells (the vector path computes tau0 per cell)"""
+    cfg = _pressure_channel((24, 32, 96), collision=coll, sigma=0.7, fringe_len=20, fringe_factor=8.0)
+    check_parity(cfg, dtype)
+
+
+def test_fringe_zone_scalar_kernel_and_bad_arguments():
+    check_parity(_pressure_channel((12, 10, 37), fringe_len=9, fringe_factor=3.0), "f64")
+    with P.LBM(19, 8, 8, 8, "f32") as sim:
+        sim.init_equilibrium(np.ones((8, 8, 8), np.float32), np.zeros((3, 8, 8, 8), np.float32))
+        for bad in (dict(fringe_len=-1), dict(fringe_factor=-0.5)):
+            with pytest.raises(P.LbmError):
+                sim.step(1, P.LbmParams(0.6, **bad))

@@ -276,7 +276,7 @@ def test_error_codes():
         assert e.value.code == B.LBM_ESTATE
         f = np.full((19, 8, 8, 8), 0.05, dtype=np.float32)
         bad = np.zeros((8, 8, 8), dtype=np.uint8)
-        bad[3, 3, 3] = 7
+        bad[3, 3, 3] = 8                            # type > 7
         with pytest.raises(P.LbmError) as e:
             sim.set_fields(f, None, bad)
         assert e.value.code == B.LBM_EINVAL
