@@ -59,6 +59,10 @@ WORKLOADS["cavity_512_f32_hrr"] = (6, (512, 512, 512), "f32", HRR)
 VM = dict(n_vortices=256, sigma_v=6.0, intensity=0.15)
 WORKLOADS["config3_urban_channel_384x192x128_f32_vm"] = (3, None, "f32", {}, VM)
 WORKLOADS["config3_urban_channel_384x192x128_f32_hrr_vm"] = (3, None, "f32", HRR, VM)
+# the urban channel in the paper's own boundary set (l.255: fixed-pressure outlet + fringe zone, full-slip outer walls, wall-modelled
+# floor) with the VM inlet; "_hrr_vm" is the paper's HHRRLBM-LES urban set-up as far as the paper defines it
+WORKLOADS["paperbc_urban_channel_384x192x128_f32_vm"] = (7, (128, 192, 384), "f32", {}, VM)
+WORKLOADS["paperbc_urban_channel_384x192x128_f32_hrr_vm"] = (7, (128, 192, 384), "f32", HRR, VM)
 DEFAULT_WORKLOAD = "config3_urban_channel_384x192x128_f32"
 
 
@@ -209,7 +213,7 @@ def run_reference(args, rank, world):
     if number == 1:
         sample = (32, 32, 32)
     else:
-        base = {2: (256, 256, 256), 3: (128, 192, 384), 4: (512, 512, 512), 5: shape, 6: shape}[number]
+        base = {2: (256, 256, 256), 3: (128, 192, 384), 4: (512, 512, 512), 5: shape, 6: shape, 7: shape}[number]
         scale = min(1.0, (cells_budget / float(np.prod(base))) ** (1.0 / 3.0))
         sample = tuple(max(16, int(round(b * scale / 8)) * 8) for b in base)
     cfg = make_cfg(number, sample, extra)

@@ -220,6 +220,23 @@ def make_config(number, shape=None, k_max=None, n_modes=None):
         u[:, (flags & 0x0F) == SOLID] = 0.0
         return dict(number=4, Q=27, dtype="f32", shape=tuple(shape), steps=200, rho=np.ones(shape), u=u, d=None,
                     flags=flags, params=dict(tau0=tau_les, cs_smago=0.12, use_hlbm=0))
+    if number == 7:
+        # the urban channel in the PAPER's boundary set (not a BASELINE.json config): config 3's
+        # geometry with a fixed-pressure outlet + fringe zone, full-slip lateral walls (planes y = 0, ny-1) and top (z = nz-1),
+        # wall-modelled bounce-back floor, velocity inlet (bench.py adds the Vortex Method to it)
+        cfg = make_config(3, shape=shape)
+        nz, ny, nx = cfg["shape"]
+        fl = cfg["flags"]
+        fl[(fl & 0x0F) == OUTLET] = POUTLET
+        fl[nz - 1] = SLIPWALL
+        fl[1:, 0] = SLIPWALL
+        fl[1:, ny - 1] = SLIPWALL
+        wall = is_wall(fl)
+        cfg["d"][wall] = 0.0
+        cfg["u"][:, wall] = 0.0
+        cfg["number"] = 7
+        cfg["params"] = dict(cfg["params"], rho_out=1.0, fringe_len=max(nx // 8, 1), fringe_factor=10.0)
+        return cfg
     if number == 6:
         # lid-driven cavity (the paper's scaling benchmark; not a BASELINE.json config):
         # closed box, five resting walls, the z = nz-1 plane moves with u_wall = (0.05, 0, 0); fluid at rest, rho = 1;

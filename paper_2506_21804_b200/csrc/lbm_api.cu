@@ -215,7 +215,7 @@ int launch_one(lbm_ctx* c, const lbm_params* p, int in, int out, int z0, int nzs
     }
     grid.z = nzs + a.list_z;
     if (grid.z == 0) return LBM_OK;
-    if (((c->n_moving > 0 && may_meet_lid) || c->n_slip > 0) && lbm::mode_pulls(MODE)) lbm::k_step_vec<Q, T, MODE, COLL, true><<<grid, block, 0, c->stream>>>(a);
+    if (c->n_moving > 0 && may_meet_lid && lbm::mode_pulls(MODE)) lbm::k_step_vec<Q, T, MODE, COLL, true><<<grid, block, 0, c->stream>>>(a);
     else                                          lbm::k_step_vec<Q, T, MODE, COLL, false><<<grid, block, 0, c->stream>>>(a);
   } else {
     if (nzs == 0) return LBM_OK;
@@ -266,7 +266,7 @@ int launch_hrr_t(lbm_ctx* c, const lbm_params* p, int in, int out) {
 template <int Q, typename T>
 int launch_bgk_pull_t(lbm_ctx* c, const lbm_params* p, int in, int out) {
   const int nz = c->nz;
-  if (c->n_moving == 0 || c->n_slip > 0 || nz < 8)
+  if (c->n_moving == 0 || nz < 8)
     return launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 0, nz, true);
   int rc = launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 1, nz - 3, true, false);
   if (rc == LBM_OK) rc = launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, nz - 2, 2, false);

@@ -22,8 +22,8 @@ enum : int { T_FLUID = 0, T_SOLID = 1, T_INLET = 2, T_OUTLET = 3, T_WM = 4, T_MO
 __host__ __device__ constexpr bool is_wall(int cls_or_type) { return ((0xA2 >> (cls_or_type & 7)) & 1) != 0; }
 // internal class byte: bits 0-2 type, bits 3-5 wall-normal code,
 //   bit 6 = ADJ:     the (non-SOLID) cell has at least one SOLID lattice neighbour (nbmask[] says which);
-//   bit 7 = SPECIAL: the cell needs the per-cell path (list blocks): WALLMODEL cells (A8) and OUTLET cells with a
-//                    SOLID neighbour (their clamped pull needs a class lookup).
+//   bit 7 = SPECIAL: the cell needs the per-cell path (list blocks): WALLMODEL cells (A8), OUTLET cells with a wall neighbour
+//                    (their clamped pull needs a class lookup) and cells next to a SLIPWALL (specular pull, G37).
 // Halfway bounce-back (A7, reading R5) on the READ side: the pull of direction i at a cell x whose source x - c_i is
 // SOLID takes the cell's own F_opp(i)(x) instead.  Nobody ever consumes the lattice slots of a SOLID cell, so the
 // step kernels write every 128-byte line they touch IN FULL (zeros on SOLID cells): a store stream with holes at
@@ -868,7 +868,7 @@ __device__ __forceinline__ void ld_uhat_nb(const T* pu, long long N, int dyp, in
 // of the cells of SPECIAL sectors (A8 wall model; OUTLET cells next to a wall), one cell per thread: the masked
 // boundary kernel as a block role of the same launch (scheduled first, overlaps with the row blocks).
 // Everything else -- bulk, solid-adjacent (read-side bounce-back), INLET and OUTLET cells -- runs in the vector path.
-// MW: the launch may meet MOVINGWALL / SLIPWALL cells (compiled out otherwise: the test costs the wall-adjacent warps registers).
+// MW: the launch may meet MOVINGWALL cells (compiled out otherwise: the test costs the wall-adjacent warps registers).
 template <int Q, typename T, int MODE, int COLL, bool MW>
 __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ StepArgs<T> a) {
   constexpr Stencil<Q> L{};
@@ -1049,11 +1049,13 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
       for (int v = 0; v < V; ++v)
         if (nbm[v] & (1u << j)) f[L.opp[j]][v] = __ldg(pown + static_cast<long long>(j) * N + v);
     }
-    // moving wall (G33) / slip wall (G37): the class byte of the wall the population bounced off decides (this kernel variant
-    // runs only where the geometry has such cells: the lid slices, or everywhere with slip walls)
-    if (MW) {
+    // moving wall (G33): MOVINGWALL cells exist only on the plane z = nz-1, so only directions towards that plane can meet one
+    // (block-uniform test); the neighbour's class byte decides.  (Cells next to a SLIPWALL are SPECIAL: list blocks.)
+    if (MW && (z >= nz - 2 || z == 0)) {
 #pragma unroll
       for (int j = 1; j < Q; ++j) {
+        const int zn = z + L.c[j][2];
+        if (((zn < 0) ? zn + nz : ((zn >= nz) ? zn - nz : zn)) != nz - 1) continue;
         const long long off = static_cast<long long>((L.c[j][1] == 0) ? 0 : ((L.c[j][1] == 1) ? dyp : dym)) +
                               static_cast<long long>((L.c[j][2] == 0) ? 0 : ((L.c[j][2] == 1) ? dzp : dzm));
         const uint8_t* pc = a.cls + self + off;
@@ -1063,14 +1065,7 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
             int ex = v + L.c[j][0];
             if (L.c[j][0] == -1 && v == 0) ex = exl;
             if (L.c[j][0] == 1 && v == V - 1) ex = exr;
-            const int st = pc[ex] & CLS_TYPE;
-            if (st == T_MOVING) f[L.opp[j]][v] += moving_wall_term<Q, T>(L.opp[j], a.u_wall);
-            else if (st == T_SLIP) {
-              const int xg = x0 + v;
-              const int t = xg + L.c[j][0];
-              f[L.opp[j]][v] = slip_pull<Q, T>(a, xg, y, z, -L.c[j][0], -L.c[j][1], -L.c[j][2],
-                                               (t < 0) ? t + nx : ((t >= nx) ? t - nx : t), f[L.opp[j]][v]);
-            }
+            if ((pc[ex] & CLS_TYPE) == T_MOVING) f[L.opp[j]][v] += moving_wall_term<Q, T>(L.opp[j], a.u_wall);
           }
         }
       }
@@ -1403,6 +1398,7 @@ __global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ fl
   if (type == T_MOVING && z != nz - 1) bad = true;
   if (bad) { atomicAdd(counters, 1ull); return; }
   uint32_t m = 0u;
+  bool slipnb = false;
   if (!is_wall(type)) {
 #pragma unroll
     for (int j = 1; j < Q; ++j) {
@@ -1410,11 +1406,15 @@ __global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ fl
       sx = (sx < 0) ? sx + nx : ((sx >= nx) ? sx - nx : sx);
       sy = (sy < 0) ? sy + ny : ((sy >= ny) ? sy - ny : sy);
       sz = (sz < 0) ? sz + nz : ((sz >= nz) ? sz - nz : sz);
-      if (is_wall(flags[cell_index(sx, sy, sz, nx, ny)] & 0x0F)) m |= (1u << j);
+      const int nt = flags[cell_index(sx, sy, sz, nx, ny)] & 0x0F;
+      if (is_wall(nt)) m |= (1u << j);
+      if (nt == T_SLIP) slipnb = true;
     }
   }
   const bool adj = (m != 0u);
-  const bool special = (type == T_WM) || (type == T_OUTLET && adj);
+  // cells next to a slip wall take the per-cell path: the specular pull (slip_pull) is a call with many operands, which does not
+  // belong into the vector kernel's register budget
+  const bool special = (type == T_WM) || (type == T_OUTLET && adj) || slipnb;
   cls[self] = static_cast<uint8_t>(type | ((type == T_WM ? hi : 0) << CLS_NORMAL_SHIFT) | (adj ? CLS_ADJ : 0) |
                                    (special ? CLS_SPECIAL : 0));
   if (is_wall(type)) atomicAdd(counters + 1, 1ull);

@@ -76,14 +76,19 @@ def _check_windows(cfg, dtype, windows, closed_axes, steps=S, u_scale=0.0, vm=No
         fc = np.ascontiguousarray(f[(slice(None),) + sel]).astype(np.float64)
         dc = None if d is None else np.ascontiguousarray(d[sel]).astype(np.float64)
         flc = None if cfg["flags"] is None else np.ascontiguousarray(cfg["flags"][sel])
+        par_c = dict(cfg["params"])
+        if par_c.get("fringe_len", 0) > 0 and ix[-1] != nx - 1:
+            # the fringe zone is measured from the last plane: a crop that does not end there must not reach into it
+            assert ix.max() + 1 < nx - 1 - par_c["fringe_len"], "window crop cuts the fringe zone"
+            par_c["fringe_len"] = 0
         if fields is None:
-            ref = O.step(fc, d=dc, flags=flc, nsteps=steps, nthreads=min(O.max_threads(), 8), **cfg["params"])
+            ref = O.step(fc, d=dc, flags=flc, nsteps=steps, nthreads=min(O.max_threads(), 8), **par_c)
         else:
             ref = fc
             for fld in fields:
                 uc = np.ascontiguousarray(fld[:, iz][:, :, iy])
                 ref, _ = O.step_vm(ref, uc, uc, np.zeros((0, 2)), np.zeros(0), 1.0, 0.0, d=dc, flags=flc, nsteps=1,
-                                   nthreads=min(O.max_threads(), 8), **cfg["params"])
+                                   nthreads=min(O.max_threads(), 8), **par_c)
         inner = (slice(None), slice(wz, wz + W), slice(wy, wy + W), slice(wx, wx + W))
         refw = ref[inner]
         gz, gy, gx = iz[wz:wz + W], iy[wy:wy + W], ix[wx:wx + W]
@@ -184,6 +189,17 @@ def test_config3_vm_inlet_full_size_windows():
     vm = I.vm_inlet(cfg["shape"], 1303, n_vortices=256, sigma_v=6.0, intensity=0.15)
     wins = [(1, 10, 0), (60, 100, 0), (nz - 1 - W, 50, 0), (30, ny - 4, 0), (90, 0, 0), (40, 150, 6), (1, 60, 150), (60, 90, 190)]
     _check_windows(cfg, "f32", wins, (True, False, True), vm=vm)
+
+
+def test_paper_boundary_set_full_size_windows():
+    """bench.py paperbc_urban_channel_384x192x128_f32_vm: VM inlet, pressure outlet + fringe zone, slip lateral walls and top,
+    wall-modelled floor; windows at the slip walls / edges, in the fringe zone, on the inflow and outflow planes"""
+    cfg = I.make_config(7, shape=(128, 192, 384))
+    nz, ny, nx = cfg["shape"]
+    vm = I.vm_inlet(cfg["shape"], 1307, n_vortices=256, sigma_v=6.0, intensity=0.15)
+    wins = [(1, 1, 0), (nz - 1 - W, ny - 1 - W, 0), (60, 1, nx - W), (nz - 1 - W, 90, nx - W), (1, ny - 1 - W, 200), (nz - 1 - W, 1, 150),
+            (40, 100, nx - 20), (60, 90, 190)]
+    _check_windows(cfg, "f32", wins, (True, True, True), vm=vm)
 
 
 def test_cavity_full_size_windows():
