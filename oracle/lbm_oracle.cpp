@@ -56,8 +56,9 @@
 // idempotence, P11a long-double brute force on 4^3, P12 bounce-back pulse + mass, P13 second
 // order convergence, P14 lattice symmetry, P15 D3Q27.
 // PARITY UNPINNED against the paper (no worked example printed): the wall-model coupling
-// reading G17, the outlet rule G16 and the inlet variant G15.  They are pinned only as
-// textbook definitions through P8, P9, P10.
+// reading G17, the outlet rules G16 / G36, the inlet variant G15, the moving-wall rule G33 and the
+// fringe zone G38.  They are pinned only as textbook definitions through P8, P9, P10, B1-B4,
+// M1-M6, Z1-Z3.
 //
 // Layouts (all row-major, x fastest): f[Q][nz][ny][nx] double, d[nz][ny][nx] double,
 // flag[nz][ny][nx] uint8.  Cell index = (z*ny + y)*nx + x.
