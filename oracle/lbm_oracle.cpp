@@ -35,6 +35,10 @@
 //                          off a wall moving with u_w: + 2 w_i rho_w (c_i.u_w)/c_s^2 on the returned population, rho_w = 1
 //                          (reading G33; the paper does not say how its lid is imposed -> PARITY UNPINNED against the
 //                          paper, pinned as the textbook rule by M1-M4 in tests/test_oracle_cavity.py)
+//   O2b solid velocity    Eq. 12 (l.99) with u^B(x,t) != 0 prescribed per cell (l.106 "non-zero solid velocities"; the moving
+//                          bodies of Fig. 1) through orc_step_body; d(x,t) varies by stepping with a new d.  Pinned
+//                          by U1-U4 in tests/test_oracle_body.py (closed-form relaxation towards u^B, Galilean image of P5,
+//                          d = 1 drives u to u^B, u^B = 0 equals orc_step)
 //   O6 moments             l.97 "fluid velocity moment u" (G19)
 //   O2h collide, HRR form  (params.collision = 1; the paper's own collision)
 //                          Eq. 6 (l.70) with f~(1) of Eq. 7 (l.74); Eq. 8-9 (l.81-86) regularised
@@ -585,7 +589,7 @@ int orc_init_equilibrium(int Q, int64_t N, const double* rho, const double* u, d
 namespace {
 int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const uint8_t* flags,
              const double* par /* tau0, cs, use_hlbm, uin0, uin1, uin2, wm_enable, kappa, E, collision, sigma, uwall0, uwall1, uwall2, rho_out, fringe_len, fringe_factor */,
-             int nsteps, int nthreads, VortexInlet* vm) {
+             int nsteps, int nthreads, VortexInlet* vm, const double* u_body = nullptr) {
   Lattice L;
   if (!make_lattice(Q, L)) return -1;
   if (nx < 1 || ny < 1 || nz < 1 || nsteps < 0) return -1;
@@ -667,6 +671,8 @@ int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const u
           raw_moments(L, fc, rho, u);
           const double dd = (p.use_hlbm && d) ? d[x] : 0.0;
           double ub[3] = {0.0, 0.0, 0.0};
+          if (u_body)                                                      // O2b: prescribed solid velocity u^B(x,t), Eq. 12
+            for (int a = 0; a < 3; ++a) ub[a] = u_body[a * N + x];
           if (type == WALLMODEL && p.wm_enable && !wm_slot.empty()) {
             const int32_t k = wm_slot[x];
             ub[0] = uB[3 * k];  ub[1] = uB[3 * k + 1];  ub[2] = uB[3 * k + 2];
@@ -692,7 +698,9 @@ int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const u
           for (int i = 0; i < Q; ++i) fc[i] = cur[i * N + x];
           const double dd = (p.use_hlbm && d) ? d[x] : 0.0;
           double ub[3] = {0.0, 0.0, 0.0};
-          if (type == WALLMODEL && p.wm_enable && !wm_slot.empty()) {
+          if (u_body)                                                      // O2b: prescribed solid velocity u^B(x,t), Eq. 12
+            for (int a = 0; a < 3; ++a) ub[a] = u_body[a * N + x];
+          if (type == WALLMODEL && p.wm_enable && !wm_slot.empty()) {      // the wall model prescribes u^B there (l.106)
             const int32_t k = wm_slot[x];
             ub[0] = uB[3 * k];  ub[1] = uB[3 * k + 1];  ub[2] = uB[3 * k + 2];
           }
@@ -836,6 +844,14 @@ extern "C" {
 int orc_step(int Q, int nx, int ny, int nz, double* f, const double* d, const uint8_t* flags, const double* par, int nsteps,
              int nthreads) {
   return step_impl(Q, nx, ny, nz, f, d, flags, par, nsteps, nthreads, nullptr);
+}
+
+// the step with a prescribed solid velocity field u^B(x,t) of Eq. 12 (l.99-106: "non-zero solid velocities"; the moving porous
+// bodies of the FSI cases of Fig. 1): u_body [3][nz][ny][nx], constant over the nsteps steps (a body that moves
+// is stepped one step at a time with new d and u_body).  WALLMODEL cells keep the wall model's u^B when wm_enable.
+int orc_step_body(int Q, int nx, int ny, int nz, double* f, const double* d, const uint8_t* flags, const double* par, int nsteps,
+                  int nthreads, const double* u_body) {
+  return step_impl(Q, nx, ny, nz, f, d, flags, par, nsteps, nthreads, nullptr, u_body);
 }
 
 // the step with the Vortex Method inlet: u_inflow [3][nz][ny] holds the inflow of the previous step on entry (u_mean

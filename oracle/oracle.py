@@ -53,6 +53,7 @@ def lib():
         L.orc_wallmodel_speed.restype = ctypes.c_double
         L.orc_init_equilibrium.argtypes = [ctypes.c_int, ctypes.c_int64, _c_dp, _c_dp, _c_dp]
         L.orc_step.argtypes = [ctypes.c_int] * 4 + [_c_dp, _c_dp, _c_u8p, _c_dp, ctypes.c_int, ctypes.c_int]
+        L.orc_step_body.argtypes = [ctypes.c_int] * 4 + [_c_dp, _c_dp, _c_u8p, _c_dp, ctypes.c_int, ctypes.c_int, _c_dp]
         L.orc_moments.argtypes = [ctypes.c_int, ctypes.c_int64, _c_dp, _c_dp, _c_dp]
         L.orc_step_vm.argtypes = [ctypes.c_int] * 4 + [_c_dp, _c_dp, _c_u8p, _c_dp, ctypes.c_int, ctypes.c_int,
                                   _c_dp, _c_dp, ctypes.c_int, _c_dp, _c_dp, ctypes.c_double, ctypes.c_double]
@@ -166,8 +167,9 @@ def pack_params(tau0, cs_smago=0.0, use_hlbm=0, u_in=(0.0, 0.0, 0.0), wm_enable=
                     dtype=np.float64)
 
 
-def step(f, d=None, flags=None, nsteps=1, nthreads=1, **params):
-    """Advance S_t -> S_{t+nsteps}.  f[Q,nz,ny,nx] float64 (a new array is returned)."""
+def step(f, d=None, flags=None, nsteps=1, nthreads=1, u_body=None, **params):
+    """Advance S_t -> S_{t+nsteps}.  f[Q,nz,ny,nx] float64 (a new array is returned).  u_body[3,nz,ny,nx]: the solid
+    velocity u^B of Eq. 12 (None = 0)."""
     f = _f64(f).copy()
     Q, nz, ny, nx = f.shape
     par = pack_params(**params)
@@ -181,7 +183,12 @@ def step(f, d=None, flags=None, nsteps=1, nthreads=1, **params):
         flags = np.ascontiguousarray(flags, dtype=np.uint8)
         assert flags.shape == (nz, ny, nx)
         fptr = flags.ctypes.data_as(_c_u8p)
-    rc = lib().orc_step(Q, nx, ny, nz, _dp(f), dptr, fptr, _dp(par), int(nsteps), int(nthreads))
+    if u_body is not None:
+        u_body = _f64(u_body)
+        assert u_body.shape == (3, nz, ny, nx)
+        rc = lib().orc_step_body(Q, nx, ny, nz, _dp(f), dptr, fptr, _dp(par), int(nsteps), int(nthreads), _dp(u_body))
+    else:
+        rc = lib().orc_step(Q, nx, ny, nz, _dp(f), dptr, fptr, _dp(par), int(nsteps), int(nthreads))
     if rc != 0:
         raise ValueError("orc_step rejected its arguments")
     return f
