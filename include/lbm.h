@@ -115,6 +115,22 @@ int lbm_init_equilibrium(lbm_ctx* ctx, const void* rho, const void* u);
 /* Replace porosity and flags only (same rules as lbm_set_fields); the populations are kept. */
 int lbm_set_geometry(lbm_ctx* ctx, const void* porosity, const uint8_t* cell_flags);
 
+/* Time-varying porosity d(x,t) (Eq. 12-13, l.99-103: "d(x,t)"): replace the porosity field only.
+ *   porosity : [nz][ny][nx] dtype, host or device (copied); NULL => d = 0 everywhere.
+ * Flags and populations are kept.  d enters the collision only, so -- unlike lbm_set_geometry -- this costs no pass over
+ * the lattice: the next lbm_step collides S_t with the new field.  Errors: LBM_EINVAL (NULL ctx), LBM_ECUDA. */
+int lbm_set_porosity(lbm_ctx* ctx, const void* porosity);
+
+/* Solid velocity field u^B(x,t) of Eq. 12 (l.99: u^ = (1-d) u + d u^B; l.106 "non-zero solid velocities"; the moving bodies of
+ * the FSI cases of Fig. 1).
+ *   u_body : [3][nz][ny][nx] dtype (component, z, y, x), host or device (copied into 3 N values of library memory);
+ *            NULL => u^B = 0 everywhere again (the memory is released).
+ * The field stays until the next call; a body that moves is stepped with lbm_set_porosity + lbm_set_body_velocity before each
+ * lbm_step(1).  It is read only where d != 0 and only when lbm_params.use_hlbm; WALLMODEL cells keep the wall model's u^B when
+ * wm_enable (reading G39); SOLID cells ignore it.  Both collision forms.  No pass over the lattice.
+ * Errors: LBM_EINVAL (NULL ctx), LBM_ENOMEM, LBM_ECUDA. */
+int lbm_set_body_velocity(lbm_ctx* ctx, const void* u_body);
+
 /* Inflow velocity field of the INLET cells (plane x = 0) and the Vortex Method that perturbs it (Eq. 18-21;
  * SURVEY 8(f)-3; readings G11, G34, G35 of DESIGN.md).
  *   u_mean : [3][nz][ny] dtype (component, z, y), host or device: the mean velocity profile u_mean(x) of Eq. 21; entries of

@@ -15,7 +15,8 @@ LBM_D3Q19, LBM_D3Q27 = 19, 27
 LBM_F32, LBM_F64 = 4, 8
 EXPORTS = ["lbm_create", "lbm_destroy", "lbm_set_fields", "lbm_init_equilibrium", "lbm_set_geometry", "lbm_step",
            "lbm_moments", "lbm_get_populations", "lbm_totals", "lbm_set_stream", "lbm_synchronize", "lbm_last_error",
-           "lbm_query", "lbm_set_option", "lbm_set_inflow", "lbm_set_vortices", "lbm_get_inflow"]
+           "lbm_query", "lbm_set_option", "lbm_set_inflow", "lbm_set_vortices", "lbm_get_inflow",
+           "lbm_set_porosity", "lbm_set_body_velocity"]
 
 
 class LbmError(RuntimeError):
@@ -67,6 +68,8 @@ def load_library():
     L.lbm_init_equilibrium.argtypes = [vp, vp, vp]
     L.lbm_set_geometry.argtypes = [vp, vp, vp]
     L.lbm_step.argtypes = [vp, ip, ctypes.POINTER(LbmParams)]
+    L.lbm_set_porosity.argtypes = [vp, vp]
+    L.lbm_set_body_velocity.argtypes = [vp, vp]
     L.lbm_set_inflow.argtypes = [vp, vp]
     L.lbm_set_vortices.argtypes = [vp, ip, vp, vp, ctypes.c_double, ctypes.c_double]
     L.lbm_get_inflow.argtypes = [vp, vp]
@@ -133,6 +136,14 @@ def lbm_init_equilibrium(ctx, rho, u):
 
 def lbm_set_geometry(ctx, porosity=None, cell_flags=None):
     return _check(ctx, load_library().lbm_set_geometry(ctx, _ptr(porosity), _ptr(cell_flags)))
+
+
+def lbm_set_porosity(ctx, porosity=None):
+    return _check(ctx, load_library().lbm_set_porosity(ctx, _ptr(porosity)))
+
+
+def lbm_set_body_velocity(ctx, u_body=None):
+    return _check(ctx, load_library().lbm_set_body_velocity(ctx, _ptr(u_body)))
 
 
 def lbm_set_inflow(ctx, u_mean):
@@ -221,6 +232,12 @@ class LBM:
 
     def set_geometry(self, porosity=None, cell_flags=None):
         return lbm_set_geometry(self.ctx, porosity, cell_flags)
+
+    def set_porosity(self, porosity=None):
+        return lbm_set_porosity(self.ctx, porosity)
+
+    def set_body_velocity(self, u_body=None):
+        return lbm_set_body_velocity(self.ctx, u_body)
 
     def init_equilibrium(self, rho, u):
         return lbm_init_equilibrium(self.ctx, rho, u)

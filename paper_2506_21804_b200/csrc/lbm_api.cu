@@ -71,6 +71,7 @@ struct lbm_ctx {
   cudaEvent_t ev_vm, ev_step[2];
   bool vm_pending;          // the newest field is still being written on vm_stream
   long long ev_step_level[2];   // time level of the step after which ev_step[k] was recorded (-1: never)
+  void* ub;              // prescribed solid velocity u^B [3][N] (lbm_set_body_velocity), nullptr = 0 everywhere
   void* uhat;            // HRR form: u^(x,t) [3][N], allocated on the first HRR step
   int hrr_slab;          // HRR form: z-slices per slab of the two-pass step (0 = whole lattice)
   lbm_params last;       // parameters of the last lbm_step: the inlet rule is part of how S_t is formed from F_{t-1}
@@ -149,6 +150,7 @@ lbm::StepArgs<T> make_args(const lbm_ctx* c, const lbm_params* p, int in, int ou
   a.fin = static_cast<const T*>(c->f[in]);
   a.fout = static_cast<T*>(c->f[out]);
   a.d = (p && p->use_hlbm && c->has_d) ? static_cast<const T*>(c->d) : nullptr;
+  a.ub = (a.d != nullptr && c->ub) ? static_cast<const T*>(c->ub) : nullptr;
   a.cls = c->cls;
   a.nbmask = c->nbmask;
   a.nx = c->nx;  a.ny = c->ny;  a.nz = c->nz;
@@ -616,7 +618,7 @@ void lbm_destroy(lbm_ctx* c) {
     cudaStreamDestroy(c->vm_stream);
     cudaEventDestroy(c->ev_vm);  cudaEventDestroy(c->ev_step[0]);  cudaEventDestroy(c->ev_step[1]);
   }
-  cudaFree(c->f[0]);  cudaFree(c->f[1]);  cudaFree(c->d);  cudaFree(c->uhat);
+  cudaFree(c->f[0]);  cudaFree(c->f[1]);  cudaFree(c->d);  cudaFree(c->uhat);  cudaFree(c->ub);
   cudaFree(c->uin_mean);  cudaFree(c->uin_field[0]);  cudaFree(c->uin_field[1]);  cudaFree(c->vpos);  cudaFree(c->vsign);  cudaFree(c->vgamma);
   cudaFree(c->cls);  cudaFree(c->cls_alt);  cudaFree(c->flags_raw);
   cudaFree(c->counters);  cudaFree(c->totals_dev);  cudaFree(c->staging);
@@ -714,6 +716,41 @@ int lbm_set_geometry(lbm_ctx* c, const void* porosity, const uint8_t* cell_flags
   rc = set_geometry_fields(c, porosity, cell_flags);
   if (rc != LBM_OK) return rc;
   if (c->phase == PHASE_PRE) return solid_values(c, true);   // the SOLID set changed: save the new set's values
+  return LBM_OK;
+}
+
+// Neither call touches the populations or the pull: d and u^B enter the collision only (Eq. 12), so the stored
+// post-collision state F_{t-1} stays valid and no pass over the lattice is needed (unlike lbm_set_geometry).
+int lbm_set_porosity(lbm_ctx* c, const void* porosity) {
+  if (!c) return LBM_EINVAL;
+  if (!porosity) {
+    c->has_d = false;
+    return LBM_OK;
+  }
+  LBM_CUDA(c, cudaMemcpyAsync(c->d, porosity, static_cast<size_t>(c->N) * c->dtype, cudaMemcpyDefault, c->stream));
+  if (!is_device_pointer(porosity)) LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  c->has_d = true;
+  return LBM_OK;
+}
+
+int lbm_set_body_velocity(lbm_ctx* c, const void* u_body) {
+  if (!c) return LBM_EINVAL;
+  const size_t bytes = 3 * static_cast<size_t>(c->N) * c->dtype;
+  if (!u_body) {
+    if (c->ub) {
+      LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+      cudaFree(c->ub);
+      c->ub = nullptr;
+      c->device_bytes -= bytes;
+    }
+    return LBM_OK;
+  }
+  if (!c->ub) {
+    int rc = dev_alloc(c, &c->ub, bytes);
+    if (rc != LBM_OK) return rc;
+  }
+  LBM_CUDA(c, cudaMemcpyAsync(c->ub, u_body, bytes, cudaMemcpyDefault, c->stream));
+  if (!is_device_pointer(u_body)) LBM_CUDA(c, cudaStreamSynchronize(c->stream));
   return LBM_OK;
 }
 

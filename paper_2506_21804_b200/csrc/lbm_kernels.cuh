@@ -115,6 +115,8 @@ struct StepArgs {
   T fringe_k;                     // fringe zone (reading G38): tau0(x) = tau0 + fringe_k max(0, x - fringe_x0)^2
   int fringe_x0;
   T u_wall[3];                    // velocity of the MOVINGWALL cells (only ever on the plane z = nz-1), reading G33
+  const T* __restrict__ ub;       // [3][N] prescribed solid velocity u^B(x,t) of Eq. 12 (moving porous bodies, l.99-106) or nullptr => 0;
+                                  // read only where d != 0 (it enters with weight d); WALLMODEL cells take the wall model's u^B (G39)
 };
 
 // ---- math helpers ---------------------------------------------------------------------------------
@@ -709,6 +711,17 @@ __device__ __forceinline__ void uhat_of(const T (&f)[Q], T d, T ubx, T uby, T ub
   uz = keep * (jz * inv_rho) + d * ubz;
 }
 
+// prescribed solid velocity u^B of one cell (Eq. 12): three element loads, and only where the porosity gives it a weight
+template <typename T>
+__device__ __forceinline__ void body_velocity(const T* __restrict__ pub, long long N, T d, T& ubx, T& uby, T& ubz) {
+  ubx = uby = ubz = T(0);
+  if (pub != nullptr && d != T(0)) {
+    ubx = __ldg(pub);
+    uby = __ldg(pub + N);
+    ubz = __ldg(pub + 2 * N);
+  }
+}
+
 // ---- the per-cell step (scalar kernel; list blocks of the vector kernel) ------------------------------
 // One non-SOLID cell of any type: pull (modes that pull), wall model, then collide + store (collide modes), store S_t
 // (MODE_STREAM) or store u^ (MODE_UHAT_*).
@@ -722,6 +735,7 @@ __device__ __forceinline__ void step_cell_any(const StepArgs<T>& a, int x, int y
   if (MODE != MODE_STREAM) {
     if (a.d != nullptr) d = __ldg(a.d + self);
     if (wm) wallmodel_ub<Q, T, PULL>(a, x, y, z, cls, ubx, uby, ubz);
+    else if (a.ub != nullptr) body_velocity<T>(a.ub + self, a.N, d, ubx, uby, ubz);
   }
   T f[Q];
   load_state<Q, T, PULL>(a, x, y, z, cls, f);
@@ -1096,7 +1110,9 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
       T fc[Q];
 #pragma unroll
       for (int i = 0; i < Q; ++i) fc[i] = f[i][v];
-      uhat_of<Q, T>(fc, d[v], T(0), T(0), T(0), uo[0][v], uo[1][v], uo[2][v]);
+      T ubx, uby, ubz;
+      body_velocity<T>(a.ub == nullptr ? nullptr : a.ub + (pout - a.uhat) + v, N, d[v], ubx, uby, ubz);
+      uhat_of<Q, T>(fc, d[v], ubx, uby, ubz, uo[0][v], uo[1][v], uo[2][v]);
       if (solid_bits & (1u << v)) {
         const bool mv = ((clsw >> (8 * v)) & CLS_TYPE) == T_MOVING;
         uo[0][v] = mv ? a.u_wall[0] : T(0);
@@ -1117,6 +1133,8 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
       T fc[Q];
 #pragma unroll
       for (int i = 0; i < Q; ++i) fc[i] = f[i][v];
+      T ubx, uby, ubz;
+      body_velocity<T>(a.ub == nullptr ? nullptr : a.ub + (pout - a.fout) + v, N, d[v], ubx, uby, ubz);
       if constexpr (HRR) {
         T D[3][3];   // D[a][b] = u^_b(x + e_a) - u^_b(x - e_a); G32: the planes beyond INLET / OUTLET copy those planes
 #pragma unroll
@@ -1131,9 +1149,9 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
         }
         const T S[6] = {T(0.5) * D[0][0], T(0.5) * D[1][1], T(0.5) * D[2][2], T(0.25) * (D[0][1] + D[1][0]),
                         T(0.25) * (D[0][2] + D[2][0]), T(0.25) * (D[1][2] + D[2][1])};
-        collide_cell_hrr<Q, T>(fc, d[v], T(0), T(0), T(0), tau0_at<T>(a, x0 + v), a.smago_k, a.sigma, S);
+        collide_cell_hrr<Q, T>(fc, d[v], ubx, uby, ubz, tau0_at<T>(a, x0 + v), a.smago_k, a.sigma, S);
       } else {
-        collide_cell<Q, T>(fc, d[v], T(0), T(0), T(0), tau0_at<T>(a, x0 + v), a.smago_k);
+        collide_cell<Q, T>(fc, d[v], ubx, uby, ubz, tau0_at<T>(a, x0 + v), a.smago_k);
       }
 #pragma unroll
       for (int i = 0; i < Q; ++i) f[i][v] = fc[i];
