@@ -63,6 +63,11 @@ WORKLOADS["config3_urban_channel_384x192x128_f32_hrr_vm"] = (3, None, "f32", HRR
 # floor) with the VM inlet; "_hrr_vm" is the paper's HHRRLBM-LES urban set-up as far as the paper defines it
 WORKLOADS["paperbc_urban_channel_384x192x128_f32_vm"] = (7, (128, 192, 384), "f32", {}, VM)
 WORKLOADS["paperbc_urban_channel_384x192x128_f32_hrr_vm"] = (7, (128, 192, 384), "f32", HRR, VM)
+# moving porous bodies (Eq. 12 with u^B != 0): the trees of config 3 (0 < d < 1, 5 % of the cells) sway with a seeded
+# solid velocity field (lbm_inputs.body_velocity), set once through lbm_set_body_velocity
+BODY = dict(amp=0.02)
+WORKLOADS["config3_urban_channel_384x192x128_f32_body"] = (3, None, "f32", {}, None, BODY)
+WORKLOADS["config3_urban_channel_384x192x128_f32_hrr_body"] = (3, None, "f32", HRR, None, BODY)
 DEFAULT_WORKLOAD = "config3_urban_channel_384x192x128_f32"
 
 
@@ -75,14 +80,24 @@ def workload(name):
 def workload_vm(name, shape):
     """Vortex Method inlet inputs of the workload (lbm_inputs.vm_inlet) or None"""
     w = WORKLOADS[name]
-    if len(w) < 5:
+    if len(w) < 5 or w[4] is None:
         return None
     return I.vm_inlet(shape, 1300 + w[0], **w[4])
+
+
+def workload_body(name, cfg):
+    """solid velocity field u^B of the workload (lbm_inputs.body_velocity) or None"""
+    w = WORKLOADS[name]
+    if len(w) < 6 or w[5] is None:
+        return None
+    return I.body_velocity(cfg, 1400 + w[0], **w[5])
 
 
 def oracle_steps(O, f, cfg, vm, state, nsteps, nthreads):
     """the oracle's step loop, with the VM inlet when the workload has one (state = the previous inflow, carried along)"""
     kw = dict(d=cfg["d"], flags=cfg["flags"], nsteps=nsteps, nthreads=nthreads, **cfg["params"])
+    if cfg.get("u_body") is not None:
+        kw["u_body"] = cfg["u_body"]
     if vm is None:
         return O.step(f, **kw), None
     return O.step_vm(f, vm["u_mean"], vm["u_mean"] if state is None else state, vm["pos"], vm["sign"], vm["sigma_v"],
@@ -92,6 +107,12 @@ def oracle_steps(O, f, cfg, vm, state, nsteps, nthreads):
 def make_cfg(number, shape, extra):
     cfg = I.make_config(number, shape=shape) if number != 1 else I.make_config(1)
     cfg["params"] = dict(cfg["params"], **extra)
+    return cfg
+
+
+def make_cfg_named(name, number, shape, extra):
+    cfg = make_cfg(number, shape, extra)
+    cfg["u_body"] = workload_body(name, cfg)
     return cfg
 
 
@@ -189,7 +210,7 @@ class ClockSampler(threading.Thread):
 def cpu_oracle_time(cfg_number, sample_shape, nsteps, nthreads, extra, name):
     """Time the oracle, as it stands, on a bounded sample of the workload."""
     from oracle import oracle as O
-    cfg = make_cfg(cfg_number, sample_shape, extra)
+    cfg = make_cfg_named(name, cfg_number, sample_shape, extra)
     vm = workload_vm(name, cfg["shape"])
     f = O.init_equilibrium(cfg["Q"], cfg["rho"], cfg["u"])
     nonsolid = f[0].size if cfg["flags"] is None else int((~I.is_wall(cfg["flags"])).sum())
@@ -216,7 +237,7 @@ def run_reference(args, rank, world):
         base = {2: (256, 256, 256), 3: (128, 192, 384), 4: (512, 512, 512), 5: shape, 6: shape, 7: shape}[number]
         scale = min(1.0, (cells_budget / float(np.prod(base))) ** (1.0 / 3.0))
         sample = tuple(max(16, int(round(b * scale / 8)) * 8) for b in base)
-    cfg = make_cfg(number, sample, extra)
+    cfg = make_cfg_named(args.workload, number, sample, extra)
     f = O.init_equilibrium(cfg["Q"], cfg["rho"], cfg["u"])
     nonsolid = f[0].size if cfg["flags"] is None else int((~I.is_wall(cfg["flags"])).sum())
     vm = workload_vm(args.workload, cfg["shape"])
@@ -272,7 +293,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     number, shape, dtype, extra = workload(args.workload)
-    cfg = make_cfg(number, shape, extra)
+    cfg = make_cfg_named(args.workload, number, shape, extra)
     hrr = cfg["params"].get("collision", 0) == 1
     if args.steps is None:
         args.steps = cfg["steps"]
@@ -296,6 +317,8 @@ def main():
     fl_d = None if cfg["flags"] is None else torch.from_numpy(cfg["flags"]).cuda()
     sim.set_geometry(d_d, fl_d)
     sim.init_equilibrium(rho_d, u_d)
+    if cfg.get("u_body") is not None:
+        sim.set_body_velocity(torch.from_numpy(cfg["u_body"].astype(npdt)).cuda())
     vm = workload_vm(args.workload, cfg["shape"])
     if vm is not None:
         sim.set_inflow(torch.from_numpy(vm["u_mean"].astype(npdt)).cuda())

@@ -262,6 +262,25 @@ def vm_inlet(shape, seed, n_vortices=256, sigma_v=6.0, intensity=0.15, u_ref=0.0
     return dict(u_mean=u_mean, pos=pos, sign=sign, sigma_v=float(sigma_v), intensity=float(intensity))
 
 
+def body_velocity(cfg, seed, amp=0.02):
+    """Solid velocity field u^B(x,t) of Eq. 12 for a workload: the partly porous cells
+    (0 < d < 1: the trees of config 3) sway with a seeded smooth velocity (three plane waves per component), cells with d = 1
+    (buildings) and d = 0 carry 0.  [3][nz][ny][nx] float64.  No method arithmetic: inputs only."""
+    nz, ny, nx = cfg["shape"]
+    rng = _rng(seed)
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij", sparse=True)
+    ub = np.zeros((3, nz, ny, nx))
+    for a in range(3):
+        for _ in range(3):
+            k = rng.integers(1, 4, size=3)
+            ph = rng.uniform(0.0, 2.0 * np.pi)
+            ub[a] += (amp / 3.0) * np.sin(2.0 * np.pi * (k[0] * x / nx + k[1] * y / ny + k[2] * z / nz) + ph)
+    d = cfg["d"]
+    moving = (d > 0.0) & (d < 1.0) if d is not None else np.zeros((nz, ny, nx), dtype=bool)
+    ub[:, ~moving] = 0.0
+    return ub
+
+
 def cavity_flags(shape):
     """closed box: SOLID on x = 0, nx-1, y = 0, ny-1, z = 0; MOVINGWALL on the whole plane z = nz-1 (the lid)"""
     flags = np.zeros(shape, dtype=np.uint8)
