@@ -68,6 +68,9 @@ WORKLOADS["paperbc_urban_channel_384x192x128_f32_hrr_vm"] = (7, (128, 192, 384),
 BODY = dict(amp=0.02)
 WORKLOADS["config3_urban_channel_384x192x128_f32_body"] = (3, None, "f32", {}, None, BODY)
 WORKLOADS["config3_urban_channel_384x192x128_f32_hrr_body"] = (3, None, "f32", HRR, None, BODY)
+# the paper's boundary set with the wall model on the building faces too (config 8; SURVEY 8(f)-2 "wall model on building faces")
+WORKLOADS["paperbc_wmfaces_urban_channel_384x192x128_f32_vm"] = (8, (128, 192, 384), "f32", {}, VM)
+WORKLOADS["paperbc_wmfaces_urban_channel_384x192x128_f32_hrr_vm"] = (8, (128, 192, 384), "f32", HRR, VM)
 DEFAULT_WORKLOAD = "config3_urban_channel_384x192x128_f32"
 
 
@@ -234,7 +237,7 @@ def run_reference(args, rank, world):
     if number == 1:
         sample = (32, 32, 32)
     else:
-        base = {2: (256, 256, 256), 3: (128, 192, 384), 4: (512, 512, 512), 5: shape, 6: shape, 7: shape}[number]
+        base = {2: (256, 256, 256), 3: (128, 192, 384), 4: (512, 512, 512), 5: shape, 6: shape, 7: shape, 8: shape}[number]
         scale = min(1.0, (cells_budget / float(np.prod(base))) ** (1.0 / 3.0))
         sample = tuple(max(16, int(round(b * scale / 8)) * 8) for b in base)
     cfg = make_cfg_named(args.workload, number, sample, extra)

@@ -237,6 +237,16 @@ def make_config(number, shape=None, k_max=None, n_modes=None):
         cfg["number"] = 7
         cfg["params"] = dict(cfg["params"], rho_out=1.0, fringe_len=max(nx // 8, 1), fringe_factor=10.0)
         return cfg
+    if number == 8:
+        # config 7 with the wall model on the building faces as well ("wall-modelled"; SURVEY 8(f)-2 "wall model on
+        # building faces of all six orientations"): every plain fluid cell (FLUID, d = 0) with a building cell (d = 1) as axis
+        # neighbour becomes a WALLMODEL cell with the normal pointing away from that face (roofs first, then x, then y faces) and
+        # d := 1 (reading R8), like the floor cells
+        cfg = make_config(7, shape=shape)
+        n_faces = wallmodel_faces(cfg["flags"], cfg["d"])
+        cfg["number"] = 8
+        cfg["wm_face_cells"] = n_faces
+        return cfg
     if number == 6:
         # lid-driven cavity (the paper's scaling benchmark; not a BASELINE.json config):
         # closed box, five resting walls, the z = nz-1 plane moves with u_wall = (0.05, 0, 0); fluid at rest, rho = 1;
@@ -279,6 +289,24 @@ def body_velocity(cfg, seed, amp=0.02):
     moving = (d > 0.0) & (d < 1.0) if d is not None else np.zeros((nz, ny, nx), dtype=bool)
     ub[:, ~moving] = 0.0
     return ub
+
+
+def wallmodel_faces(flags, d):
+    """Flag the plain fluid cells next to a building face (a FLUID cell with d = 1) as WALLMODEL cells, in place; the normal code
+    {0:+x, 1:-x, 2:+y, 3:-y, 4:+z, 5:-z} points from the face into the fluid.  Returns the number of cells per normal code."""
+    building = (d == 1.0) & ((flags & 0x0F) == FLUID)
+    plain = (d == 0.0) & (flags == FLUID)
+    taken = np.zeros_like(plain)
+    counts = []
+    # (normal code, axis, shift): the building lies at x - n, i.e. building rolled by +n along the axis
+    order = [(4, 0, 1), (5, 0, -1), (0, 2, 1), (1, 2, -1), (2, 1, 1), (3, 1, -1)]
+    for code, axis, sh in order:
+        m = plain & ~taken & np.roll(building, sh, axis=axis)
+        flags[m] = WALLMODEL | (code << 4)
+        taken |= m
+        counts.append((code, int(m.sum())))
+    d[taken] = 1.0
+    return dict(counts)
 
 
 def cavity_flags(shape):

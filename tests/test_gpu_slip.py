@@ -39,6 +39,18 @@ def test_paper_boundary_set_hrr(dtype):
     check_parity(_paper_channel((24, 32, 64), collision=1, sigma=0.7), dtype)
 
 
+@pytest.mark.parametrize("dtype,Q,extra", [("f32", 19, {}), ("f64", 19, {}), ("f32", 27, {}), ("f64", 19, dict(collision=1, sigma=0.7)),
+                                           ("f32", 19, dict(collision=1, sigma=0.7))])
+def test_paper_boundary_set_with_wall_model_on_the_building_faces(dtype, Q, extra):
+    """config 8: config 7 + WALLMODEL cells on the roofs and the four side faces of the buildings"""
+    cfg = I.make_config(8, shape=(40, 48, 160))
+    cfg["Q"] = Q
+    cfg["params"] = dict(cfg["params"], **extra)
+    n = cfg["wm_face_cells"]
+    assert all(n[c] > 100 for c in (0, 1, 2, 3, 4))
+    check_parity(cfg, dtype)
+
+
 @pytest.mark.parametrize("Q", [19, 27])
 def test_closed_slip_box_with_obstacles_and_zero_gradient_outlet_corner_cases(Q):
     shape = (14, 12, 32)

@@ -60,3 +60,21 @@ def test_config_table():
     assert abs(c2["params"]["tau0"] - 0.50003) < 1e-12 and c2["params"]["cs_smago"] == 0.1
     c4 = I.make_config(4, shape=(48, 48, 48), k_max=4, n_modes=32)
     assert c4["Q"] == 27 and np.abs(c4["u"][:, c4["flags"] == I.SOLID]).max() == 0.0
+
+
+def test_config8_wall_model_cells_on_building_faces_point_away_from_the_face():
+    cfg = I.make_config(8, shape=(40, 48, 160))
+    base = I.make_config(7, shape=(40, 48, 160))
+    fl, d = cfg["flags"], cfg["d"]
+    building = (base["d"] == 1.0) & ((base["flags"] & 15) == I.FLUID)
+    new = ((fl & 15) == I.WALLMODEL) & ((base["flags"] & 15) != I.WALLMODEL)
+    assert new.sum() == sum(cfg["wm_face_cells"].values()) > 1000
+    assert (base["d"][new] == 0.0).all() and (d[new] == 1.0).all()
+    # the cell behind every new wall-model cell (x - n) is a building cell
+    for z, y, x in np.argwhere(new)[::7]:
+        code = fl[z, y, x] >> 4
+        n = [0, 0, 0]
+        n[code >> 1] = -1 if (code & 1) else 1
+        assert building[z - n[2], y - n[1], x - n[0]]
+    # nothing else changed
+    assert np.array_equal(fl[~new], base["flags"][~new]) and np.array_equal(d[~new], base["d"][~new])
