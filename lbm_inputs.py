@@ -297,16 +297,25 @@ def wallmodel_faces(flags, d):
     building = (d == 1.0) & ((flags & 0x0F) == FLUID)
     plain = (d == 0.0) & (flags == FLUID)
     taken = np.zeros_like(plain)
-    counts = []
+    cand = []
     # (normal code, axis, shift): the building lies at x - n, i.e. building rolled by +n along the axis
     order = [(4, 0, 1), (5, 0, -1), (0, 2, 1), (1, 2, -1), (2, 1, 1), (3, 1, -1)]
     for code, axis, sh in order:
         m = plain & ~taken & np.roll(building, sh, axis=axis)
-        flags[m] = WALLMODEL | (code << 4)
         taken |= m
-        counts.append((code, int(m.sum())))
-    d[taken] = 1.0
-    return dict(counts)
+        cand.append(m)
+    # the wall model samples the velocity at x + n: that cell must be plain fluid and not a candidate itself (a gap of one or two
+    # cells between two buildings has no such point: two wall-model cells sampling each other feed back and blow up within 40 steps)
+    free = plain & ~taken
+    counts = {}
+    chosen = np.zeros_like(plain)
+    for (code, axis, sh), m in zip(order, cand):
+        ok = m & np.roll(free, -sh, axis=axis)
+        flags[ok] = WALLMODEL | (code << 4)
+        chosen |= ok
+        counts[code] = int(ok.sum())
+    d[chosen] = 1.0
+    return counts
 
 
 def cavity_flags(shape):

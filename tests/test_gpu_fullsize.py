@@ -202,6 +202,24 @@ def test_paper_boundary_set_full_size_windows():
     _check_windows(cfg, "f32", wins, (True, True, True), vm=vm)
 
 
+def test_wall_model_on_building_faces_full_size_windows():
+    """bench.py paperbc_wmfaces_urban_channel_384x192x128_f32_*: config 8 (the paper's boundary set + wall-model cells on the roofs
+    and the four side faces of the buildings); one window around a wall-model cell of every orientation the geometry has"""
+    cfg = I.make_config(8, shape=(128, 192, 384))
+    nz, ny, nx = cfg["shape"]
+    fl = cfg["flags"]
+    wins = []
+    for code in (0, 1, 2, 3, 4):
+        idx = np.argwhere((fl == (I.WALLMODEL | (code << 4))) & (np.arange(nz)[:, None, None] > 1))
+        assert len(idx) > 1000
+        for k in (len(idx) // 3, 2 * len(idx) // 3):
+            z, y, x = idx[k]
+            wins.append((int(np.clip(z - W // 2, 1, nz - 1 - W)), int(np.clip(y - W // 2, 1, ny - 1 - W)), int(np.clip(x - W // 2, 0, nx - W))))
+    _check_windows(cfg, "f32", wins, (True, True, True))
+    cfg["params"] = dict(cfg["params"], collision=1, sigma=0.7)
+    _check_windows(cfg, "f32", wins[::2], (True, True, True), steps=6)
+
+
 def test_cavity_full_size_windows():
     """lid-driven cavity 512^3 (bench.py cavity_512_f32: three launches per step, lid slices on the MW kernel variant):
     windows at the lid's corners and edges, under the lid, at the floor and in the bulk; the walls close every axis"""

@@ -76,5 +76,11 @@ def test_config8_wall_model_cells_on_building_faces_point_away_from_the_face():
         n = [0, 0, 0]
         n[code >> 1] = -1 if (code & 1) else 1
         assert building[z - n[2], y - n[1], x - n[0]]
+    # ... and the cell in front of it (x + n, where the wall model samples the velocity) is plain fluid
+    for z, y, x in np.argwhere(new)[::5]:
+        code = fl[z, y, x] >> 4
+        n = [0, 0, 0]
+        n[code >> 1] = -1 if (code & 1) else 1
+        assert fl[z + n[2], y + n[1], x + n[0]] == I.FLUID and d[z + n[2], y + n[1], x + n[0]] == 0.0
     # nothing else changed
     assert np.array_equal(fl[~new], base["flags"][~new]) and np.array_equal(d[~new], base["d"][~new])
