@@ -36,7 +36,7 @@ def _axis_crop(lo, n, closed):
     return idx, lo - a
 
 
-def _check_windows(cfg, dtype, windows, closed_axes, steps=S, u_scale=0.0, vm=None):
+def _check_windows(cfg, dtype, windows, closed_axes, steps=S, u_scale=0.0, vm=None, u_body=None):
     """u_scale: velocity scale of the whole field (R12 normalises by the field's maximum; a window of fluid at rest has none)"""
     nz, ny, nx = cfg["shape"]
     Q = cfg["Q"]
@@ -47,6 +47,9 @@ def _check_windows(cfg, dtype, windows, closed_axes, steps=S, u_scale=0.0, vm=No
     par = P.LbmParams(**cfg["params"])
     with P.LBM(Q, nx, ny, nz, dtype) as sim:
         sim.set_fields(f, d, cfg["flags"])                  # host pointers, library defaults = bench configuration
+        if u_body is not None:
+            u_body = u_body.astype(npdt)
+            sim.set_body_velocity(u_body)
         if vm is not None:
             sim.set_inflow(vm["u_mean"].astype(npdt))
             sim.set_vortices(vm["pos"], vm["sign"], vm["sigma_v"], vm["intensity"])
@@ -82,7 +85,8 @@ def _check_windows(cfg, dtype, windows, closed_axes, steps=S, u_scale=0.0, vm=No
             assert ix.max() + 1 < nx - 1 - par_c["fringe_len"], "window crop cuts the fringe zone"
             par_c["fringe_len"] = 0
         if fields is None:
-            ref = O.step(fc, d=dc, flags=flc, nsteps=steps, nthreads=min(O.max_threads(), 8), **par_c)
+            ubc = None if u_body is None else np.ascontiguousarray(u_body[(slice(None),) + sel]).astype(np.float64)
+            ref = O.step(fc, d=dc, flags=flc, nsteps=steps, nthreads=min(O.max_threads(), 8), u_body=ubc, **par_c)
         else:
             ref = fc
             for fld in fields:
@@ -200,6 +204,23 @@ def test_paper_boundary_set_full_size_windows():
     wins = [(1, 1, 0), (nz - 1 - W, ny - 1 - W, 0), (60, 1, nx - W), (nz - 1 - W, 90, nx - W), (1, ny - 1 - W, 200), (nz - 1 - W, 1, 150),
             (40, 100, nx - 20), (60, 90, 190)]
     _check_windows(cfg, "f32", wins, (True, True, True), vm=vm)
+
+
+def test_moving_bodies_full_size_windows():
+    """bench.py config3_urban_channel_384x192x128_f32_body / _hrr_body: the trees of config 3 carry a solid velocity field
+    (lbm_inputs.body_velocity, same seed as bench.py); windows centred on tree cells (0 < d < 1)"""
+    cfg = I.make_config(3)
+    nz, ny, nx = cfg["shape"]
+    ub = I.body_velocity(cfg, 1403, amp=0.02)
+    trees = np.argwhere((cfg["d"] > 0) & (cfg["d"] < 1))
+    assert len(trees) > 100000 and np.abs(ub[:, cfg["d"] == 1.0]).max() == 0.0
+    wins = []
+    for k in range(1, 9):
+        z, y, x = trees[k * len(trees) // 9]
+        wins.append((int(np.clip(z - W // 2, 1, nz - 1 - W)), int(y - W // 2) % ny, int(np.clip(x - W // 2, 0, nx - W))))
+    _check_windows(cfg, "f32", wins, (True, False, True), u_body=ub)
+    cfg["params"] = dict(cfg["params"], collision=1, sigma=0.7)
+    _check_windows(cfg, "f32", wins[::2], (True, False, True), steps=6, u_body=ub)
 
 
 def test_wall_model_on_building_faces_full_size_windows():
