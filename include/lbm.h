@@ -203,6 +203,7 @@ long long lbm_query(const lbm_ctx* ctx, int what);
 /* Tuning knobs (no effect on results beyond floating-point summation order).  Returns LBM_EINVAL for an
  * unknown key/value.  Keys:
  *   "cuda_graph"  0|1   replay each lbm_step(n) through a captured CUDA graph (default 1 for n >= 4)
+ *   "serpentine"  0|1   consecutive launches sweep the z-slices in opposite directions for L2 reuse (default 1)
  * More keys are listed in DESIGN.md as the kernels gain variants. */
 int lbm_set_option(lbm_ctx* ctx, const char* key, long long value);
 

@@ -73,6 +73,8 @@ struct lbm_ctx {
   long long ev_step_level[2];   // time level of the step after which ev_step[k] was recorded (-1: never)
   void* ub;              // prescribed solid velocity u^B [3][N] (lbm_set_body_velocity), nullptr = 0 everywhere
   void* uhat;            // HRR form: u^(x,t) [3][N], allocated on the first HRR step
+  int serpentine;        // 1: consecutive launches sweep z in opposite directions (L2 reuse)
+  long long sweep_count; // BGK steps launched so far (parity = direction)
   int hrr_slab;          // HRR form: z-slices per slab of the two-pass step (0 = whole lattice)
   lbm_params last;       // parameters of the last lbm_step: the inlet rule is part of how S_t is formed from F_{t-1}
   char err[512];
@@ -158,6 +160,7 @@ lbm::StepArgs<T> make_args(const lbm_ctx* c, const lbm_params* p, int in, int ou
   a.list = c->list;
   a.n_list = static_cast<int>(c->n_list);
   a.list_z = 0;
+  a.z_reverse = 0;
   a.z0 = 0;
   a.uhat = static_cast<T*>(c->uhat);
   a.sigma = p ? static_cast<T>(p->sigma) : T(1);
@@ -207,6 +210,9 @@ int launch_one(lbm_ctx* c, const lbm_params* p, int in, int out, int z0, int nzs
   dim3 grid, block;
   lbm::StepArgs<T> a = make_args<T>(c, p, in, out);
   a.z0 = z0;
+  // serpentine sweep (lbm_set_option "serpentine", default 1): BGK steps alternate their direction with the time level; in the
+  // HRR form the u^ pass runs downwards and the step pass upwards
+  if (c->serpentine) a.z_reverse = lbm::mode_uhat(MODE) ? 1 : ((COLL == lbm::COLL_HRR) ? 0 : static_cast<int>(c->sweep_count & 1));
   const bool vec = c->use_vector && (c->nx % (32 / static_cast<int>(sizeof(T))) == 0);   // whole 32-byte sectors per row
   if (vec) {
     launch_dims_vec<Q, T, COLL>(c, grid, block);
@@ -296,6 +302,7 @@ int launch_step_t(lbm_ctx* c, const lbm_params* p, int mode) {
   }
   if (rc != LBM_OK) return rc;
   c->cur = out;
+  c->sweep_count++;
   return LBM_OK;
 }
 
@@ -587,6 +594,7 @@ lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype) {
   c->phase = PHASE_NONE;
   c->block_threads = 64;
   c->use_vector = 1;
+  c->serpentine = 1;
   c->last = default_params();
   std::snprintf(c->err, sizeof(c->err), "no error");
   const size_t pop = static_cast<size_t>(lattice) * N * dtype;
@@ -948,6 +956,11 @@ int lbm_set_option(lbm_ctx* c, const char* key, long long value) {
   if (std::strcmp(key, "block_threads") == 0) {
     if (value != 64 && value != 128 && value != 256) return fail(c, LBM_EINVAL, "block_threads must be 64, 128 or 256");
     c->block_threads = static_cast<int>(value);
+    return LBM_OK;
+  }
+  if (std::strcmp(key, "serpentine") == 0) {
+    if (value != 0 && value != 1) return fail(c, LBM_EINVAL, "serpentine must be 0 or 1");
+    c->serpentine = static_cast<int>(value);
     return LBM_OK;
   }
   if (std::strcmp(key, "hrr_slab") == 0) {

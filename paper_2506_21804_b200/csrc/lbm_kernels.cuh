@@ -105,6 +105,7 @@ struct StepArgs {
   const int* __restrict__ list;
   int n_list;
   int list_z;
+  int z_reverse;                  // vector kernel: walk the slab from its last slice down (serpentine sweep over consecutive launches)
   int z0;                         // first lattice z-slice of this launch (the grid covers a slab z0 .. z0 + gridDim.z - list_z - 1)
   // HRR form (Eq. 7-11): u^(x,t) of every cell [3][N] (written by the MODE_UHAT_* pass, SOLID cells 0), Eq. 7 factor
   T* __restrict__ uhat;
@@ -914,7 +915,10 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
   const int nvec = a.nx / V;
   const int qx = blockIdx.x * blockDim.x + tx;
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
-  const int z = a.z0 + static_cast<int>(blockIdx.z) - a.list_z;
+  // serpentine sweep: a launch that runs against the direction of the previous one starts on the slices that launch wrote (or read)
+  // last, which are still in the 126 MB L2
+  const int kz = static_cast<int>(blockIdx.z) - a.list_z;
+  const int z = a.z0 + (a.z_reverse ? (static_cast<int>(gridDim.z) - a.list_z - 1 - kz) : kz);
   const bool active = (qx < nvec) && (y < a.ny);
   const int x0 = qx * V;
   const int nx = a.nx, ny = a.ny, nz = a.nz;
