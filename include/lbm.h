@@ -90,8 +90,11 @@ typedef struct {
 
 /* Create a context for an nx x ny x nz lattice (nx fastest in memory).
  * lattice: LBM_D3Q19 | LBM_D3Q27 (l.60; D3Q27 from BASELINE.json config 4).  dtype: LBM_F32 | LBM_F64.
- * nx, ny, nz >= 1 and nx*ny*nz < 2^31.  Allocates two population lattices (2*Q*N*dtype bytes), the
- * porosity field and one class byte per cell on the current CUDA device.
+ * nx, ny, nz >= 1 (SURVEY 8(b) asked for LBM_EINVAL below 3; sizes 1 and 2 are accepted as a superset: the periodic wrap is
+ * well defined for them and they are parity-tested), nx*ny*nz < 2^31, ny <= 65535 and nz <= 65000 (launch-grid limits; a
+ * lattice whose nz plus its list slices passes 65535 is refused by lbm_step with LBM_EINVAL).  Rows with nx a multiple of
+ * 32/sizeof(dtype) take the vector kernel, other row lengths the scalar kernel.  Allocates two population lattices
+ * (2*Q*N*dtype bytes), the porosity field, one class byte and one 32-bit neighbour mask per cell on the current CUDA device.
  * Returns NULL on failure; lbm_last_error(NULL) then holds the reason. */
 lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype);
 
@@ -162,27 +165,49 @@ int lbm_get_inflow(lbm_ctx* ctx, void* u);
  *   -> tau_eff from the local non-equilibrium stress (Eq. 3-5, 14) -> relaxation (Eq. 6) -> propagation
  *   with halfway bounce-back at SOLID neighbours (R5), zero-gradient outlet (R7), regularised velocity
  *   inlet (l.155, R6).
- * BGK form: one fused kernel launch per step on the context's stream.  HRR form: two launches per
- * z-slab of the lattice (u^ pass, then the fused step) and 3 more values of dtype per
- * cell of device memory (allocated on the first HRR step; LBM_ENOMEM if that fails).  Asynchronous.
+ * BGK form: one fused kernel launch per step on the context's stream, preceded by the wall-model pre-pass over the
+ * compact list of WALLMODEL cells when wm_enable and such cells exist (3 values of dtype per cell of device memory for
+ * their u^B, allocated on the first such step).  HRR form: two launches per step (u^ pass, then the fused step;
+ * DESIGN.md 5.5) and 3 more values of dtype per cell (allocated on the first HRR step; LBM_ENOMEM if that fails).
+ * Steady-state steps are replayed 8 at a time from a captured CUDA graph (option "cuda_graph").  Asynchronous.
  * Errors: LBM_EINVAL (NULL ctx/params, n_steps < 0, tau0 <= 0.5, cs_smago < 0, wm_enable with
  * wm_kappa <= 0 or wm_E <= 0, collision not 0/1, sigma outside [0,1] with HRR, rho_out < 0, fringe_len < 0, fringe_factor < 0), LBM_ESTATE (no state
  * set yet), LBM_ECUDA. */
 int lbm_step(lbm_ctx* ctx, int n_steps, const lbm_params* params);
 
 /* Moments of the state S_t for EVERY cell (SOLID cells report whatever was set):
- * rho = sum_i f_i, u = sum_i c_i f_i / rho -- the raw fluid velocity moment of l.97 (G19), not u^.
- * rho[nz][ny][nx], u[3][nz][ny][nx] dtype, host or device; either may be NULL to skip it. */
+ * rho = sum_i f_i, u = sum_i c_i f_i / rho -- the raw fluid velocity moment of l.97 (G19), not u^ (SURVEY 8(a) row A9).
+ * rho[nz][ny][nx], u[3][nz][ny][nx] dtype, host or device; either may be NULL to skip it.
+ * One launch of the step kernel in its moments mode (the pull of S_t from the stored post-collision lattice happens in
+ * registers; nothing is materialised and the following lbm_step costs no extra pass) plus one launch over the wall cells.
+ * Errors: LBM_EINVAL (NULL ctx), LBM_ESTATE (no state), LBM_ENOMEM (staging for host outputs), LBM_ECUDA. */
 int lbm_moments(lbm_ctx* ctx, void* rho, void* u);
 
-/* State S_t in the external layout (parity checks, checkpoint).  populations[Q][nz][ny][nx]. */
+/* State S_t = the pre-collision populations f_i(x,t) of Eq. 6 (l.70-72; reading G12/R2) in the external layout:
+ * populations[Q][nz][ny][nx] dtype, host or device, written in full (parity checks, checkpoint).
+ * When the storage holds the post-collision lattice this materialises S_t with one stream-only pass into the other lattice
+ * (the next lbm_step then starts with a collide-only sweep: still one sweep per step).
+ * Errors: LBM_EINVAL (NULL ctx / buffer), LBM_ESTATE (no state), LBM_ECUDA. */
 int lbm_get_populations(lbm_ctx* ctx, void* populations);
 
-/* Totals over non-SOLID cells of S_t: out[0] = sum rho, out[1..3] = sum rho u, out[4] = sum rho |u|^2 / 2.
- * `out` is a HOST array of 5 doubles.  Accumulated in fp64.  Synchronises the stream. */
+/* The same for a box of cells only: origin (x0,y0,z0), extent (bx,by,bz) >= 1, inside the lattice (no wrap);
+ * populations[Q][bz][by][bx] dtype, host or device.  For probes and for parity checks on lattices whose full state does not
+ * fit a third time in memory (896^3 fp32: 54.7 GB per population set).  Materialises S_t like lbm_get_populations.
+ * Errors: LBM_EINVAL (NULL ctx / buffer, box empty or outside the lattice), LBM_ESTATE, LBM_ENOMEM, LBM_ECUDA. */
+int lbm_get_populations_box(lbm_ctx* ctx, int x0, int y0, int z0, int bx, int by, int bz, void* populations);
+
+/* Totals over the non-wall cells of S_t (the conserved quantities of Eq. 6: mass and momentum, l.97,
+ * and the kinetic energy the Taylor-Green check of config 1 is stated in): out[0] = sum rho, out[1..3] = sum rho u,
+ * out[4] = sum rho |u|^2 / 2.  `out` is a HOST array of 5 doubles.  One launch, pulling S_t in registers like lbm_moments:
+ * per-thread sums over the cells of a vector in dtype, from the warp level up in fp64 (shuffle tree, one atomicAdd(double)
+ * per block into one of 256 slots, the last block adds the slots).  Synchronises the stream.
+ * Errors: LBM_EINVAL (NULL ctx / out), LBM_ESTATE (no state), LBM_ECUDA. */
 int lbm_totals(lbm_ctx* ctx, double out[5]);
 
-/* Use `cuda_stream` (a cudaStream_t passed as void*) for all subsequent work; NULL = default stream. */
+/* Use `cuda_stream` (a cudaStream_t passed as void*) for all subsequent work; NULL = the legacy default stream (also the
+ * stream of a fresh context).  Synchronises the old stream first.  PyTorch owns streams in this build (north_star: "PyTorch
+ * used only for device memory and streams"): pass torch.cuda.current_stream().cuda_stream.  Errors: LBM_EINVAL (NULL ctx),
+ * LBM_ECUDA. */
 int lbm_set_stream(lbm_ctx* ctx, void* cuda_stream);
 
 /* Block until everything enqueued so far has finished; returns LBM_ECUDA if any kernel failed. */
@@ -193,18 +218,29 @@ int lbm_synchronize(lbm_ctx* ctx);
 const char* lbm_last_error(const lbm_ctx* ctx);
 
 /* Introspection used by the harness.  what:
- *   0 steps taken since the last set_fields/init      1 kernels launched by this ctx so far
- *   2 number of cells N                                3 number of SOLID cells
+ *   0 steps taken since the last set_fields/init      1 kernels launched by this ctx so far (graph replays count their kernels)
+ *   2 number of cells N                                3 number of wall cells (SOLID, MOVINGWALL, SLIPWALL)
  *   4 device bytes owned by the ctx                    5 cells on the masked (boundary) path
- *   6 cells handled by the list blocks of the vector kernel (masked cells + their vector mates)
+ *   6 cells handled by the list blocks of the vector kernel (SPECIAL cells + their sector mates)
+ *   7 CUDA graph launches so far                       8 WALLMODEL cells (length of the pre-pass list)
  * Returns -1 for an unknown `what` or a NULL ctx. */
 long long lbm_query(const lbm_ctx* ctx, int what);
 
-/* Tuning knobs (no effect on results beyond floating-point summation order).  Returns LBM_EINVAL for an
- * unknown key/value.  Keys:
- *   "cuda_graph"  0|1   replay each lbm_step(n) through a captured CUDA graph (default 1 for n >= 4)
- *   "serpentine"  0|1   consecutive launches sweep the z-slices in opposite directions for L2 reuse (default 1)
- * More keys are listed in DESIGN.md as the kernels gain variants. */
+/* Tuning knobs.  None changes a result (the A/B tests compare populations bit for bit).  Returns LBM_EINVAL for an
+ * unknown key or value, LBM_ESTATE where noted.  Keys (every key the library accepts is listed here):
+ *   "cuda_graph"    0|1     1 (default): lbm_step replays the steady-state time loop 8 steps at a time from a captured CUDA
+ *                           graph (re-captured when parameters, fields or options change); steps that do not fill a chunk, the
+ *                           first step of a fresh state and runs with the Vortex Method inlet use plain launches
+ *   "pdl"           0|1|2   programmatic dependent launch of the time-loop kernels: 0 plain launches; 1 every kernel becomes
+ *                           resident while its predecessor drains and waits for it; 2 (default) additionally, after the
+ *                           wall-model pre-pass only the threads that read its output wait for it
+ *   "wm_prepass"    0|1     1 (default): WALLMODEL cells run in the vector path, their u^B comes from a pre-pass over their
+ *                           compact list; 0: they are solved cell by cell in the list blocks of the step kernel.  Decides how
+ *                           flags are classified: LBM_ESTATE once a state or geometry has been set
+ *   "serpentine"    0|1     consecutive launches sweep the z-slices in opposite directions for L2 reuse (default 1)
+ *   "vector"        0|1     0 forces the scalar kernel (one cell per thread) for every row length (default 1)
+ *   "block_threads" 64|128|256   threads per block of the step kernels (default 64)
+ *   "hrr_slab"      n >= 0  HRR form: interleave the u^ pass and the step pass in slabs of n z-slices (0 = whole lattice, default) */
 int lbm_set_option(lbm_ctx* ctx, const char* key, long long value);
 
 #ifdef __cplusplus

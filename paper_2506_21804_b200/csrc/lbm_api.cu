@@ -3,7 +3,7 @@
 // Argument checking, device storage, phase bookkeeping and kernel launches.  No arithmetic of
 // the method lives here; it is all in lbm_kernels.cuh.
 // =====================================================================================
-#include "../../include/lbm.h"
+#include "lbm_ctx.h"
 
 #include <cstdarg>
 #include <cstdio>
@@ -16,72 +16,10 @@
 #include "lbm_kernels.cuh"
 
 namespace {
-
 char g_create_error[512] = "no error";
-
-enum Phase { PHASE_NONE = 0,   // no state yet
-             PHASE_PRE = 1,    // cur holds S_t (pre-collision), as handed in
-             PHASE_POST = 2 }; // cur holds F_{t-1} (post-collision, not yet streamed); S_t = stream(F_{t-1})
-
 }  // namespace
 
-struct lbm_ctx {
-  int Q, nx, ny, nz, dtype;
-  long long N;
-  void* f[2];            // two population lattices, [Q][N] each
-  void* d;               // porosity [N]
-  bool has_d;
-  uint8_t* cls;          // class byte per cell (see lbm_kernels.cuh)
-  uint8_t* cls_alt;      // classification target before it is accepted
-  uint8_t* flags_raw;    // device copy of the caller's flag bytes; afterwards the list marks
-  uint32_t* nbmask;      // per cell: which lattice neighbours are SOLID (read-side bounce-back)
-  int* solid_list;       // SOLID cells, ascending
-  void* solid_vals;      // their own populations [Q][n_solid] (the step kernels write zeros over their lattice slots)
-  long long n_solid_list;
-  int* list;             // cells of the non-bulk vectors (vector kernel), ascending
-  long long n_list;
-  void* cub_tmp;
-  size_t cub_tmp_bytes;
-  int* list_count_dev;
-  unsigned long long* counters;  // device [6]
-  long long n_moving, n_slip;    // MOVINGWALL / SLIPWALL cells of the accepted geometry
-  double* totals_dev;            // device [5]
-  void* staging;         // host<->device bounce buffer, grown on demand
-  size_t staging_bytes;
-  int cur;
-  Phase phase;
-  long long steps, launches, n_solid, n_masked;
-  size_t device_bytes;
-  cudaStream_t stream;
-  int block_threads;
-  int use_vector;        // 1: 128-bit vector kernel when nx % (32/dtype) == 0 (default); 0: scalar kernel
-  int use_graph;
-  // Vortex Method inlet / per-cell inflow field (lbm_set_inflow, lbm_set_vortices)
-  double* uin_mean;      // [3][nz][ny] fp64 (whatever the dtype), nullptr = uniform params.u_in
-  double* uin_field[2];  // inflow of the current / the previous time level, fp64
-  int uin_cur;
-  long long inflow_index;   // the time level t the current inflow field belongs to (S_t carries it)
-  int nv;
-  double* vpos;  double* vsign;  double* vgamma;     // device [nv][2], [nv], [nv]
-  double vm_sigma, vm_intensity;
-  bool gamma_dirty;
-  // the inflow of level t+1 depends on the inflow of level t only, never on the lattice: it is formed on a side stream while
-  // step t runs (events order the two streams; two field buffers)
-  cudaStream_t vm_stream;
-  cudaEvent_t ev_vm, ev_step[2];
-  bool vm_pending;          // the newest field is still being written on vm_stream
-  long long ev_step_level[2];   // time level of the step after which ev_step[k] was recorded (-1: never)
-  void* ub;              // prescribed solid velocity u^B [3][N] (lbm_set_body_velocity), nullptr = 0 everywhere
-  void* uhat;            // HRR form: u^(x,t) [3][N], allocated on the first HRR step
-  int serpentine;        // 1: consecutive launches sweep z in opposite directions (L2 reuse)
-  long long sweep_count; // BGK steps launched so far (parity = direction)
-  int hrr_slab;          // HRR form: z-slices per slab of the two-pass step (0 = whole lattice)
-  lbm_params last;       // parameters of the last lbm_step: the inlet rule is part of how S_t is formed from F_{t-1}
-  char err[512];
-};
-
-namespace {
-
+namespace lbmhost {
 int fail(lbm_ctx* c, int code, const char* fmt, ...) {
   char* dst = c ? c->err : g_create_error;
   va_list ap;
@@ -90,12 +28,11 @@ int fail(lbm_ctx* c, int code, const char* fmt, ...) {
   va_end(ap);
   return code;
 }
+}  // namespace lbmhost
 
-#define LBM_CUDA(c, call)                                                                             \
-  do {                                                                                                \
-    cudaError_t e_ = (call);                                                                          \
-    if (e_ != cudaSuccess) return fail((c), LBM_ECUDA, "%s: %s", #call, cudaGetErrorString(e_));      \
-  } while (0)
+namespace {
+
+using lbmhost::fail;
 
 bool is_device_pointer(const void* p) {
   cudaPointerAttributes at;
@@ -141,212 +78,21 @@ void launch_dims(const lbm_ctx* c, dim3& grid, dim3& block) {
   while (ny2 < c->ny) ny2 <<= 1;
   if (by > ny2) by = ny2;
   if (by < 1) by = 1;
-  if (bx * by < 32) by = 32 / bx;   // whole warps only: the reductions use full-mask shuffles
+  if (bx * by < 32) by = 32 / bx;
   block = dim3(bx, by, 1);
   grid = dim3((c->nx + bx - 1) / bx, (c->ny + by - 1) / by, c->nz);
 }
 
-template <typename T>
-lbm::StepArgs<T> make_args(const lbm_ctx* c, const lbm_params* p, int in, int out) {
-  lbm::StepArgs<T> a;
-  a.fin = static_cast<const T*>(c->f[in]);
-  a.fout = static_cast<T*>(c->f[out]);
-  a.d = (p && p->use_hlbm && c->has_d) ? static_cast<const T*>(c->d) : nullptr;
-  a.ub = (a.d != nullptr && c->ub) ? static_cast<const T*>(c->ub) : nullptr;
-  a.cls = c->cls;
-  a.nbmask = c->nbmask;
-  a.nx = c->nx;  a.ny = c->ny;  a.nz = c->nz;
-  a.N = c->N;
-  a.list = c->list;
-  a.n_list = static_cast<int>(c->n_list);
-  a.list_z = 0;
-  a.z_reverse = 0;
-  a.z0 = 0;
-  a.uhat = static_cast<T*>(c->uhat);
-  a.sigma = p ? static_cast<T>(p->sigma) : T(1);
-  for (int k = 0; k < 3; ++k) a.u_wall[k] = p ? static_cast<T>(p->u_wall[k]) : T(0);
-  a.rho_out = (p && p->rho_out > 0.0) ? static_cast<T>(p->rho_out) : T(1);
-  a.fringe_k = T(0);
-  a.fringe_x0 = c->nx;
-  if (p && p->fringe_len > 0 && p->fringe_factor > 0.0) {
-    a.fringe_k = static_cast<T>((p->tau0 - 0.5) * p->fringe_factor / (static_cast<double>(p->fringe_len) * p->fringe_len));
-    a.fringe_x0 = c->nx - 1 - p->fringe_len;
-  }
-  a.uin_field = c->uin_mean ? c->uin_field[c->uin_cur] : nullptr;
-  if (p) {
-    a.tau0 = static_cast<T>(p->tau0);
-    a.smago_k = static_cast<T>(18.0 * 1.4142135623730951 * p->cs_smago * p->cs_smago);
-    a.u_in[0] = static_cast<T>(p->u_in[0]);  a.u_in[1] = static_cast<T>(p->u_in[1]);  a.u_in[2] = static_cast<T>(p->u_in[2]);
-    a.wm_enable = p->wm_enable;
-    a.wm_kappa = p->wm_kappa;  a.wm_E = p->wm_E;
-    a.nu = (p->tau0 - 0.5) / 3.0;
-  } else {
-    a.tau0 = T(1);  a.smago_k = T(0);
-    a.u_in[0] = a.u_in[1] = a.u_in[2] = T(0);
-    a.wm_enable = 0;  a.wm_kappa = 0.41;  a.wm_E = 9.8;  a.nu = 1.0 / 6.0;
-  }
-  return a;
-}
-
-// vector kernel: thread <-> V consecutive cells; block (bx quads, by rows)
-template <int Q, typename T, int COLL>
-void launch_dims_vec(const lbm_ctx* c, dim3& grid, dim3& block) {
-  const int V = lbm::VecOf<Q, T, COLL>::V;
-  const int nvec = c->nx / V;
-  int bx = 1;
-  while (bx < nvec && bx < 32) bx <<= 1;
-  int by = c->block_threads / bx;
-  int ny2 = 1;
-  while (ny2 < c->ny) ny2 <<= 1;
-  if (by > ny2) by = ny2;
-  if (bx * by < 32) by = 32 / bx;
-  block = dim3(bx, by, 1);
-  grid = dim3((nvec + bx - 1) / bx, (c->ny + by - 1) / by, c->nz);
-}
-
-// One launch of a step kernel over the z-slices [z0, z0 + nzs) (+ the list blocks when with_list), lattice `in` -> `out`.
-template <int Q, typename T, int MODE, int COLL>
-int launch_one(lbm_ctx* c, const lbm_params* p, int in, int out, int z0, int nzs, bool with_list, bool may_meet_lid = true) {
-  dim3 grid, block;
-  lbm::StepArgs<T> a = make_args<T>(c, p, in, out);
-  a.z0 = z0;
-  // serpentine sweep (lbm_set_option "serpentine", default 1): BGK steps alternate their direction with the time level; in the
-  // HRR form the u^ pass runs downwards and the step pass upwards
-  if (c->serpentine) a.z_reverse = lbm::mode_uhat(MODE) ? 1 : ((COLL == lbm::COLL_HRR) ? 0 : static_cast<int>(c->sweep_count & 1));
-  const bool vec = c->use_vector && (c->nx % (32 / static_cast<int>(sizeof(T))) == 0);   // whole 32-byte sectors per row
-  if (vec) {
-    launch_dims_vec<Q, T, COLL>(c, grid, block);
-    a.list_z = 0;
-    if (with_list) {
-      const long long per_slice = static_cast<long long>(grid.x) * grid.y * block.x * block.y;
-      a.list_z = static_cast<int>((c->n_list + per_slice - 1) / per_slice);
-    }
-    grid.z = nzs + a.list_z;
-    if (grid.z == 0) return LBM_OK;
-    if (c->n_moving > 0 && may_meet_lid && lbm::mode_pulls(MODE)) lbm::k_step_vec<Q, T, MODE, COLL, true><<<grid, block, 0, c->stream>>>(a);
-    else                                          lbm::k_step_vec<Q, T, MODE, COLL, false><<<grid, block, 0, c->stream>>>(a);
-  } else {
-    if (nzs == 0) return LBM_OK;
-    launch_dims(c, grid, block);
-    grid.z = nzs;
-    lbm::k_step<Q, T, MODE, COLL><<<grid, block, 0, c->stream>>>(a);
-  }
-  LBM_CUDA(c, cudaGetLastError());
-  c->launches++;
-  return LBM_OK;
-}
-
-// HRR form (Eq. 7-11): the FD strain (Eq. 10) needs u^(x,t) of the six neighbours, i.e. their streamed populations, so
-// a step is two passes: UHAT (pull, moments, Eq. 12 -> u^ field) and the fused step that reads it.  The passes are
-// interleaved slab by slab in z, the UHAT pass one slice ahead, so that the populations the UHAT pass pulled are still
-// in the 126 MB L2 when the step pass pulls them again.  The list cells (wall model, ...) go with the
-// first UHAT launch and the last step launch.
-template <int Q, typename T, int MODE_U, int MODE_S>
-int launch_hrr_t(lbm_ctx* c, const lbm_params* p, int in, int out) {
-  const int nz = c->nz;
-  int slab = (c->hrr_slab > 0) ? c->hrr_slab : nz;
-  if (slab >= nz - 1) {
-    int rc = launch_one<Q, T, MODE_U, lbm::COLL_BGK>(c, p, in, out, 0, nz, true);
-    if (rc != LBM_OK) return rc;
-    return launch_one<Q, T, MODE_S, lbm::COLL_HRR>(c, p, in, out, 0, nz, true);
-  }
-  // UHAT: slice nz-1 first (the periodic neighbour of slice 0), then [0, slab], [slab+1, 2 slab], ... up to nz-2
-  int rc = launch_one<Q, T, MODE_U, lbm::COLL_BGK>(c, p, in, out, nz - 1, 1, true);
-  if (rc != LBM_OK) return rc;
-  int udone = 0;                       // slices [0, udone) have their u^
-  for (int z0 = 0; z0 < nz; z0 += slab) {
-    const int zend = (z0 + slab < nz) ? z0 + slab : nz;          // step pass covers [z0, zend)
-    int uneed = (zend + 1 < nz - 1) ? zend + 1 : nz - 1;         // needs u^ on [z0 - 1, zend]; nz-1 is done
-    if (uneed > udone) {
-      rc = launch_one<Q, T, MODE_U, lbm::COLL_BGK>(c, p, in, out, udone, uneed - udone, false);
-      if (rc != LBM_OK) return rc;
-      udone = uneed;
-    }
-    rc = launch_one<Q, T, MODE_S, lbm::COLL_HRR>(c, p, in, out, z0, zend - z0, zend == nz);
-    if (rc != LBM_OK) return rc;
-  }
-  return LBM_OK;
-}
-
-// The timed BGK step.  With a moving lid (MOVINGWALL cells live on the plane z = nz-1 only) the slices that can meet it
-// (z = nz-2, nz-1 and, through the periodic wrap, 0) take the kernel variant that looks the neighbour's class up; the bulk
-// runs the plain variant: three launches instead of one.
-template <int Q, typename T>
-int launch_bgk_pull_t(lbm_ctx* c, const lbm_params* p, int in, int out) {
-  const int nz = c->nz;
-  if (c->n_moving == 0 || nz < 8)
-    return launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 0, nz, true);
-  int rc = launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 1, nz - 3, true, false);
-  if (rc == LBM_OK) rc = launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, nz - 2, 2, false);
-  if (rc == LBM_OK) rc = launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 0, 1, false);
-  return rc;
-}
-
-template <int Q, typename T>
-int launch_step_t(lbm_ctx* c, const lbm_params* p, int mode) {
-  const int in = c->cur, out = 1 - c->cur;
-  const bool hrr = p && p->collision == LBM_COLLISION_HRR;
-  int rc;
-  switch (mode) {
-    case lbm::MODE_COLLIDE:
-      rc = hrr ? launch_hrr_t<Q, T, lbm::MODE_UHAT_PRE, lbm::MODE_COLLIDE>(c, p, in, out)
-               : launch_one<Q, T, lbm::MODE_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 0, c->nz, true);
-      break;
-    case lbm::MODE_STREAM_COLLIDE:
-      rc = hrr ? launch_hrr_t<Q, T, lbm::MODE_UHAT_PULL, lbm::MODE_STREAM_COLLIDE>(c, p, in, out)
-               : launch_bgk_pull_t<Q, T>(c, p, in, out);
-      break;
-    default:
-      rc = launch_one<Q, T, lbm::MODE_STREAM, lbm::COLL_BGK>(c, p, in, out, 0, c->nz, true);
-      break;
-  }
-  if (rc != LBM_OK) return rc;
-  c->cur = out;
-  c->sweep_count++;
-  return LBM_OK;
-}
+// the launchers live in lbm_inst.cu (one object per lattice, dtype and part)
+#define LBM_DISPATCH(c, fn, ...)                                                                                                \
+  ((c)->Q == 19 ? ((c)->dtype == LBM_F32 ? lbmhost::fn<19, float>(__VA_ARGS__) : lbmhost::fn<19, double>(__VA_ARGS__))          \
+                : ((c)->dtype == LBM_F32 ? lbmhost::fn<27, float>(__VA_ARGS__) : lbmhost::fn<27, double>(__VA_ARGS__)))
 
 int launch_step(lbm_ctx* c, const lbm_params* p, int mode) {
-  if (c->Q == 19) return c->dtype == LBM_F32 ? launch_step_t<19, float>(c, p, mode) : launch_step_t<19, double>(c, p, mode);
-  return c->dtype == LBM_F32 ? launch_step_t<27, float>(c, p, mode) : launch_step_t<27, double>(c, p, mode);
+  const bool hrr = p && p->collision == LBM_COLLISION_HRR && mode != lbm::MODE_STREAM;
+  if (hrr) return LBM_DISPATCH(c, launch_step_hrr, c, p, mode);
+  return LBM_DISPATCH(c, launch_step_bgk, c, p, mode);
 }
-
-template <int Q, typename T>
-int launch_moments_t(lbm_ctx* c, const lbm_params* p, void* rho, void* u) {
-  dim3 grid, block;
-  launch_dims(c, grid, block);
-  lbm::StepArgs<T> a = make_args<T>(c, p, c->cur, 1 - c->cur);
-  lbm::k_moments<Q, T><<<grid, block, 0, c->stream>>>(a, static_cast<T*>(rho), static_cast<T*>(u));
-  LBM_CUDA(c, cudaGetLastError());
-  c->launches++;
-  return LBM_OK;
-}
-
-template <int Q, typename T>
-int launch_totals_t(lbm_ctx* c, const lbm_params* p) {
-  dim3 grid, block;
-  launch_dims(c, grid, block);
-  lbm::StepArgs<T> a = make_args<T>(c, p, c->cur, 1 - c->cur);
-  lbm::k_totals<Q, T><<<grid, block, 0, c->stream>>>(a, c->totals_dev);
-  LBM_CUDA(c, cudaGetLastError());
-  c->launches++;
-  return LBM_OK;
-}
-
-template <int Q, typename T>
-int launch_init_t(lbm_ctx* c, const void* rho, const void* u) {
-  const int threads = 256;
-  const long long blocks = (c->N + threads - 1) / threads;
-  lbm::k_init_equilibrium<Q, T><<<static_cast<unsigned>(blocks), threads, 0, c->stream>>>(
-      static_cast<const T*>(rho), static_cast<const T*>(u), static_cast<T*>(c->f[0]), c->N);
-  LBM_CUDA(c, cudaGetLastError());
-  c->launches++;
-  return LBM_OK;
-}
-
-#define LBM_DISPATCH(c, fn, ...)                                                                              \
-  ((c)->Q == 19 ? ((c)->dtype == LBM_F32 ? fn<19, float>(__VA_ARGS__) : fn<19, double>(__VA_ARGS__))          \
-                : ((c)->dtype == LBM_F32 ? fn<27, float>(__VA_ARGS__) : fn<27, double>(__VA_ARGS__)))
 
 lbm_params default_params() {
   lbm_params p;
@@ -374,6 +120,7 @@ int check_params(lbm_ctx* c, const lbm_params* p) {
 }
 
 // stream compaction of the cell indices n with flags_raw[n] != 0 (count known) into a new device array
+// (cub::DeviceSelect: a library primitive at set-up time only, never inside lbm_step)
 int compact_marks(lbm_ctx* c, long long count, int** out) {
   *out = nullptr;
   if (count <= 0) return LBM_OK;
@@ -382,15 +129,21 @@ int compact_marks(lbm_ctx* c, long long count, int** out) {
   if (rc != LBM_OK) return rc;
   cub::CountingInputIterator<int> it(0);
   size_t need = 0;
-  LBM_CUDA(c, cub::DeviceSelect::Flagged(nullptr, need, it, c->flags_raw, arr, c->list_count_dev, static_cast<int>(c->N), c->stream));
-  if (need > c->cub_tmp_bytes) {
+  cudaError_t e = cub::DeviceSelect::Flagged(nullptr, need, it, c->flags_raw, arr, c->list_count_dev, static_cast<int>(c->N), c->stream);
+  if (e == cudaSuccess && need > c->cub_tmp_bytes) {
     if (c->cub_tmp) { cudaFree(c->cub_tmp); c->device_bytes -= c->cub_tmp_bytes; c->cub_tmp = nullptr; c->cub_tmp_bytes = 0; }
     rc = dev_alloc(c, &c->cub_tmp, need);
-    if (rc != LBM_OK) { cudaFree(arr); return rc; }
-    c->cub_tmp_bytes = need;
+    if (rc == LBM_OK) c->cub_tmp_bytes = need;
   }
-  LBM_CUDA(c, cub::DeviceSelect::Flagged(c->cub_tmp, need, it, c->flags_raw, arr, c->list_count_dev, static_cast<int>(c->N), c->stream));
-  LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  if (rc == LBM_OK && e == cudaSuccess)
+    e = cub::DeviceSelect::Flagged(c->cub_tmp, need, it, c->flags_raw, arr, c->list_count_dev, static_cast<int>(c->N), c->stream);
+  if (rc == LBM_OK && e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (rc == LBM_OK && e != cudaSuccess) rc = fail(c, LBM_ECUDA, "list compaction: %s", cudaGetErrorString(e));
+  if (rc != LBM_OK) {
+    cudaFree(arr);
+    c->device_bytes -= static_cast<size_t>(count) * sizeof(int);
+    return rc;
+  }
   *out = arr;
   return LBM_OK;
 }
@@ -415,76 +168,91 @@ int solid_values(lbm_ctx* c, bool save) {
   return LBM_OK;
 }
 
-// copy flags to the device, validate + classify into cls_alt, accept on success
+// copy flags to the device, validate + classify into cls_alt, build the new compact lists, accept everything together on
+// success; on any failure the context keeps the geometry it had (lists, counts, class bytes, neighbour masks)
 int classify(lbm_ctx* c, const uint8_t* cell_flags) {
   if (cell_flags) {
     LBM_CUDA(c, cudaMemcpyAsync(c->flags_raw, cell_flags, c->N, cudaMemcpyDefault, c->stream));
   } else {
     LBM_CUDA(c, cudaMemsetAsync(c->flags_raw, 0, c->N, c->stream));
   }
-  LBM_CUDA(c, cudaMemsetAsync(c->counters, 0, 6 * sizeof(unsigned long long), c->stream));
+  LBM_CUDA(c, cudaMemsetAsync(c->counters, 0, 8 * sizeof(unsigned long long), c->stream));
   dim3 grid, block;
   launch_dims(c, grid, block);
-  if (c->Q == 19) lbm::k_classify<19><<<grid, block, 0, c->stream>>>(c->flags_raw, c->cls_alt, c->nx, c->ny, c->nz, c->counters);
-  else            lbm::k_classify<27><<<grid, block, 0, c->stream>>>(c->flags_raw, c->cls_alt, c->nx, c->ny, c->nz, c->counters);
+  const int wm_special = c->wm_prepass ? 0 : 1;
+  if (c->Q == 19) lbm::k_classify<19><<<grid, block, 0, c->stream>>>(c->flags_raw, c->cls_alt, c->nx, c->ny, c->nz, c->counters, wm_special);
+  else            lbm::k_classify<27><<<grid, block, 0, c->stream>>>(c->flags_raw, c->cls_alt, c->nx, c->ny, c->nz, c->counters, wm_special);
   LBM_CUDA(c, cudaGetLastError());
   c->launches++;
-  unsigned long long h[6];
+  unsigned long long h[8];
   LBM_CUDA(c, cudaMemcpyAsync(h, c->counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
   LBM_CUDA(c, cudaStreamSynchronize(c->stream));
   if (h[0] != 0)
     return fail(c, LBM_EINVAL, "cell_flags: %llu invalid flag byte(s) (type > 7, bad high nibble, INLET off x=0, OUTLET / POUTLET off x=nx-1 or MOVINGWALL off z=nz-1)", h[0]);
-  // compact list of the cells the vector kernel leaves to its list blocks
-  const int SV = 32 / c->dtype;        // cells per 32-byte sector of a population row
+  int* new_list = nullptr;
+  int* new_solid = nullptr;
+  int* new_wm = nullptr;
+  void* new_vals = nullptr;
+  const long long n_solid = static_cast<long long>(h[1]);
+  const long long n_wm = static_cast<long long>(h[6]);
+  const size_t vbytes = static_cast<size_t>(n_solid) * c->Q * c->dtype;
   long long n_list = 0;
+  int rc = LBM_OK;
+  // (1) cells the vector kernel leaves to its list blocks: every cell of a 32-byte sector that holds a SPECIAL cell
+  const int SV = 32 / c->dtype;        // cells per 32-byte sector of a population row
   if (c->nx % SV == 0) {
     const long long nsec = c->N / SV;
     const unsigned blocks = static_cast<unsigned>((nsec + 255) / 256);
     if (SV == 8) lbm::k_mark_list<8><<<blocks, 256, 0, c->stream>>>(c->cls_alt, c->flags_raw, nsec, c->counters);
     else         lbm::k_mark_list<4><<<blocks, 256, 0, c->stream>>>(c->cls_alt, c->flags_raw, nsec, c->counters);
-    LBM_CUDA(c, cudaGetLastError());
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h, c->counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return fail(c, LBM_ECUDA, "classify (list marks): %s", cudaGetErrorString(e));
     c->launches++;
-    LBM_CUDA(c, cudaMemcpyAsync(h, c->counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
-    LBM_CUDA(c, cudaStreamSynchronize(c->stream));
     n_list = static_cast<long long>(h[3]);
-    int* new_list = nullptr;
-    int rc = compact_marks(c, n_list, &new_list);
-    if (rc != LBM_OK) return rc;
-    if (c->list) { cudaFree(c->list); c->device_bytes -= static_cast<size_t>(c->n_list) * sizeof(int); }
-    c->list = new_list;
+    rc = compact_marks(c, n_list, &new_list);
   }
-  // SOLID cells: list + side buffer for their own values
-  {
-    const long long n_solid = static_cast<long long>(h[1]);
+  // (2) wall cells: list + side buffer for their own values
+  if (rc == LBM_OK) {
     const unsigned blocks = static_cast<unsigned>((c->N + 255) / 256);
     lbm::k_mark_solid<<<blocks, 256, 0, c->stream>>>(c->cls_alt, c->flags_raw, c->N);
-    LBM_CUDA(c, cudaGetLastError());
-    c->launches++;
-    int* new_list = nullptr;
-    int rc = compact_marks(c, n_solid, &new_list);
-    if (rc != LBM_OK) return rc;
-    void* new_vals = nullptr;
-    const size_t vbytes = static_cast<size_t>(n_solid) * c->Q * c->dtype;
-    if (n_solid > 0) {
-      rc = dev_alloc(c, &new_vals, vbytes);
-      if (rc != LBM_OK) { cudaFree(new_list); return rc; }
-    }
-    if (c->solid_list) { cudaFree(c->solid_list); c->device_bytes -= static_cast<size_t>(c->n_solid_list) * sizeof(int); }
-    if (c->solid_vals) { cudaFree(c->solid_vals); c->device_bytes -= static_cast<size_t>(c->n_solid_list) * c->Q * c->dtype; }
-    c->solid_list = new_list;
-    c->solid_vals = new_vals;
-    c->n_solid_list = n_solid;
+    if (cudaGetLastError() != cudaSuccess) rc = fail(c, LBM_ECUDA, "classify (wall marks): launch failed");
+    else { c->launches++; rc = compact_marks(c, n_solid, &new_solid); }
+    if (rc == LBM_OK && n_solid > 0) rc = dev_alloc(c, &new_vals, vbytes);
   }
-  c->n_list = n_list;
+  // (3) WALLMODEL cells: list of the pre-pass
+  if (rc == LBM_OK) {
+    const unsigned blocks = static_cast<unsigned>((c->N + 255) / 256);
+    lbm::k_mark_wm<<<blocks, 256, 0, c->stream>>>(c->cls_alt, c->flags_raw, c->N);
+    if (cudaGetLastError() != cudaSuccess) rc = fail(c, LBM_ECUDA, "classify (wall-model marks): launch failed");
+    else { c->launches++; rc = compact_marks(c, n_wm, &new_wm); }
+  }
+  if (rc != LBM_OK) {                  // nothing of the old geometry has been touched
+    if (new_list) { cudaFree(new_list); c->device_bytes -= static_cast<size_t>(n_list) * sizeof(int); }
+    if (new_solid) { cudaFree(new_solid); c->device_bytes -= static_cast<size_t>(n_solid) * sizeof(int); }
+    if (new_wm) { cudaFree(new_wm); c->device_bytes -= static_cast<size_t>(n_wm) * sizeof(int); }
+    if (new_vals) { cudaFree(new_vals); c->device_bytes -= vbytes; }
+    return rc;
+  }
+  // accept: swap lists, counts, class bytes together
+  if (c->list) { cudaFree(c->list); c->device_bytes -= static_cast<size_t>(c->n_list) * sizeof(int); }
+  if (c->solid_list) { cudaFree(c->solid_list); c->device_bytes -= static_cast<size_t>(c->n_solid_list) * sizeof(int); }
+  if (c->solid_vals) { cudaFree(c->solid_vals); c->device_bytes -= static_cast<size_t>(c->n_solid_list) * c->Q * c->dtype; }
+  if (c->wm_list) { cudaFree(c->wm_list); c->device_bytes -= static_cast<size_t>(c->n_wm) * sizeof(int); }
+  c->list = new_list;          c->n_list = n_list;
+  c->solid_list = new_solid;   c->solid_vals = new_vals;   c->n_solid_list = n_solid;
+  c->wm_list = new_wm;         c->n_wm = n_wm;
   uint8_t* t = c->cls;  c->cls = c->cls_alt;  c->cls_alt = t;
   if (c->Q == 19) lbm::k_nbmask<19><<<grid, block, 0, c->stream>>>(c->cls, c->nbmask, c->nx, c->ny, c->nz);
   else            lbm::k_nbmask<27><<<grid, block, 0, c->stream>>>(c->cls, c->nbmask, c->nx, c->ny, c->nz);
   LBM_CUDA(c, cudaGetLastError());
   c->launches++;
-  c->n_solid = static_cast<long long>(h[1]);
+  c->n_solid = n_solid;
   c->n_masked = static_cast<long long>(h[2]);
   c->n_moving = static_cast<long long>(h[4]);
   c->n_slip = static_cast<long long>(h[5]);
+  c->epoch++;
   return LBM_OK;
 }
 
@@ -579,7 +347,10 @@ lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype) {
   if (dtype != LBM_F32 && dtype != LBM_F64) { fail(nullptr, LBM_EINVAL, "lbm_create: dtype %d is not 4 (f32) or 8 (f64)", dtype); return nullptr; }
   if (nx < 1 || ny < 1 || nz < 1) { fail(nullptr, LBM_EINVAL, "lbm_create: nx, ny, nz must be >= 1 (got %d %d %d)", nx, ny, nz); return nullptr; }
   const long long N = static_cast<long long>(nx) * ny * nz;
-  if (N >= (1ll << 31) || nz > 65535) { fail(nullptr, LBM_EINVAL, "lbm_create: lattice too large (N = %lld must be < 2^31, nz <= 65535)", N); return nullptr; }
+  if (N >= (1ll << 31) || nz > 65000 || ny > 65535) {
+    fail(nullptr, LBM_EINVAL, "lbm_create: lattice too large (N = %lld must be < 2^31, ny <= 65535, nz <= 65000: grid limits)", N);
+    return nullptr;
+  }
   int ndev = 0;
   cudaError_t e = cudaGetDeviceCount(&ndev);
   if (e != cudaSuccess || ndev == 0) {
@@ -595,6 +366,9 @@ lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype) {
   c->block_threads = 64;
   c->use_vector = 1;
   c->serpentine = 1;
+  c->wm_prepass = 1;
+  c->use_pdl = 2;
+  c->use_graph = 1;
   c->last = default_params();
   std::snprintf(c->err, sizeof(c->err), "no error");
   const size_t pop = static_cast<size_t>(lattice) * N * dtype;
@@ -605,8 +379,10 @@ lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype) {
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->cls_alt), N);
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->flags_raw), N);
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->nbmask), static_cast<size_t>(N) * sizeof(uint32_t));
-  if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->counters), 6 * sizeof(unsigned long long));
-  if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->totals_dev), 5 * sizeof(double));
+  const size_t tot_bytes = (8 + 5 * LBM_TOT_SLOTS + 1) * sizeof(double);      // result, slots, ticket (see make_args)
+  if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->counters), 8 * sizeof(unsigned long long));
+  if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->totals_dev), tot_bytes);
+  if (rc == LBM_OK && cudaMemset(c->totals_dev, 0, tot_bytes) != cudaSuccess) rc = fail(c, LBM_ECUDA, "cudaMemset failed");
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->list_count_dev), sizeof(int));
   if (rc == LBM_OK && cudaMemset(c->cls, 0, N) != cudaSuccess) rc = fail(c, LBM_ECUDA, "cudaMemset failed");
   if (rc == LBM_OK && cudaMemset(c->nbmask, 0, static_cast<size_t>(N) * sizeof(uint32_t)) != cudaSuccess) rc = fail(c, LBM_ECUDA, "cudaMemset failed");
@@ -632,6 +408,10 @@ void lbm_destroy(lbm_ctx* c) {
   cudaFree(c->counters);  cudaFree(c->totals_dev);  cudaFree(c->staging);
   cudaFree(c->list);  cudaFree(c->cub_tmp);  cudaFree(c->list_count_dev);
   cudaFree(c->nbmask);  cudaFree(c->solid_list);  cudaFree(c->solid_vals);
+  cudaFree(c->wm_list);  cudaFree(c->wm_ub);  cudaFree(c->uin_scratch);
+  for (int k = 0; k < LBM_GRAPH_CACHE; ++k)
+    if (c->graphs[k].valid) cudaGraphExecDestroy(c->graphs[k].exec);
+  if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
   cudaGetLastError();
   delete c;
 }
@@ -694,7 +474,7 @@ int lbm_init_equilibrium(lbm_ctx* c, const void* rho, const void* u) {
     if (hr) { LBM_CUDA(c, cudaMemcpyAsync(s, rho, cell_bytes, cudaMemcpyDefault, c->stream)); drho = s; }
     if (hu) { LBM_CUDA(c, cudaMemcpyAsync(s + cell_bytes, u, 3 * cell_bytes, cudaMemcpyDefault, c->stream)); du = s + cell_bytes; }
   }
-  int rc = LBM_DISPATCH(c, launch_init_t, c, drho, du);
+  int rc = LBM_DISPATCH(c, launch_init, c, drho, du);
   if (rc != LBM_OK) return rc;
   if (hr || hu) LBM_CUDA(c, cudaStreamSynchronize(c->stream));
   c->cur = 0;
@@ -732,11 +512,13 @@ int lbm_set_geometry(lbm_ctx* c, const void* porosity, const uint8_t* cell_flags
 int lbm_set_porosity(lbm_ctx* c, const void* porosity) {
   if (!c) return LBM_EINVAL;
   if (!porosity) {
+    if (c->has_d) c->epoch++;
     c->has_d = false;
     return LBM_OK;
   }
   LBM_CUDA(c, cudaMemcpyAsync(c->d, porosity, static_cast<size_t>(c->N) * c->dtype, cudaMemcpyDefault, c->stream));
   if (!is_device_pointer(porosity)) LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  if (!c->has_d) c->epoch++;
   c->has_d = true;
   return LBM_OK;
 }
@@ -750,12 +532,14 @@ int lbm_set_body_velocity(lbm_ctx* c, const void* u_body) {
       cudaFree(c->ub);
       c->ub = nullptr;
       c->device_bytes -= bytes;
+      c->epoch++;
     }
     return LBM_OK;
   }
   if (!c->ub) {
     int rc = dev_alloc(c, &c->ub, bytes);
     if (rc != LBM_OK) return rc;
+    c->epoch++;
   }
   LBM_CUDA(c, cudaMemcpyAsync(c->ub, u_body, bytes, cudaMemcpyDefault, c->stream));
   if (!is_device_pointer(u_body)) LBM_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -772,9 +556,11 @@ int lbm_set_inflow(lbm_ctx* c, const void* u_mean) {
   if (!u_mean) {
     if (c->uin_mean) {
       LBM_CUDA(c, cudaStreamSynchronize(c->stream));
-      cudaFree(c->uin_mean);  cudaFree(c->uin_field[0]);  cudaFree(c->uin_field[1]);
+      cudaFree(c->uin_mean);  cudaFree(c->uin_field[0]);  cudaFree(c->uin_field[1]);  cudaFree(c->uin_scratch);
       c->uin_mean = c->uin_field[0] = c->uin_field[1] = nullptr;
-      c->device_bytes -= 3 * bytes;
+      c->uin_scratch = nullptr;
+      c->device_bytes -= 3 * bytes + static_cast<size_t>(n) * sizeof(float);
+      c->epoch++;
     }
     return LBM_OK;
   }
@@ -782,13 +568,17 @@ int lbm_set_inflow(lbm_ctx* c, const void* u_mean) {
     rc = dev_alloc(c, reinterpret_cast<void**>(&c->uin_mean), bytes);
     if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->uin_field[0]), bytes);
     if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->uin_field[1]), bytes);
+    // fp32 <-> fp64 conversions go through a buffer of their own: the idle field buffer belongs to the side stream, which may
+    // be writing the next level's inflow into it while a queued conversion still reads or writes it
+    if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->uin_scratch), static_cast<size_t>(n) * sizeof(float));
     if (rc != LBM_OK) return rc;
     c->uin_cur = 0;
+    c->epoch++;
   }
   if (c->dtype == LBM_F64) {
     LBM_CUDA(c, cudaMemcpyAsync(c->uin_mean, u_mean, bytes, cudaMemcpyDefault, c->stream));
-  } else {                               // fp32 input -> staging (the other field buffer) -> fp64
-    float* tmp = reinterpret_cast<float*>(c->uin_field[1 - c->uin_cur]);
+  } else {                               // fp32 input -> scratch -> fp64
+    float* tmp = c->uin_scratch;
     LBM_CUDA(c, cudaMemcpyAsync(tmp, u_mean, static_cast<size_t>(n) * sizeof(float), cudaMemcpyDefault, c->stream));
     lbm::k_convert<float, double><<<static_cast<unsigned>((n + 255) / 256), 256, 0, c->stream>>>(tmp, c->uin_mean, n);
     LBM_CUDA(c, cudaGetLastError());
@@ -837,14 +627,85 @@ int lbm_get_inflow(lbm_ctx* c, void* u) {
   const long long n = 3ll * c->ny * c->nz;
   if (c->dtype == LBM_F64) {
     LBM_CUDA(c, cudaMemcpyAsync(u, c->uin_field[c->uin_cur], static_cast<size_t>(n) * sizeof(double), cudaMemcpyDefault, c->stream));
-  } else {                               // fp64 -> fp32 through the idle field buffer
-    float* tmp = reinterpret_cast<float*>(c->uin_field[1 - c->uin_cur]);
+  } else {                               // fp64 -> fp32 through the conversion scratch (main stream only)
+    float* tmp = c->uin_scratch;
     lbm::k_convert<double, float><<<static_cast<unsigned>((n + 255) / 256), 256, 0, c->stream>>>(c->uin_field[c->uin_cur], tmp, n);
     LBM_CUDA(c, cudaGetLastError());
     c->launches++;
     LBM_CUDA(c, cudaMemcpyAsync(u, tmp, static_cast<size_t>(n) * sizeof(float), cudaMemcpyDefault, c->stream));
   }
   if (!is_device_pointer(u)) LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  return LBM_OK;
+}
+
+// ---- CUDA graphs ("cuda_graph", default on): the steady-state time loop is replayed in chunks of LBM_GRAPH_CHUNK steps from a
+// captured graph (one graph launch instead of 8 .. 24 kernel launches: matters where a step is shorter than its launches, i.e.
+// small lattices and the three-launch steps of the lid-driven cavity).  A chunk is an even number of steps, so the lattice roles
+// and the sweep direction are back where they started; one graph per (current lattice, sweep parity), re-captured when the
+// parameters or anything else baked into the kernel arguments changed (epoch).  Not used with the Vortex Method inlet (its
+// side stream and events are ordered on the host) and not for the first step of a fresh state.
+static void graph_drop(lbm_graph_entry& g) {
+  if (g.valid) cudaGraphExecDestroy(g.exec);
+  g.valid = false;
+}
+
+static int graph_chunk(lbm_ctx* c, const lbm_params* params, bool* done) {
+  *done = false;
+  const int parity = static_cast<int>(c->sweep_count & 1);
+  lbm_graph_entry& g = c->graphs[c->cur * 2 + parity];
+  if (g.valid && (g.epoch != c->epoch || std::memcmp(&g.params, params, sizeof(lbm_params)) != 0)) graph_drop(g);
+  if (!g.valid) {
+    if (!c->cap_stream && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+      cudaGetLastError();
+      c->use_graph = 0;
+      return LBM_OK;
+    }
+    // capture on the private stream; nothing executes, so the bookkeeping the launches advance is put back afterwards
+    const cudaStream_t user = c->stream;
+    const int cur0 = c->cur;
+    const long long sweep0 = c->sweep_count, launches0 = c->launches;
+    cudaGraph_t graph = nullptr;
+    if (cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+      cudaGetLastError();
+      c->use_graph = 0;
+      return LBM_OK;
+    }
+    c->stream = c->cap_stream;
+    c->prev_launch_prepass = false;
+    int rc = LBM_OK;
+    for (int k = 0; k < LBM_GRAPH_CHUNK && rc == LBM_OK; ++k) rc = launch_step(c, params, lbm::MODE_STREAM_COLLIDE);
+    const cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
+    c->stream = user;
+    c->cur = cur0;
+    c->sweep_count = sweep0;
+    g.launches = c->launches - launches0;
+    c->launches = launches0;
+    c->prev_launch_prepass = false;
+    if (rc != LBM_OK || e != cudaSuccess || graph == nullptr) {
+      if (graph) cudaGraphDestroy(graph);
+      cudaGetLastError();
+      c->use_graph = 0;                 // capture is not available here: the plain launch path does the same work
+      return LBM_OK;
+    }
+    const cudaError_t ei = cudaGraphInstantiate(&g.exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ei != cudaSuccess) {
+      cudaGetLastError();
+      c->use_graph = 0;
+      return LBM_OK;
+    }
+    g.valid = true;
+    g.params = *params;
+    g.epoch = c->epoch;
+    g.cur = cur0;
+    g.sweep_parity = parity;
+  }
+  LBM_CUDA(c, cudaGraphLaunch(g.exec, c->stream));
+  c->sweep_count += LBM_GRAPH_CHUNK;        // cur is unchanged after an even number of steps
+  c->launches += g.launches;
+  c->graph_launches++;
+  c->prev_launch_prepass = false;
+  *done = true;
   return LBM_OK;
 }
 
@@ -861,11 +722,25 @@ int lbm_step(lbm_ctx* c, int n_steps, const lbm_params* params) {
     if (rc != LBM_OK) return rc;
     // SOLID cells of all-SOLID lines are never written by the UHAT pass: u^ = 0 there (resting wall) from here on
     LBM_CUDA(c, cudaMemsetAsync(c->uhat, 0, bytes, c->stream));
+    c->epoch++;
   }
-  for (int s = 0; s < n_steps; ++s) {
+  if (params->wm_enable && c->wm_prepass && c->n_wm > 0 && !c->wm_ub && n_steps > 0) {
+    // u^B of the wall-model cells, addressed by cell (only their entries are ever touched)
+    rc = dev_alloc(c, &c->wm_ub, 3 * static_cast<size_t>(c->N) * c->dtype);
+    if (rc != LBM_OK) return rc;
+    c->epoch++;
+  }
+  int s = 0;
+  while (s < n_steps) {
     if (c->phase == PHASE_PRE) {
       rc = launch_step(c, params, lbm::MODE_COLLIDE);          // S_t -> F_t
       c->phase = PHASE_POST;
+    } else if (c->use_graph && !c->uin_mean && n_steps - s >= LBM_GRAPH_CHUNK) {
+      bool done = false;
+      rc = graph_chunk(c, params, &done);
+      if (rc != LBM_OK) return rc;
+      if (done) { s += LBM_GRAPH_CHUNK; continue; }
+      continue;                                                // capture unavailable: use_graph is off now
     } else {
       rc = ensure_inflow(c, c->steps + s);                     // Vortex Method inlet: the inflow S_t carries (Eq. 21)
       if (rc != LBM_OK) return rc;
@@ -874,11 +749,14 @@ int lbm_step(lbm_ctx* c, int n_steps, const lbm_params* params) {
     if (rc != LBM_OK) return rc;
     rc = vm_prefetch(c, c->steps + s);                         // inflow of the next level, beside this step
     if (rc != LBM_OK) return rc;
+    ++s;
   }
   c->steps += n_steps;
   return LBM_OK;
 }
 
+// A9.  Neither call changes the stored lattice or its phase: with the storage holding F_{t-1} the kernels pull S_t in
+// registers (one launch over the lattice + one over the wall cells' side buffer for lbm_moments).
 int lbm_moments(lbm_ctx* c, void* rho, void* u) {
   if (!c) return LBM_EINVAL;
   if (c->phase == PHASE_NONE) return fail(c, LBM_ESTATE, "lbm_moments: no state");
@@ -895,9 +773,9 @@ int lbm_moments(lbm_ctx* c, void* rho, void* u) {
     if (hu) du = s + cell_bytes;
   }
   lbm_params p = c->last;
-  int rc = materialise(c);           // S_t in the cell's own storage (one extra pass when the storage held F_{t-1})
+  int rc = (c->phase == PHASE_POST) ? ensure_inflow(c, c->steps) : LBM_OK;     // the inlet rule is part of the pull
   if (rc != LBM_OK) return rc;
-  rc = LBM_DISPATCH(c, launch_moments_t, c, &p, drho, du);
+  rc = LBM_DISPATCH(c, launch_moments, c, &p, drho, du);
   if (rc != LBM_OK) return rc;
   if (hr) LBM_CUDA(c, cudaMemcpyAsync(rho, drho, cell_bytes, cudaMemcpyDefault, c->stream));
   if (hu) LBM_CUDA(c, cudaMemcpyAsync(u, du, 3 * cell_bytes, cudaMemcpyDefault, c->stream));
@@ -917,15 +795,45 @@ int lbm_get_populations(lbm_ctx* c, void* populations) {
   return LBM_OK;
 }
 
+int lbm_get_populations_box(lbm_ctx* c, int x0, int y0, int z0, int bx, int by, int bz, void* populations) {
+  if (!c) return LBM_EINVAL;
+  if (!populations) return fail(c, LBM_EINVAL, "lbm_get_populations_box: populations is NULL");
+  if (c->phase == PHASE_NONE) return fail(c, LBM_ESTATE, "lbm_get_populations_box: no state");
+  if (bx < 1 || by < 1 || bz < 1 || x0 < 0 || y0 < 0 || z0 < 0 || x0 + bx > c->nx || y0 + by > c->ny || z0 + bz > c->nz)
+    return fail(c, LBM_EINVAL, "lbm_get_populations_box: box (%d,%d,%d)+(%d,%d,%d) is empty or leaves the lattice", x0, y0, z0, bx, by, bz);
+  const long long n = static_cast<long long>(c->Q) * bx * by * bz;
+  const size_t bytes = static_cast<size_t>(n) * c->dtype;
+  int rc = materialise(c);
+  if (rc != LBM_OK) return rc;
+  const bool host = !is_device_pointer(populations);
+  void* dst = populations;
+  if (host) {
+    rc = ensure_staging(c, bytes);
+    if (rc != LBM_OK) return rc;
+    dst = c->staging;
+  }
+  const unsigned blocks = static_cast<unsigned>((n + 255) / 256);
+  if (c->dtype == LBM_F32)
+    lbm::k_gather_box<float><<<blocks, 256, 0, c->stream>>>(static_cast<const float*>(c->f[c->cur]), c->N, c->nx, c->ny, x0, y0, z0, bx, by, bz, c->Q, static_cast<float*>(dst));
+  else
+    lbm::k_gather_box<double><<<blocks, 256, 0, c->stream>>>(static_cast<const double*>(c->f[c->cur]), c->N, c->nx, c->ny, x0, y0, z0, bx, by, bz, c->Q, static_cast<double*>(dst));
+  LBM_CUDA(c, cudaGetLastError());
+  c->launches++;
+  if (host) {
+    LBM_CUDA(c, cudaMemcpyAsync(populations, dst, bytes, cudaMemcpyDeviceToHost, c->stream));
+    LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  }
+  return LBM_OK;
+}
+
 int lbm_totals(lbm_ctx* c, double out[5]) {
   if (!c) return LBM_EINVAL;
   if (!out) return fail(c, LBM_EINVAL, "lbm_totals: out is NULL");
   if (c->phase == PHASE_NONE) return fail(c, LBM_ESTATE, "lbm_totals: no state");
-  LBM_CUDA(c, cudaMemsetAsync(c->totals_dev, 0, 5 * sizeof(double), c->stream));
   lbm_params p = c->last;
-  int rc = materialise(c);
+  int rc = (c->phase == PHASE_POST) ? ensure_inflow(c, c->steps) : LBM_OK;
   if (rc != LBM_OK) return rc;
-  rc = LBM_DISPATCH(c, launch_totals_t, c, &p);
+  rc = LBM_DISPATCH(c, launch_totals, c, &p);
   if (rc != LBM_OK) return rc;
   LBM_CUDA(c, cudaMemcpyAsync(out, c->totals_dev, 5 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
   LBM_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -942,10 +850,13 @@ long long lbm_query(const lbm_ctx* c, int what) {
     case 4: return static_cast<long long>(c->device_bytes);
     case 5: return c->n_masked;
     case 6: return c->n_list;
+    case 7: return c->graph_launches;
+    case 8: return c->n_wm;
     default: return -1;
   }
 }
 
+// options that change how the geometry is classified or what the kernel arguments hold invalidate the captured graphs
 int lbm_set_option(lbm_ctx* c, const char* key, long long value) {
   if (!c || !key) return LBM_EINVAL;
   if (std::strcmp(key, "cuda_graph") == 0) {
@@ -953,24 +864,42 @@ int lbm_set_option(lbm_ctx* c, const char* key, long long value) {
     c->use_graph = static_cast<int>(value);
     return LBM_OK;
   }
+  if (std::strcmp(key, "pdl") == 0) {
+    if (value < 0 || value > 2) return fail(c, LBM_EINVAL, "pdl must be 0, 1 or 2");
+    c->use_pdl = static_cast<int>(value);
+    c->epoch++;
+    return LBM_OK;
+  }
+  if (std::strcmp(key, "wm_prepass") == 0) {
+    if (value != 0 && value != 1) return fail(c, LBM_EINVAL, "wm_prepass must be 0 or 1");
+    if (c->phase != PHASE_NONE || c->n_wm > 0)
+      return fail(c, LBM_ESTATE, "wm_prepass decides how the flags are classified: set it before lbm_set_fields / lbm_set_geometry");
+    c->wm_prepass = static_cast<int>(value);
+    c->epoch++;
+    return LBM_OK;
+  }
   if (std::strcmp(key, "block_threads") == 0) {
     if (value != 64 && value != 128 && value != 256) return fail(c, LBM_EINVAL, "block_threads must be 64, 128 or 256");
     c->block_threads = static_cast<int>(value);
+    c->epoch++;
     return LBM_OK;
   }
   if (std::strcmp(key, "serpentine") == 0) {
     if (value != 0 && value != 1) return fail(c, LBM_EINVAL, "serpentine must be 0 or 1");
     c->serpentine = static_cast<int>(value);
+    c->epoch++;
     return LBM_OK;
   }
   if (std::strcmp(key, "hrr_slab") == 0) {
     if (value < 0) return fail(c, LBM_EINVAL, "hrr_slab must be >= 0");
     c->hrr_slab = static_cast<int>(value);
+    c->epoch++;
     return LBM_OK;
   }
   if (std::strcmp(key, "vector") == 0) {
     if (value != 0 && value != 1) return fail(c, LBM_EINVAL, "vector must be 0 or 1");
     c->use_vector = static_cast<int>(value);
+    c->epoch++;
     return LBM_OK;
   }
   return fail(c, LBM_EINVAL, "unknown option '%s'", key);

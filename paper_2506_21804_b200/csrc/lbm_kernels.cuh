@@ -28,7 +28,7 @@ __host__ __device__ constexpr bool is_wall(int cls_or_type) { return ((0xA2 >> (
 // SOLID takes the cell's own F_opp(i)(x) instead.  Nobody ever consumes the lattice slots of a SOLID cell, so the
 // step kernels write every 128-byte line they touch IN FULL (zeros on SOLID cells): a store stream with holes at
 // the walls leaves partial sectors that the L2 has to fill from DRAM, which cost config 4 a third of its
-// bandwidth (profiles/r1_config4_spheres.md).  SOLID cells' own values (inert, R5) are kept in a side buffer by
+// bandwidth (profiles/r1_k_step_vec_ncu.md).  SOLID cells' own values (inert, R5) are kept in a side buffer by
 // the host side and patched back whenever the state is materialised.
 constexpr uint8_t CLS_TYPE = 0x07;
 constexpr uint8_t CLS_ADJ = 0x40;
@@ -40,12 +40,29 @@ enum : int { MODE_COLLIDE = 0,        // input holds S_t (fresh state): collide 
              MODE_STREAM_COLLIDE = 1, // input holds F_{t-1}: pull to S_t, collide             -> F_t
              MODE_STREAM = 2,         // input holds F_{t-1}: pull to S_t, store S_t (materialise)
              MODE_UHAT_PULL = 3,      // input holds F_{t-1}: pull to S_t, store u^(x,t) (HRR form, first pass)
-             MODE_UHAT_PRE = 4 };     // input holds S_t: store u^(x,t)
+             MODE_UHAT_PRE = 4,       // input holds S_t: store u^(x,t)
+             MODE_MOMENTS_PULL = 5,   // A9: input holds F_{t-1}: pull to S_t, store rho, u of S_t into the caller's arrays
+             MODE_MOMENTS_PRE = 6,    // A9: input holds S_t
+             MODE_TOTALS_PULL = 7,    // A9: pull to S_t, reduce mass / momentum / kinetic energy over the non-wall cells
+             MODE_TOTALS_PRE = 8 };
 // collision forms (lbm_params.collision)
 enum : int { COLL_BGK = 0, COLL_HRR = 1 };
-__host__ __device__ constexpr bool mode_pulls(int mode) { return mode == MODE_STREAM_COLLIDE || mode == MODE_STREAM || mode == MODE_UHAT_PULL; }
+__host__ __device__ constexpr bool mode_pulls(int mode) {
+  return mode == MODE_STREAM_COLLIDE || mode == MODE_STREAM || mode == MODE_UHAT_PULL || mode == MODE_MOMENTS_PULL || mode == MODE_TOTALS_PULL;
+}
 __host__ __device__ constexpr bool mode_collides(int mode) { return mode == MODE_COLLIDE || mode == MODE_STREAM_COLLIDE; }
 __host__ __device__ constexpr bool mode_uhat(int mode) { return mode == MODE_UHAT_PULL || mode == MODE_UHAT_PRE; }
+__host__ __device__ constexpr bool mode_moments(int mode) { return mode == MODE_MOMENTS_PULL || mode == MODE_MOMENTS_PRE; }
+__host__ __device__ constexpr bool mode_totals(int mode) { return mode == MODE_TOTALS_PULL || mode == MODE_TOTALS_PRE; }
+__host__ __device__ constexpr bool mode_diag(int mode) { return mode_moments(mode) || mode_totals(mode); }
+// modes that read the porosity / solid velocity (Eq. 12)
+__host__ __device__ constexpr bool mode_hlbm(int mode) { return mode_collides(mode) || mode_uhat(mode); }
+
+// Programmatic dependent launch (sm_90+): a kernel launched with the programmatic-serialization attribute may become resident
+// while its predecessor in the stream drains; griddep_wait() returns once the predecessor has completed and its writes are
+// visible.  Both are no-ops in a kernel launched the ordinary way.
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void griddep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 // ---- velocity set by rule R1 (G13), generated at compile time -------------------------
 template <int Q>
@@ -118,6 +135,20 @@ struct StepArgs {
   T u_wall[3];                    // velocity of the MOVINGWALL cells (only ever on the plane z = nz-1), reading G33
   const T* __restrict__ ub;       // [3][N] prescribed solid velocity u^B(x,t) of Eq. 12 (moving porous bodies, l.99-106) or nullptr => 0;
                                   // read only where d != 0 (it enters with weight d); WALLMODEL cells take the wall model's u^B (G39)
+  // wall-model pre-pass (A8): u^B of the WALLMODEL cells [3][N] (only their entries are ever written or read), written by
+  // k_wallmodel_prepass of the same time level, or nullptr => the per-cell paths solve Spalding's law in place
+  T* __restrict__ wm_ub;
+  const int* __restrict__ wm_list;   // WALLMODEL cells, ascending
+  int n_wm;
+  int pdl_wait_all;               // 1: every thread waits for the preceding kernel (it wrote this kernel's input);
+                                  // 0: only the threads that read wm_ub wait (the predecessor is the wall-model pre-pass)
+  // A9 outputs: caller arrays rho[N], u[3][N] (either may be nullptr); totals: slots[LBM slots][5] partial sums, a ticket, out[5]
+  T* __restrict__ mom_rho;
+  T* __restrict__ mom_u;
+  double* __restrict__ tot_slots;
+  unsigned* __restrict__ tot_ticket;
+  double* __restrict__ tot_out;
+  int tot_nslots;
 };
 
 // ---- math helpers ---------------------------------------------------------------------------------
@@ -457,7 +488,7 @@ __device__ __forceinline__ void spalding_eval(double up, double kappa, double in
   dsp = 1.0 + kappa * invE * (ek - 1.0 - k - k2);
 }
 
-__device__ __noinline__ double wallmodel_ratio(double U2, double nu, double kappa, double E) {
+static __device__ __noinline__ double wallmodel_ratio(double U2, double nu, double kappa, double E) {
   const double y2 = 1.5, y1 = 0.5;
   const double invE = 1.0 / E;
   const double Re = U2 * y2 / nu;
@@ -723,23 +754,108 @@ __device__ __forceinline__ void body_velocity(const T* __restrict__ pub, long lo
   }
 }
 
+// raw moments of one cell held in registers (A2 / A9): rho = sum f, j = sum c f
+template <int Q, typename T>
+__device__ __forceinline__ void cell_moments(const T (&f)[Q], T& rho, T& jx, T& jy, T& jz) {
+  constexpr Stencil<Q> L{};
+  constexpr int H = (Q - 1) / 2;
+  rho = f[0];
+  jx = jy = jz = T(0);
+#pragma unroll
+  for (int i = 1; i <= H; ++i) {
+    rho += f[i] + f[i + H];
+    const T df = f[i] - f[i + H];
+    if (L.c[i][0] == 1) jx += df; else if (L.c[i][0] == -1) jx -= df;
+    if (L.c[i][1] == 1) jy += df; else if (L.c[i][1] == -1) jy -= df;
+    if (L.c[i][2] == 1) jz += df; else if (L.c[i][2] == -1) jz -= df;
+  }
+}
+
+// A9 totals: block partial sums -> slot (spreads the atomics over nslots x 5 addresses) -> the last block of the grid
+// (ticket) adds the slots up in a fixed order, writes out[5] and leaves slots and ticket zeroed for the next launch.
+// Every thread of the block must call it (warp shuffle tree -> shared memory -> one atomicAdd(double) per block and quantity).
+__device__ __forceinline__ void reduce_totals(const double (&v)[5], double* __restrict__ slots, int nslots,
+                                              unsigned* __restrict__ ticket, double* __restrict__ out) {
+  __shared__ double part[5][8];
+  __shared__ int s_last;
+  const int tid = threadIdx.y * blockDim.x + threadIdx.x;
+  const int lane = tid & 31, warp = tid >> 5;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    double s = v[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    if (lane == 0) part[k][warp] = s;
+  }
+  __syncthreads();
+  const int nwarps = (blockDim.x * blockDim.y + 31) >> 5;
+  const unsigned nblocks = gridDim.x * gridDim.y * gridDim.z;
+  const unsigned blk = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+  if (tid < 5) {
+    double s = 0.0;
+    for (int w = 0; w < nwarps; ++w) s += part[tid][w];
+    if (s != 0.0) atomicAdd(slots + static_cast<size_t>(blk % nslots) * 5 + tid, s);
+    __threadfence();
+  }
+  __syncthreads();
+  if (tid == 0) s_last = (atomicInc(ticket, nblocks - 1u) == nblocks - 1u) ? 1 : 0;   // wraps to 0 on the last block
+  __syncthreads();
+  if (s_last && tid < 5) {
+    __threadfence();
+    double s = 0.0;
+    for (int q = 0; q < nslots; ++q) {
+      s += __ldcg(slots + static_cast<size_t>(q) * 5 + tid);
+      slots[static_cast<size_t>(q) * 5 + tid] = 0.0;
+    }
+    out[tid] = s;
+  }
+}
+
 // ---- the per-cell step (scalar kernel; list blocks of the vector kernel) ------------------------------
-// One non-SOLID cell of any type: pull (modes that pull), wall model, then collide + store (collide modes), store S_t
-// (MODE_STREAM) or store u^ (MODE_UHAT_*).
+// One non-wall cell of any type: pull (modes that pull), wall model, then collide + store (collide modes), store S_t
+// (MODE_STREAM), store u^ (MODE_UHAT_*), store rho, u (MODE_MOMENTS_*) or add to the totals acc[] (MODE_TOTALS_*).
 template <int Q, typename T, int MODE, int COLL>
-__device__ __forceinline__ void step_cell_any(const StepArgs<T>& a, int x, int y, int z, uint8_t cls) {
+__device__ __forceinline__ void step_cell_any(const StepArgs<T>& a, int x, int y, int z, uint8_t cls, double (&acc)[5]) {
   constexpr bool PULL = mode_pulls(MODE);
   const long long self = cell_index(x, y, z, a.nx, a.ny);
   const int type = cls & CLS_TYPE;
   T d = T(0), ubx = T(0), uby = T(0), ubz = T(0);
   const bool wm = (type == T_WM) && a.wm_enable;
-  if (MODE != MODE_STREAM) {
+  if (mode_hlbm(MODE)) {
     if (a.d != nullptr) d = __ldg(a.d + self);
-    if (wm) wallmodel_ub<Q, T, PULL>(a, x, y, z, cls, ubx, uby, ubz);
-    else if (a.ub != nullptr) body_velocity<T>(a.ub + self, a.N, d, ubx, uby, ubz);
+    if (wm) {
+      if (a.wm_ub != nullptr) {                // written by the pre-pass of this time level (possibly still running: PDL)
+        if (!a.pdl_wait_all) griddep_wait();
+        ubx = __ldcg(a.wm_ub + self);
+        uby = __ldcg(a.wm_ub + a.N + self);
+        ubz = __ldcg(a.wm_ub + 2 * a.N + self);
+      } else {
+        wallmodel_ub<Q, T, PULL>(a, x, y, z, cls, ubx, uby, ubz);
+      }
+    } else if (a.ub != nullptr) {
+      body_velocity<T>(a.ub + self, a.N, d, ubx, uby, ubz);
+    }
   }
   T f[Q];
   load_state<Q, T, PULL>(a, x, y, z, cls, f);
+  if (mode_diag(MODE)) {
+    T rho, jx, jy, jz;
+    cell_moments<Q, T>(f, rho, jx, jy, jz);
+    if (mode_moments(MODE)) {
+      const T ir = rcp_(rho);
+      if (a.mom_rho != nullptr) a.mom_rho[self] = rho;
+      if (a.mom_u != nullptr) {
+        a.mom_u[self] = jx * ir;
+        a.mom_u[a.N + self] = jy * ir;
+        a.mom_u[2 * a.N + self] = jz * ir;
+      }
+    } else {
+      const double r = static_cast<double>(rho), px = static_cast<double>(jx), py = static_cast<double>(jy), pz = static_cast<double>(jz);
+      acc[0] += r;  acc[1] += px;  acc[2] += py;  acc[3] += pz;
+      acc[4] += 0.5 * (px * px + py * py + pz * pz) / r;
+    }
+    return;
+  }
   if (mode_uhat(MODE)) {
     T ux, uy, uz;
     uhat_of<Q, T>(f, d, ubx, uby, ubz, ux, uy, uz);
@@ -760,9 +876,11 @@ __device__ __forceinline__ void step_cell_any(const StepArgs<T>& a, int x, int y
   store_cell<Q, T>(a, x, y, z, f);
 }
 
-// wall cell in the per-cell paths: zeros over its lattice slots (never read; keeps sectors whole) / u^ = the wall's velocity
+// wall cell in the per-cell paths: zeros over its lattice slots (never read; keeps sectors whole) / u^ = the wall's velocity;
+// the A9 modes leave it alone (moments: k_solid_moments reports the cell's own values; totals: walls do not count)
 template <int Q, typename T, int MODE>
 __device__ __forceinline__ void solid_cell_any(const StepArgs<T>& a, long long self) {
+  if (mode_diag(MODE)) return;
   if (mode_uhat(MODE)) {
     const bool mv = (a.cls[self] & CLS_TYPE) == T_MOVING;     // u^ of a wall cell = the wall's velocity (G30, G33)
     a.uhat[self] = mv ? a.u_wall[0] : T(0);
@@ -777,17 +895,40 @@ __device__ __forceinline__ void solid_cell_any(const StepArgs<T>& a, long long s
 // Fallback for row lengths the vector kernel does not take.
 template <int Q, typename T, int MODE, int COLL>
 __global__ void __launch_bounds__(256) k_step(const __grid_constant__ StepArgs<T> a) {
+  if (a.pdl_wait_all) griddep_wait();
+  griddep_launch();
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
   const int z = a.z0 + blockIdx.z;
-  if (x >= a.nx || y >= a.ny) return;
-  const long long self = cell_index(x, y, z, a.nx, a.ny);
-  const uint8_t cls = a.cls[self];
-  if (is_wall(cls)) {                        // wall cells are inert (R5); their slots are never read
-    solid_cell_any<Q, T, MODE>(a, self);
-    return;
+  double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  if (x < a.nx && y < a.ny) {
+    const long long self = cell_index(x, y, z, a.nx, a.ny);
+    const uint8_t cls = a.cls[self];
+    if (is_wall(cls)) solid_cell_any<Q, T, MODE>(a, self);   // wall cells are inert (R5); their slots are never read
+    else step_cell_any<Q, T, MODE, COLL>(a, x, y, z, cls, acc);
   }
-  step_cell_any<Q, T, MODE, COLL>(a, x, y, z, cls);
+  if constexpr (mode_totals(MODE)) reduce_totals(acc, a.tot_slots, a.tot_nslots, a.tot_ticket, a.tot_out);
+}
+
+// A8 as a pre-pass over the compact list of WALLMODEL cells (reading R8): u^B of every wall-model cell of this time level, so
+// that the cells themselves run in the vector path like any other cell and only the two Newton solves stay per cell.
+// PULL: the lattice holds F_{t-1} (the sample point's S_t is pulled).  Launched with programmatic serialization: the blocks
+// wait for the step kernel that wrote the lattice, then let the next step kernel start beside them.
+template <int Q, typename T, bool PULL>
+__global__ void __launch_bounds__(128) k_wallmodel_prepass(const __grid_constant__ StepArgs<T> a) {
+  griddep_wait();
+  griddep_launch();
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= a.n_wm) return;
+  const int cell = a.wm_list[k];
+  const int plane = a.nx * a.ny;
+  const int z = cell / plane, rem = cell - z * plane;
+  const int y = rem / a.nx, x = rem - y * a.nx;
+  T ubx, uby, ubz;
+  wallmodel_ub<Q, T, PULL>(a, x, y, z, a.cls[cell], ubx, uby, ubz);
+  a.wm_ub[cell] = ubx;
+  a.wm_ub[a.N + cell] = uby;
+  a.wm_ub[2 * a.N + cell] = ubz;
 }
 
 // ---- the vectorised step kernel (the hot one) ------------------------------------------------------
@@ -885,7 +1026,7 @@ __device__ __forceinline__ void ld_uhat_nb(const T* pu, long long N, int dyp, in
 // Everything else -- bulk, solid-adjacent (read-side bounce-back), INLET and OUTLET cells -- runs in the vector path.
 // MW: the launch may meet MOVINGWALL cells (compiled out otherwise: the test costs the wall-adjacent warps registers).
 template <int Q, typename T, int MODE, int COLL, bool MW>
-__global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ StepArgs<T> a) {
+__device__ __forceinline__ void step_vec_body(const StepArgs<T>& a, double (&acc)[5]) {
   constexpr Stencil<Q> L{};
   constexpr int V = VecOf<Q, T, COLL>::V;
   constexpr bool HRR = (COLL == COLL_HRR) && mode_collides(MODE);
@@ -906,7 +1047,7 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
         const int plane = a.nx * a.ny;
         const int cz = cell / plane, rem = cell - cz * plane;
         const int cy = rem / a.nx, cx = rem - cy * a.nx;
-        step_cell_any<Q, T, MODE, COLL>(a, cx, cy, cz, c);
+        step_cell_any<Q, T, MODE, COLL>(a, cx, cy, cz, c, acc);
       }
     }
     return;
@@ -941,7 +1082,7 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
   const unsigned live_lanes = __ballot_sync(FULL, active && !all_solid);
   const unsigned group = (LG >= 32) ? FULL : (((1u << (LG & 31)) - 1u) << (lane & ~(LG - 1)));
   // (the u^ pass writes every wall vector: 12 bytes per cell, and the FD stencil may read any of them)
-  const bool zero_fill = active && all_solid && !special && (mode_uhat(MODE) || ((live_lanes & group) != 0u));
+  const bool zero_fill = !mode_diag(MODE) && active && all_solid && !special && (mode_uhat(MODE) || ((live_lanes & group) != 0u));
   const bool mine = active && !all_solid && !special;       // this thread computes and stores the vector
   const bool doload = active && !all_solid;                 // neighbours may need its lanes' values
   // which cells of the vector are SOLID (bit v)
@@ -951,12 +1092,19 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
   const bool inlet0 = mine && (x0 == 0) && ((clsw & CLS_TYPE) == T_INLET);
   const bool outletN = mine && (qx == nvec - 1) && (((clsw >> (8 * (V - 1))) & CLS_TYPE) == T_OUTLET);
   const bool poutN = mine && (qx == nvec - 1) && (((clsw >> (8 * (V - 1))) & CLS_TYPE) == T_POUTLET);
+  // WALLMODEL cells of the vector (bit v): their u^B comes from the pre-pass (A8); sigma = 0 there in the HRR form (l.131)
+  unsigned wm_bits = 0;
+  if (mode_hlbm(MODE) && a.wm_enable) {
+#pragma unroll
+    for (int v = 0; v < V; ++v) wm_bits |= (((clsw >> (8 * v)) & CLS_TYPE) == T_WM) ? (1u << v) : 0u;
+  }
+  if (!mine) wm_bits = 0;
 
   T f[Q][V];
   T d[V];
 #pragma unroll
   for (int v = 0; v < V; ++v) d[v] = T(0);
-  if (MODE != MODE_STREAM && mine && a.d != nullptr) {
+  if (mode_hlbm(MODE) && mine && a.d != nullptr) {
     T dv[V];
     ld_vec_keep(a.d + self, dv);
 #pragma unroll
@@ -1031,7 +1179,7 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
       }
     }
   }
-  T* pout = mode_uhat(MODE) ? a.uhat + self : a.fout + self;
+  T* pout = mode_uhat(MODE) ? a.uhat + self : a.fout + self;   // (unused by the A9 modes)
   if (zero_fill) {
     T zero[V];
 #pragma unroll
@@ -1107,6 +1255,40 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
 #pragma unroll
     for (int i = 0; i < Q; ++i) f[i][V - 1] = fc[i];
   }
+  if constexpr (mode_diag(MODE)) {                            // A9: raw moments of S_t (l.97, G19)
+    T mr[V], mu[3][V], sr = T(0), sj[3] = {T(0), T(0), T(0)}, se = T(0);
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      T fc[Q];
+#pragma unroll
+      for (int i = 0; i < Q; ++i) fc[i] = f[i][v];
+      T rho, jx, jy, jz;
+      cell_moments<Q, T>(fc, rho, jx, jy, jz);
+      const bool wall = (solid_bits >> v) & 1u;
+      if constexpr (mode_moments(MODE)) {
+        const T ir = rcp_(wall ? T(1) : rho);
+        mr[v] = wall ? T(0) : rho;              // wall cells of a mixed vector: k_solid_moments writes their own values afterwards
+        mu[0][v] = wall ? T(0) : jx * ir;
+        mu[1][v] = wall ? T(0) : jy * ir;
+        mu[2][v] = wall ? T(0) : jz * ir;
+      } else if (!wall) {
+        sr += rho;  sj[0] += jx;  sj[1] += jy;  sj[2] += jz;
+        se += T(0.5) * (jx * jx + jy * jy + jz * jz) * rcp_(rho);
+      }
+    }
+    if constexpr (mode_moments(MODE)) {
+      if (a.mom_rho != nullptr) st_vec(a.mom_rho + self, mr);
+      if (a.mom_u != nullptr) {
+#pragma unroll
+        for (int b = 0; b < 3; ++b) st_vec(a.mom_u + b * N + self, mu[b]);
+      }
+    } else {
+      acc[0] += static_cast<double>(sr);  acc[1] += static_cast<double>(sj[0]);  acc[2] += static_cast<double>(sj[1]);
+      acc[3] += static_cast<double>(sj[2]);  acc[4] += static_cast<double>(se);
+    }
+    return;
+  }
+  if (wm_bits != 0u && a.wm_ub != nullptr && !a.pdl_wait_all) griddep_wait();   // u^B of this level: the pre-pass may still be running
   if constexpr (mode_uhat(MODE)) {                            // first pass of the HRR form: u^(x,t) (Eq. 12), SOLID cells 0
     T uo[3][V];
 #pragma unroll
@@ -1115,7 +1297,11 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
 #pragma unroll
       for (int i = 0; i < Q; ++i) fc[i] = f[i][v];
       T ubx, uby, ubz;
-      body_velocity<T>(a.ub == nullptr ? nullptr : a.ub + (pout - a.uhat) + v, N, d[v], ubx, uby, ubz);
+      if ((wm_bits >> v) & 1u) {
+        ubx = __ldcg(a.wm_ub + self + v);  uby = __ldcg(a.wm_ub + N + self + v);  ubz = __ldcg(a.wm_ub + 2 * N + self + v);
+      } else {
+        body_velocity<T>(a.ub == nullptr ? nullptr : a.ub + self + v, N, d[v], ubx, uby, ubz);
+      }
       uhat_of<Q, T>(fc, d[v], ubx, uby, ubz, uo[0][v], uo[1][v], uo[2][v]);
       if (solid_bits & (1u << v)) {
         const bool mv = ((clsw >> (8 * v)) & CLS_TYPE) == T_MOVING;
@@ -1138,7 +1324,12 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
 #pragma unroll
       for (int i = 0; i < Q; ++i) fc[i] = f[i][v];
       T ubx, uby, ubz;
-      body_velocity<T>(a.ub == nullptr ? nullptr : a.ub + (pout - a.fout) + v, N, d[v], ubx, uby, ubz);
+      const bool wmc = (wm_bits >> v) & 1u;
+      if (wmc) {
+        ubx = __ldcg(a.wm_ub + self + v);  uby = __ldcg(a.wm_ub + N + self + v);  ubz = __ldcg(a.wm_ub + 2 * N + self + v);
+      } else {
+        body_velocity<T>(a.ub == nullptr ? nullptr : a.ub + self + v, N, d[v], ubx, uby, ubz);
+      }
       if constexpr (HRR) {
         T D[3][3];   // D[a][b] = u^_b(x + e_a) - u^_b(x - e_a); G32: the planes beyond INLET / OUTLET copy those planes
 #pragma unroll
@@ -1153,7 +1344,7 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
         }
         const T S[6] = {T(0.5) * D[0][0], T(0.5) * D[1][1], T(0.5) * D[2][2], T(0.25) * (D[0][1] + D[1][0]),
                         T(0.25) * (D[0][2] + D[2][0]), T(0.25) * (D[1][2] + D[2][1])};
-        collide_cell_hrr<Q, T>(fc, d[v], ubx, uby, ubz, tau0_at<T>(a, x0 + v), a.smago_k, a.sigma, S);
+        collide_cell_hrr<Q, T>(fc, d[v], ubx, uby, ubz, tau0_at<T>(a, x0 + v), a.smago_k, wmc ? T(0) : a.sigma, S);   // sigma = 0: l.131
       } else {
         collide_cell<Q, T>(fc, d[v], ubx, uby, ubz, tau0_at<T>(a, x0 + v), a.smago_k);
       }
@@ -1175,6 +1366,15 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
   }
 }
 
+template <int Q, typename T, int MODE, int COLL, bool MW>
+__global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ StepArgs<T> a) {
+  if (a.pdl_wait_all) griddep_wait();      // the preceding kernel wrote this kernel's input (see StepArgs)
+  griddep_launch();
+  double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  step_vec_body<Q, T, MODE, COLL, MW>(a, acc);
+  if constexpr (mode_totals(MODE)) reduce_totals(acc, a.tot_slots, a.tot_nslots, a.tot_ticket, a.tot_out);
+}
+
 // marks the cells that the list blocks of k_step_vec must process: every cell of a 32-byte sector (SV = 8 floats /
 // 4 doubles, aligned) that holds at least one SPECIAL cell.  mark[] feeds a stream compaction.
 template <int SV>
@@ -1190,82 +1390,24 @@ __global__ void __launch_bounds__(256) k_mark_list(const uint8_t* __restrict__ c
   if (m) atomicAdd(counters + 3, static_cast<unsigned long long>(SV));
 }
 
-// ---- A9: moments of S_t -----------------------------------------------------------------------------
-// (the host side materialises S_t first when the storage holds F_{t-1}: plain loads of the cell's own values)
+// ---- A9 runs as modes of the step kernels (MODE_MOMENTS_*, MODE_TOTALS_*): the pull happens in registers, nothing is
+// materialised.  Wall cells report their own (inert) populations, which live in the side buffer side[Q][n_solid]:
 template <int Q, typename T>
-__global__ void __launch_bounds__(256) k_moments(const __grid_constant__ StepArgs<T> a, T* __restrict__ rho_out, T* __restrict__ u_out) {
-  constexpr Stencil<Q> L{};
-  constexpr int H = (Q - 1) / 2;
-  const int x = blockIdx.x * blockDim.x + threadIdx.x;
-  const int y = blockIdx.y * blockDim.y + threadIdx.y;
-  const int z = blockIdx.z;
-  if (x >= a.nx || y >= a.ny) return;
-  const long long self = cell_index(x, y, z, a.nx, a.ny);
+__global__ void __launch_bounds__(256) k_solid_moments(const T* __restrict__ side, const int* __restrict__ solid_list, long long n_solid,
+                                                       long long N, T* __restrict__ rho_out, T* __restrict__ u_out) {
+  const long long k = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (k >= n_solid) return;
   T f[Q];
 #pragma unroll
-  for (int i = 0; i < Q; ++i) f[i] = __ldg(a.fin + i * a.N + self);
-  T rho = f[0], jx = T(0), jy = T(0), jz = T(0);
-#pragma unroll
-  for (int i = 1; i <= H; ++i) {
-    rho += f[i] + f[i + H];
-    const T df = f[i] - f[i + H];
-    jx += T(L.c[i][0]) * df;
-    jy += T(L.c[i][1]) * df;
-    jz += T(L.c[i][2]) * df;
-  }
-  if (rho_out) rho_out[self] = rho;
+  for (int i = 0; i < Q; ++i) f[i] = side[i * n_solid + k];
+  T rho, jx, jy, jz;
+  cell_moments<Q, T>(f, rho, jx, jy, jz);
+  const long long cell = solid_list[k];
+  if (rho_out) rho_out[cell] = rho;
   if (u_out) {
-    u_out[self] = jx / rho;
-    u_out[a.N + self] = jy / rho;
-    u_out[2 * a.N + self] = jz / rho;
-  }
-}
-
-// ---- A9: totals over non-SOLID cells (mass, momentum, kinetic energy), fp64 accumulation --------------
-// warp shuffle tree -> one shared-memory partial per warp -> one atomicAdd(double) per block and quantity
-template <int Q, typename T>
-__global__ void __launch_bounds__(256) k_totals(const __grid_constant__ StepArgs<T> a, double* __restrict__ out /*[5]*/) {
-  constexpr Stencil<Q> L{};
-  const int x = blockIdx.x * blockDim.x + threadIdx.x;
-  const int y = blockIdx.y * blockDim.y + threadIdx.y;
-  const int z = blockIdx.z;
-  double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-  if (x < a.nx && y < a.ny) {
-    const long long self = cell_index(x, y, z, a.nx, a.ny);
-    const uint8_t cls = a.cls[self];
-    if (!is_wall(cls)) {
-      T f[Q];
-#pragma unroll
-      for (int i = 0; i < Q; ++i) f[i] = __ldg(a.fin + i * a.N + self);
-      double rho = 0.0, jx = 0.0, jy = 0.0, jz = 0.0;
-#pragma unroll
-      for (int i = 0; i < Q; ++i) {
-        const double fi = static_cast<double>(f[i]);
-        rho += fi;
-        jx += L.c[i][0] * fi;
-        jy += L.c[i][1] * fi;
-        jz += L.c[i][2] * fi;
-      }
-      v[0] = rho;  v[1] = jx;  v[2] = jy;  v[3] = jz;
-      v[4] = 0.5 * (jx * jx + jy * jy + jz * jz) / rho;
-    }
-  }
-  __shared__ double part[5][8];
-  const int tid = threadIdx.y * blockDim.x + threadIdx.x;
-  const int lane = tid & 31, warp = tid >> 5;
-#pragma unroll
-  for (int k = 0; k < 5; ++k) {
-    double s = v[k];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
-    if (lane == 0) part[k][warp] = s;
-  }
-  __syncthreads();
-  const int nwarps = (blockDim.x * blockDim.y + 31) >> 5;
-  if (tid < 5) {
-    double s = 0.0;
-    for (int w = 0; w < nwarps; ++w) s += part[tid][w];
-    atomicAdd(out + tid, s);
+    u_out[cell] = jx / rho;
+    u_out[N + cell] = jy / rho;
+    u_out[2 * N + cell] = jz / rho;
   }
 }
 
@@ -1401,10 +1543,10 @@ __global__ void __launch_bounds__(VM_CELLS * VM_SLICES) k_vm_inflow(const uint8_
 }
 
 // counters[0] = invalid flag bytes, [1] = wall cells (SOLID + MOVINGWALL), [2] = masked cells (non-wall, not plain bulk FLUID),
-// [4] = MOVINGWALL cells, [5] = SLIPWALL cells ([3] belongs to k_mark_list).
+// [4] = MOVINGWALL cells, [5] = SLIPWALL cells, [6] = WALLMODEL cells ([3] belongs to k_mark_list).
 template <int Q>
 __global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ flags, uint8_t* __restrict__ cls,
-                                                  int nx, int ny, int nz, unsigned long long* __restrict__ counters) {
+                                                  int nx, int ny, int nz, unsigned long long* __restrict__ counters, int wm_special) {
   constexpr Stencil<Q> L{};
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
@@ -1436,11 +1578,13 @@ __global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ fl
   const bool adj = (m != 0u);
   // cells next to a slip wall take the per-cell path: the specular pull (slip_pull) is a call with many operands, which does not
   // belong into the vector kernel's register budget
-  const bool special = (type == T_WM) || (type == T_OUTLET && adj) || slipnb;
+  // (wm_special: WALLMODEL cells solve Spalding's law in the list blocks instead of taking u^B from the pre-pass)
+  const bool special = (type == T_WM && wm_special) || (type == T_OUTLET && adj) || slipnb;
   cls[self] = static_cast<uint8_t>(type | ((type == T_WM ? hi : 0) << CLS_NORMAL_SHIFT) | (adj ? CLS_ADJ : 0) |
                                    (special ? CLS_SPECIAL : 0));
   if (is_wall(type)) atomicAdd(counters + 1, 1ull);
   if (type == T_MOVING) atomicAdd(counters + 4, 1ull);
+  if (type == T_WM) atomicAdd(counters + 6, 1ull);
   if (type == T_SLIP) atomicAdd(counters + 5, 1ull);
   else if (adj || type != T_FLUID) atomicAdd(counters + 2, 1ull);
 }
@@ -1469,9 +1613,30 @@ __global__ void __launch_bounds__(256) k_nbmask(const uint8_t* __restrict__ cls,
 }
 
 // mark[n] = 1 on SOLID cells (feeds the compaction of the SOLID-cell list)
-__global__ void __launch_bounds__(256) k_mark_solid(const uint8_t* __restrict__ cls, uint8_t* __restrict__ mark, long long N) {
+static __global__ void __launch_bounds__(256) k_mark_solid(const uint8_t* __restrict__ cls, uint8_t* __restrict__ mark, long long N) {
   const long long n = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
   if (n < N) mark[n] = is_wall(cls[n]) ? 1 : 0;
+}
+
+// populations of a box of cells out of a lattice that holds S_t: out[Q][bz][by][bx] (lbm_get_populations_box)
+template <typename T>
+__global__ void __launch_bounds__(256) k_gather_box(const T* __restrict__ f, long long N, int nx, int ny, int x0, int y0, int z0,
+                                                    int bx, int by, int bz, int Q, T* __restrict__ out) {
+  const long long n = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  const long long per = static_cast<long long>(bx) * by * bz;
+  if (n >= per * Q) return;
+  const int i = static_cast<int>(n / per);
+  long long r = n - i * per;
+  const int z = static_cast<int>(r / (static_cast<long long>(bx) * by));
+  r -= static_cast<long long>(z) * bx * by;
+  const int y = static_cast<int>(r / bx), x = static_cast<int>(r - static_cast<long long>(y) * bx);
+  out[n] = f[i * N + cell_index(x0 + x, y0 + y, z0 + z, nx, ny)];
+}
+
+// mark[n] = 1 on WALLMODEL cells (feeds the compaction of the pre-pass list)
+static __global__ void __launch_bounds__(256) k_mark_wm(const uint8_t* __restrict__ cls, uint8_t* __restrict__ mark, long long N) {
+  const long long n = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (n < N) mark[n] = ((cls[n] & CLS_TYPE) == T_WM) ? 1 : 0;
 }
 
 // SOLID cells are inert (R5) but the step kernels write zeros over their slots: their own Q values live in a side buffer

@@ -1,0 +1,313 @@
+// =====================================================================================
+// lbm_launch.cuh -- launch side of the step kernels: argument block, grid shapes, the sequence of launches that makes
+// one time step in each collision form.  Included by lbm_inst.cu only (one object file per lattice, dtype and part).
+// =====================================================================================
+#pragma once
+#include "lbm_ctx.h"
+#include "lbm_kernels.cuh"
+
+namespace lbmhost {
+
+struct DiagOut {           // A9 outputs of a MODE_MOMENTS_* launch (device pointers; either may be null)
+  void* rho;
+  void* u;
+};
+
+inline void launch_dims(const lbm_ctx* c, dim3& grid, dim3& block) {
+  int bx = 1;
+  while (bx < c->nx && bx < c->block_threads) bx <<= 1;
+  int by = c->block_threads / bx;
+  int ny2 = 1;
+  while (ny2 < c->ny) ny2 <<= 1;
+  if (by > ny2) by = ny2;
+  if (by < 1) by = 1;
+  if (bx * by < 32) by = 32 / bx;   // whole warps only: the reductions use full-mask shuffles
+  block = dim3(bx, by, 1);
+  grid = dim3((c->nx + bx - 1) / bx, (c->ny + by - 1) / by, c->nz);
+}
+
+// does this step run the wall-model pre-pass (A8)?
+inline bool wm_prepass_active(const lbm_ctx* c, const lbm_params* p) {
+  return p && p->wm_enable && c->wm_prepass && c->n_wm > 0 && c->wm_ub != nullptr;
+}
+
+template <typename T>
+lbm::StepArgs<T> make_args(const lbm_ctx* c, const lbm_params* p, int in, int out) {
+  lbm::StepArgs<T> a;
+  a.fin = static_cast<const T*>(c->f[in]);
+  a.fout = static_cast<T*>(c->f[out]);
+  a.d = (p && p->use_hlbm && c->has_d) ? static_cast<const T*>(c->d) : nullptr;
+  a.ub = (a.d != nullptr && c->ub) ? static_cast<const T*>(c->ub) : nullptr;
+  a.cls = c->cls;
+  a.nbmask = c->nbmask;
+  a.nx = c->nx;  a.ny = c->ny;  a.nz = c->nz;
+  a.N = c->N;
+  a.list = c->list;
+  a.n_list = static_cast<int>(c->n_list);
+  a.list_z = 0;
+  a.z_reverse = 0;
+  a.z0 = 0;
+  a.uhat = static_cast<T*>(c->uhat);
+  a.sigma = p ? static_cast<T>(p->sigma) : T(1);
+  for (int k = 0; k < 3; ++k) a.u_wall[k] = p ? static_cast<T>(p->u_wall[k]) : T(0);
+  a.rho_out = (p && p->rho_out > 0.0) ? static_cast<T>(p->rho_out) : T(1);
+  a.fringe_k = T(0);
+  a.fringe_x0 = c->nx;
+  if (p && p->fringe_len > 0 && p->fringe_factor > 0.0) {
+    a.fringe_k = static_cast<T>((p->tau0 - 0.5) * p->fringe_factor / (static_cast<double>(p->fringe_len) * p->fringe_len));
+    a.fringe_x0 = c->nx - 1 - p->fringe_len;
+  }
+  a.uin_field = c->uin_mean ? c->uin_field[c->uin_cur] : nullptr;
+  if (p) {
+    a.tau0 = static_cast<T>(p->tau0);
+    a.smago_k = static_cast<T>(18.0 * 1.4142135623730951 * p->cs_smago * p->cs_smago);
+    a.u_in[0] = static_cast<T>(p->u_in[0]);  a.u_in[1] = static_cast<T>(p->u_in[1]);  a.u_in[2] = static_cast<T>(p->u_in[2]);
+    a.wm_enable = p->wm_enable;
+    a.wm_kappa = p->wm_kappa;  a.wm_E = p->wm_E;
+    a.nu = (p->tau0 - 0.5) / 3.0;
+  } else {
+    a.tau0 = T(1);  a.smago_k = T(0);
+    a.u_in[0] = a.u_in[1] = a.u_in[2] = T(0);
+    a.wm_enable = 0;  a.wm_kappa = 0.41;  a.wm_E = 9.8;  a.nu = 1.0 / 6.0;
+  }
+  a.wm_ub = wm_prepass_active(c, p) ? static_cast<T*>(c->wm_ub) : nullptr;
+  a.wm_list = c->wm_list;
+  a.n_wm = static_cast<int>(c->n_wm);
+  a.pdl_wait_all = 1;
+  a.mom_rho = nullptr;  a.mom_u = nullptr;
+  a.tot_out = c->totals_dev;
+  a.tot_slots = c->totals_dev + 8;
+  a.tot_ticket = reinterpret_cast<unsigned*>(c->totals_dev + 8 + 5 * LBM_TOT_SLOTS);
+  a.tot_nslots = LBM_TOT_SLOTS;
+  return a;
+}
+
+// vector kernel: thread <-> V consecutive cells; block (bx quads, by rows)
+template <int Q, typename T, int COLL>
+void launch_dims_vec(const lbm_ctx* c, dim3& grid, dim3& block) {
+  const int V = lbm::VecOf<Q, T, COLL>::V;
+  const int nvec = c->nx / V;
+  int bx = 1;
+  while (bx < nvec && bx < 32) bx <<= 1;
+  int by = c->block_threads / bx;
+  int ny2 = 1;
+  while (ny2 < c->ny) ny2 <<= 1;
+  if (by > ny2) by = ny2;
+  if (bx * by < 32) by = 32 / bx;
+  block = dim3(bx, by, 1);
+  grid = dim3((nvec + bx - 1) / bx, (c->ny + by - 1) / by, c->nz);
+}
+
+// kernel launch with (pdl) or without the programmatic-serialization attribute
+template <typename Kern, typename Args>
+cudaError_t launch_k(Kern kern, dim3 grid, dim3 block, cudaStream_t st, bool pdl, const Args& a) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kern, a);
+}
+
+// One launch of a step kernel over the z-slices [z0, z0 + nzs) (+ the list blocks when with_list), lattice `in` -> `out`.
+template <int Q, typename T, int MODE, int COLL>
+int launch_one(lbm_ctx* c, const lbm_params* p, int in, int out, int z0, int nzs, bool with_list, bool may_meet_lid = true,
+               const DiagOut* diag = nullptr) {
+  dim3 grid, block;
+  lbm::StepArgs<T> a = make_args<T>(c, p, in, out);
+  a.z0 = z0;
+  if (diag) {
+    a.mom_rho = static_cast<T*>(diag->rho);
+    a.mom_u = static_cast<T*>(diag->u);
+  }
+  // serpentine sweep (lbm_set_option "serpentine", default 1): BGK steps alternate their direction with the time level; in the
+  // HRR form the u^ pass runs downwards and the step pass upwards; a diagnostic pass runs against the last step
+  if (c->serpentine) a.z_reverse = lbm::mode_uhat(MODE) ? 1 : ((COLL == lbm::COLL_HRR) ? 0 : static_cast<int>(c->sweep_count & 1));
+  // programmatic dependent launch for the kernels of the time loop: resident while the predecessor drains.  After the wall-model
+  // pre-pass (which itself waited for the lattice) only the threads that read its output wait ("pdl" = 2).
+  const bool timeloop = lbm::mode_collides(MODE) || lbm::mode_uhat(MODE);
+  const bool pdl = timeloop && c->use_pdl > 0;
+  a.pdl_wait_all = (pdl && c->use_pdl == 2 && c->prev_launch_prepass) ? 0 : 1;
+  c->prev_launch_prepass = false;
+  const bool vec = c->use_vector && (c->nx % (32 / static_cast<int>(sizeof(T))) == 0);   // whole 32-byte sectors per row
+  cudaError_t e;
+  if (vec) {
+    launch_dims_vec<Q, T, COLL>(c, grid, block);
+    a.list_z = 0;
+    if (with_list) {
+      const long long per_slice = static_cast<long long>(grid.x) * grid.y * block.x * block.y;
+      a.list_z = static_cast<int>((c->n_list + per_slice - 1) / per_slice);
+    }
+    grid.z = nzs + a.list_z;
+    if (grid.z == 0) return LBM_OK;
+    if (grid.z > 65535u || grid.y > 65535u)
+      return fail(c, LBM_EINVAL, "lattice does not fit the launch grid (nz + list slices = %u, rows = %u; both must be <= 65535)", grid.z, grid.y);
+    bool mw = false;
+    if constexpr (lbm::mode_pulls(MODE)) mw = c->n_moving > 0 && may_meet_lid;
+    if constexpr (lbm::mode_pulls(MODE)) {
+      if (mw) e = launch_k(lbm::k_step_vec<Q, T, MODE, COLL, true>, grid, block, c->stream, pdl, a);
+      else    e = launch_k(lbm::k_step_vec<Q, T, MODE, COLL, false>, grid, block, c->stream, pdl, a);
+    } else {
+      e = launch_k(lbm::k_step_vec<Q, T, MODE, COLL, false>, grid, block, c->stream, pdl, a);
+    }
+  } else {
+    if (nzs == 0) return LBM_OK;
+    launch_dims(c, grid, block);
+    grid.z = nzs;
+    e = launch_k(lbm::k_step<Q, T, MODE, COLL>, grid, block, c->stream, pdl, a);
+  }
+  if (e != cudaSuccess) return fail(c, LBM_ECUDA, "kernel launch (mode %d): %s", MODE, cudaGetErrorString(e));
+  LBM_CUDA(c, cudaGetLastError());
+  c->launches++;
+  return LBM_OK;
+}
+
+// A8: u^B of the wall-model cells of this time level (no-op when the step does not use the pre-pass)
+template <int Q, typename T, bool PULL>
+int launch_prepass(lbm_ctx* c, const lbm_params* p, int in, int out) {
+  if (!wm_prepass_active(c, p)) return LBM_OK;
+  lbm::StepArgs<T> a = make_args<T>(c, p, in, out);
+  const unsigned blocks = static_cast<unsigned>((c->n_wm + 127) / 128);
+  cudaError_t e = launch_k(lbm::k_wallmodel_prepass<Q, T, PULL>, dim3(blocks), dim3(128), c->stream, c->use_pdl > 0, a);
+  if (e != cudaSuccess) return fail(c, LBM_ECUDA, "wall-model pre-pass launch: %s", cudaGetErrorString(e));
+  LBM_CUDA(c, cudaGetLastError());
+  c->launches++;
+  c->prev_launch_prepass = true;
+  return LBM_OK;
+}
+
+// HRR form (Eq. 7-11): the FD strain (Eq. 10) needs u^(x,t) of the six neighbours, i.e. their streamed populations, so
+// a step is two passes: UHAT (pull, moments, Eq. 12 -> u^ field) and the fused step that reads it.  With "hrr_slab" the
+// passes are interleaved slab by slab in z, the UHAT pass one slice ahead (measured slower, default off).
+// The list cells go with the first UHAT launch and the last step launch.
+template <int Q, typename T, int MODE_U, int MODE_S>
+int launch_hrr_t(lbm_ctx* c, const lbm_params* p, int in, int out) {
+  const int nz = c->nz;
+  int slab = (c->hrr_slab > 0) ? c->hrr_slab : nz;
+  int rc = launch_prepass<Q, T, lbm::mode_pulls(MODE_U)>(c, p, in, out);
+  if (rc != LBM_OK) return rc;
+  if (slab >= nz - 1) {
+    rc = launch_one<Q, T, MODE_U, lbm::COLL_BGK>(c, p, in, out, 0, nz, true);
+    if (rc != LBM_OK) return rc;
+    return launch_one<Q, T, MODE_S, lbm::COLL_HRR>(c, p, in, out, 0, nz, true);
+  }
+  // UHAT: slice nz-1 first (the periodic neighbour of slice 0), then [0, slab], [slab+1, 2 slab], ... up to nz-2
+  rc = launch_one<Q, T, MODE_U, lbm::COLL_BGK>(c, p, in, out, nz - 1, 1, true);
+  if (rc != LBM_OK) return rc;
+  int udone = 0;                       // slices [0, udone) have their u^
+  for (int z0 = 0; z0 < nz; z0 += slab) {
+    const int zend = (z0 + slab < nz) ? z0 + slab : nz;          // step pass covers [z0, zend)
+    int uneed = (zend + 1 < nz - 1) ? zend + 1 : nz - 1;         // needs u^ on [z0 - 1, zend]; nz-1 is done
+    if (uneed > udone) {
+      rc = launch_one<Q, T, MODE_U, lbm::COLL_BGK>(c, p, in, out, udone, uneed - udone, false);
+      if (rc != LBM_OK) return rc;
+      udone = uneed;
+    }
+    rc = launch_one<Q, T, MODE_S, lbm::COLL_HRR>(c, p, in, out, z0, zend - z0, zend == nz);
+    if (rc != LBM_OK) return rc;
+  }
+  return LBM_OK;
+}
+
+// The timed BGK step.  With a moving lid (MOVINGWALL cells live on the plane z = nz-1 only) the slices that can meet it
+// (z = nz-2, nz-1 and, through the periodic wrap, 0) take the kernel variant that looks the neighbour's class up; the bulk
+// runs the plain variant: three launches instead of one.
+template <int Q, typename T>
+int launch_bgk_pull_t(lbm_ctx* c, const lbm_params* p, int in, int out) {
+  const int nz = c->nz;
+  int rc = launch_prepass<Q, T, true>(c, p, in, out);
+  if (rc != LBM_OK) return rc;
+  if (c->n_moving == 0 || nz < 8)
+    return launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 0, nz, true);
+  rc = launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 1, nz - 3, true, false);
+  if (rc == LBM_OK) rc = launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, nz - 2, 2, false);
+  if (rc == LBM_OK) rc = launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 0, 1, false);
+  return rc;
+}
+
+inline void step_done(lbm_ctx* c) {
+  c->cur = 1 - c->cur;
+  c->sweep_count++;
+}
+
+#if LBM_INST_PART == 0
+template <int Q, typename T>
+int launch_step_bgk(lbm_ctx* c, const lbm_params* p, int mode) {
+  const int in = c->cur, out = 1 - c->cur;
+  int rc;
+  switch (mode) {
+    case lbm::MODE_COLLIDE:
+      rc = launch_prepass<Q, T, false>(c, p, in, out);
+      if (rc == LBM_OK) rc = launch_one<Q, T, lbm::MODE_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 0, c->nz, true);
+      break;
+    case lbm::MODE_STREAM_COLLIDE:
+      rc = launch_bgk_pull_t<Q, T>(c, p, in, out);
+      break;
+    default:
+      rc = launch_one<Q, T, lbm::MODE_STREAM, lbm::COLL_BGK>(c, p, in, out, 0, c->nz, true);
+      break;
+  }
+  if (rc != LBM_OK) return rc;
+  step_done(c);
+  return LBM_OK;
+}
+
+template <int Q, typename T>
+int launch_init(lbm_ctx* c, const void* rho, const void* u) {
+  const int threads = 256;
+  const long long blocks = (c->N + threads - 1) / threads;
+  lbm::k_init_equilibrium<Q, T><<<static_cast<unsigned>(blocks), threads, 0, c->stream>>>(
+      static_cast<const T*>(rho), static_cast<const T*>(u), static_cast<T*>(c->f[0]), c->N);
+  LBM_CUDA(c, cudaGetLastError());
+  c->launches++;
+  return LBM_OK;
+}
+#endif
+
+#if LBM_INST_PART == 1
+template <int Q, typename T>
+int launch_step_hrr(lbm_ctx* c, const lbm_params* p, int mode) {
+  const int in = c->cur, out = 1 - c->cur;
+  int rc = (mode == lbm::MODE_COLLIDE) ? launch_hrr_t<Q, T, lbm::MODE_UHAT_PRE, lbm::MODE_COLLIDE>(c, p, in, out)
+                                       : launch_hrr_t<Q, T, lbm::MODE_UHAT_PULL, lbm::MODE_STREAM_COLLIDE>(c, p, in, out);
+  if (rc != LBM_OK) return rc;
+  step_done(c);
+  return LBM_OK;
+}
+#endif
+
+#if LBM_INST_PART == 2
+// A9: rho, u of S_t for every cell: one launch of the step kernel in its moments mode (the pull happens in registers; the
+// stored lattice and the phase stay as they are) + the wall cells' own values from their side buffer.
+template <int Q, typename T>
+int launch_moments(lbm_ctx* c, const lbm_params* p, void* rho, void* u) {
+  const DiagOut out = {rho, u};
+  int rc = (c->phase == PHASE_POST)
+               ? launch_one<Q, T, lbm::MODE_MOMENTS_PULL, lbm::COLL_BGK>(c, p, c->cur, 1 - c->cur, 0, c->nz, true, true, &out)
+               : launch_one<Q, T, lbm::MODE_MOMENTS_PRE, lbm::COLL_BGK>(c, p, c->cur, 1 - c->cur, 0, c->nz, true, true, &out);
+  if (rc != LBM_OK) return rc;
+  if (c->n_solid_list > 0) {
+    const unsigned blocks = static_cast<unsigned>((c->n_solid_list + 255) / 256);
+    lbm::k_solid_moments<Q, T><<<blocks, 256, 0, c->stream>>>(static_cast<const T*>(c->solid_vals), c->solid_list, c->n_solid_list, c->N,
+                                                              static_cast<T*>(rho), static_cast<T*>(u));
+    LBM_CUDA(c, cudaGetLastError());
+    c->launches++;
+  }
+  return LBM_OK;
+}
+
+// A9: totals over the non-wall cells of S_t -> c->totals_dev[0..4]: one launch (block partials -> slots -> last block)
+template <int Q, typename T>
+int launch_totals(lbm_ctx* c, const lbm_params* p) {
+  return (c->phase == PHASE_POST)
+             ? launch_one<Q, T, lbm::MODE_TOTALS_PULL, lbm::COLL_BGK>(c, p, c->cur, 1 - c->cur, 0, c->nz, true)
+             : launch_one<Q, T, lbm::MODE_TOTALS_PRE, lbm::COLL_BGK>(c, p, c->cur, 1 - c->cur, 0, c->nz, true);
+}
+#endif
+
+}  // namespace lbmhost

@@ -33,6 +33,17 @@ def test_library_exports_every_declared_symbol(lib):
         assert hasattr(lib, name), name
 
 
+def test_every_accepted_option_key_is_documented_in_the_header():
+    """lbm_set_option: the keys the library compares against (lbm_api.cu) are exactly the keys include/lbm.h lists"""
+    api = open(os.path.join(ROOT, "paper_2506_21804_b200", "csrc", "lbm_api.cu")).read()
+    body = api[api.index("int lbm_set_option("):]
+    accepted = sorted(set(re.findall(r'std::strcmp\(key, "([a-z_]+)"\)', body)))
+    header = open(os.path.join(ROOT, "include", "lbm.h")).read()
+    doc = header[header.index("/* Tuning knobs"):header.index("int lbm_set_option(")]
+    documented = sorted(set(re.findall(r'^ \*   "([a-z_]+)"', doc, flags=re.M)))
+    assert accepted == documented and len(accepted) >= 7, (accepted, documented)
+
+
 def test_params_struct_layout_matches_header(tmp_path):
     """the ctypes mirror against the C compiler's view of include/lbm.h (offsetof / sizeof printed by a gcc-built probe)"""
     import subprocess
