@@ -6,8 +6,12 @@
 Workload at N = 1: BASELINE.json config 3 (configs[2]) -- D3Q19 Smagorinsky + HLBM, fp32, 384x192x128
 urban channel -- the configuration the metric "MLUPs ... for D3Q19 Smagorinsky+HLBM" and the
 north_star target are quoted on.  A "step" is one lattice time step = one pass of the whole hot path
- over all cells = one fused kernel launch.  One step moves 1.48 GB, far more
-than the 126 MB L2, so no L2 flush is needed between steps.
+ over all cells = one fused kernel launch (preceded by the wall-model pre-pass over the compact list of
+WALLMODEL cells).  One step moves 1.46 GB, far more than the 126 MB L2, so no L2 flush is needed between steps.
+Protocol: --repeats R (default 3) timed regions of exactly K steps, each from a fresh
+lbm_init_equilibrium + W warm-up steps, CUDA events on the library's stream; the line reports the MEDIAN region
+(all of them are listed in config.repeats_ms_per_step).  lbm_moments / lbm_totals (row A9) are timed separately
+("moments" block) and are not part of MLUPs.
 N > 1: the path does not shard in this build ("replicas only"): every rank runs the same
 workload on its own GPU, no data-path collective; value = sum over ranks / max time.
 --impl reference: the CPU oracle (oracle/), as it stands, timed on the host cores on a bounded sample.
@@ -201,7 +205,7 @@ class ClockSampler(threading.Thread):
                         self.reasons.add(k)
             except Exception:
                 pass
-            time.sleep(0.02)
+            time.sleep(0.005)
 
     def stop(self):
         self._stop_evt.set()
@@ -270,6 +274,8 @@ def main():
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--repeats", type=int, default=3, help="timed regions of K steps each, every one from a fresh state; the median is reported")
+    ap.add_argument("--no-moments", action="store_true", help="skip the separate timing of lbm_moments / lbm_totals (A9)")
     ap.add_argument("--option", action="append", default=[], help="library option key=value (tuning)")
     args = ap.parse_args()
 
@@ -335,29 +341,68 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident timing -------------------------------------------------------------------
-    sim.step(args.warmup, par)
-    barrier()
+    # ---- device-resident timing: R regions of exactly K steps, each from a fresh state + W warm-up steps -----------
     sampler = ClockSampler(local_rank)
     sampler.start()
-    l0 = sim.query("launches")
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    sim.step(args.steps, par)
-    e1.record(stream)
-    barrier()
+    region_ms, launches = [], 0
+    for rep in range(max(args.repeats, 1)):
+        if rep > 0:
+            sim.init_equilibrium(rho_d, u_d)                  # fresh S_0 (also resets the inflow history of the VM inlet)
+        sim.step(args.warmup, par)
+        barrier()
+        l0 = sim.query("launches")
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        sim.step(args.steps, par)
+        e1.record(stream)
+        barrier()
+        launches = sim.query("launches") - l0
+        region_ms.append(max_over_ranks(e0.elapsed_time(e1), world))
     clocks = sampler.stop()
-    launches = sim.query("launches") - l0
-    ms = e0.elapsed_time(e1)
-    ms = max_over_ranks(ms, world)
+    ms = float(np.median(region_ms))
     tot1 = sim.totals()
     finite = bool(np.isfinite(tot1).all())
     value = job_mlups(world, n_fluid, args.steps, ms * 1e-3)
     step_bytes, per_cell = algorithmic_bytes_per_step(cfg, dtype, n_solid)
     peak, peak_src = measured_peak()
-    # BGK form: one launch = one step.  HRR form: a step is several launches (u^ pass + fused step per z-slab); the
-    # figure is then algorithmic bytes per STEP / time per step, i.e. it charges the u^ pass to the step kernel
+    # BGK form: one launch over the lattice = one step.  HRR form: a step is two launches over the lattice (u^ pass + fused step);
+    # the figure is then algorithmic bytes per STEP / time per step, i.e. it charges the u^ pass to the step kernel
     achieved = step_bytes / (ms * 1e-3 / max(args.steps, 1)) / 1e9    # GB/s
+
+    # ---- A9, timed separately (not part of MLUPs): lbm_moments / lbm_totals on the stepped state (post-collision storage:
+    # the pull happens in registers).  Algorithmic bytes: (Q + 4) sizeof(T) N resp. Q sizeof(T) N (+ 1 class byte per cell)
+    moments = None
+    if not args.no_moments:
+        sz = 4 if dtype == "f32" else 8
+        rho_o = torch.empty((nz, ny, nx), dtype=tdt, device="cuda")
+        u_o = torch.empty((3, nz, ny, nx), dtype=tdt, device="cuda")
+
+        def timed(fn, n=7):
+            fn()
+            ts = []
+            for _ in range(n):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                fn()
+                b.record(stream)
+                torch.cuda.synchronize()
+                ts.append(a.elapsed_time(b))
+            return max_over_ranks(float(np.median(ts)), world)
+
+        lm0 = sim.query("launches")
+        t_mom = timed(lambda: sim.moments(rho_o, u_o))
+        lm1 = sim.query("launches")
+        t_tot = timed(lambda: sim.totals())
+        lm2 = sim.query("launches")
+        b_mom = (Q + 4) * sz * n_fluid + N
+        b_tot = Q * sz * n_fluid + N
+        moments = {"lbm_moments": {"ms": t_mom, "algorithmic_bytes": b_mom, "achieved_gbs": b_mom / (t_mom * 1e-3) / 1e9,
+                                   "frac": b_mom / (t_mom * 1e-3) / 1e9 / peak, "launches_per_call": (lm1 - lm0) / 8.0},
+                   "lbm_totals": {"ms": t_tot, "algorithmic_bytes": b_tot, "achieved_gbs": b_tot / (t_tot * 1e-3) / 1e9,
+                                  "frac": b_tot / (t_tot * 1e-3) / 1e9 / peak, "launches_per_call": (lm2 - lm1) / 8.0,
+                                  "note": "includes the 40-byte result copy to the host and its stream synchronisation"},
+                   "what": "median of 7 calls on the stepped state, CUDA events; device outputs rho[N], u[3][N]; not part of MLUPs"}
+        del rho_o, u_o
 
     # ---- end to end through the C ABI with HOST buffers ------------------------------------------
     e2e = None
@@ -398,9 +443,13 @@ def main():
             sample_shape = tuple(max(16, int(round(b * scale / 8)) * 8) for b in base)
             ns = 100   # ~1.5e8 cell updates: about 10 s of host work at the oracle's ~15 MLUPs
         v, dt_cpu, shp = cpu_oracle_time(number, sample_shape, ns, cores, extra, args.workload)
+        ns1 = max(ns // 10, 1)                                 # the same sample on ONE thread, a tenth of the steps
+        v1, dt1, _ = cpu_oracle_time(number, sample_shape, ns1, 1, extra, args.workload)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": "fp64 oracle, %d OpenMP threads, workload generator at (nz,ny,nx)=%s, %d steps after 1 warm-up, %.1f s"
-                         % (cores, str(tuple(shp)), ns, dt_cpu)}
+                         % (cores, str(tuple(shp)), ns, dt_cpu),
+               "single_thread": {"value": v1, "unit": UNIT, "cores": 1,
+                                 "sample": "the same sample, 1 thread, %d steps after 1 warm-up, %.1f s" % (ns1, dt1)}}
 
     if rank == 0:
         line = {
@@ -412,12 +461,15 @@ def main():
                        "l2": "inputs larger than L2 (%.2f GB per step)" % (step_bytes / 1e9),
                        "mlups_all_cells": world * N * args.steps / (ms * 1e-3) / 1e6, "parallelism": "replicas only",
                        "finite": finite, "mass_drift_rel": (tot1[0] - tot0[0]) / tot0[0],
+                       "repeats_ms_per_step": [t / args.steps for t in region_ms],
+                       "protocol": "median of %d timed regions of %d steps, each from a fresh lbm_init_equilibrium + %d warm-up steps" % (len(region_ms), args.steps, args.warmup),
                        "bytes_per_update": per_cell},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": ncu_traffic(args.workload), "peak_source": peak_src, "frac_of_8000_datasheet": achieved / 8000.0,
+                         "traffic": ncu_traffic(args.workload), "traffic_source": "profiles/ncu_traffic.csv (ncu --set full capture of this workload, DRAM read + write bytes per launch)",
+                         "peak_source": peak_src, "frac_of_8000_datasheet": achieved / 8000.0,
                          "algorithmic_bytes_per_launch": step_bytes, "kernel": "lbm::k_step_vec<%d,%s,MODE_STREAM_COLLIDE,%s>" % (Q, "float" if dtype == "f32" else "double", "COLL_HRR" if hrr else "COLL_BGK"),
                          "launches_per_step": launches / max(args.steps, 1)},
-            "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+            "moments": moments, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         }
         print(json.dumps(line), flush=True)
     sim.close()

@@ -196,6 +196,14 @@ int lbm_get_populations(lbm_ctx* ctx, void* populations);
  * Errors: LBM_EINVAL (NULL ctx / buffer, box empty or outside the lattice), LBM_ESTATE, LBM_ENOMEM, LBM_ECUDA. */
 int lbm_get_populations_box(lbm_ctx* ctx, int x0, int y0, int z0, int bx, int by, int bz, void* populations);
 
+/* The inverse of lbm_get_populations_box: replace the populations f_i(x,t) of the state S_t (Eq. 6 l.70-72) on a box of cells;
+ * populations[Q][bz][by][bx] dtype, host or device (copied), box inside the lattice (no wrap).  Everything else of the state is
+ * kept (step counter, geometry, fields).  On a context without a state the call starts one at step 0: the caller then covers the
+ * whole lattice box by box before stepping (cells not covered hold unspecified values) -- the way to set a lattice whose
+ * populations do not fit a third time in memory (896^3 fp32).  Materialises S_t like lbm_get_populations.
+ * Errors: LBM_EINVAL (NULL ctx / buffer, box empty or outside the lattice), LBM_ENOMEM (staging), LBM_ECUDA. */
+int lbm_set_populations_box(lbm_ctx* ctx, int x0, int y0, int z0, int bx, int by, int bz, const void* populations);
+
 /* Totals over the non-wall cells of S_t (the conserved quantities of Eq. 6: mass and momentum, l.97,
  * and the kinetic energy the Taylor-Green check of config 1 is stated in): out[0] = sum rho, out[1..3] = sum rho u,
  * out[4] = sum rho |u|^2 / 2.  `out` is a HOST array of 5 doubles.  One launch, pulling S_t in registers like lbm_moments:

@@ -16,7 +16,7 @@ LBM_F32, LBM_F64 = 4, 8
 EXPORTS = ["lbm_create", "lbm_destroy", "lbm_set_fields", "lbm_init_equilibrium", "lbm_set_geometry", "lbm_step",
            "lbm_moments", "lbm_get_populations", "lbm_totals", "lbm_set_stream", "lbm_synchronize", "lbm_last_error",
            "lbm_query", "lbm_set_option", "lbm_set_inflow", "lbm_set_vortices", "lbm_get_inflow",
-           "lbm_set_porosity", "lbm_set_body_velocity", "lbm_get_populations_box"]
+           "lbm_set_porosity", "lbm_set_body_velocity", "lbm_get_populations_box", "lbm_set_populations_box"]
 
 
 class LbmError(RuntimeError):
@@ -76,6 +76,7 @@ def load_library():
     L.lbm_moments.argtypes = [vp, vp, vp]
     L.lbm_get_populations.argtypes = [vp, vp]
     L.lbm_get_populations_box.argtypes = [vp, ip, ip, ip, ip, ip, ip, vp]
+    L.lbm_set_populations_box.argtypes = [vp, ip, ip, ip, ip, ip, ip, vp]
     L.lbm_totals.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
     L.lbm_set_stream.argtypes = [vp, vp]
     L.lbm_synchronize.argtypes = [vp]
@@ -185,6 +186,13 @@ def lbm_get_populations_box(ctx, origin, extent, populations):
     return _check(ctx, load_library().lbm_get_populations_box(ctx, x0, y0, z0, bx, by, bz, _ptr(populations)))
 
 
+def lbm_set_populations_box(ctx, origin, extent, populations):
+    """origin = (x0, y0, z0), extent = (bx, by, bz); populations[Q][bz][by][bx]"""
+    x0, y0, z0 = (int(v) for v in origin)
+    bx, by, bz = (int(v) for v in extent)
+    return _check(ctx, load_library().lbm_set_populations_box(ctx, x0, y0, z0, bx, by, bz, _ptr(populations)))
+
+
 def lbm_totals(ctx):
     out = (ctypes.c_double * 5)()
     _check(ctx, load_library().lbm_totals(ctx, out))
@@ -271,6 +279,9 @@ class LBM:
 
     def get_populations_box(self, origin, extent, populations):
         return lbm_get_populations_box(self.ctx, origin, extent, populations)
+
+    def set_populations_box(self, origin, extent, populations):
+        return lbm_set_populations_box(self.ctx, origin, extent, populations)
 
     def totals(self):
         return lbm_totals(self.ctx)

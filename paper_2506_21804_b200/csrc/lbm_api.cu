@@ -826,6 +826,42 @@ int lbm_get_populations_box(lbm_ctx* c, int x0, int y0, int z0, int bx, int by, 
   return LBM_OK;
 }
 
+int lbm_set_populations_box(lbm_ctx* c, int x0, int y0, int z0, int bx, int by, int bz, const void* populations) {
+  if (!c) return LBM_EINVAL;
+  if (!populations) return fail(c, LBM_EINVAL, "lbm_set_populations_box: populations is NULL");
+  if (bx < 1 || by < 1 || bz < 1 || x0 < 0 || y0 < 0 || z0 < 0 || x0 + bx > c->nx || y0 + by > c->ny || z0 + bz > c->nz)
+    return fail(c, LBM_EINVAL, "lbm_set_populations_box: box (%d,%d,%d)+(%d,%d,%d) is empty or leaves the lattice", x0, y0, z0, bx, by, bz);
+  const long long n = static_cast<long long>(c->Q) * bx * by * bz;
+  const size_t bytes = static_cast<size_t>(n) * c->dtype;
+  int rc = LBM_OK;
+  if (c->phase == PHASE_NONE) {          // no state yet: this call starts one (the caller covers the lattice box by box)
+    c->cur = 0;
+    c->phase = PHASE_PRE;
+    c->steps = 0;
+    rc = reset_inflow(c);
+  } else {
+    rc = materialise(c);                 // the lattice must hold S_t itself (wall cells' own values included)
+  }
+  if (rc != LBM_OK) return rc;
+  const bool host = !is_device_pointer(populations);
+  const void* src = populations;
+  if (host) {
+    rc = ensure_staging(c, bytes);
+    if (rc != LBM_OK) return rc;
+    LBM_CUDA(c, cudaMemcpyAsync(c->staging, populations, bytes, cudaMemcpyHostToDevice, c->stream));
+    src = c->staging;
+  }
+  const unsigned blocks = static_cast<unsigned>((n + 255) / 256);
+  if (c->dtype == LBM_F32)
+    lbm::k_scatter_box<float><<<blocks, 256, 0, c->stream>>>(static_cast<float*>(c->f[c->cur]), c->N, c->nx, c->ny, x0, y0, z0, bx, by, bz, c->Q, static_cast<const float*>(src));
+  else
+    lbm::k_scatter_box<double><<<blocks, 256, 0, c->stream>>>(static_cast<double*>(c->f[c->cur]), c->N, c->nx, c->ny, x0, y0, z0, bx, by, bz, c->Q, static_cast<const double*>(src));
+  LBM_CUDA(c, cudaGetLastError());
+  c->launches++;
+  if (host) LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  return solid_values(c, true);          // wall cells inside the box: their own values live in the side buffer
+}
+
 int lbm_totals(lbm_ctx* c, double out[5]) {
   if (!c) return LBM_EINVAL;
   if (!out) return fail(c, LBM_EINVAL, "lbm_totals: out is NULL");

@@ -1633,6 +1633,21 @@ __global__ void __launch_bounds__(256) k_gather_box(const T* __restrict__ f, lon
   out[n] = f[i * N + cell_index(x0 + x, y0 + y, z0 + z, nx, ny)];
 }
 
+// the inverse: in[Q][bz][by][bx] -> the box's cells of a lattice that holds S_t (lbm_set_populations_box)
+template <typename T>
+__global__ void __launch_bounds__(256) k_scatter_box(T* __restrict__ f, long long N, int nx, int ny, int x0, int y0, int z0,
+                                                     int bx, int by, int bz, int Q, const T* __restrict__ in) {
+  const long long n = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  const long long per = static_cast<long long>(bx) * by * bz;
+  if (n >= per * Q) return;
+  const int i = static_cast<int>(n / per);
+  long long r = n - i * per;
+  const int z = static_cast<int>(r / (static_cast<long long>(bx) * by));
+  r -= static_cast<long long>(z) * bx * by;
+  const int y = static_cast<int>(r / bx), x = static_cast<int>(r - static_cast<long long>(y) * bx);
+  f[i * N + cell_index(x0 + x, y0 + y, z0 + z, nx, ny)] = in[n];
+}
+
 // mark[n] = 1 on WALLMODEL cells (feeds the compaction of the pre-pass list)
 static __global__ void __launch_bounds__(256) k_mark_wm(const uint8_t* __restrict__ cls, uint8_t* __restrict__ mark, long long N) {
   const long long n = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;

@@ -11,8 +11,11 @@ from parity_util import NP_DTYPE, TOL, field_error, nonsolid, oracle_inputs
 pytestmark = pytest.mark.gpu
 # Eq. 21 divides by the norm of a central difference of the previous inflow: rounding differences between the two sides (exp,
 # FMA contraction, summation order: ~1e-16) are amplified by |u_prev| / |grad u_prev| (1e2 .. 1e4 on these profiles) at every
-# step and fed back.  DESIGN.md (G35) derives 1e-9 for the fp64 path with the VM inlet; fp32 keeps 2e-5 (the inflow is fp64 inside).
-TOL_VM = {"f32": TOL["f32"], "f64": 1e-9}
+# step and fed back (G35).  MEASURED fp64 GPU-vs-oracle errors (B200, round 2): after 10 steps inflow field 7.5e-13
+# (24x32x64, 40 seeds) / 1.0e-11 (40x48x96, 120 seeds), populations 1.4e-13 / 9.5e-13; after 30 steps inflow 1.0e-10 / 8.3e-11,
+# populations 1.2e-11 / 1.1e-11; full-size config 3 + VM windows (10 steps, 256 seeds) 3.0e-11.  The tolerance is < 10x the figure of the case
+# this file runs (24x32x64, 10 steps: 7.5e-13); fp32 keeps 2e-5 (the inflow is fp64 inside: measured 5e-8 / 2e-6).
+TOL_VM = {"f32": TOL["f32"], "f64": 5e-12}
 
 
 def _case(shape=(24, 32, 64), nv=40, sigma_v=3.0, extra=None):
