@@ -56,6 +56,8 @@ enum { LBM_D3Q19 = 19, LBM_D3Q27 = 27 };
 enum { LBM_F32 = 4, LBM_F64 = 8 };
 enum { LBM_FLUID = 0, LBM_SOLID = 1, LBM_INLET = 2, LBM_OUTLET = 3, LBM_WALLMODEL = 4, LBM_MOVINGWALL = 5, LBM_POUTLET = 6, LBM_SLIPWALL = 7 };
 enum { LBM_COLLISION_BGK = 0, LBM_COLLISION_HRR = 1 };
+enum { LBM_HALO_POPULATIONS = 0, LBM_HALO_UHAT = 1 };
+enum { LBM_SIDE_LOW = 0, LBM_SIDE_HIGH = 1 };
 
 typedef struct lbm_ctx lbm_ctx; /* opaque; owned by the library */
 
@@ -212,6 +214,44 @@ int lbm_set_populations_box(lbm_ctx* ctx, int x0, int y0, int z0, int bx, int by
  * Errors: LBM_EINVAL (NULL ctx / out), LBM_ESTATE (no state), LBM_ECUDA. */
 int lbm_totals(lbm_ctx* ctx, double out[5]);
 
+/* ---- Slab decomposition in z: one context per sub-domain (PAPER.md l.214-218 and Table 1 l.227-239: the
+ * paper's scaling runs decompose the lattice over MPI ranks with a halo exchange per step).  The library provides the
+ * sub-domain mechanics; the transfer itself (NCCL send/recv, peer copies, or a device copy between two contexts on one GPU)
+ * is the caller's, on the context's stream.
+ *
+ * lbm_set_halo: declare the first ghost_lo and the last ghost_hi z-slices (0 or 1 each) of this context's lattice GHOST slices:
+ * copies of the neighbouring sub-domain's boundary slices.  Their flags and porosity are set by the caller like any other cell
+ * (copies of the neighbour's), their populations arrive through lbm_halo_unpack; every pass (step, moments, totals, state
+ * getters) then covers the interior slices only, and the entries of the ghost slices in any output are unspecified.
+ * A sub-domain is advanced with lbm_step_halo (lbm_step returns LBM_ESTATE), one time step in two stages:
+ *     stage 0   HRR form: wall-model pre-pass + u^ pass (Eq. 12) over the interior; BGK form: nothing
+ *               -> exchange LBM_HALO_UHAT (HRR form only): the FD strain of Eq. 10 reads u^ of the slices z +- 1
+ *     stage 1   the fused step over the interior (Eq. 6; stream + collide)
+ *               -> exchange LBM_HALO_POPULATIONS: the next step's pull (l.70, A1) reads the ghost slices
+ * No exchange is needed before the first step of a fresh state (it collides S_0 in place).  Per face the exchange moves the
+ * populations that cross the cut, 5 of 19 (D3Q19) or 9 of 27 (D3Q27) per cell, and 3 values of u^ per cell in the HRR form.
+ * Not available with the Vortex Method inlet (it works on the whole inflow plane); a WALLMODEL cell whose sample point x + n lies
+ * in a ghost slice is refused (LBM_EINVAL: move the cut); CUDA graphs and "hrr_slab" are not used.
+ * Errors: LBM_EINVAL (NULL ctx, counts not 0/1, no interior slice left, wall-model cell on a cut), LBM_ESTATE (VM inlet), LBM_ECUDA. */
+int lbm_set_halo(lbm_ctx* ctx, int ghost_lo, int ghost_hi);
+
+/* One stage (0, then 1) of one time step of a sub-domain; see lbm_set_halo.  Also valid without ghost slices (the two stages
+ * together are lbm_step(1) without the CUDA-graph path).  Asynchronous.
+ * Errors: as lbm_step, plus LBM_EINVAL (stage not 0 / 1) and LBM_ESTATE (stages out of order, VM inlet). */
+int lbm_step_halo(lbm_ctx* ctx, const lbm_params* params, int stage);
+
+/* Face buffers of the halo exchange.  what: LBM_HALO_POPULATIONS | LBM_HALO_UHAT; side: LBM_SIDE_LOW (z = 0 end) | LBM_SIDE_HIGH.
+ * lbm_halo_pack copies out of the boundary INTERIOR slice of that side what the neighbour on that side needs:
+ *     populations: [n_cross][ny][nx] dtype, the populations leaving through that face (c_z = -1 on the low side, +1 on the high
+ *                  side) in ascending population order, as stored (post-collision F_t: call it after stage 1);
+ *     u^:          [3][ny][nx] dtype (after stage 0 of an HRR step).
+ * lbm_halo_unpack writes a buffer packed by the neighbour (its pack of the OPPOSITE side) into the GHOST slice of that side.
+ * lbm_query(ctx, 9 | 10) gives the number of values of a populations / u^ face buffer.  Host or device buffers (device buffers
+ * are used in place, asynchronously on the context's stream; host buffers synchronise).
+ * Errors: LBM_EINVAL (NULL, bad what / side), LBM_ESTATE (no ghost slice on that side, no state, no u^ field yet), LBM_ENOMEM, LBM_ECUDA. */
+int lbm_halo_pack(lbm_ctx* ctx, int what, int side, void* buf);
+int lbm_halo_unpack(lbm_ctx* ctx, int what, int side, const void* buf);
+
 /* Use `cuda_stream` (a cudaStream_t passed as void*) for all subsequent work; NULL = the legacy default stream (also the
  * stream of a fresh context).  Synchronises the old stream first.  PyTorch owns streams in this build (north_star: "PyTorch
  * used only for device memory and streams"): pass torch.cuda.current_stream().cuda_stream.  Errors: LBM_EINVAL (NULL ctx),
@@ -231,6 +271,8 @@ const char* lbm_last_error(const lbm_ctx* ctx);
  *   4 device bytes owned by the ctx                    5 cells on the masked (boundary) path
  *   6 cells handled by the list blocks of the vector kernel (SPECIAL cells + their sector mates)
  *   7 CUDA graph launches so far                       8 WALLMODEL cells (length of the pre-pass list)
+ *   9 values of a populations face buffer (halo)        10 values of a u^ face buffer (halo)
+ *   11 interior z-slices (nz minus the ghost slices)
  * Returns -1 for an unknown `what` or a NULL ctx. */
 long long lbm_query(const lbm_ctx* ctx, int what);
 

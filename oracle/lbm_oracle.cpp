@@ -657,7 +657,8 @@ int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const u
     }
 
     // ---- O1b (HRR form): u^(x,t) of every cell, the field the FD strain is taken of (G30) ------
-    // SOLID cells: u^ = 0 (a resting wall).
+    // Wall cells at rest (SOLID, SLIPWALL): u^ = 0 whatever populations they hold (G30; G37: "the FD stencil sees u^ = 0 on
+    // slip wall cells like on any resting wall").
     if (p.collision == 1) {
 #pragma omp parallel for num_threads(nth) if (nth > 1)
       for (int64_t x = 0; x < N; ++x) {
@@ -665,7 +666,7 @@ int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const u
         double uh[3] = {0.0, 0.0, 0.0};
         if (type == MOVINGWALL) {
           for (int a = 0; a < 3; ++a) uh[a] = p.u_wall[a];                 // the wall's own velocity (G33)
-        } else if (type != SOLID) {
+        } else if (!is_wall(type)) {
           double fc[QMAX], rho, u[3];
           for (int i = 0; i < Q; ++i) fc[i] = cur[i * N + x];
           raw_moments(L, fc, rho, u);

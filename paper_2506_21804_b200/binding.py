@@ -13,10 +13,13 @@ _lib = None
 LBM_OK, LBM_EINVAL, LBM_ENOMEM, LBM_ECUDA, LBM_ESTATE = 0, -1, -2, -3, -4
 LBM_D3Q19, LBM_D3Q27 = 19, 27
 LBM_F32, LBM_F64 = 4, 8
+LBM_HALO_POPULATIONS, LBM_HALO_UHAT = 0, 1
+LBM_SIDE_LOW, LBM_SIDE_HIGH = 0, 1
 EXPORTS = ["lbm_create", "lbm_destroy", "lbm_set_fields", "lbm_init_equilibrium", "lbm_set_geometry", "lbm_step",
            "lbm_moments", "lbm_get_populations", "lbm_totals", "lbm_set_stream", "lbm_synchronize", "lbm_last_error",
            "lbm_query", "lbm_set_option", "lbm_set_inflow", "lbm_set_vortices", "lbm_get_inflow",
-           "lbm_set_porosity", "lbm_set_body_velocity", "lbm_get_populations_box", "lbm_set_populations_box"]
+           "lbm_set_porosity", "lbm_set_body_velocity", "lbm_get_populations_box", "lbm_set_populations_box",
+           "lbm_set_halo", "lbm_step_halo", "lbm_halo_pack", "lbm_halo_unpack"]
 
 
 class LbmError(RuntimeError):
@@ -77,6 +80,10 @@ def load_library():
     L.lbm_get_populations.argtypes = [vp, vp]
     L.lbm_get_populations_box.argtypes = [vp, ip, ip, ip, ip, ip, ip, vp]
     L.lbm_set_populations_box.argtypes = [vp, ip, ip, ip, ip, ip, ip, vp]
+    L.lbm_set_halo.argtypes = [vp, ip, ip]
+    L.lbm_step_halo.argtypes = [vp, ctypes.POINTER(LbmParams), ip]
+    L.lbm_halo_pack.argtypes = [vp, ip, ip, vp]
+    L.lbm_halo_unpack.argtypes = [vp, ip, ip, vp]
     L.lbm_totals.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
     L.lbm_set_stream.argtypes = [vp, vp]
     L.lbm_synchronize.argtypes = [vp]
@@ -193,6 +200,22 @@ def lbm_set_populations_box(ctx, origin, extent, populations):
     return _check(ctx, load_library().lbm_set_populations_box(ctx, x0, y0, z0, bx, by, bz, _ptr(populations)))
 
 
+def lbm_set_halo(ctx, ghost_lo, ghost_hi):
+    return _check(ctx, load_library().lbm_set_halo(ctx, int(ghost_lo), int(ghost_hi)))
+
+
+def lbm_step_halo(ctx, params, stage):
+    return _check(ctx, load_library().lbm_step_halo(ctx, ctypes.byref(params), int(stage)))
+
+
+def lbm_halo_pack(ctx, what, side, buf):
+    return _check(ctx, load_library().lbm_halo_pack(ctx, int(what), int(side), _ptr(buf)))
+
+
+def lbm_halo_unpack(ctx, what, side, buf):
+    return _check(ctx, load_library().lbm_halo_unpack(ctx, int(what), int(side), _ptr(buf)))
+
+
 def lbm_totals(ctx):
     out = (ctypes.c_double * 5)()
     _check(ctx, load_library().lbm_totals(ctx, out))
@@ -218,7 +241,7 @@ def lbm_set_option(ctx, key, value):
 class LBM:
     """Convenience owner of one lbm_ctx (still marshalling only)."""
     QUERY = dict(steps=0, launches=1, cells=2, solid_cells=3, device_bytes=4, masked_cells=5, list_cells=6, graph_launches=7,
-                 wallmodel_cells=8)
+                 wallmodel_cells=8, halo_population_values=9, halo_uhat_values=10, interior_slices=11)
 
     def __init__(self, lattice, nx, ny, nz, dtype="f32", stream=None):
         self.Q, self.nx, self.ny, self.nz = lattice, nx, ny, nz
@@ -282,6 +305,18 @@ class LBM:
 
     def set_populations_box(self, origin, extent, populations):
         return lbm_set_populations_box(self.ctx, origin, extent, populations)
+
+    def set_halo(self, ghost_lo, ghost_hi):
+        return lbm_set_halo(self.ctx, ghost_lo, ghost_hi)
+
+    def step_halo(self, params, stage):
+        return lbm_step_halo(self.ctx, params, stage)
+
+    def halo_pack(self, what, side, buf):
+        return lbm_halo_pack(self.ctx, what, side, buf)
+
+    def halo_unpack(self, what, side, buf):
+        return lbm_halo_unpack(self.ctx, what, side, buf)
 
     def totals(self):
         return lbm_totals(self.ctx)

@@ -88,9 +88,11 @@ void launch_dims(const lbm_ctx* c, dim3& grid, dim3& block) {
   ((c)->Q == 19 ? ((c)->dtype == LBM_F32 ? lbmhost::fn<19, float>(__VA_ARGS__) : lbmhost::fn<19, double>(__VA_ARGS__))          \
                 : ((c)->dtype == LBM_F32 ? lbmhost::fn<27, float>(__VA_ARGS__) : lbmhost::fn<27, double>(__VA_ARGS__)))
 
-int launch_step(lbm_ctx* c, const lbm_params* p, int mode) {
+// stage: -1 = the whole step; 0 / 1 = the two stages of a step on a sub-domain (lbm_step_halo; the BGK form has no stage 0)
+int launch_step(lbm_ctx* c, const lbm_params* p, int mode, int stage = -1) {
   const bool hrr = p && p->collision == LBM_COLLISION_HRR && mode != lbm::MODE_STREAM;
-  if (hrr) return LBM_DISPATCH(c, launch_step_hrr, c, p, mode);
+  if (hrr) return LBM_DISPATCH(c, launch_step_hrr, c, p, mode, stage);
+  if (stage == 0) return LBM_OK;
   return LBM_DISPATCH(c, launch_step_bgk, c, p, mode);
 }
 
@@ -408,7 +410,7 @@ void lbm_destroy(lbm_ctx* c) {
   cudaFree(c->counters);  cudaFree(c->totals_dev);  cudaFree(c->staging);
   cudaFree(c->list);  cudaFree(c->cub_tmp);  cudaFree(c->list_count_dev);
   cudaFree(c->nbmask);  cudaFree(c->solid_list);  cudaFree(c->solid_vals);
-  cudaFree(c->wm_list);  cudaFree(c->wm_ub);  cudaFree(c->uin_scratch);
+  cudaFree(c->wm_list);  cudaFree(c->wm_ub);  cudaFree(c->uin_scratch);  cudaFree(c->halo_buf);
   for (int k = 0; k < LBM_GRAPH_CACHE; ++k)
     if (c->graphs[k].valid) cudaGraphExecDestroy(c->graphs[k].exec);
   if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
@@ -550,6 +552,8 @@ int lbm_set_inflow(lbm_ctx* c, const void* u_mean) {
   if (!c) return LBM_EINVAL;
   const long long n = 3ll * c->ny * c->nz;
   const size_t bytes = static_cast<size_t>(n) * sizeof(double);       // kept in fp64 whatever the dtype
+  if (u_mean && (c->ghost_lo || c->ghost_hi))
+    return fail(c, LBM_ESTATE, "lbm_set_inflow: the Vortex Method inlet works on the whole inflow plane; not available on a sub-domain (lbm_set_halo)");
   // the state S_t keeps the inflow it was formed with
   int rc = materialise(c);
   if (rc != LBM_OK) return rc;
@@ -709,13 +713,9 @@ static int graph_chunk(lbm_ctx* c, const lbm_params* params, bool* done) {
   return LBM_OK;
 }
 
-int lbm_step(lbm_ctx* c, int n_steps, const lbm_params* params) {
-  if (!c) return LBM_EINVAL;
-  int rc = check_params(c, params);
-  if (rc != LBM_OK) return rc;
-  if (n_steps < 0) return fail(c, LBM_EINVAL, "lbm_step: n_steps = %d must be >= 0", n_steps);
-  if (c->phase == PHASE_NONE) return fail(c, LBM_ESTATE, "lbm_step: no state; call lbm_set_fields or lbm_init_equilibrium first");
-  c->last = *params;
+// buffers a step needs beyond the lattices: u^ field (HRR form), u^B of the wall-model cells (pre-pass)
+static int step_buffers(lbm_ctx* c, const lbm_params* params, int n_steps) {
+  int rc = LBM_OK;
   if (params->collision == LBM_COLLISION_HRR && !c->uhat && n_steps > 0) {
     const size_t bytes = 3 * static_cast<size_t>(c->N) * c->dtype;
     rc = dev_alloc(c, &c->uhat, bytes);
@@ -730,6 +730,20 @@ int lbm_step(lbm_ctx* c, int n_steps, const lbm_params* params) {
     if (rc != LBM_OK) return rc;
     c->epoch++;
   }
+  return LBM_OK;
+}
+
+int lbm_step(lbm_ctx* c, int n_steps, const lbm_params* params) {
+  if (!c) return LBM_EINVAL;
+  int rc = check_params(c, params);
+  if (rc != LBM_OK) return rc;
+  if (n_steps < 0) return fail(c, LBM_EINVAL, "lbm_step: n_steps = %d must be >= 0", n_steps);
+  if (c->phase == PHASE_NONE) return fail(c, LBM_ESTATE, "lbm_step: no state; call lbm_set_fields or lbm_init_equilibrium first");
+  if (c->ghost_lo + c->ghost_hi > 0)
+    return fail(c, LBM_ESTATE, "lbm_step: the context is a sub-domain with ghost slices (lbm_set_halo): advance it with lbm_step_halo and exchange the halos");
+  c->last = *params;
+  rc = step_buffers(c, params, n_steps);
+  if (rc != LBM_OK) return rc;
   int s = 0;
   while (s < n_steps) {
     if (c->phase == PHASE_PRE) {
@@ -876,6 +890,150 @@ int lbm_totals(lbm_ctx* c, double out[5]) {
   return LBM_OK;
 }
 
+// ---- slab decomposition in z: ghost slices, staged step, halo pack / unpack ------
+// wall-model cells whose sample point lies in a ghost slice cannot be served (their pre-pass would pull from beyond the halo)
+static int check_wm_cut(lbm_ctx* c, int ghost_lo, int ghost_hi) {
+  c->halo_wm_epoch = c->epoch;
+  if (!(ghost_lo || ghost_hi) || c->n_wm <= 0) return LBM_OK;
+  LBM_CUDA(c, cudaMemsetAsync(c->counters, 0, sizeof(unsigned long long), c->stream));
+  const long long plane = static_cast<long long>(c->nx) * c->ny;
+  lbm::k_count_wm_on_cut<<<static_cast<unsigned>((plane + 255) / 256), 256, 0, c->stream>>>(c->cls, plane, c->nz, ghost_lo, ghost_hi, c->counters);
+  LBM_CUDA(c, cudaGetLastError());
+  c->launches++;
+  unsigned long long bad = 0;
+  LBM_CUDA(c, cudaMemcpyAsync(&bad, c->counters, sizeof(bad), cudaMemcpyDeviceToHost, c->stream));
+  LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  if (bad) {
+    c->halo_wm_epoch = -1;
+    return fail(c, LBM_EINVAL, "halo: %llu WALLMODEL cell(s) sample their velocity in a ghost slice (wall normal across the cut): move the cut", bad);
+  }
+  return LBM_OK;
+}
+
+int lbm_set_halo(lbm_ctx* c, int ghost_lo, int ghost_hi) {
+  if (!c) return LBM_EINVAL;
+  if ((ghost_lo != 0 && ghost_lo != 1) || (ghost_hi != 0 && ghost_hi != 1))
+    return fail(c, LBM_EINVAL, "lbm_set_halo: ghost_lo = %d, ghost_hi = %d must be 0 or 1", ghost_lo, ghost_hi);
+  if (c->nz - ghost_lo - ghost_hi < 1) return fail(c, LBM_EINVAL, "lbm_set_halo: no interior slice left (nz = %d)", c->nz);
+  if ((ghost_lo || ghost_hi) && c->uin_mean)
+    return fail(c, LBM_ESTATE, "lbm_set_halo: the Vortex Method inlet works on the whole inflow plane; not available on a sub-domain");
+  { int rcw = check_wm_cut(c, ghost_lo, ghost_hi); if (rcw != LBM_OK) return rcw; }
+  int rc = materialise(c);               // a pass over the old interior; the ghost slices start without valid contents
+  if (rc != LBM_OK) return rc;
+  c->ghost_lo = ghost_lo;
+  c->ghost_hi = ghost_hi;
+  c->halo_stage = 0;
+  c->epoch++;
+  c->halo_wm_epoch = c->epoch;
+  return LBM_OK;
+}
+
+int lbm_step_halo(lbm_ctx* c, const lbm_params* params, int stage) {
+  if (!c) return LBM_EINVAL;
+  int rc = check_params(c, params);
+  if (rc != LBM_OK) return rc;
+  if (stage != 0 && stage != 1) return fail(c, LBM_EINVAL, "lbm_step_halo: stage = %d must be 0 or 1", stage);
+  if (c->phase == PHASE_NONE) return fail(c, LBM_ESTATE, "lbm_step_halo: no state");
+  if (c->uin_mean) return fail(c, LBM_ESTATE, "lbm_step_halo: not available with the Vortex Method inlet");
+  if (stage != c->halo_stage) return fail(c, LBM_ESTATE, "lbm_step_halo: stage %d called where stage %d is due", stage, c->halo_stage);
+  if (params->wm_enable && c->halo_wm_epoch != c->epoch) {       // the geometry changed since the cut was checked
+    rc = check_wm_cut(c, c->ghost_lo, c->ghost_hi);
+    if (rc != LBM_OK) return rc;
+  }
+  c->last = *params;
+  rc = step_buffers(c, params, 1);
+  if (rc != LBM_OK) return rc;
+  const int mode = (c->phase == PHASE_PRE) ? lbm::MODE_COLLIDE : lbm::MODE_STREAM_COLLIDE;
+  rc = launch_step(c, params, mode, stage);
+  if (rc != LBM_OK) return rc;
+  if (stage == 0) {
+    c->halo_stage = 1;
+  } else {
+    c->halo_stage = 0;
+    c->phase = PHASE_POST;
+    c->steps += 1;
+  }
+  return LBM_OK;
+}
+
+// planes of one face buffer and the slice they live in
+static int halo_planes(lbm_ctx* c, const char* who, int what, int side, bool pack, lbm::HaloPlanes* hp, int* z, void** field) {
+  if (what != LBM_HALO_POPULATIONS && what != LBM_HALO_UHAT) return fail(c, LBM_EINVAL, "%s: what = %d must be 0 (populations) or 1 (u^)", who, what);
+  if (side != LBM_SIDE_LOW && side != LBM_SIDE_HIGH) return fail(c, LBM_EINVAL, "%s: side = %d must be 0 (low) or 1 (high)", who, side);
+  if ((side == LBM_SIDE_LOW && !c->ghost_lo) || (side == LBM_SIDE_HIGH && !c->ghost_hi))
+    return fail(c, LBM_ESTATE, "%s: no ghost slice on side %d (lbm_set_halo)", who, side);
+  if (c->phase == PHASE_NONE) return fail(c, LBM_ESTATE, "%s: no state", who);
+  // pack reads the boundary INTERIOR slice, unpack writes the GHOST slice
+  if (side == LBM_SIDE_LOW) *z = pack ? c->ghost_lo : 0;
+  else *z = pack ? c->nz - 1 - c->ghost_hi : c->nz - 1;
+  if (what == LBM_HALO_UHAT) {
+    if (!c->uhat) return fail(c, LBM_ESTATE, "%s: no u^ field (the HRR form has not run yet)", who);
+    hp->n = 3;
+    hp->idx[0] = 0;  hp->idx[1] = 1;  hp->idx[2] = 2;
+    *field = c->uhat;
+    return LBM_OK;
+  }
+  // the populations that cross the cut: leaving downwards (c_z = -1) from the low boundary slice, upwards from the high one;
+  // the ghost slice on the low side receives what travels upwards (c_z = +1), the one on the high side c_z = -1
+  const int want = ((side == LBM_SIDE_LOW) == pack) ? -1 : +1;
+  hp->n = 0;
+  if (c->Q == 19) {
+    constexpr lbm::Stencil<19> L{};
+    for (int i = 0; i < 19; ++i) if (L.c[i][2] == want) hp->idx[hp->n++] = i;
+  } else {
+    constexpr lbm::Stencil<27> L{};
+    for (int i = 0; i < 27; ++i) if (L.c[i][2] == want) hp->idx[hp->n++] = i;
+  }
+  *field = c->f[c->cur];
+  return LBM_OK;
+}
+
+static int halo_copy(lbm_ctx* c, const char* who, int what, int side, void* buf, bool pack) {
+  if (!c) return LBM_EINVAL;
+  if (!buf) return fail(c, LBM_EINVAL, "%s: buffer is NULL", who);
+  lbm::HaloPlanes hp;
+  int z = 0;
+  void* field = nullptr;
+  int rc = halo_planes(c, who, what, side, pack, &hp, &z, &field);
+  if (rc != LBM_OK) return rc;
+  const long long plane = static_cast<long long>(c->nx) * c->ny;
+  const size_t bytes = static_cast<size_t>(hp.n) * plane * c->dtype;
+  const bool host = !is_device_pointer(buf);
+  void* dbuf = buf;
+  if (host) {
+    if (c->halo_buf_bytes < bytes) {
+      if (c->halo_buf) { cudaStreamSynchronize(c->stream); cudaFree(c->halo_buf); c->device_bytes -= c->halo_buf_bytes; c->halo_buf = nullptr; c->halo_buf_bytes = 0; }
+      rc = dev_alloc(c, &c->halo_buf, bytes);
+      if (rc != LBM_OK) return rc;
+      c->halo_buf_bytes = bytes;
+    }
+    dbuf = c->halo_buf;
+    if (!pack) LBM_CUDA(c, cudaMemcpyAsync(dbuf, buf, bytes, cudaMemcpyHostToDevice, c->stream));
+  }
+  unsigned blocks = static_cast<unsigned>((plane + 255) / 256);
+  if (blocks > 148u * 8u) blocks = 148u * 8u;
+  const long long off = static_cast<long long>(z) * plane;
+  if (c->dtype == LBM_F32) {
+    if (pack) lbm::k_halo_planes<float, true><<<blocks, 256, 0, c->stream>>>(static_cast<float*>(field), c->N, off, plane, hp, static_cast<float*>(dbuf));
+    else      lbm::k_halo_planes<float, false><<<blocks, 256, 0, c->stream>>>(static_cast<float*>(field), c->N, off, plane, hp, static_cast<float*>(dbuf));
+  } else {
+    if (pack) lbm::k_halo_planes<double, true><<<blocks, 256, 0, c->stream>>>(static_cast<double*>(field), c->N, off, plane, hp, static_cast<double*>(dbuf));
+    else      lbm::k_halo_planes<double, false><<<blocks, 256, 0, c->stream>>>(static_cast<double*>(field), c->N, off, plane, hp, static_cast<double*>(dbuf));
+  }
+  LBM_CUDA(c, cudaGetLastError());
+  c->launches++;
+  if (host) {
+    if (pack) LBM_CUDA(c, cudaMemcpyAsync(buf, dbuf, bytes, cudaMemcpyDeviceToHost, c->stream));
+    LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  }
+  return LBM_OK;
+}
+
+int lbm_halo_pack(lbm_ctx* c, int what, int side, void* buf) { return halo_copy(c, "lbm_halo_pack", what, side, buf, true); }
+int lbm_halo_unpack(lbm_ctx* c, int what, int side, const void* buf) {
+  return halo_copy(c, "lbm_halo_unpack", what, side, const_cast<void*>(buf), false);
+}
+
 long long lbm_query(const lbm_ctx* c, int what) {
   if (!c) return -1;
   switch (what) {
@@ -888,6 +1046,9 @@ long long lbm_query(const lbm_ctx* c, int what) {
     case 6: return c->n_list;
     case 7: return c->graph_launches;
     case 8: return c->n_wm;
+    case 9: return static_cast<long long>(c->Q == 19 ? 5 : 9) * c->nx * c->ny;
+    case 10: return 3ll * c->nx * c->ny;
+    case 11: return c->nz - c->ghost_lo - c->ghost_hi;
     default: return -1;
   }
 }

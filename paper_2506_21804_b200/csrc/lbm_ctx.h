@@ -90,11 +90,22 @@ struct lbm_ctx {
   int use_pdl;           // programmatic dependent launch of the time-loop kernels: 0 off, 1 every thread waits for the predecessor,
                          // 2 (default) after the wall-model pre-pass only the threads that read its output wait
   bool prev_launch_prepass;   // the last kernel enqueued on the stream was the wall-model pre-pass
+  // slab decomposition in z (lbm_set_halo): the first ghost_lo / last ghost_hi slices (0 or 1 each) are ghost slices that hold
+  // copies of the neighbouring sub-domain's boundary slices (lbm_halo_unpack); every pass covers the interior slices only
+  int ghost_lo, ghost_hi;
+  long long halo_wm_epoch;   // epoch at which the wall-model cells were last checked against the cuts
+  int halo_stage;        // lbm_step_halo: 0 = a step may begin, 1 = stage 0 of the current step is done
+  void* halo_buf;        // device staging of lbm_halo_pack / lbm_halo_unpack for host buffers
+  size_t halo_buf_bytes;
   lbm_params last;       // parameters of the last lbm_step: the inlet rule is part of how S_t is formed from F_{t-1}
   char err[512];
 };
 
 namespace lbmhost {
+
+// interior slices [zlo, zlo + zcount) of the local lattice (all of it without ghost slices)
+inline int zlo(const lbm_ctx* c) { return c->ghost_lo; }
+inline int zcount(const lbm_ctx* c) { return c->nz - c->ghost_lo - c->ghost_hi; }
 
 int fail(lbm_ctx* c, int code, const char* fmt, ...);
 
@@ -106,7 +117,7 @@ int fail(lbm_ctx* c, int code, const char* fmt, ...);
 
 // one time step (or one materialising pass) in the BGK / HRR form; `mode` is a lbm:: MODE_* value
 template <int Q, typename T> int launch_step_bgk(lbm_ctx* c, const lbm_params* p, int mode);
-template <int Q, typename T> int launch_step_hrr(lbm_ctx* c, const lbm_params* p, int mode);
+template <int Q, typename T> int launch_step_hrr(lbm_ctx* c, const lbm_params* p, int mode, int stage);
 // A9: rho, u of S_t into caller buffers (device pointers); totals into c->totals_dev[0..4]
 template <int Q, typename T> int launch_moments(lbm_ctx* c, const lbm_params* p, void* rho, void* u);
 template <int Q, typename T> int launch_totals(lbm_ctx* c, const lbm_params* p);

@@ -11,7 +11,7 @@ namespace lbmhost {
 template int launch_step_bgk<LBM_INST_Q, LBM_INST_T>(lbm_ctx*, const lbm_params*, int);
 template int launch_init<LBM_INST_Q, LBM_INST_T>(lbm_ctx*, const void*, const void*);
 #elif LBM_INST_PART == 1
-template int launch_step_hrr<LBM_INST_Q, LBM_INST_T>(lbm_ctx*, const lbm_params*, int);
+template int launch_step_hrr<LBM_INST_Q, LBM_INST_T>(lbm_ctx*, const lbm_params*, int, int);
 #elif LBM_INST_PART == 2
 template int launch_moments<LBM_INST_Q, LBM_INST_T>(lbm_ctx*, const lbm_params*, void*, void*);
 template int launch_totals<LBM_INST_Q, LBM_INST_T>(lbm_ctx*, const lbm_params*);

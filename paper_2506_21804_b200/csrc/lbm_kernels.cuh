@@ -123,7 +123,8 @@ struct StepArgs {
   int n_list;
   int list_z;
   int z_reverse;                  // vector kernel: walk the slab from its last slice down (serpentine sweep over consecutive launches)
-  int z0;                         // first lattice z-slice of this launch (the grid covers a slab z0 .. z0 + gridDim.z - list_z - 1)
+  int z0;                         // first lattice z-slice of this launch (the launch covers the slab z0 .. z0 + nzs - 1)
+  int nzs;                        // z-slices of this launch (grid.z = list_z + nzs, except in the totals modes, whose blocks loop over z)
   // HRR form (Eq. 7-11): u^(x,t) of every cell [3][N] (written by the MODE_UHAT_* pass, SOLID cells 0), Eq. 7 factor
   T* __restrict__ uhat;
   T sigma;
@@ -1026,7 +1027,7 @@ __device__ __forceinline__ void ld_uhat_nb(const T* pu, long long N, int dyp, in
 // Everything else -- bulk, solid-adjacent (read-side bounce-back), INLET and OUTLET cells -- runs in the vector path.
 // MW: the launch may meet MOVINGWALL cells (compiled out otherwise: the test costs the wall-adjacent warps registers).
 template <int Q, typename T, int MODE, int COLL, bool MW>
-__device__ __forceinline__ void step_vec_body(const StepArgs<T>& a, double (&acc)[5]) {
+__device__ __forceinline__ void step_vec_body(const StepArgs<T>& a, double (&acc)[5], const int bz) {   // bz: the block's z index in the (virtual) grid
   constexpr Stencil<Q> L{};
   constexpr int V = VecOf<Q, T, COLL>::V;
   constexpr bool HRR = (COLL == COLL_HRR) && mode_collides(MODE);
@@ -1035,8 +1036,8 @@ __device__ __forceinline__ void step_vec_body(const StepArgs<T>& a, double (&acc
   constexpr unsigned FULL = 0xffffffffu;
   constexpr bool PULL = mode_pulls(MODE);
   const int tx = threadIdx.x;
-  if (static_cast<int>(blockIdx.z) < a.list_z) {
-    const long long blk = (static_cast<long long>(blockIdx.z) * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+  if (bz < a.list_z) {
+    const long long blk = (static_cast<long long>(bz) * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
     const long long k = blk * (blockDim.x * blockDim.y) + threadIdx.y * blockDim.x + tx;
     if (k < a.n_list) {
       const int cell = a.list[k];
@@ -1058,8 +1059,8 @@ __device__ __forceinline__ void step_vec_body(const StepArgs<T>& a, double (&acc
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
   // serpentine sweep: a launch that runs against the direction of the previous one starts on the slices that launch wrote (or read)
   // last, which are still in the 126 MB L2
-  const int kz = static_cast<int>(blockIdx.z) - a.list_z;
-  const int z = a.z0 + (a.z_reverse ? (static_cast<int>(gridDim.z) - a.list_z - 1 - kz) : kz);
+  const int kz = bz - a.list_z;
+  const int z = a.z0 + (a.z_reverse ? (a.nzs - 1 - kz) : kz);
   const bool active = (qx < nvec) && (y < a.ny);
   const int x0 = qx * V;
   const int nx = a.nx, ny = a.ny, nz = a.nz;
@@ -1371,8 +1372,14 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
   if (a.pdl_wait_all) griddep_wait();      // the preceding kernel wrote this kernel's input (see StepArgs)
   griddep_launch();
   double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-  step_vec_body<Q, T, MODE, COLL, MW>(a, acc);
-  if constexpr (mode_totals(MODE)) reduce_totals(acc, a.tot_slots, a.tot_nslots, a.tot_ticket, a.tot_out);
+  if constexpr (mode_totals(MODE)) {
+    // the blocks walk the z-slices with stride gridDim.z, so that one block-level reduction (shuffle trees, atomics, ticket)
+    // serves many vectors per thread
+    for (int bz = blockIdx.z; bz < a.list_z + a.nzs; bz += gridDim.z) step_vec_body<Q, T, MODE, COLL, MW>(a, acc, bz);
+    reduce_totals(acc, a.tot_slots, a.tot_nslots, a.tot_ticket, a.tot_out);
+  } else {
+    step_vec_body<Q, T, MODE, COLL, MW>(a, acc, static_cast<int>(blockIdx.z));
+  }
 }
 
 // marks the cells that the list blocks of k_step_vec must process: every cell of a 32-byte sector (SV = 8 floats /
@@ -1646,6 +1653,46 @@ __global__ void __launch_bounds__(256) k_scatter_box(T* __restrict__ f, long lon
   r -= static_cast<long long>(z) * bx * by;
   const int y = static_cast<int>(r / bx), x = static_cast<int>(r - static_cast<long long>(y) * bx);
   f[i * N + cell_index(x0 + x, y0 + y, z0 + z, nx, ny)] = in[n];
+}
+
+// ---- halo exchange of a slab decomposition in z ----------------------------------------
+// A face buffer holds n_planes planes of nx*ny values: the populations that cross the cut (c_z = -1 towards the lower, c_z = +1
+// towards the upper neighbour: 5 of 19, 9 of 27) of one boundary slice, or the three components of u^ of that slice (HRR form).
+// In the SoA layout every such plane is contiguous: base + idx[k] * N + z * plane.  PACK: lattice -> buffer, else buffer -> lattice.
+struct HaloPlanes {
+  int n;
+  int idx[9];          // population (or component) index of plane k
+};
+template <typename T, bool PACK>
+__global__ void __launch_bounds__(256) k_halo_planes(T* __restrict__ field, long long N, long long slice_off, long long plane,
+                                                     HaloPlanes hp, T* __restrict__ buf) {
+  const long long stride = static_cast<long long>(gridDim.x) * blockDim.x;
+  for (int k = 0; k < hp.n; ++k) {
+    T* __restrict__ row = field + hp.idx[k] * N + slice_off;
+    T* __restrict__ b = buf + k * plane;
+    for (long long n = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; n < plane; n += stride) {
+      if (PACK) b[n] = row[n];
+      else row[n] = b[n];
+    }
+  }
+}
+
+// wall-model cells whose sample point x + n lies in a ghost slice (their pre-pass would pull from beyond the halo): counted
+// when a halo is set, the decomposition is refused if there are any
+static __global__ void __launch_bounds__(256) k_count_wm_on_cut(const uint8_t* __restrict__ cls, long long plane, int nz, int ghost_lo,
+                                                                int ghost_hi, unsigned long long* __restrict__ count) {
+  const long long n = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (n >= plane) return;
+  unsigned bad = 0;
+  if (ghost_lo) {                       // first interior slice, normal -z (code 5)
+    const uint8_t c = cls[static_cast<long long>(ghost_lo) * plane + n];
+    if ((c & CLS_TYPE) == T_WM && ((c >> CLS_NORMAL_SHIFT) & 7) == 5) ++bad;
+  }
+  if (ghost_hi) {                       // last interior slice, normal +z (code 4)
+    const uint8_t c = cls[static_cast<long long>(nz - 1 - ghost_hi) * plane + n];
+    if ((c & CLS_TYPE) == T_WM && ((c >> CLS_NORMAL_SHIFT) & 7) == 4) ++bad;
+  }
+  if (bad) atomicAdd(count, static_cast<unsigned long long>(bad));
 }
 
 // mark[n] = 1 on WALLMODEL cells (feeds the compaction of the pre-pass list)

@@ -47,6 +47,7 @@ lbm::StepArgs<T> make_args(const lbm_ctx* c, const lbm_params* p, int in, int ou
   a.list_z = 0;
   a.z_reverse = 0;
   a.z0 = 0;
+  a.nzs = c->nz;
   a.uhat = static_cast<T*>(c->uhat);
   a.sigma = p ? static_cast<T>(p->sigma) : T(1);
   for (int k = 0; k < 3; ++k) a.u_wall[k] = p ? static_cast<T>(p->u_wall[k]) : T(0);
@@ -121,6 +122,7 @@ int launch_one(lbm_ctx* c, const lbm_params* p, int in, int out, int z0, int nzs
   dim3 grid, block;
   lbm::StepArgs<T> a = make_args<T>(c, p, in, out);
   a.z0 = z0;
+  a.nzs = nzs;
   if (diag) {
     a.mom_rho = static_cast<T*>(diag->rho);
     a.mom_u = static_cast<T*>(diag->u);
@@ -145,6 +147,11 @@ int launch_one(lbm_ctx* c, const lbm_params* p, int in, int out, int z0, int nzs
     }
     grid.z = nzs + a.list_z;
     if (grid.z == 0) return LBM_OK;
+    if constexpr (lbm::mode_totals(MODE)) {     // ~16 blocks per SM; every block loops over the z-slices (one reduction per block)
+      const unsigned per_slice = grid.x * grid.y;
+      const unsigned want = (148u * 16u + per_slice - 1) / per_slice;
+      if (grid.z > want) grid.z = want;
+    }
     if (grid.z > 65535u || grid.y > 65535u)
       return fail(c, LBM_EINVAL, "lattice does not fit the launch grid (nz + list slices = %u, rows = %u; both must be <= 65535)", grid.z, grid.y);
     bool mw = false;
@@ -186,15 +193,19 @@ int launch_prepass(lbm_ctx* c, const lbm_params* p, int in, int out) {
 // passes are interleaved slab by slab in z, the UHAT pass one slice ahead (measured slower, default off).
 // The list cells go with the first UHAT launch and the last step launch.
 template <int Q, typename T, int MODE_U, int MODE_S>
-int launch_hrr_t(lbm_ctx* c, const lbm_params* p, int in, int out) {
+int launch_hrr_t(lbm_ctx* c, const lbm_params* p, int in, int out, int stage) {
   const int nz = c->nz;
-  int slab = (c->hrr_slab > 0) ? c->hrr_slab : nz;
-  int rc = launch_prepass<Q, T, lbm::mode_pulls(MODE_U)>(c, p, in, out);
+  const bool halo = (c->ghost_lo + c->ghost_hi) > 0;
+  int slab = (c->hrr_slab > 0 && !halo) ? c->hrr_slab : nz;
+  int rc = LBM_OK;
+  // stages of a step on a sub-domain (lbm_step_halo): 0 = pre-pass + u^ pass (the caller then exchanges the u^ boundary
+  // slices), 1 = the fused step pass; stage < 0: the whole step
+  if (stage != 1) rc = launch_prepass<Q, T, lbm::mode_pulls(MODE_U)>(c, p, in, out);
   if (rc != LBM_OK) return rc;
   if (slab >= nz - 1) {
-    rc = launch_one<Q, T, MODE_U, lbm::COLL_BGK>(c, p, in, out, 0, nz, true);
-    if (rc != LBM_OK) return rc;
-    return launch_one<Q, T, MODE_S, lbm::COLL_HRR>(c, p, in, out, 0, nz, true);
+    if (stage != 1) rc = launch_one<Q, T, MODE_U, lbm::COLL_BGK>(c, p, in, out, zlo(c), zcount(c), true);
+    if (rc != LBM_OK || stage == 0) return rc;
+    return launch_one<Q, T, MODE_S, lbm::COLL_HRR>(c, p, in, out, zlo(c), zcount(c), true);
   }
   // UHAT: slice nz-1 first (the periodic neighbour of slice 0), then [0, slab], [slab+1, 2 slab], ... up to nz-2
   rc = launch_one<Q, T, MODE_U, lbm::COLL_BGK>(c, p, in, out, nz - 1, 1, true);
@@ -222,11 +233,19 @@ int launch_bgk_pull_t(lbm_ctx* c, const lbm_params* p, int in, int out) {
   const int nz = c->nz;
   int rc = launch_prepass<Q, T, true>(c, p, in, out);
   if (rc != LBM_OK) return rc;
+  const int z0 = zlo(c), z1 = zlo(c) + zcount(c);            // interior slices [z0, z1)
   if (c->n_moving == 0 || nz < 8)
-    return launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 0, nz, true);
-  rc = launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 1, nz - 3, true, false);
-  if (rc == LBM_OK) rc = launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, nz - 2, 2, false);
-  if (rc == LBM_OK) rc = launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 0, 1, false);
+    return launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, z0, z1 - z0, true);
+  // [1, nz-2) plain, [nz-2, nz) and [0, 1) on the variant that looks for the lid, each clipped to the interior
+  auto piece = [&](int a, int b, bool with_list, bool lid) {
+    a = a < z0 ? z0 : a;
+    b = b > z1 ? z1 : b;
+    if (b <= a && !with_list) return static_cast<int>(LBM_OK);
+    return launch_one<Q, T, lbm::MODE_STREAM_COLLIDE, lbm::COLL_BGK>(c, p, in, out, a, b > a ? b - a : 0, with_list, lid);
+  };
+  rc = piece(1, nz - 2, true, false);
+  if (rc == LBM_OK) rc = piece(nz - 2, nz, false, true);
+  if (rc == LBM_OK) rc = piece(0, 1, false, true);
   return rc;
 }
 
@@ -243,13 +262,13 @@ int launch_step_bgk(lbm_ctx* c, const lbm_params* p, int mode) {
   switch (mode) {
     case lbm::MODE_COLLIDE:
       rc = launch_prepass<Q, T, false>(c, p, in, out);
-      if (rc == LBM_OK) rc = launch_one<Q, T, lbm::MODE_COLLIDE, lbm::COLL_BGK>(c, p, in, out, 0, c->nz, true);
+      if (rc == LBM_OK) rc = launch_one<Q, T, lbm::MODE_COLLIDE, lbm::COLL_BGK>(c, p, in, out, zlo(c), zcount(c), true);
       break;
     case lbm::MODE_STREAM_COLLIDE:
       rc = launch_bgk_pull_t<Q, T>(c, p, in, out);
       break;
     default:
-      rc = launch_one<Q, T, lbm::MODE_STREAM, lbm::COLL_BGK>(c, p, in, out, 0, c->nz, true);
+      rc = launch_one<Q, T, lbm::MODE_STREAM, lbm::COLL_BGK>(c, p, in, out, zlo(c), zcount(c), true);
       break;
   }
   if (rc != LBM_OK) return rc;
@@ -271,12 +290,12 @@ int launch_init(lbm_ctx* c, const void* rho, const void* u) {
 
 #if LBM_INST_PART == 1
 template <int Q, typename T>
-int launch_step_hrr(lbm_ctx* c, const lbm_params* p, int mode) {
+int launch_step_hrr(lbm_ctx* c, const lbm_params* p, int mode, int stage) {
   const int in = c->cur, out = 1 - c->cur;
-  int rc = (mode == lbm::MODE_COLLIDE) ? launch_hrr_t<Q, T, lbm::MODE_UHAT_PRE, lbm::MODE_COLLIDE>(c, p, in, out)
-                                       : launch_hrr_t<Q, T, lbm::MODE_UHAT_PULL, lbm::MODE_STREAM_COLLIDE>(c, p, in, out);
+  int rc = (mode == lbm::MODE_COLLIDE) ? launch_hrr_t<Q, T, lbm::MODE_UHAT_PRE, lbm::MODE_COLLIDE>(c, p, in, out, stage)
+                                       : launch_hrr_t<Q, T, lbm::MODE_UHAT_PULL, lbm::MODE_STREAM_COLLIDE>(c, p, in, out, stage);
   if (rc != LBM_OK) return rc;
-  step_done(c);
+  if (stage != 0) step_done(c);
   return LBM_OK;
 }
 #endif
@@ -288,8 +307,8 @@ template <int Q, typename T>
 int launch_moments(lbm_ctx* c, const lbm_params* p, void* rho, void* u) {
   const DiagOut out = {rho, u};
   int rc = (c->phase == PHASE_POST)
-               ? launch_one<Q, T, lbm::MODE_MOMENTS_PULL, lbm::COLL_BGK>(c, p, c->cur, 1 - c->cur, 0, c->nz, true, true, &out)
-               : launch_one<Q, T, lbm::MODE_MOMENTS_PRE, lbm::COLL_BGK>(c, p, c->cur, 1 - c->cur, 0, c->nz, true, true, &out);
+               ? launch_one<Q, T, lbm::MODE_MOMENTS_PULL, lbm::COLL_BGK>(c, p, c->cur, 1 - c->cur, zlo(c), zcount(c), true, true, &out)
+               : launch_one<Q, T, lbm::MODE_MOMENTS_PRE, lbm::COLL_BGK>(c, p, c->cur, 1 - c->cur, zlo(c), zcount(c), true, true, &out);
   if (rc != LBM_OK) return rc;
   if (c->n_solid_list > 0) {
     const unsigned blocks = static_cast<unsigned>((c->n_solid_list + 255) / 256);
@@ -305,8 +324,8 @@ int launch_moments(lbm_ctx* c, const lbm_params* p, void* rho, void* u) {
 template <int Q, typename T>
 int launch_totals(lbm_ctx* c, const lbm_params* p) {
   return (c->phase == PHASE_POST)
-             ? launch_one<Q, T, lbm::MODE_TOTALS_PULL, lbm::COLL_BGK>(c, p, c->cur, 1 - c->cur, 0, c->nz, true)
-             : launch_one<Q, T, lbm::MODE_TOTALS_PRE, lbm::COLL_BGK>(c, p, c->cur, 1 - c->cur, 0, c->nz, true);
+             ? launch_one<Q, T, lbm::MODE_TOTALS_PULL, lbm::COLL_BGK>(c, p, c->cur, 1 - c->cur, zlo(c), zcount(c), true)
+             : launch_one<Q, T, lbm::MODE_TOTALS_PRE, lbm::COLL_BGK>(c, p, c->cur, 1 - c->cur, zlo(c), zcount(c), true);
 }
 #endif
 

@@ -7,6 +7,8 @@ and comes out window by window (lbm_get_populations_box), so that neither the ho
 Both sides start from the ORACLE's equilibrium populations rounded to the run's dtype: the slabs handed to the library and the
 crops handed to the oracle are the same cell-local function (orc_init_equilibrium) of the same rho, u arrays.
 """
+from concurrent.futures import ThreadPoolExecutor
+
 import numpy as np
 import pytest
 import torch
@@ -57,10 +59,16 @@ def _lean_windows(n, dtype, steps=S, slab=8):
     got, got_rho, got_u = {}, {}, {}
     with P.LBM(Q, nx, ny, nz, dtype) as sim:
         sim.set_geometry(d, cfg["flags"])
-        for z0 in range(0, nz, slab):
-            zs = min(slab, nz - z0)
-            fs = O.init_equilibrium(Q, np.ascontiguousarray(cfg["rho"][z0:z0 + zs]), np.ascontiguousarray(cfg["u"][:, z0:z0 + zs])).astype(npdt)
-            sim.set_populations_box((0, 0, z0), (nx, ny, zs), fs)
+        def slab_populations(z0):                              # the oracle's routine, one call per slab (it is serial: the
+            zs = min(slab, nz - z0)                            # harness runs several slabs at a time; ctypes drops the GIL)
+            return z0, zs, O.init_equilibrium(Q, np.ascontiguousarray(cfg["rho"][z0:z0 + zs]),
+                                              np.ascontiguousarray(cfg["u"][:, z0:z0 + zs])).astype(npdt)
+
+        starts = list(range(0, nz, slab))
+        with ThreadPoolExecutor(max_workers=min(O.max_threads(), 12)) as pool:
+            for k0 in range(0, len(starts), 24):               # bounded: at most 24 slabs in memory
+                for z0, zs, fs in pool.map(slab_populations, starts[k0:k0 + 24]):
+                    sim.set_populations_box((0, 0, z0), (nx, ny, zs), fs)
         assert sim.query("steps") == 0
         sim.step(steps, par)
         rho = torch.empty((nz, ny, nx), dtype=TORCH_DTYPE[dtype], device="cuda")
@@ -99,7 +107,11 @@ def _lean_windows(n, dtype, steps=S, slab=8):
         rr, ru = O.moments(ref)
         e_f = field_error(gotw, refw, mask)
         e_rho = field_error(got_rho[(z0, y0, x0)], rr[inner[1:]], mask)
-        e_u = field_error(got_u[(z0, y0, x0)], ru[(slice(None),) + inner[1:]], mask)
+        uw = ru[(slice(None),) + inner[1:]]
+        e_u = field_error(got_u[(z0, y0, x0)], uw, mask)
+        # R12 normalises by the maximum of the whole FIELD, which a window inside a building (u ~ 0) does not see; the field's
+        # maximum is at least the inlet speed (the INLET plane carries u_in exactly)
+        e_u *= np.abs(uw[..., mask]).max() / max(np.abs(uw[..., mask]).max(), cfg["params"]["u_in"][0])
         worst = max(worst, e_f, e_rho, e_u)
         assert e_f <= TOL[dtype], ("populations", (z0, y0, x0), e_f)
         assert e_rho <= TOL[dtype], ("rho", (z0, y0, x0), e_rho)

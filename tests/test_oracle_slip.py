@@ -101,3 +101,27 @@ def test_W3_uniform_flow_fixed_point_and_fallback(Q):
     t0 = O.totals(f, flags)
     t1 = O.totals(O.step(f, flags=flags, nsteps=30, tau0=0.7), flags)
     assert abs(t1[0] / t0[0] - 1.0) <= 1e-13 and t1[1] < t0[1]
+
+
+@pytest.mark.parametrize("Q", [19, 27])
+@pytest.mark.parametrize("coll", [0, 1])
+def test_W4_wall_cells_are_inert_whatever_populations_they_hold(Q, coll):
+    """Readings R5 / G30 / G37: SOLID and SLIPWALL cells are inert -- nothing a fluid cell computes may depend on the populations
+    stored in them; in the HRR form the FD stencil sees u^ = 0 there (a resting wall), not the moment of those stored values.
+    (Found by the GPU parity test from a non-equilibrium start: the oracle took u^ of SLIPWALL cells from their own populations,
+    which only shows once those populations carry momentum.)"""
+    nz, ny, nx = 9, 8, 12
+    rng = np.random.Generator(np.random.PCG64(40 + Q + coll))
+    flags = _slip_box(nz, ny, nx)
+    flags[2:4, 2:4, 5:8] = I.SOLID
+    rho = 1.0 + 0.02 * rng.standard_normal(flags.shape)
+    u = 0.04 * rng.standard_normal((3,) + flags.shape)
+    f = O.init_equilibrium(Q, rho, u) * (1 + 0.01 * rng.standard_normal((Q,) + flags.shape))
+    wall = I.is_wall(flags)
+    par = dict(tau0=0.58, cs_smago=0.1, collision=coll, sigma=0.5)
+    a = O.step(f, flags=flags, nsteps=5, **par)
+    g = f.copy()
+    g[:, wall] = O.feq(Q, 1.3, [0.1, -0.2, 0.15])[:, None] * (1 + 0.3 * rng.uniform(-1, 1, size=(Q, int(wall.sum()))))
+    b = O.step(g, flags=flags, nsteps=5, **par)
+    assert np.array_equal(a[:, ~wall], b[:, ~wall])
+    assert np.array_equal(b[:, wall], g[:, wall])                # and they keep what they hold
