@@ -12,8 +12,11 @@ Protocol: --repeats R (default 3) timed regions of exactly K steps
 lbm_init_equilibrium + W warm-up steps, CUDA events on the library's stream; the line reports the MEDIAN region
 (all of them are listed in config.repeats_ms_per_step).  lbm_moments / lbm_totals (row A9) are timed separately
 ("moments" block) and are not part of MLUPs.
-N > 1: the path does not shard in this build ("replicas only"): every rank runs the same
-workload on its own GPU, no data-path collective; value = sum over ranks / max time.
+N > 1: the lattice is cut into z-slabs, one per GPU (one process per GPU), with one halo exchange per step over NCCL
+send/recv (two in the HRR form): the 5 of 19 populations that cross each cut, lbm_set_halo / lbm_step_halo / lbm_halo_pack /
+lbm_halo_unpack + paper_2506_21804_b200/slab.py.  Weak scaling by default: N copies of the workload's height stacked in z
+(the same generator at (N nz, ny, nx)), value = all cell updates of the job / max time over ranks; --strong cuts the
+workload's own lattice; --replicas (and the Vortex-Method workloads) run N independent replicas with no data-path collective.
 --impl reference: the CPU oracle (oracle/), as it stands, timed on the host cores on a bounded sample.
 Prints ONE JSON line on rank 0.
 """
@@ -275,6 +278,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--repeats", type=int, default=3, help="timed regions of K steps each, every one from a fresh state; the median is reported")
+    ap.add_argument("--replicas", action="store_true", help="N > 1: independent replicas instead of the z-slab decomposition")
+    ap.add_argument("--strong", action="store_true", help="N > 1: cut the workload's own lattice N ways (strong scaling) instead of stacking N of them in z")
     ap.add_argument("--no-moments", action="store_true", help="skip the separate timing of lbm_moments / lbm_totals (A9)")
     ap.add_argument("--option", action="append", default=[], help="library option key=value (tuning)")
     args = ap.parse_args()
@@ -302,22 +307,49 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     number, shape, dtype, extra = workload(args.workload)
+    # N > 1: the lattice is cut into z-slabs, one per GPU, with a halo exchange per step.  Weak scaling
+    # (default): N copies of the workload's height stacked in z -- the same generator at (N nz, ny, nx) -- so every GPU keeps the
+    # workload's own cell count; --strong cuts the workload's own lattice.  Workloads with the Vortex Method inlet (it needs the
+    # whole inflow plane) and config 1 run as independent replicas.
+    decomposed = world > 1 and not args.replicas and number != 1 and workload_vm(args.workload, (8, 8, 8)) is None
+    if decomposed and not args.strong:
+        base = shape or make_cfg(number, None, {})["shape"]
+        shape = (base[0] * world, base[1], base[2])
     cfg = make_cfg_named(args.workload, number, shape, extra)
     hrr = cfg["params"].get("collision", 0) == 1
     if args.steps is None:
         args.steps = cfg["steps"]
-    nz, ny, nx = cfg["shape"]
-    N = nx * ny * nz
     Q = cfg["Q"]
     tdt = torch.float32 if dtype == "f32" else torch.float64
     npdt = np.float32 if dtype == "f32" else np.float64
     par = P.LbmParams(**cfg["params"])
-
     stream = torch.cuda.current_stream()
-    sim = P.LBM(Q, nx, ny, nz, dtype, stream=stream.cuda_stream)
+    part = None
+    n_wall_global = 0 if cfg["flags"] is None else int(I.is_wall(cfg["flags"]).sum())
+    cells_global = int(np.prod(cfg["shape"]))
+    if decomposed:
+        from paper_2506_21804_b200 import slab as S
+        gnz, ny, nx = cfg["shape"]
+        part = S.SlabLBM(Q, nx, ny, gnz, dtype, rank, world, S.z_is_closed(cfg["flags"]), stream=stream.cuda_stream)
+        sim = part.sim
+        sl = part.slab
+        for key, axis in (("rho", 0), ("u", 1), ("d", 0), ("flags", 0), ("u_body", 1)):
+            if cfg.get(key) is not None:
+                cfg[key] = sl.take(cfg[key], axis=axis)           # this rank's slices, ghost slices included
+        nz = sl.nz_local
+    else:
+        nz, ny, nx = cfg["shape"]
+        sim = P.LBM(Q, nx, ny, nz, dtype, stream=stream.cuda_stream)
+    N = nx * ny * nz
     for kv in args.option:
         k, v = kv.split("=")
         sim.set_option(k, int(v))
+
+    def do_steps(n):
+        if part is not None:
+            part.step(n, par)
+        else:
+            sim.step(n, par)
 
     # inputs resident in HBM before the timed region
     rho_d = torch.from_numpy(cfg["rho"].astype(npdt)).cuda()
@@ -325,16 +357,32 @@ def main():
     d_d = None if cfg["d"] is None else torch.from_numpy(cfg["d"].astype(npdt)).cuda()
     fl_d = None if cfg["flags"] is None else torch.from_numpy(cfg["flags"]).cuda()
     sim.set_geometry(d_d, fl_d)
-    sim.init_equilibrium(rho_d, u_d)
+    if part is not None:
+        part.init_equilibrium(rho_d, u_d)                     # + lbm_set_halo
+    else:
+        sim.init_equilibrium(rho_d, u_d)
     if cfg.get("u_body") is not None:
         sim.set_body_velocity(torch.from_numpy(cfg["u_body"].astype(npdt)).cuda())
     vm = workload_vm(args.workload, cfg["shape"])
     if vm is not None:
         sim.set_inflow(torch.from_numpy(vm["u_mean"].astype(npdt)).cuda())
         sim.set_vortices(vm["pos"], vm["sign"], vm["sigma_v"], vm["intensity"])
-    n_solid = sim.query("solid_cells")
-    n_fluid = N - n_solid
-    tot0 = sim.totals()
+    if decomposed:
+        n_solid = n_wall_global                               # job-wide counts (every rank generated the global geometry)
+        n_fluid = (cells_global - n_wall_global) / world      # per rank on average: job value = world * n_fluid * steps / time
+    else:
+        n_solid = sim.query("solid_cells")
+        n_fluid = N - n_solid
+
+    def job_totals():
+        t = np.array(sim.totals())
+        if decomposed:
+            tt = torch.tensor(t, device="cuda", dtype=torch.float64)
+            dist.all_reduce(tt)
+            t = tt.cpu().numpy()
+        return t
+
+    tot0 = job_totals()
 
     def barrier():
         if world > 1:
@@ -347,23 +395,25 @@ def main():
     region_ms, launches = [], 0
     for rep in range(max(args.repeats, 1)):
         if rep > 0:
-            sim.init_equilibrium(rho_d, u_d)                  # fresh S_0 (also resets the inflow history of the VM inlet)
-        sim.step(args.warmup, par)
+            (part or sim).init_equilibrium(rho_d, u_d)        # fresh S_0 (also resets the inflow history of the VM inlet)
+        do_steps(args.warmup)
         barrier()
         l0 = sim.query("launches")
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
-        sim.step(args.steps, par)
+        do_steps(args.steps)
         e1.record(stream)
         barrier()
         launches = sim.query("launches") - l0
         region_ms.append(max_over_ranks(e0.elapsed_time(e1), world))
     clocks = sampler.stop()
     ms = float(np.median(region_ms))
-    tot1 = sim.totals()
+    tot1 = job_totals()
     finite = bool(np.isfinite(tot1).all())
     value = job_mlups(world, n_fluid, args.steps, ms * 1e-3)
     step_bytes, per_cell = algorithmic_bytes_per_step(cfg, dtype, n_solid)
+    if decomposed:
+        step_bytes //= world                                  # per GPU (the roofline figures are per GPU)
     peak, peak_src = measured_peak()
     # BGK form: one launch over the lattice = one step.  HRR form: a step is two launches over the lattice (u^ pass + fused step);
     # the figure is then algorithmic bytes per STEP / time per step, i.e. it charges the u^ pass to the step kernel
@@ -392,7 +442,8 @@ def main():
         lm0 = sim.query("launches")
         t_mom = timed(lambda: sim.moments(rho_o, u_o))
         lm1 = sim.query("launches")
-        t_tot = timed(lambda: sim.totals())
+        tot_o = torch.empty(5, dtype=torch.float64, device="cuda")
+        t_tot = timed(lambda: sim.totals(tot_o))
         lm2 = sim.query("launches")
         b_mom = (Q + 4) * sz * n_fluid + N
         b_tot = Q * sz * n_fluid + N
@@ -400,7 +451,7 @@ def main():
                                    "frac": b_mom / (t_mom * 1e-3) / 1e9 / peak, "launches_per_call": (lm1 - lm0) / 8.0},
                    "lbm_totals": {"ms": t_tot, "algorithmic_bytes": b_tot, "achieved_gbs": b_tot / (t_tot * 1e-3) / 1e9,
                                   "frac": b_tot / (t_tot * 1e-3) / 1e9 / peak, "launches_per_call": (lm2 - lm1) / 8.0,
-                                  "note": "includes the 40-byte result copy to the host and its stream synchronisation"},
+                                  "note": "result into a device buffer (asynchronous; a host buffer adds the copy and a stream synchronisation)"},
                    "what": "median of 7 calls on the stepped state, CUDA events; device outputs rho[N], u[3][N]; not part of MLUPs"}
         del rho_o, u_o
 
@@ -418,7 +469,7 @@ def main():
         barrier()
         t0 = time.perf_counter()
         sim.set_fields(h_f, h_d, h_fl)                 # H2D: populations + porosity + flags
-        sim.step(args.steps, par)
+        do_steps(args.steps)
         sim.moments(h_rho, h_u)                        # D2H: rho, u
         sim.synchronize()
         dt = time.perf_counter() - t0
@@ -454,12 +505,15 @@ def main():
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong" if (decomposed and args.strong) else "weak", "vs_baseline": None,
             "dtype": dtype, "data": "synthetic",
             "config": {"workload": args.workload, "lattice": "D3Q%d" % Q, "nx": nx, "ny": ny, "nz": nz, "cells": N,
                        "solid_cells": n_solid, "masked_cells": sim.query("masked_cells"), "params": cfg["params"],
                        "l2": "inputs larger than L2 (%.2f GB per step)" % (step_bytes / 1e9),
-                       "mlups_all_cells": world * N * args.steps / (ms * 1e-3) / 1e6, "parallelism": "replicas only",
+                       "mlups_all_cells": (cells_global if decomposed else world * N) * args.steps / (ms * 1e-3) / 1e6,
+                       "parallelism": ("z-slabs, one per GPU, halo exchange per step over NCCL send/recv (%s scaling): global lattice %s"
+                                       % ("strong" if args.strong else "weak", "x".join(str(v) for v in cfg["shape"][::-1]))) if decomposed
+                                      else ("replicas only" if world > 1 else "single GPU"),
                        "finite": finite, "mass_drift_rel": (tot1[0] - tot0[0]) / tot0[0],
                        "repeats_ms_per_step": [t / args.steps for t in region_ms],
                        "protocol": "median of %d timed regions of %d steps, each from a fresh lbm_init_equilibrium + %d warm-up steps" % (len(region_ms), args.steps, args.warmup),

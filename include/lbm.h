@@ -208,9 +208,9 @@ int lbm_set_populations_box(lbm_ctx* ctx, int x0, int y0, int z0, int bx, int by
 
 /* Totals over the non-wall cells of S_t (the conserved quantities of Eq. 6: mass and momentum, l.97,
  * and the kinetic energy the Taylor-Green check of config 1 is stated in): out[0] = sum rho, out[1..3] = sum rho u,
- * out[4] = sum rho |u|^2 / 2.  `out` is a HOST array of 5 doubles.  One launch, pulling S_t in registers like lbm_moments:
+ * out[4] = sum rho |u|^2 / 2.  `out`: 5 doubles, host (the call synchronises the stream) or device (asynchronous).  One launch, pulling S_t in registers like lbm_moments:
  * per-thread sums over the cells of a vector in dtype, from the warp level up in fp64 (shuffle tree, one atomicAdd(double)
- * per block into one of 256 slots, the last block adds the slots).  Synchronises the stream.
+ * per block into one of 256 slots, the last block adds the slots).  On a sub-domain (lbm_set_halo): the interior cells only.
  * Errors: LBM_EINVAL (NULL ctx / out), LBM_ESTATE (no state), LBM_ECUDA. */
 int lbm_totals(lbm_ctx* ctx, double out[5]);
 

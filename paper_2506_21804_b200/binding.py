@@ -84,7 +84,7 @@ def load_library():
     L.lbm_step_halo.argtypes = [vp, ctypes.POINTER(LbmParams), ip]
     L.lbm_halo_pack.argtypes = [vp, ip, ip, vp]
     L.lbm_halo_unpack.argtypes = [vp, ip, ip, vp]
-    L.lbm_totals.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
+    L.lbm_totals.argtypes = [vp, vp]
     L.lbm_set_stream.argtypes = [vp, vp]
     L.lbm_synchronize.argtypes = [vp]
     L.lbm_last_error.argtypes = [vp]
@@ -216,9 +216,13 @@ def lbm_halo_unpack(ctx, what, side, buf):
     return _check(ctx, load_library().lbm_halo_unpack(ctx, int(what), int(side), _ptr(buf)))
 
 
-def lbm_totals(ctx):
+def lbm_totals(ctx, out=None):
+    """out = None: returns the five totals as a list (host, synchronises); out = a buffer of 5 doubles (host or device):
+    filled in place (a device buffer asynchronously)"""
+    if out is not None:
+        return _check(ctx, load_library().lbm_totals(ctx, _ptr(out)))
     out = (ctypes.c_double * 5)()
-    _check(ctx, load_library().lbm_totals(ctx, out))
+    _check(ctx, load_library().lbm_totals(ctx, ctypes.addressof(out)))
     return list(out)
 
 
@@ -318,8 +322,8 @@ class LBM:
     def halo_unpack(self, what, side, buf):
         return lbm_halo_unpack(self.ctx, what, side, buf)
 
-    def totals(self):
-        return lbm_totals(self.ctx)
+    def totals(self, out=None):
+        return lbm_totals(self.ctx, out)
 
     def synchronize(self):
         return lbm_synchronize(self.ctx)

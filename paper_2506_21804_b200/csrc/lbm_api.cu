@@ -885,8 +885,9 @@ int lbm_totals(lbm_ctx* c, double out[5]) {
   if (rc != LBM_OK) return rc;
   rc = LBM_DISPATCH(c, launch_totals, c, &p);
   if (rc != LBM_OK) return rc;
-  LBM_CUDA(c, cudaMemcpyAsync(out, c->totals_dev, 5 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
-  LBM_CUDA(c, cudaStreamSynchronize(c->stream));
+  const bool dev = is_device_pointer(out);
+  LBM_CUDA(c, cudaMemcpyAsync(out, c->totals_dev, 5 * sizeof(double), cudaMemcpyDefault, c->stream));
+  if (!dev) LBM_CUDA(c, cudaStreamSynchronize(c->stream));
   return LBM_OK;
 }
 

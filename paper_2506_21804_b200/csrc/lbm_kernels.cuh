@@ -124,6 +124,8 @@ struct StepArgs {
   int list_z;
   int z_reverse;                  // vector kernel: walk the slab from its last slice down (serpentine sweep over consecutive launches)
   int z0;                         // first lattice z-slice of this launch (the launch covers the slab z0 .. z0 + nzs - 1)
+  int zi0, zi1;                   // interior slices [zi0, zi1) of the lattice (all of it unless ghost slices are declared: lbm_set_halo);
+                                  // list cells outside belong to ghost slices and are skipped
   int nzs;                        // z-slices of this launch (grid.z = list_z + nzs, except in the totals modes, whose blocks loop over z)
   // HRR form (Eq. 7-11): u^(x,t) of every cell [3][N] (written by the MODE_UHAT_* pass, SOLID cells 0), Eq. 7 factor
   T* __restrict__ uhat;
@@ -1042,11 +1044,12 @@ __device__ __forceinline__ void step_vec_body(const StepArgs<T>& a, double (&acc
     if (k < a.n_list) {
       const int cell = a.list[k];
       const uint8_t c = a.cls[cell];
+      const int plane = a.nx * a.ny;
+      const int cz = cell / plane, rem = cell - cz * plane;
+      if (cz < a.zi0 || cz >= a.zi1) return;   // a cell of a ghost slice: its values come from the neighbouring sub-domain
       if (is_wall(c)) {                    // wall sector-mate: zeros keep the sector whole
         solid_cell_any<Q, T, MODE>(a, cell);
       } else {
-        const int plane = a.nx * a.ny;
-        const int cz = cell / plane, rem = cell - cz * plane;
         const int cy = rem / a.nx, cx = rem - cy * a.nx;
         step_cell_any<Q, T, MODE, COLL>(a, cx, cy, cz, c, acc);
       }

@@ -48,6 +48,8 @@ lbm::StepArgs<T> make_args(const lbm_ctx* c, const lbm_params* p, int in, int ou
   a.z_reverse = 0;
   a.z0 = 0;
   a.nzs = c->nz;
+  a.zi0 = zlo(c);
+  a.zi1 = zlo(c) + zcount(c);
   a.uhat = static_cast<T*>(c->uhat);
   a.sigma = p ? static_cast<T>(p->sigma) : T(1);
   for (int k = 0; k < 3; ++k) a.u_wall[k] = p ? static_cast<T>(p->u_wall[k]) : T(0);
