@@ -95,8 +95,8 @@ typedef struct {
  * nx, ny, nz >= 1 (SURVEY 8(b) asked for LBM_EINVAL below 3; sizes 1 and 2 are accepted as a superset: the periodic wrap is
  * well defined for them and they are parity-tested), nx*ny*nz < 2^31, ny <= 65535 and nz <= 65000 (launch-grid limits; a
  * lattice whose nz plus its list slices passes 65535 is refused by lbm_step with LBM_EINVAL).  Rows with nx a multiple of
- * 32/sizeof(dtype) take the vector kernel, other row lengths the scalar kernel.  Allocates two population lattices
- * (2*Q*N*dtype bytes), the porosity field, one class byte and one 32-bit neighbour mask per cell on the current CUDA device.
+ * 32/sizeof(dtype) take the vector kernel, other row lengths the scalar kernel.  Allocates one population lattice (Q*N*dtype
+ * bytes; the second one when the first two-lattice pass runs), the porosity field, one class byte and one 32-bit neighbour mask per cell on the current CUDA device.
  * Returns NULL on failure; lbm_last_error(NULL) then holds the reason. */
 lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype);
 
@@ -288,6 +288,10 @@ long long lbm_query(const lbm_ctx* ctx, int what);
  *                           compact list; 0: they are solved cell by cell in the list blocks of the step kernel.  Decides how
  *                           flags are classified: LBM_ESTATE once a state or geometry has been set
  *   "serpentine"    0|1     consecutive launches sweep the z-slices in opposite directions for L2 reuse (default 1)
+ *   "inplace"       0|1     1: a lattice without a single wall / inlet / outlet / wall-model cell (fully periodic bulk), BGK form,
+ *                           steps IN PLACE on one array (AA pattern: even steps collide locally into the opposite slots, odd
+ *                           steps pull and push through the neighbours); the second lattice is then never
+ *                           allocated unless a state read after an odd number of steps needs it.  Default 0 (two lattices)
  *   "vector"        0|1     0 forces the scalar kernel (one cell per thread) for every row length (default 1)
  *   "block_threads" 64|128|256   threads per block of the step kernels (default 64)
  *   "hrr_slab"      n >= 0  HRR form: interleave the u^ pass and the step pass in slabs of n z-slices (0 = whole lattice, default) */

@@ -1,6 +1,6 @@
 """Build step for the CUDA library (nvcc, sm_100a only).  `python -m paper_2506_21804_b200.build [--force] [-v]`.
 
-csrc/lbm_api.cu (host side of the C ABI, set-up kernels) + csrc/lbm_inst.cu compiled once per (lattice, dtype, part): thirteen
+csrc/lbm_api.cu (host side of the C ABI, set-up kernels) + csrc/lbm_inst.cu compiled once per (lattice, dtype, part): seventeen
 object files, built in parallel, linked into liblbm_b200.so next to this file."""
 import os
 import subprocess
@@ -18,7 +18,7 @@ NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a",
 UNITS = [("lbm_api", "lbm_api.cu", [])]
 for _q in (19, 27):
     for _t in ("float", "double"):
-        for _part in (0, 1, 2):
+        for _part in (0, 1, 2, 3):
             UNITS.append(("lbm_inst_q%d_%s_p%d" % (_q, _t, _part), "lbm_inst.cu",
                           ["-DLBM_INST_Q=%d" % _q, "-DLBM_INST_T=%s" % _t, "-DLBM_INST_PART=%d" % _part]))
 

@@ -89,7 +89,14 @@ void launch_dims(const lbm_ctx* c, dim3& grid, dim3& block) {
                 : ((c)->dtype == LBM_F32 ? lbmhost::fn<27, float>(__VA_ARGS__) : lbmhost::fn<27, double>(__VA_ARGS__)))
 
 // stage: -1 = the whole step; 0 / 1 = the two stages of a step on a sub-domain (lbm_step_halo; the BGK form has no stage 0)
+// the second lattice is allocated when a two-lattice pass first needs it (a lattice that only ever steps in place never does)
+int ensure_lattice1(lbm_ctx* c) {
+  if (c->f[1]) return LBM_OK;
+  return dev_alloc(c, &c->f[1], static_cast<size_t>(c->Q) * c->N * c->dtype);
+}
+
 int launch_step(lbm_ctx* c, const lbm_params* p, int mode, int stage = -1) {
+  { int rca = ensure_lattice1(c); if (rca != LBM_OK) return rca; }
   const bool hrr = p && p->collision == LBM_COLLISION_HRR && mode != lbm::MODE_STREAM;
   if (hrr) return LBM_DISPATCH(c, launch_step_hrr, c, p, mode, stage);
   if (stage == 0) return LBM_OK;
@@ -374,8 +381,7 @@ lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype) {
   c->last = default_params();
   std::snprintf(c->err, sizeof(c->err), "no error");
   const size_t pop = static_cast<size_t>(lattice) * N * dtype;
-  int rc = dev_alloc(c, &c->f[0], pop);
-  if (rc == LBM_OK) rc = dev_alloc(c, &c->f[1], pop);
+  int rc = dev_alloc(c, &c->f[0], pop);          // (the second lattice: ensure_lattice1, on first use)
   if (rc == LBM_OK) rc = dev_alloc(c, &c->d, static_cast<size_t>(N) * dtype);
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->cls), N);
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->cls_alt), N);
@@ -488,6 +494,14 @@ int lbm_init_equilibrium(lbm_ctx* c, const void* rho, const void* u) {
 
 // POST -> PRE: write S_t = stream(F_{t-1}) into the other lattice and make it current
 static int materialise(lbm_ctx* c) {
+  if (c->phase == PHASE_SWAPPED) {       // in-place stepping, odd number of steps: un-swap and stream into the other lattice
+    lbm_params p = c->last;
+    int rc = ensure_lattice1(c);
+    if (rc == LBM_OK) rc = LBM_DISPATCH(c, launch_aa, c, &p, 2);
+    if (rc != LBM_OK) return rc;
+    c->phase = PHASE_PRE;
+    return LBM_OK;
+  }
   if (c->phase != PHASE_POST) return LBM_OK;
   lbm_params p = c->last;
   int rci = ensure_inflow(c, c->steps);
@@ -713,6 +727,16 @@ static int graph_chunk(lbm_ctx* c, const lbm_params* params, bool* done) {
   return LBM_OK;
 }
 
+// In-place (AA pattern) stepping applies to lattices without a single boundary cell, BGK form, rows the vector kernels take
+static bool inplace_eligible(const lbm_ctx* c, const lbm_params* p) {
+  if (!c->inplace || !c->use_vector || c->n_solid != 0 || c->n_masked != 0 || c->uin_mean || c->ghost_lo || c->ghost_hi) return false;
+  if (p->collision != LBM_COLLISION_BGK) return false;
+  const int V = (c->Q == 19 ? 16 : 8) / c->dtype;             // cells per thread of the BGK vector kernels
+  if (V < 1 || c->nx % V != 0) return false;
+  const int nvec = c->nx / V;
+  return nvec % 32 == 0 && nvec <= 256;
+}
+
 // buffers a step needs beyond the lattices: u^ field (HRR form), u^B of the wall-model cells (pre-pass)
 static int step_buffers(lbm_ctx* c, const lbm_params* params, int n_steps) {
   int rc = LBM_OK;
@@ -745,7 +769,23 @@ int lbm_step(lbm_ctx* c, int n_steps, const lbm_params* params) {
   rc = step_buffers(c, params, n_steps);
   if (rc != LBM_OK) return rc;
   int s = 0;
+  const bool inplace = inplace_eligible(c, params);
+  if (!inplace && c->phase == PHASE_SWAPPED && n_steps > 0) {
+    rc = materialise(c);
+    if (rc != LBM_OK) return rc;
+  }
   while (s < n_steps) {
+    if (inplace) {                                             // AA pattern on the current lattice alone (option "inplace")
+      if (c->phase == PHASE_POST) {
+        rc = materialise(c);
+        if (rc != LBM_OK) return rc;
+      }
+      rc = LBM_DISPATCH(c, launch_aa, c, params, c->phase == PHASE_PRE ? 0 : 1);
+      if (rc != LBM_OK) return rc;
+      c->phase = (c->phase == PHASE_PRE) ? PHASE_SWAPPED : PHASE_PRE;
+      ++s;
+      continue;
+    }
     if (c->phase == PHASE_PRE) {
       rc = launch_step(c, params, lbm::MODE_COLLIDE);          // S_t -> F_t
       c->phase = PHASE_POST;
@@ -787,7 +827,9 @@ int lbm_moments(lbm_ctx* c, void* rho, void* u) {
     if (hu) du = s + cell_bytes;
   }
   lbm_params p = c->last;
-  int rc = (c->phase == PHASE_POST) ? ensure_inflow(c, c->steps) : LBM_OK;     // the inlet rule is part of the pull
+  int rc = (c->phase == PHASE_SWAPPED) ? materialise(c) : LBM_OK;
+  if (rc != LBM_OK) return rc;
+  rc = (c->phase == PHASE_POST) ? ensure_inflow(c, c->steps) : LBM_OK;     // the inlet rule is part of the pull
   if (rc != LBM_OK) return rc;
   rc = LBM_DISPATCH(c, launch_moments, c, &p, drho, du);
   if (rc != LBM_OK) return rc;
@@ -881,7 +923,9 @@ int lbm_totals(lbm_ctx* c, double out[5]) {
   if (!out) return fail(c, LBM_EINVAL, "lbm_totals: out is NULL");
   if (c->phase == PHASE_NONE) return fail(c, LBM_ESTATE, "lbm_totals: no state");
   lbm_params p = c->last;
-  int rc = (c->phase == PHASE_POST) ? ensure_inflow(c, c->steps) : LBM_OK;
+  int rc = (c->phase == PHASE_SWAPPED) ? materialise(c) : LBM_OK;
+  if (rc != LBM_OK) return rc;
+  rc = (c->phase == PHASE_POST) ? ensure_inflow(c, c->steps) : LBM_OK;
   if (rc != LBM_OK) return rc;
   rc = LBM_DISPATCH(c, launch_totals, c, &p);
   if (rc != LBM_OK) return rc;
@@ -939,6 +983,10 @@ int lbm_step_halo(lbm_ctx* c, const lbm_params* params, int stage) {
   if (stage != c->halo_stage) return fail(c, LBM_ESTATE, "lbm_step_halo: stage %d called where stage %d is due", stage, c->halo_stage);
   if (params->wm_enable && c->halo_wm_epoch != c->epoch) {       // the geometry changed since the cut was checked
     rc = check_wm_cut(c, c->ghost_lo, c->ghost_hi);
+    if (rc != LBM_OK) return rc;
+  }
+  if (c->phase == PHASE_SWAPPED) {
+    rc = materialise(c);
     if (rc != LBM_OK) return rc;
   }
   c->last = *params;
@@ -1091,6 +1139,12 @@ int lbm_set_option(lbm_ctx* c, const char* key, long long value) {
   if (std::strcmp(key, "hrr_slab") == 0) {
     if (value < 0) return fail(c, LBM_EINVAL, "hrr_slab must be >= 0");
     c->hrr_slab = static_cast<int>(value);
+    c->epoch++;
+    return LBM_OK;
+  }
+  if (std::strcmp(key, "inplace") == 0) {
+    if (value != 0 && value != 1) return fail(c, LBM_EINVAL, "inplace must be 0 or 1");
+    c->inplace = static_cast<int>(value);
     c->epoch++;
     return LBM_OK;
   }

@@ -12,7 +12,8 @@
 
 enum Phase { PHASE_NONE = 0,   // no state yet
              PHASE_PRE = 1,    // cur holds S_t (pre-collision), as handed in
-             PHASE_POST = 2 }; // cur holds F_{t-1} (post-collision, not yet streamed); S_t = stream(F_{t-1})
+             PHASE_POST = 2,   // cur holds F_{t-1} (post-collision, not yet streamed); S_t = stream(F_{t-1})
+             PHASE_SWAPPED = 3 }; // in-place (AA) stepping after an odd number of steps: cur holds F_{t-1,i}(x) in slot opp(i)
 
 constexpr int LBM_TOT_SLOTS = 256;      // partial-sum slots of the totals reduction (spreads the atomics)
 constexpr int LBM_GRAPH_CHUNK = 8;      // time steps per captured CUDA graph (even: lattice roles and sweep direction return)
@@ -86,6 +87,7 @@ struct lbm_ctx {
   int serpentine;        // 1: consecutive launches sweep z in opposite directions (L2 reuse)
   long long sweep_count; // BGK steps launched so far (parity = direction)
   int hrr_slab;          // HRR form: z-slices per slab of the two-pass step (0 = whole lattice)
+  int inplace;           // 1: lattices without any boundary cell step in place (AA pattern), one lattice (option "inplace")
   int wm_prepass;        // 1: wall-model cells run in the vector path, u^B from a pre-pass over their compact list (default)
   int use_pdl;           // programmatic dependent launch of the time-loop kernels: 0 off, 1 every thread waits for the predecessor,
                          // 2 (default) after the wall-model pre-pass only the threads that read its output wait
@@ -122,5 +124,7 @@ template <int Q, typename T> int launch_step_hrr(lbm_ctx* c, const lbm_params* p
 template <int Q, typename T> int launch_moments(lbm_ctx* c, const lbm_params* p, void* rho, void* u);
 template <int Q, typename T> int launch_totals(lbm_ctx* c, const lbm_params* p);
 template <int Q, typename T> int launch_init(lbm_ctx* c, const void* rho, const void* u);
+// in-place AA pattern: kind 0 even step, 1 odd step, 2 un-swap into the other lattice (which becomes current)
+template <int Q, typename T> int launch_aa(lbm_ctx* c, const lbm_params* p, int kind);
 
 }  // namespace lbmhost

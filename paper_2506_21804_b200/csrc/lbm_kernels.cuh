@@ -1106,18 +1106,19 @@ __device__ __forceinline__ void step_vec_body(const StepArgs<T>& a, double (&acc
 
   T f[Q][V];
   T d[V];
+  uint32_t nbm[V];
 #pragma unroll
-  for (int v = 0; v < V; ++v) d[v] = T(0);
+  for (int v = 0; v < V; ++v) { d[v] = T(0); nbm[v] = 0u; }
+  // porosity vector and the per-cell SOLID-neighbour masks of a solid-adjacent vector (one aligned 128 / 64-bit load each), issued
+  // BEFORE the population loads (issued after them -- to take the wait for the class bytes out of the chain class bytes -> masks
+  // -> populations -> own-cell loads that ncu shows on the ADJ warps of config 4 -- every workload ran 1 - 14 % slower: measured,
+  // DESIGN.md 5.2)
   if (mode_hlbm(MODE) && mine && a.d != nullptr) {
     T dv[V];
     ld_vec_keep(a.d + self, dv);
 #pragma unroll
     for (int v = 0; v < V; ++v) d[v] = dv[v];
   }
-  // per-cell SOLID-neighbour masks of a solid-adjacent vector (one aligned 128 / 64-bit load)
-  uint32_t nbm[V];
-#pragma unroll
-  for (int v = 0; v < V; ++v) nbm[v] = 0u;
   if (adj) ld_nbmask(a.nbmask + self, nbm);
   // row offsets of the (dy, dz) neighbour rows; all deltas fit 32 bits because N < 2^31
   const int ym = (y == 0) ? ny - 1 : y - 1, yp = (y >= ny - 1) ? 0 : y + 1;
@@ -1138,29 +1139,32 @@ __device__ __forceinline__ void step_vec_body(const StepArgs<T>& a, double (&acc
       if (mine) ld_uhat_nb<T, V>(a.uhat + self, N, dyp, dym, dzp, dzm, exl, exr, gu, gl, gr);
     }
   } else {
+    // phase 1: issue every load before anything consumes one (in-order issue: a shuffle placed right
+    // after its load would serialise the loads).  One running pointer per population (+N each).
+    T e[Q];   // the one element a shifted row needs from outside the warp / row (edge lanes only)
+    auto issue_loads = [&](const bool ld, const bool el, const bool er) {
+      const T* pself = a.fin + self;
+#pragma unroll
+      for (int i = 0; i < Q; ++i) {
+        const long long off = static_cast<long long>((L.c[i][1] == 0) ? 0 : ((L.c[i][1] == 1) ? dym : dyp)) +
+                              static_cast<long long>((L.c[i][2] == 0) ? 0 : ((L.c[i][2] == 1) ? dzm : dzp));
+        const T* src = pself + off;                            // source row, at the vector's x
+        pself += N;
+#pragma unroll
+        for (int v = 0; v < V; ++v) f[i][v] = T(0);
+        e[i] = T(0);
+        if (ld) ld_vec(src, f[i]);
+        if (L.c[i][0] == 1 && el) e[i] = __ldg(src + exl);
+        if (L.c[i][0] == -1 && er) e[i] = __ldg(src + exr);
+      }
+    };
     // a vector that is SOLID throughout loads nothing, but the rows its neighbour pulls from (y -+ 1, z -+ 1) may be
     // fluid at its end cells: that neighbour fetches the one element itself, like a lane at the edge of the warp
     const bool solid_l = __shfl_up_sync(FULL, all_solid ? 1 : 0, 1) != 0;
     const bool solid_r = __shfl_down_sync(FULL, all_solid ? 1 : 0, 1) != 0;
     const bool edge_l = doload && ((lane == 0) || (tx == 0) || solid_l);
     const bool edge_r = doload && ((lane == 31) || (tx == static_cast<int>(blockDim.x) - 1) || (qx == nvec - 1) || solid_r);
-    // phase 1: issue every load before anything consumes one (in-order issue: a shuffle placed right
-    // after its load would serialise the loads).  One running pointer per population (+N each).
-    const T* pself = a.fin + self;
-    T e[Q];   // the one element a shifted row needs from outside the warp / row (edge lanes only)
-#pragma unroll
-    for (int i = 0; i < Q; ++i) {
-      const long long off = static_cast<long long>((L.c[i][1] == 0) ? 0 : ((L.c[i][1] == 1) ? dym : dyp)) +
-                            static_cast<long long>((L.c[i][2] == 0) ? 0 : ((L.c[i][2] == 1) ? dzm : dzp));
-      const T* src = pself + off;                            // source row, at the vector's x
-      pself += N;
-#pragma unroll
-      for (int v = 0; v < V; ++v) f[i][v] = T(0);
-      e[i] = T(0);
-      if (doload) ld_vec(src, f[i]);
-      if (L.c[i][0] == 1 && edge_l) e[i] = __ldg(src + exl);
-      if (L.c[i][0] == -1 && edge_r) e[i] = __ldg(src + exr);
-    }
+    issue_loads(doload, edge_l, edge_r);
     if constexpr (HRR) {
       if (mine) ld_uhat_nb<T, V>(a.uhat + self, N, dyp, dym, dzp, dzm, exl, exr, gu, gl, gr);
     }
@@ -1382,6 +1386,191 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
     reduce_totals(acc, a.tot_slots, a.tot_nslots, a.tot_ticket, a.tot_out);
   } else {
     step_vec_body<Q, T, MODE, COLL, MW>(a, acc, static_cast<int>(blockIdx.z));
+  }
+}
+
+// ---- in-place propagation, AA pattern (one lattice) -- the propagation bake-off of DESIGN.md section 4 --------------------
+// Lattices without a single wall / inlet / outlet / wall-model cell only (fully periodic bulk), BGK form.  Two alternating
+// kernels on ONE array a[Q][N]:
+//   even step (array holds S_t as a[i][x] = f_i(x,t)):           read a[i][x], collide, write F_i(x) to a[opp(i)][x]  -- all local;
+//   odd step  (array holds F_t with swapped slots):               read S_{t+1,i}(x) = a[opp(i)][x - c_i], collide, write
+//             F_{t+1,j}(x) to a[j][x + c_j], the slot and cell the value of direction opp(j) was read from: afterwards the
+//             array holds S_{t+2} in the plain layout.
+// Every location is read and written by the same cell, so one array suffices.  The vector form keeps all global accesses
+// aligned: the thread that loads the aligned vector (slot, row, x0) is the one that stores it; the c_x = +-1 shift is a warp
+// shuffle on the way in and on the way out, and at warp edges one scalar load on the way in and a shared-memory hand-over on
+// the way out.  A block covers whole rows in x, so the one __syncthreads between the load phase and the store phase orders
+// the edge loads of a thread before the stores of its x-neighbours.
+template <typename T>
+struct AAArgs {
+  T* __restrict__ a;               // [Q][N], updated in place
+  const T* __restrict__ d;         // porosity or nullptr
+  const T* __restrict__ ub;        // solid velocity [3][N] or nullptr
+  int nx, ny, nz;
+  long long N;
+  T tau0, smago_k, fringe_k;
+  int fringe_x0;
+};
+
+template <int Q, typename T>
+__device__ __forceinline__ void aa_collide_vec(const AAArgs<T>& a, long long self, int x0, T (&f)[Q][VecOf<Q, T, COLL_BGK>::V]) {
+  constexpr int V = VecOf<Q, T, COLL_BGK>::V;
+  T d[V];
+#pragma unroll
+  for (int v = 0; v < V; ++v) d[v] = T(0);
+  if (a.d != nullptr) ld_vec_keep(a.d + self, d);
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    T fc[Q];
+#pragma unroll
+    for (int i = 0; i < Q; ++i) fc[i] = f[i][v];
+    T ubx, uby, ubz;
+    body_velocity<T>(a.ub == nullptr ? nullptr : a.ub + self + v, a.N, d[v], ubx, uby, ubz);
+    const int xd = (x0 + v > a.fringe_x0) ? x0 + v - a.fringe_x0 : 0;
+    collide_cell<Q, T>(fc, d[v], ubx, uby, ubz, a.tau0 + a.fringe_k * static_cast<T>(xd * xd), a.smago_k);
+#pragma unroll
+    for (int i = 0; i < Q; ++i) f[i][v] = fc[i];
+  }
+}
+
+// grid (ceil(nvec / bx), ceil(ny / by), nz), block (bx, by)
+template <int Q, typename T>
+__global__ void __launch_bounds__(256, 2) k_aa_even(const __grid_constant__ AAArgs<T> a) {
+  constexpr Stencil<Q> L{};
+  constexpr int V = VecOf<Q, T, COLL_BGK>::V;
+  const int qx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int y = blockIdx.y * blockDim.y + threadIdx.y;
+  const int z = blockIdx.z;
+  if (qx >= a.nx / V || y >= a.ny) return;
+  const int x0 = qx * V;
+  const long long self = (static_cast<long long>(z) * a.ny + y) * a.nx + x0;
+  T f[Q][V];
+  T* p = a.a + self;
+#pragma unroll
+  for (int i = 0; i < Q; ++i) ld_vec(p + i * a.N, f[i]);
+  aa_collide_vec<Q, T>(a, self, x0, f);
+#pragma unroll
+  for (int i = 0; i < Q; ++i) st_vec(p + L.opp[i] * a.N, f[i]);
+}
+
+// grid (1, ceil(ny / by), nz), block (nvec, by): whole rows in x (nvec = nx / V a multiple of 32, nvec * by <= 256)
+template <int Q, typename T>
+__global__ void __launch_bounds__(256, 2) k_aa_odd(const __grid_constant__ AAArgs<T> a) {
+  constexpr Stencil<Q> L{};
+  constexpr int V = VecOf<Q, T, COLL_BGK>::V;
+  constexpr unsigned FULL = 0xffffffffu;
+  constexpr int NXP = (Q == 19) ? 5 : 9;                  // populations with c_x = +1 (and as many with c_x = -1)
+  __shared__ T edge_r[NXP][8];                           // F_j of the LAST cell of every warp, j with c_x = +1 (goes to the next warp)
+  __shared__ T edge_l[NXP][8];                           // F_j of the FIRST cell of every warp, j with c_x = -1 (goes to the previous warp)
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  const int lane = tx & 31;
+  const int wrow = blockDim.x >> 5;                       // warps per row
+  const int warp = ty * wrow + (tx >> 5);                 // warp of the block (rows are whole warps)
+  const int y = blockIdx.y * blockDim.y + ty;
+  const int z = blockIdx.z;
+  const bool active = y < a.ny;
+  const int nx = a.nx, ny = a.ny, nz = a.nz;
+  const long long N = a.N;
+  const int x0 = tx * V;
+  const int yy = active ? y : 0;
+  const long long self = (static_cast<long long>(z) * ny + yy) * nx + x0;
+  const int ym = (yy == 0) ? ny - 1 : yy - 1, yp = (yy >= ny - 1) ? 0 : yy + 1;
+  const int zm = (z == 0) ? nz - 1 : z - 1, zp = (z == nz - 1) ? 0 : z + 1;
+  const int dym = (ym - yy) * nx, dyp = (yp - yy) * nx;
+  const int plane = nx * ny;
+  const int dzm = (zm - z) * plane, dzp = (zp - z) * plane;
+  const int exl = ((x0 == 0) ? nx - 1 : x0 - 1) - x0, exr = ((x0 + V >= nx) ? 0 : x0 + V) - x0;
+  T f[Q][V], e[Q];
+  // load phase: S_{t+1,i}(x) = a[opp(i)][x - c_i]: the aligned vector of the source row, realigned by one element for c_x = +-1
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    const long long off = static_cast<long long>((L.c[i][1] == 0) ? 0 : ((L.c[i][1] == 1) ? dym : dyp)) +
+                          static_cast<long long>((L.c[i][2] == 0) ? 0 : ((L.c[i][2] == 1) ? dzm : dzp));
+    const T* src = a.a + L.opp[i] * N + self + off;
+#pragma unroll
+    for (int v = 0; v < V; ++v) f[i][v] = T(0);
+    e[i] = T(0);
+    if (active) ld_vec(src, f[i]);
+    if (L.c[i][0] == 1 && active && lane == 0) e[i] = __ldg(src + exl);
+    if (L.c[i][0] == -1 && active && lane == 31) e[i] = __ldg(src + exr);
+  }
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    if (L.c[i][0] == 1) {
+      T nb = __shfl_up_sync(FULL, f[i][V - 1], 1);
+      if (lane == 0) nb = e[i];
+#pragma unroll
+      for (int v = V - 1; v > 0; --v) f[i][v] = f[i][v - 1];
+      f[i][0] = nb;
+    } else if (L.c[i][0] == -1) {
+      T nb = __shfl_down_sync(FULL, f[i][0], 1);
+      if (lane == 31) nb = e[i];
+#pragma unroll
+      for (int v = 0; v < V - 1; ++v) f[i][v] = f[i][v + 1];
+      f[i][V - 1] = nb;
+    }
+  }
+  if (active) aa_collide_vec<Q, T>(a, self, x0, f);
+  // store phase: F_j(x) goes to a[j][x + c_j]; the aligned vector (j, row + (c_y, c_z), x0) takes F_j(x - c_x)
+  {
+    int kp = 0, km = 0;
+#pragma unroll
+    for (int j = 0; j < Q; ++j) {
+      if (L.c[j][0] == 1) { if (lane == 31) edge_r[kp][warp] = f[j][V - 1]; ++kp; }
+      else if (L.c[j][0] == -1) { if (lane == 0) edge_l[km][warp] = f[j][0]; ++km; }
+    }
+  }
+  __syncthreads();                                       // every load of the block is done; the edge values are in place
+  {
+    const int wl = ty * wrow + (((tx >> 5) == 0) ? wrow - 1 : (tx >> 5) - 1);          // previous / next warp of the row (periodic)
+    const int wr = ty * wrow + (((tx >> 5) == wrow - 1) ? 0 : (tx >> 5) + 1);
+    int kp = 0, km = 0;
+#pragma unroll
+    for (int j = 0; j < Q; ++j) {
+      const long long off = static_cast<long long>((L.c[j][1] == 0) ? 0 : ((L.c[j][1] == 1) ? dyp : dym)) +
+                            static_cast<long long>((L.c[j][2] == 0) ? 0 : ((L.c[j][2] == 1) ? dzp : dzm));
+      T* dst = a.a + j * N + self + off;
+      T o[V];
+      if (L.c[j][0] == 1) {
+        T nb = __shfl_up_sync(FULL, f[j][V - 1], 1);
+        if (lane == 0) nb = edge_r[kp][wl];
+        ++kp;
+#pragma unroll
+        for (int v = V - 1; v > 0; --v) o[v] = f[j][v - 1];
+        o[0] = nb;
+      } else if (L.c[j][0] == -1) {
+        T nb = __shfl_down_sync(FULL, f[j][0], 1);
+        if (lane == 31) nb = edge_l[km][wr];
+        ++km;
+#pragma unroll
+        for (int v = 0; v < V - 1; ++v) o[v] = f[j][v + 1];
+        o[V - 1] = nb;
+      } else {
+#pragma unroll
+        for (int v = 0; v < V; ++v) o[v] = f[j][v];
+      }
+      if (active) st_vec(dst, o);
+    }
+  }
+}
+
+// the state S_{t+1} out of an array that holds F_t with swapped slots: out[i][x] = a[opp(i)][x - c_i] (materialisation; off the
+// timed path: one thread per value)
+template <int Q, typename T>
+__global__ void __launch_bounds__(256) k_aa_unswap(const T* __restrict__ a, T* __restrict__ out, int nx, int ny, int nz, long long N) {
+  constexpr Stencil<Q> L{};
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  const int y = blockIdx.y * blockDim.y + threadIdx.y;
+  const int z = blockIdx.z;
+  if (x >= nx || y >= ny) return;
+  const long long self = cell_index(x, y, z, nx, ny);
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    int sx = x - L.c[i][0], sy = y - L.c[i][1], sz = z - L.c[i][2];
+    sx = (sx < 0) ? sx + nx : ((sx >= nx) ? sx - nx : sx);
+    sy = (sy < 0) ? sy + ny : ((sy >= ny) ? sy - ny : sy);
+    sz = (sz < 0) ? sz + nz : ((sz >= nz) ? sz - nz : sz);
+    out[i * N + self] = a[L.opp[i] * N + cell_index(sx, sy, sz, nx, ny)];
   }
 }
 

@@ -302,6 +302,45 @@ int launch_step_hrr(lbm_ctx* c, const lbm_params* p, int mode, int stage) {
 }
 #endif
 
+#if LBM_INST_PART == 3
+// In-place AA pattern (propagation bake-off): one launch per step on the current lattice alone.
+// odd = 0: even step (plain layout -> swapped slots), 1: odd step (swapped -> plain), 2: un-swap into the other lattice.
+template <int Q, typename T>
+int launch_aa(lbm_ctx* c, const lbm_params* p, int kind) {
+  constexpr int V = lbm::VecOf<Q, T, lbm::COLL_BGK>::V;
+  if (kind == 2) {
+    dim3 grid, block;
+    launch_dims(c, grid, block);
+    lbm::k_aa_unswap<Q, T><<<grid, block, 0, c->stream>>>(static_cast<const T*>(c->f[c->cur]), static_cast<T*>(c->f[1 - c->cur]), c->nx, c->ny, c->nz, c->N);
+    LBM_CUDA(c, cudaGetLastError());
+    c->launches++;
+    c->cur = 1 - c->cur;
+    return LBM_OK;
+  }
+  lbm::StepArgs<T> sa = make_args<T>(c, p, c->cur, c->cur);
+  lbm::AAArgs<T> a;
+  a.a = static_cast<T*>(c->f[c->cur]);
+  a.d = sa.d;  a.ub = sa.ub;
+  a.nx = c->nx;  a.ny = c->ny;  a.nz = c->nz;  a.N = c->N;
+  a.tau0 = sa.tau0;  a.smago_k = sa.smago_k;  a.fringe_k = sa.fringe_k;  a.fringe_x0 = sa.fringe_x0;
+  const int nvec = c->nx / V;
+  if (kind == 0) {
+    dim3 grid, block;
+    launch_dims_vec<Q, T, lbm::COLL_BGK>(c, grid, block);
+    lbm::k_aa_even<Q, T><<<grid, block, 0, c->stream>>>(a);
+  } else {
+    int by = 64 / nvec;
+    if (by < 1) by = 1;
+    dim3 block(nvec, by, 1), grid(1, (c->ny + by - 1) / by, c->nz);
+    lbm::k_aa_odd<Q, T><<<grid, block, 0, c->stream>>>(a);
+  }
+  LBM_CUDA(c, cudaGetLastError());
+  c->launches++;
+  c->sweep_count++;
+  return LBM_OK;
+}
+#endif
+
 #if LBM_INST_PART == 2
 // A9: rho, u of S_t for every cell: one launch of the step kernel in its moments mode (the pull happens in registers; the
 // stored lattice and the phase stay as they are) + the wall cells' own values from their side buffer.
