@@ -171,7 +171,7 @@ int lbm_get_inflow(lbm_ctx* ctx, void* u);
  * compact list of WALLMODEL cells when wm_enable and such cells exist (3 values of dtype per cell of device memory for
  * their u^B, allocated on the first such step).  HRR form: two launches per step (u^ pass, then the fused step;
  * DESIGN.md 5.5) and 3 more values of dtype per cell (allocated on the first HRR step; LBM_ENOMEM if that fails).
- * Steady-state steps are replayed 8 at a time from a captured CUDA graph (option "cuda_graph").  Asynchronous.
+ * With option "cuda_graph" steady-state steps are replayed 8 at a time from a captured CUDA graph.  Asynchronous.
  * Errors: LBM_EINVAL (NULL ctx/params, n_steps < 0, tau0 <= 0.5, cs_smago < 0, wm_enable with
  * wm_kappa <= 0 or wm_E <= 0, collision not 0/1, sigma outside [0,1] with HRR, rho_out < 0, fringe_len < 0, fringe_factor < 0), LBM_ESTATE (no state
  * set yet), LBM_ECUDA. */
@@ -278,9 +278,11 @@ long long lbm_query(const lbm_ctx* ctx, int what);
 
 /* Tuning knobs.  None changes a result (the A/B tests compare populations bit for bit).  Returns LBM_EINVAL for an
  * unknown key or value, LBM_ESTATE where noted.  Keys (every key the library accepts is listed here):
- *   "cuda_graph"    0|1     1 (default): lbm_step replays the steady-state time loop 8 steps at a time from a captured CUDA
- *                           graph (re-captured when parameters, fields or options change); steps that do not fill a chunk, the
- *                           first step of a fresh state and runs with the Vortex Method inlet use plain launches
+ *   "cuda_graph"    0|1     1: lbm_step replays the steady-state time loop 8 steps at a time from a captured CUDA graph
+ *                           (re-captured when parameters, fields or options change); steps that do not fill a chunk, the first
+ *                           step of a fresh state, runs with the Vortex Method inlet and sub-domains use plain launches.
+ *                           Default 0: beside "pdl" it measured neutral (config 1: 4.4 -> 4.2 us per step, everything else
+ *                           within noise), and a capture that lands in a caller's timed region costs more than it wins
  *   "pdl"           0|1|2   programmatic dependent launch of the time-loop kernels: 0 plain launches; 1 every kernel becomes
  *                           resident while its predecessor drains and waits for it; 2 (default) additionally, after the
  *                           wall-model pre-pass only the threads that read its output wait for it

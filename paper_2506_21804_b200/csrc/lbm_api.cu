@@ -377,7 +377,7 @@ lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype) {
   c->serpentine = 1;
   c->wm_prepass = 1;
   c->use_pdl = 2;
-  c->use_graph = 1;
+  c->use_graph = 0;
   c->last = default_params();
   std::snprintf(c->err, sizeof(c->err), "no error");
   const size_t pop = static_cast<size_t>(lattice) * N * dtype;
@@ -656,7 +656,8 @@ int lbm_get_inflow(lbm_ctx* c, void* u) {
   return LBM_OK;
 }
 
-// ---- CUDA graphs ("cuda_graph", default on): the steady-state time loop is replayed in chunks of LBM_GRAPH_CHUNK steps from a
+// ---- CUDA graphs ("cuda_graph", default off: measured neutral beside programmatic dependent launch, and a capture inside a
+// caller's timed region costs more than it can win): the steady-state time loop is replayed in chunks of LBM_GRAPH_CHUNK steps from a
 // captured graph (one graph launch instead of 8 .. 24 kernel launches: matters where a step is shorter than its launches, i.e.
 // small lattices and the three-launch steps of the lid-driven cavity).  A chunk is an even number of steps, so the lattice roles
 // and the sweep direction are back where they started; one graph per (current lattice, sweep parity), re-captured when the

@@ -61,7 +61,7 @@ struct lbm_ctx {
   cudaStream_t stream;
   int block_threads;
   int use_vector;        // 1: 128-bit vector kernel when nx % (32/dtype) == 0 (default); 0: scalar kernel
-  int use_graph;         // 1: lbm_step replays captured CUDA graphs of LBM_GRAPH_CHUNK steps (default)
+  int use_graph;         // 1: lbm_step replays captured CUDA graphs of LBM_GRAPH_CHUNK steps (default 0)
   cudaStream_t cap_stream;   // capture happens on a private stream (the caller's may be the legacy default stream)
   lbm_graph_entry graphs[LBM_GRAPH_CACHE];
   long long epoch;       // bumped whenever something baked into a captured graph changes (geometry, fields, options)

@@ -83,6 +83,7 @@ def test_graph_is_recaptured_when_parameters_or_fields_change():
     p2 = dict(cfg["params"], tau0=0.56, cs_smago=0.15)
     d2 = np.where(d > 0, 0.5 * d, d)
     with P.LBM(19, nx, ny, nz, "f64") as sim:
+        sim.set_option("cuda_graph", 1)
         sim.set_fields(f, d, cfg["flags"])
         sim.step(17, P.LbmParams(**p1))
         g1 = sim.query("graph_launches")
