@@ -79,13 +79,12 @@ WORKLOADS["config3_urban_channel_384x192x128_f32_hrr_body"] = (3, None, "f32", H
 WORKLOADS["paperbc_wmfaces_urban_channel_384x192x128_f32_vm"] = (8, (128, 192, 384), "f32", {}, VM)
 WORKLOADS["paperbc_wmfaces_urban_channel_384x192x128_f32_hrr_vm"] = (8, (128, 192, 384), "f32", HRR, VM)
 # propagation bake-off: the fully periodic LES box of config 2 on two lattices (pull) and in place (AA pattern,
-# option "inplace"); 896^3 fp64 is the size only the one-lattice scheme holds (109 GB per population set)
+# option "inplace"); at 768^3 fp64 one population set is 68.9 GB
 INPLACE = dict(inplace=1)
 WORKLOADS["config2_les_periodic_256_f32_inplace"] = (2, None, "f32", {}, None, None, INPLACE)
 for _n, _t in ((512, "f32"), (768, "f64")):
     WORKLOADS["config2_les_periodic_%d_%s" % (_n, _t)] = (2, (_n, _n, _n), _t)
     WORKLOADS["config2_les_periodic_%d_%s_inplace" % (_n, _t)] = (2, (_n, _n, _n), _t, {}, None, None, INPLACE)
-WORKLOADS["config2_les_periodic_896_f64_inplace"] = (2, (896, 896, 896), "f64", {}, None, None, INPLACE)
 DEFAULT_WORKLOAD = "config3_urban_channel_384x192x128_f32"
 
 

@@ -272,7 +272,7 @@ const char* lbm_last_error(const lbm_ctx* ctx);
  *   6 cells handled by the list blocks of the vector kernel (SPECIAL cells + their sector mates)
  *   7 CUDA graph launches so far                       8 WALLMODEL cells (length of the pre-pass list)
  *   9 values of a populations face buffer (halo)        10 values of a u^ face buffer (halo)
- *   11 interior z-slices (nz minus the ghost slices)
+ *   11 interior z-slices (nz minus the ghost slices)   12 cells with a slip plane code (slip-adjacent cells in the vector path)
  * Returns -1 for an unknown `what` or a NULL ctx. */
 long long lbm_query(const lbm_ctx* ctx, int what);
 
@@ -289,6 +289,10 @@ long long lbm_query(const lbm_ctx* ctx, int what);
  *   "wm_prepass"    0|1     1 (default): WALLMODEL cells run in the vector path, their u^B comes from a pre-pass over their
  *                           compact list; 0: they are solved cell by cell in the list blocks of the step kernel.  Decides how
  *                           flags are classified: LBM_ESTATE once a state or geometry has been set
+ *   "slip_planes"   0|1     1 (default): cells next to ONE plane slip wall normal to y or z (and nothing else that complicates the
+ *                           specular pull) run in the vector path, pulling the reflected populations from their own plane; 0: every
+ *                           cell next to a slip wall is handled cell by cell in the list blocks.  Decides how flags are
+ *                           classified: LBM_ESTATE once a state or geometry has been set
  *   "serpentine"    0|1     consecutive launches sweep the z-slices in opposite directions for L2 reuse (default 1)
  *   "inplace"       0|1     1: a lattice without a single wall / inlet / outlet / wall-model cell (fully periodic bulk), BGK form,
  *                           steps IN PLACE on one array (AA pattern: even steps collide locally into the opposite slots, odd

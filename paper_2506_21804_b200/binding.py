@@ -245,7 +245,7 @@ def lbm_set_option(ctx, key, value):
 class LBM:
     """Convenience owner of one lbm_ctx (still marshalling only)."""
     QUERY = dict(steps=0, launches=1, cells=2, solid_cells=3, device_bytes=4, masked_cells=5, list_cells=6, graph_launches=7,
-                 wallmodel_cells=8, halo_population_values=9, halo_uhat_values=10, interior_slices=11)
+                 wallmodel_cells=8, halo_population_values=9, halo_uhat_values=10, interior_slices=11, slip_plane_cells=12)
 
     def __init__(self, lattice, nx, ny, nz, dtype="f32", stream=None):
         self.Q, self.nx, self.ny, self.nz = lattice, nx, ny, nz

@@ -189,8 +189,9 @@ int classify(lbm_ctx* c, const uint8_t* cell_flags) {
   dim3 grid, block;
   launch_dims(c, grid, block);
   const int wm_special = c->wm_prepass ? 0 : 1;
-  if (c->Q == 19) lbm::k_classify<19><<<grid, block, 0, c->stream>>>(c->flags_raw, c->cls_alt, c->nx, c->ny, c->nz, c->counters, wm_special);
-  else            lbm::k_classify<27><<<grid, block, 0, c->stream>>>(c->flags_raw, c->cls_alt, c->nx, c->ny, c->nz, c->counters, wm_special);
+  const int slip_planes = c->slip_planes;
+  if (c->Q == 19) lbm::k_classify<19><<<grid, block, 0, c->stream>>>(c->flags_raw, c->cls_alt, c->nx, c->ny, c->nz, c->counters, wm_special, slip_planes);
+  else            lbm::k_classify<27><<<grid, block, 0, c->stream>>>(c->flags_raw, c->cls_alt, c->nx, c->ny, c->nz, c->counters, wm_special, slip_planes);
   LBM_CUDA(c, cudaGetLastError());
   c->launches++;
   unsigned long long h[8];
@@ -212,6 +213,11 @@ int classify(lbm_ctx* c, const uint8_t* cell_flags) {
   if (c->nx % SV == 0) {
     const long long nsec = c->N / SV;
     const unsigned blocks = static_cast<unsigned>((nsec + 255) / 256);
+    if (h[7] != 0) {                   // cells with a slip plane code: the cells of a sector must agree (vector path)
+      if (SV == 8) lbm::k_slip_uniform<8><<<blocks, 256, 0, c->stream>>>(c->cls_alt, nsec, c->counters);
+      else         lbm::k_slip_uniform<4><<<blocks, 256, 0, c->stream>>>(c->cls_alt, nsec, c->counters);
+      c->launches++;
+    }
     if (SV == 8) lbm::k_mark_list<8><<<blocks, 256, 0, c->stream>>>(c->cls_alt, c->flags_raw, nsec, c->counters);
     else         lbm::k_mark_list<4><<<blocks, 256, 0, c->stream>>>(c->cls_alt, c->flags_raw, nsec, c->counters);
     cudaError_t e = cudaGetLastError();
@@ -261,6 +267,7 @@ int classify(lbm_ctx* c, const uint8_t* cell_flags) {
   c->n_masked = static_cast<long long>(h[2]);
   c->n_moving = static_cast<long long>(h[4]);
   c->n_slip = static_cast<long long>(h[5]);
+  c->n_slipcode = static_cast<long long>(h[7]);
   c->epoch++;
   return LBM_OK;
 }
@@ -376,6 +383,7 @@ lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype) {
   c->use_vector = 1;
   c->serpentine = 1;
   c->wm_prepass = 1;
+  c->slip_planes = 1;
   c->use_pdl = 2;
   c->use_graph = 0;
   c->last = default_params();
@@ -1099,6 +1107,7 @@ long long lbm_query(const lbm_ctx* c, int what) {
     case 9: return static_cast<long long>(c->Q == 19 ? 5 : 9) * c->nx * c->ny;
     case 10: return 3ll * c->nx * c->ny;
     case 11: return c->nz - c->ghost_lo - c->ghost_hi;
+    case 12: return c->n_slipcode;
     default: return -1;
   }
 }
@@ -1122,6 +1131,14 @@ int lbm_set_option(lbm_ctx* c, const char* key, long long value) {
     if (c->phase != PHASE_NONE || c->n_wm > 0)
       return fail(c, LBM_ESTATE, "wm_prepass decides how the flags are classified: set it before lbm_set_fields / lbm_set_geometry");
     c->wm_prepass = static_cast<int>(value);
+    c->epoch++;
+    return LBM_OK;
+  }
+  if (std::strcmp(key, "slip_planes") == 0) {
+    if (value != 0 && value != 1) return fail(c, LBM_EINVAL, "slip_planes must be 0 or 1");
+    if (c->phase != PHASE_NONE || c->n_slip > 0)
+      return fail(c, LBM_ESTATE, "slip_planes decides how the flags are classified: set it before lbm_set_fields / lbm_set_geometry");
+    c->slip_planes = static_cast<int>(value);
     c->epoch++;
     return LBM_OK;
   }

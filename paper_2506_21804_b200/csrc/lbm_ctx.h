@@ -51,6 +51,7 @@ struct lbm_ctx {
   int* list_count_dev;
   unsigned long long* counters;  // device [8]
   long long n_moving, n_slip;    // MOVINGWALL / SLIPWALL cells of the accepted geometry
+  long long n_slipcode;          // cells next to a plane slip wall that run in the vector path (slip plane code in their class byte)
   double* totals_dev;            // device [5] result + [LBM_TOT_SLOTS][5] partial sums + ticket counter
   void* staging;         // host<->device bounce buffer, grown on demand
   size_t staging_bytes;
@@ -88,6 +89,7 @@ struct lbm_ctx {
   long long sweep_count; // BGK steps launched so far (parity = direction)
   int hrr_slab;          // HRR form: z-slices per slab of the two-pass step (0 = whole lattice)
   int inplace;           // 1: lattices without any boundary cell step in place (AA pattern), one lattice (option "inplace")
+  int slip_planes;       // 1: cells next to a plane slip wall normal to y or z get a slip plane code and run in the vector path (default)
   int wm_prepass;        // 1: wall-model cells run in the vector path, u^B from a pre-pass over their compact list (default)
   int use_pdl;           // programmatic dependent launch of the time-loop kernels: 0 off, 1 every thread waits for the predecessor,
                          // 2 (default) after the wall-model pre-pass only the threads that read its output wait

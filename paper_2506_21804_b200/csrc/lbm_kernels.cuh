@@ -15,6 +15,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 namespace lbm {
 
 enum : int { T_FLUID = 0, T_SOLID = 1, T_INLET = 2, T_OUTLET = 3, T_WM = 4, T_MOVING = 5, T_POUTLET = 6, T_SLIP = 7 };
@@ -95,6 +97,32 @@ __host__ __device__ constexpr T weight(int c2) {
   return (Q == 19) ? (c2 == 0 ? T(1.0 / 3.0) : (c2 == 1 ? T(1.0 / 18.0) : T(1.0 / 36.0)))
                    : (c2 == 0 ? T(8.0 / 27.0) : (c2 == 1 ? T(2.0 / 27.0) : (c2 == 2 ? T(1.0 / 54.0) : T(1.0 / 216.0))));
 }
+
+// Slip plane code of a cell (bits 3-5 of the class byte of a cell that is not a WALLMODEL cell; 0 = none): the cell lies next to ONE
+// plane slip wall normal to y or z and nothing else complicates its specular pull (reading G37): 2 = wall at y-1 (normal +y),
+// 3 = wall at y+1, 4 = wall at z-1, 5 = wall at z+1 -- the numbering of the wall-normal codes.  For such a cell the population i
+// with c_i . n = +1 is pulled as the population with the n-component of c_i reversed from the cell x - c_i + n of its OWN plane:
+// a different source row and slot, but the same aligned access pattern, so these cells run in the vector path (kernel variant
+// WV bit 1) instead of the per-cell list path.  Everything less regular (edges, corners, wall-model cells at a slip wall, slip walls
+// normal to x, a sector whose cells disagree) keeps the SPECIAL bit and the general rule slip_pull.
+__host__ __device__ constexpr int slip_axis(int code) { return code >> 1; }                  // 1 = y, 2 = z
+__host__ __device__ constexpr int slip_sign(int code) { return (code & 1) ? -1 : 1; }        // of the normal (wall -> fluid)
+// population index of c_i with its y (my) or z (mz) component reversed
+template <int Q>
+struct Mirror {
+  int my[Q], mz[Q];      // ... reversed
+  int zy[Q], zz[Q];      // ... set to zero (0 = the rest population: the cell itself)
+  constexpr Mirror() : my{}, mz{}, zy{}, zz{} {
+    constexpr Stencil<Q> L{};
+    for (int i = 0; i < Q; ++i)
+      for (int k = 0; k < Q; ++k) {
+        if (L.c[k][0] == L.c[i][0] && L.c[k][1] == -L.c[i][1] && L.c[k][2] == L.c[i][2]) my[i] = k;
+        if (L.c[k][0] == L.c[i][0] && L.c[k][1] == L.c[i][1] && L.c[k][2] == -L.c[i][2]) mz[i] = k;
+        if (L.c[k][0] == L.c[i][0] && L.c[k][1] == 0 && L.c[k][2] == L.c[i][2]) zy[i] = k;
+        if (L.c[k][0] == L.c[i][0] && L.c[k][1] == L.c[i][1] && L.c[k][2] == 0) zz[i] = k;
+      }
+  }
+};
 
 // Moving-wall bounce-back (reading G33; lid of the lid-driven cavity): the population i that returns
 // from a wall moving with u_w gains 2 w_i rho_w (c_i . u_w) / c_s^2 = 6 w_i (c_i . u_w), rho_w = 1, c_i = wall -> fluid.
@@ -615,11 +643,23 @@ __device__ __forceinline__ void pull_cell(const StepArgs<T>& a, int x, int y, in
   const int xp = (type == T_OUTLET) ? x : ((x == nx - 1) ? 0 : x + 1);
   const int ym = (y == 0) ? ny - 1 : y - 1, yp = (y == ny - 1) ? 0 : y + 1;
   const int zm = (z == 0) ? nz - 1 : z - 1, zp = (z == nz - 1) ? 0 : z + 1;
+  const int sc = (type == T_WM) ? 0 : ((cls >> CLS_NORMAL_SHIFT) & 7);       // slip plane code (0 = none)
+  constexpr Mirror<Q> MR{};
 #pragma unroll
   for (int i = 0; i < Q; ++i) {
     const int sx = (L.c[i][0] == 0) ? x : ((L.c[i][0] == 1) ? xm : xp);
-    const int sy = (L.c[i][1] == 0) ? y : ((L.c[i][1] == 1) ? ym : yp);
-    const int sz = (L.c[i][2] == 0) ? z : ((L.c[i][2] == 1) ? zm : zp);
+    int sy = (L.c[i][1] == 0) ? y : ((L.c[i][1] == 1) ? ym : yp);
+    int sz = (L.c[i][2] == 0) ? z : ((L.c[i][2] == 1) ? zm : zp);
+    if (sc != 0) {                                            // specular pull at a plane slip wall: own plane, mirrored slot
+      if (L.c[i][1] != 0 && sc == ((L.c[i][1] == 1) ? 2 : 3)) {
+        f[i] = __ldg(a.fin + MR.my[i] * N + cell_index(sx, y, sz, nx, ny));
+        continue;
+      }
+      if (L.c[i][2] != 0 && sc == ((L.c[i][2] == 1) ? 4 : 5)) {
+        f[i] = __ldg(a.fin + MR.mz[i] * N + cell_index(sx, sy, z, nx, ny));
+        continue;
+      }
+    }
     const long long s = cell_index(sx, sy, sz, nx, ny);
     bool own = (i > 0) && ((nbm >> L.opp[i]) & 1u);
     if (L.c[i][0] == -1 && type == T_OUTLET) own = is_wall(a.cls[s]);
@@ -1027,11 +1067,14 @@ __device__ __forceinline__ void ld_uhat_nb(const T* pu, long long N, int dyp, in
 // of the cells of SPECIAL sectors (A8 wall model; OUTLET cells next to a wall), one cell per thread: the masked
 // boundary kernel as a block role of the same launch (scheduled first, overlaps with the row blocks).
 // Everything else -- bulk, solid-adjacent (read-side bounce-back), INLET and OUTLET cells -- runs in the vector path.
-// MW: the launch may meet MOVINGWALL cells (compiled out otherwise: the test costs the wall-adjacent warps registers).
-template <int Q, typename T, int MODE, int COLL, bool MW>
+// WV: kernel variant for special walls, compiled out otherwise (they cost registers): bit 0 = the launch may meet MOVINGWALL cells,
+// bit 1 = the lattice has cells with a slip plane code (specular pull in the vector path).
+template <int Q, typename T, int MODE, int COLL, int WV>
 __device__ __forceinline__ void step_vec_body(const StepArgs<T>& a, double (&acc)[5], const int bz) {   // bz: the block's z index in the (virtual) grid
   constexpr Stencil<Q> L{};
   constexpr int V = VecOf<Q, T, COLL>::V;
+  constexpr bool MW = (WV & 1) != 0;       // the launch may meet MOVINGWALL cells
+  constexpr bool SLIPV = (WV & 2) != 0;    // the lattice has cells with a slip plane code
   constexpr bool HRR = (COLL == COLL_HRR) && mode_collides(MODE);
   constexpr int SV = 32 / static_cast<int>(sizeof(T));      // cells per 32-byte sector
   constexpr int LG = 128 / (V * static_cast<int>(sizeof(T)));  // lanes per 128-byte line
@@ -1142,13 +1185,31 @@ __device__ __forceinline__ void step_vec_body(const StepArgs<T>& a, double (&acc
     // phase 1: issue every load before anything consumes one (in-order issue: a shuffle placed right
     // after its load would serialise the loads).  One running pointer per population (+N each).
     T e[Q];   // the one element a shifted row needs from outside the warp / row (edge lanes only)
-    auto issue_loads = [&](const bool ld, const bool el, const bool er) {
+    // SLIPV variant: slip plane code of the vector (its non-wall cells agree: k_slip_uniform): the populations that would come out of
+    // the slip plane are pulled from the vector's own plane and the mirrored slot instead (specular reflection, reading G37)
+    int sc = 0;
+    if (SLIPV) {
+#pragma unroll
+      for (int v = 0; v < V; ++v) {
+        const int b = static_cast<int>(clsw >> (8 * v)) & 0xff;
+        if (!is_wall(b) && (b & CLS_TYPE) != T_WM) sc |= (b >> CLS_NORMAL_SHIFT) & 7;
+      }
+      if (!active) sc = 0;
+    }
+    auto issue_loads = [&](auto slip_tag, const bool ld, const bool el, const bool er) {
+      constexpr bool SL = decltype(slip_tag)::value;         // this warp pulls under a slip plane code
       const T* pself = a.fin + self;
+      constexpr Mirror<Q> MR{};
 #pragma unroll
       for (int i = 0; i < Q; ++i) {
-        const long long off = static_cast<long long>((L.c[i][1] == 0) ? 0 : ((L.c[i][1] == 1) ? dym : dyp)) +
-                              static_cast<long long>((L.c[i][2] == 0) ? 0 : ((L.c[i][2] == 1) ? dzm : dzp));
-        const T* src = pself + off;                            // source row, at the vector's x
+        long long offy = static_cast<long long>((L.c[i][1] == 0) ? 0 : ((L.c[i][1] == 1) ? dym : dyp));
+        long long offz = static_cast<long long>((L.c[i][2] == 0) ? 0 : ((L.c[i][2] == 1) ? dzm : dzp));
+        long long slot = 0;
+        if (SL && sc != 0) {
+          if (L.c[i][1] != 0 && sc == ((L.c[i][1] == 1) ? 2 : 3)) { offy = 0; slot = static_cast<long long>(MR.my[i] - i) * N; }
+          else if (L.c[i][2] != 0 && sc == ((L.c[i][2] == 1) ? 4 : 5)) { offz = 0; slot = static_cast<long long>(MR.mz[i] - i) * N; }
+        }
+        const T* src = pself + (offy + offz + slot);           // source row, at the vector's x
         pself += N;
 #pragma unroll
         for (int v = 0; v < V; ++v) f[i][v] = T(0);
@@ -1160,11 +1221,22 @@ __device__ __forceinline__ void step_vec_body(const StepArgs<T>& a, double (&acc
     };
     // a vector that is SOLID throughout loads nothing, but the rows its neighbour pulls from (y -+ 1, z -+ 1) may be
     // fluid at its end cells: that neighbour fetches the one element itself, like a lane at the edge of the warp
-    const bool solid_l = __shfl_up_sync(FULL, all_solid ? 1 : 0, 1) != 0;
-    const bool solid_r = __shfl_down_sync(FULL, all_solid ? 1 : 0, 1) != 0;
+    // (SLIPV variant: the same where the neighbouring vector pulls under another slip plane code: its elements come from other rows)
+    bool solid_l, solid_r;
+    if constexpr (SLIPV) {
+      const int nb_key = (all_solid ? 8 : 0) | sc;
+      const int key_l = __shfl_up_sync(FULL, nb_key, 1), key_r = __shfl_down_sync(FULL, nb_key, 1);
+      solid_l = (key_l & 8) != 0 || (key_l & 7) != sc;
+      solid_r = (key_r & 8) != 0 || (key_r & 7) != sc;
+    } else {
+      solid_l = __shfl_up_sync(FULL, all_solid ? 1 : 0, 1) != 0;
+      solid_r = __shfl_down_sync(FULL, all_solid ? 1 : 0, 1) != 0;
+    }
     const bool edge_l = doload && ((lane == 0) || (tx == 0) || solid_l);
     const bool edge_r = doload && ((lane == 31) || (tx == static_cast<int>(blockDim.x) - 1) || (qx == nvec - 1) || solid_r);
-    issue_loads(doload, edge_l, edge_r);
+    // (a warp-uniform branch: the warps of the bulk run the plain load sequence, without the slip arithmetic)
+    if (SLIPV && __any_sync(FULL, sc != 0)) issue_loads(std::true_type{}, doload, edge_l, edge_r);
+    else issue_loads(std::false_type{}, doload, edge_l, edge_r);
     if constexpr (HRR) {
       if (mine) ld_uhat_nb<T, V>(a.uhat + self, N, dyp, dym, dzp, dzm, exl, exr, gu, gl, gr);
     }
@@ -1374,7 +1446,7 @@ __device__ __forceinline__ void step_vec_body(const StepArgs<T>& a, double (&acc
   }
 }
 
-template <int Q, typename T, int MODE, int COLL, bool MW>
+template <int Q, typename T, int MODE, int COLL, int WV>
 __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ StepArgs<T> a) {
   if (a.pdl_wait_all) griddep_wait();      // the preceding kernel wrote this kernel's input (see StepArgs)
   griddep_launch();
@@ -1382,10 +1454,10 @@ __global__ void __launch_bounds__(256, 2) k_step_vec(const __grid_constant__ Ste
   if constexpr (mode_totals(MODE)) {
     // the blocks walk the z-slices with stride gridDim.z, so that one block-level reduction (shuffle trees, atomics, ticket)
     // serves many vectors per thread
-    for (int bz = blockIdx.z; bz < a.list_z + a.nzs; bz += gridDim.z) step_vec_body<Q, T, MODE, COLL, MW>(a, acc, bz);
+    for (int bz = blockIdx.z; bz < a.list_z + a.nzs; bz += gridDim.z) step_vec_body<Q, T, MODE, COLL, WV>(a, acc, bz);
     reduce_totals(acc, a.tot_slots, a.tot_nslots, a.tot_ticket, a.tot_out);
   } else {
-    step_vec_body<Q, T, MODE, COLL, MW>(a, acc, static_cast<int>(blockIdx.z));
+    step_vec_body<Q, T, MODE, COLL, WV>(a, acc, static_cast<int>(blockIdx.z));
   }
 }
 
@@ -1574,6 +1646,33 @@ __global__ void __launch_bounds__(256) k_aa_unswap(const T* __restrict__ a, T* _
   }
 }
 
+// Slip plane codes are used by the vector kernel one VECTOR at a time: the non-wall cells of a 32-byte sector must agree on the
+// code (a WALLMODEL / zero-gradient OUTLET cell counts as code 0).  Where they do not, the coded cells of the sector fall back
+// to the per-cell path: SPECIAL, code cleared, ADJ set (the neighbour masks are built afterwards and then keep all their links).
+template <int SV>
+__global__ void __launch_bounds__(256) k_slip_uniform(uint8_t* __restrict__ cls, long long nsec_total, unsigned long long* __restrict__ counters) {
+  const long long q = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (q >= nsec_total) return;
+  int first = -1;
+  bool mixed = false;
+#pragma unroll
+  for (int v = 0; v < SV; ++v) {
+    const uint8_t c = cls[q * SV + v];
+    if (is_wall(c)) continue;
+    const int code = ((c & CLS_TYPE) == T_WM) ? 0 : ((c >> CLS_NORMAL_SHIFT) & 7);
+    if (first < 0) first = code;
+    else if (code != first) mixed = true;
+  }
+  if (!mixed) return;
+#pragma unroll
+  for (int v = 0; v < SV; ++v) {
+    const uint8_t c = cls[q * SV + v];
+    if (is_wall(c) || (c & CLS_TYPE) == T_WM || ((c >> CLS_NORMAL_SHIFT) & 7) == 0) continue;
+    cls[q * SV + v] = static_cast<uint8_t>((c & CLS_TYPE) | CLS_ADJ | CLS_SPECIAL);
+    atomicAdd(counters + 7, ~0ull);      // one coded cell less
+  }
+}
+
 // marks the cells that the list blocks of k_step_vec must process: every cell of a 32-byte sector (SV = 8 floats /
 // 4 doubles, aligned) that holds at least one SPECIAL cell.  mark[] feeds a stream compaction.
 template <int SV>
@@ -1742,10 +1841,10 @@ __global__ void __launch_bounds__(VM_CELLS * VM_SLICES) k_vm_inflow(const uint8_
 }
 
 // counters[0] = invalid flag bytes, [1] = wall cells (SOLID + MOVINGWALL), [2] = masked cells (non-wall, not plain bulk FLUID),
-// [4] = MOVINGWALL cells, [5] = SLIPWALL cells, [6] = WALLMODEL cells ([3] belongs to k_mark_list).
+// [4] = MOVINGWALL cells, [5] = SLIPWALL cells, [6] = WALLMODEL cells, [7] = cells with a slip plane code ([3] belongs to k_mark_list).
 template <int Q>
 __global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ flags, uint8_t* __restrict__ cls,
-                                                  int nx, int ny, int nz, unsigned long long* __restrict__ counters, int wm_special) {
+                                                  int nx, int ny, int nz, unsigned long long* __restrict__ counters, int wm_special, int slip_planes) {
   constexpr Stencil<Q> L{};
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
@@ -1762,6 +1861,8 @@ __global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ fl
   if (bad) { atomicAdd(counters, 1ull); return; }
   uint32_t m = 0u;
   bool slipnb = false;
+  int nt[Q];
+  nt[0] = type;
   if (!is_wall(type)) {
 #pragma unroll
     for (int j = 1; j < Q; ++j) {
@@ -1769,23 +1870,50 @@ __global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ fl
       sx = (sx < 0) ? sx + nx : ((sx >= nx) ? sx - nx : sx);
       sy = (sy < 0) ? sy + ny : ((sy >= ny) ? sy - ny : sy);
       sz = (sz < 0) ? sz + nz : ((sz >= nz) ? sz - nz : sz);
-      const int nt = flags[cell_index(sx, sy, sz, nx, ny)] & 0x0F;
-      if (is_wall(nt)) m |= (1u << j);
-      if (nt == T_SLIP) slipnb = true;
+      nt[j] = flags[cell_index(sx, sy, sz, nx, ny)] & 0x0F;
+      if (is_wall(nt[j])) m |= (1u << j);
+      if (nt[j] == T_SLIP) slipnb = true;
     }
   }
+  // slip plane code (see slip_axis above): every neighbour on the wall side of ONE plane normal to y or z is a SLIPWALL cell, the
+  // specular sources x + c_j + n (in the cell's own plane) are no walls, and no other neighbour is a slip wall (other walls are
+  // fine: they stay in the neighbour mask and bounce back)
+  int scode = 0;
+  if (slipnb && slip_planes && type != T_WM && type != T_OUTLET) {
+    constexpr Mirror<Q> MR{};
+    for (int code = 2; code <= 5 && scode == 0; ++code) {
+      const int ax = slip_axis(code), side = -slip_sign(code);
+      bool ok = true;
+      uint32_t handled = 0u;
+#pragma unroll
+      for (int j = 1; j < Q; ++j) {
+        if (L.c[j][ax] == side) {
+          handled |= (1u << j);
+          const int back = (ax == 1) ? MR.zy[j] : MR.zz[j];       // x + c_j + n
+          if (nt[j] != T_SLIP || (back != 0 && is_wall(nt[back]))) ok = false;
+        } else if (nt[j] == T_SLIP) {
+          ok = false;
+        }
+      }
+      if (ok) {
+        scode = code;
+        m &= ~handled;
+      }
+    }
+  }
+  const bool adj_any = (m != 0u) || scode != 0;                // (statistics: the cell has a wall neighbour)
   const bool adj = (m != 0u);
-  // cells next to a slip wall take the per-cell path: the specular pull (slip_pull) is a call with many operands, which does not
-  // belong into the vector kernel's register budget
+  // cells next to a slip wall that have no slip plane code take the per-cell path (general specular pull slip_pull)
   // (wm_special: WALLMODEL cells solve Spalding's law in the list blocks instead of taking u^B from the pre-pass)
-  const bool special = (type == T_WM && wm_special) || (type == T_OUTLET && adj) || slipnb;
-  cls[self] = static_cast<uint8_t>(type | ((type == T_WM ? hi : 0) << CLS_NORMAL_SHIFT) | (adj ? CLS_ADJ : 0) |
+  const bool special = (type == T_WM && wm_special) || (type == T_OUTLET && adj) || (slipnb && scode == 0);
+  cls[self] = static_cast<uint8_t>(type | ((type == T_WM ? hi : scode) << CLS_NORMAL_SHIFT) | (adj ? CLS_ADJ : 0) |
                                    (special ? CLS_SPECIAL : 0));
   if (is_wall(type)) atomicAdd(counters + 1, 1ull);
   if (type == T_MOVING) atomicAdd(counters + 4, 1ull);
   if (type == T_WM) atomicAdd(counters + 6, 1ull);
   if (type == T_SLIP) atomicAdd(counters + 5, 1ull);
-  else if (adj || type != T_FLUID) atomicAdd(counters + 2, 1ull);
+  else if (adj_any || type != T_FLUID) atomicAdd(counters + 2, 1ull);
+  if (scode != 0) atomicAdd(counters + 7, 1ull);
 }
 
 // nbmask of an accepted classification (a rejected flag array must leave the old geometry intact)
@@ -1807,6 +1935,13 @@ __global__ void __launch_bounds__(256) k_nbmask(const uint8_t* __restrict__ cls,
       sz = (sz < 0) ? sz + nz : ((sz >= nz) ? sz - nz : sz);
       if (is_wall(cls[cell_index(sx, sy, sz, nx, ny)])) m |= (1u << j);
     }
+  }
+  const uint8_t c0 = cls[self];
+  const int sc = ((c0 & CLS_TYPE) == T_WM || is_wall(c0)) ? 0 : ((c0 >> CLS_NORMAL_SHIFT) & 7);
+  if (sc != 0) {                         // the links into the slip plane are served by the specular pull, not by bounce-back
+#pragma unroll
+    for (int j = 1; j < Q; ++j)
+      if (L.c[j][slip_axis(sc)] == -slip_sign(sc)) m &= ~(1u << j);
   }
   nbmask[self] = m;
 }

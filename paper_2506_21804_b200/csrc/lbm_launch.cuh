@@ -156,13 +156,17 @@ int launch_one(lbm_ctx* c, const lbm_params* p, int in, int out, int z0, int nzs
     }
     if (grid.z > 65535u || grid.y > 65535u)
       return fail(c, LBM_EINVAL, "lattice does not fit the launch grid (nz + list slices = %u, rows = %u; both must be <= 65535)", grid.z, grid.y);
-    bool mw = false;
-    if constexpr (lbm::mode_pulls(MODE)) mw = c->n_moving > 0 && may_meet_lid;
+    int wv = 0;      // kernel variant: bit 0 = the launch may meet the moving lid, bit 1 = cells with a slip plane code
+    if constexpr (lbm::mode_pulls(MODE)) wv = ((c->n_moving > 0 && may_meet_lid) ? 1 : 0) | ((c->n_slipcode > 0) ? 2 : 0);
     if constexpr (lbm::mode_pulls(MODE)) {
-      if (mw) e = launch_k(lbm::k_step_vec<Q, T, MODE, COLL, true>, grid, block, c->stream, pdl, a);
-      else    e = launch_k(lbm::k_step_vec<Q, T, MODE, COLL, false>, grid, block, c->stream, pdl, a);
+      switch (wv) {
+        case 1:  e = launch_k(lbm::k_step_vec<Q, T, MODE, COLL, 1>, grid, block, c->stream, pdl, a); break;
+        case 2:  e = launch_k(lbm::k_step_vec<Q, T, MODE, COLL, 2>, grid, block, c->stream, pdl, a); break;
+        case 3:  e = launch_k(lbm::k_step_vec<Q, T, MODE, COLL, 3>, grid, block, c->stream, pdl, a); break;
+        default: e = launch_k(lbm::k_step_vec<Q, T, MODE, COLL, 0>, grid, block, c->stream, pdl, a); break;
+      }
     } else {
-      e = launch_k(lbm::k_step_vec<Q, T, MODE, COLL, false>, grid, block, c->stream, pdl, a);
+      e = launch_k(lbm::k_step_vec<Q, T, MODE, COLL, 0>, grid, block, c->stream, pdl, a);
     }
   } else {
     if (nzs == 0) return LBM_OK;

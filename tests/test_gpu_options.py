@@ -75,6 +75,37 @@ def test_wall_model_prepass_and_in_place_solve_agree(dtype, coll):
     assert field_error(outs[0], outs[1], m) <= (1e-13 if dtype == "f64" else 2e-6)
 
 
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("Q,coll", [(19, 0), (19, 1), (27, 0)])
+def test_slip_plane_codes_and_the_general_specular_rule_agree(Q, coll, dtype):
+    """slip_planes 1 (cells next to a plane slip wall pull the reflected populations in the vector path) vs 0 (every slip-adjacent
+    cell in the list blocks, general rule slip_pull): config 7 (slip lateral walls and top) from a NON-EQUILIBRIUM state, so that a
+    wrong slot or source row cannot hide behind symmetry"""
+    cfg = I.make_config(7, shape=(24, 32, 96))
+    cfg["Q"] = Q
+    cfg["params"] = dict(cfg["params"], collision=coll, sigma=0.7)
+    f, d = oracle_inputs(cfg, "f64")
+    rng = np.random.Generator(np.random.PCG64(77 + Q + coll))
+    f = (f * (1.0 + 0.02 * rng.uniform(-1.0, 1.0, size=f.shape))).astype(NP_DTYPE[dtype])
+    d = d.astype(NP_DTYPE[dtype])
+    ref = run_oracle(cfg, f, d, 10)
+    m = nonsolid(cfg)
+    nz, ny, nx = cfg["shape"]
+    outs, coded = [], []
+    for v in (1, 0):
+        with P.LBM(Q, nx, ny, nz, dtype) as sim:
+            sim.set_option("slip_planes", v)
+            sim.set_fields(f, d, cfg["flags"])
+            coded.append((sim.query("slip_plane_cells"), sim.query("list_cells")))
+            sim.step(10, P.LbmParams(**cfg["params"]))
+            out = np.empty_like(f)
+            sim.get_populations(out)
+        assert field_error(out, ref, m) <= TOL[dtype], (v,)
+        outs.append(out)
+    assert coded[0][0] > 2000 and coded[1][0] == 0 and coded[0][1] < coded[1][1] // 4      # the list shrank to the edges and corners
+    assert field_error(outs[0], outs[1], m) <= (1e-13 if dtype == "f64" else 2e-6)
+
+
 def test_graph_is_recaptured_when_parameters_or_fields_change():
     cfg = I.make_config(3, shape=(24, 32, 96))
     f, d = oracle_inputs(cfg, "f64")
