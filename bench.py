@@ -82,6 +82,7 @@ WORKLOADS["paperbc_wmfaces_urban_channel_384x192x128_f32_hrr_vm"] = (8, (128, 19
 # option "inplace"); at 768^3 fp64 one population set is 68.9 GB
 INPLACE = dict(inplace=1)
 WORKLOADS["config2_les_periodic_256_f32_inplace"] = (2, None, "f32", {}, None, None, INPLACE)
+WORKLOADS["config4_d3q27_spheres_512_f32_inplace"] = (4, None, "f32", {}, None, None, INPLACE)
 for _n, _t in ((512, "f32"), (768, "f64")):
     WORKLOADS["config2_les_periodic_%d_%s" % (_n, _t)] = (2, (_n, _n, _n), _t)
     WORKLOADS["config2_les_periodic_%d_%s_inplace" % (_n, _t)] = (2, (_n, _n, _n), _t, {}, None, None, INPLACE)

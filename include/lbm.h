@@ -294,8 +294,8 @@ long long lbm_query(const lbm_ctx* ctx, int what);
  *                           cell next to a slip wall is handled cell by cell in the list blocks.  Decides how flags are
  *                           classified: LBM_ESTATE once a state or geometry has been set
  *   "serpentine"    0|1     consecutive launches sweep the z-slices in opposite directions for L2 reuse (default 1)
- *   "inplace"       0|1     1: a lattice without a single wall / inlet / outlet / wall-model cell (fully periodic bulk), BGK form,
- *                           steps IN PLACE on one array (AA pattern: even steps collide locally into the opposite slots, odd
+ *   "inplace"       0|1     1: a lattice of plain fluid cells, with or without resting SOLID cells (halfway bounce-back) but without
+ *                           any inlet / outlet / wall-model / moving / slip cell, BGK form, steps IN PLACE on one array (AA pattern: even steps collide locally into the opposite slots, odd
  *                           steps pull and push through the neighbours); the second lattice is then never
  *                           allocated unless a state read after an odd number of steps needs it.  Default 0 (two lattices)
  *   "vector"        0|1     0 forces the scalar kernel (one cell per thread) for every row length (default 1)

@@ -185,7 +185,7 @@ int classify(lbm_ctx* c, const uint8_t* cell_flags) {
   } else {
     LBM_CUDA(c, cudaMemsetAsync(c->flags_raw, 0, c->N, c->stream));
   }
-  LBM_CUDA(c, cudaMemsetAsync(c->counters, 0, 8 * sizeof(unsigned long long), c->stream));
+  LBM_CUDA(c, cudaMemsetAsync(c->counters, 0, 16 * sizeof(unsigned long long), c->stream));
   dim3 grid, block;
   launch_dims(c, grid, block);
   const int wm_special = c->wm_prepass ? 0 : 1;
@@ -194,7 +194,7 @@ int classify(lbm_ctx* c, const uint8_t* cell_flags) {
   else            lbm::k_classify<27><<<grid, block, 0, c->stream>>>(c->flags_raw, c->cls_alt, c->nx, c->ny, c->nz, c->counters, wm_special, slip_planes);
   LBM_CUDA(c, cudaGetLastError());
   c->launches++;
-  unsigned long long h[8];
+  unsigned long long h[16];
   LBM_CUDA(c, cudaMemcpyAsync(h, c->counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
   LBM_CUDA(c, cudaStreamSynchronize(c->stream));
   if (h[0] != 0)
@@ -268,6 +268,7 @@ int classify(lbm_ctx* c, const uint8_t* cell_flags) {
   c->n_moving = static_cast<long long>(h[4]);
   c->n_slip = static_cast<long long>(h[5]);
   c->n_slipcode = static_cast<long long>(h[7]);
+  c->n_typed = static_cast<long long>(h[8]);
   c->epoch++;
   return LBM_OK;
 }
@@ -396,7 +397,7 @@ lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype) {
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->flags_raw), N);
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->nbmask), static_cast<size_t>(N) * sizeof(uint32_t));
   const size_t tot_bytes = (8 + 5 * LBM_TOT_SLOTS + 1) * sizeof(double);      // result, slots, ticket (see make_args)
-  if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->counters), 8 * sizeof(unsigned long long));
+  if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->counters), 16 * sizeof(unsigned long long));
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->totals_dev), tot_bytes);
   if (rc == LBM_OK && cudaMemset(c->totals_dev, 0, tot_bytes) != cudaSuccess) rc = fail(c, LBM_ECUDA, "cudaMemset failed");
   if (rc == LBM_OK) rc = dev_alloc(c, reinterpret_cast<void**>(&c->list_count_dev), sizeof(int));
@@ -471,6 +472,7 @@ int lbm_set_fields(lbm_ctx* c, const void* populations, const void* porosity, co
   if (!is_device_pointer(populations)) LBM_CUDA(c, cudaStreamSynchronize(c->stream));
   c->cur = 0;
   c->phase = PHASE_PRE;
+  c->solid_dirty = false;
   c->steps = 0;
   { int rci = reset_inflow(c); if (rci != LBM_OK) return rci; }
   return solid_values(c, true);      // SOLID cells' own values -> side buffer (the step kernels overwrite their slots)
@@ -495,6 +497,7 @@ int lbm_init_equilibrium(lbm_ctx* c, const void* rho, const void* u) {
   if (hr || hu) LBM_CUDA(c, cudaStreamSynchronize(c->stream));
   c->cur = 0;
   c->phase = PHASE_PRE;
+  c->solid_dirty = false;
   c->steps = 0;
   { int rci = reset_inflow(c); if (rci != LBM_OK) return rci; }
   return solid_values(c, true);
@@ -508,7 +511,12 @@ static int materialise(lbm_ctx* c) {
     if (rc == LBM_OK) rc = LBM_DISPATCH(c, launch_aa, c, &p, 2);
     if (rc != LBM_OK) return rc;
     c->phase = PHASE_PRE;
-    return LBM_OK;
+    c->solid_dirty = false;
+    return solid_values(c, false);       // the wall cells' own values into the lattice that now holds S_t
+  }
+  if (c->phase == PHASE_PRE && c->solid_dirty) {     // in-place steps left whatever in the wall cells' slots: put their own values back
+    c->solid_dirty = false;
+    return solid_values(c, false);
   }
   if (c->phase != PHASE_POST) return LBM_OK;
   lbm_params p = c->last;
@@ -738,7 +746,9 @@ static int graph_chunk(lbm_ctx* c, const lbm_params* params, bool* done) {
 
 // In-place (AA pattern) stepping applies to lattices without a single boundary cell, BGK form, rows the vector kernels take
 static bool inplace_eligible(const lbm_ctx* c, const lbm_params* p) {
-  if (!c->inplace || !c->use_vector || c->n_solid != 0 || c->n_masked != 0 || c->uin_mean || c->ghost_lo || c->ghost_hi) return false;
+  if (!c->inplace || !c->use_vector || c->uin_mean || c->ghost_lo || c->ghost_hi) return false;
+  // plain fluid, or plain fluid + resting SOLID cells (halfway bounce-back): no inlet / outlet / wall-model / moving / slip cell
+  if (c->n_typed != 0 || c->n_moving != 0 || c->n_slip != 0 || c->n_list != 0) return false;
   if (p->collision != LBM_COLLISION_BGK) return false;
   const int V = (c->Q == 19 ? 16 : 8) / c->dtype;             // cells per thread of the BGK vector kernels
   if (V < 1 || c->nx % V != 0) return false;
@@ -792,6 +802,7 @@ int lbm_step(lbm_ctx* c, int n_steps, const lbm_params* params) {
       rc = LBM_DISPATCH(c, launch_aa, c, params, c->phase == PHASE_PRE ? 0 : 1);
       if (rc != LBM_OK) return rc;
       c->phase = (c->phase == PHASE_PRE) ? PHASE_SWAPPED : PHASE_PRE;
+      if (c->n_solid > 0) c->solid_dirty = true;
       ++s;
       continue;
     }

@@ -51,6 +51,8 @@ struct lbm_ctx {
   int* list_count_dev;
   unsigned long long* counters;  // device [8]
   long long n_moving, n_slip;    // MOVINGWALL / SLIPWALL cells of the accepted geometry
+  long long n_typed;             // non-wall cells of a type other than FLUID (inlet, outlet, wall model, ...)
+  bool solid_dirty;              // in-place steps ran over wall cells' slots: their own values must be put back before the lattice is read
   long long n_slipcode;          // cells next to a plane slip wall that run in the vector path (slip plane code in their class byte)
   double* totals_dev;            // device [5] result + [LBM_TOT_SLOTS][5] partial sums + ticket counter
   void* staging;         // host<->device bounce buffer, grown on demand

@@ -1478,14 +1478,18 @@ struct AAArgs {
   T* __restrict__ a;               // [Q][N], updated in place
   const T* __restrict__ d;         // porosity or nullptr
   const T* __restrict__ ub;        // solid velocity [3][N] or nullptr
+  const uint8_t* __restrict__ cls;      // class bytes (WALLS variants)
+  const uint32_t* __restrict__ nbmask;  // SOLID-neighbour masks (WALLS variants)
   int nx, ny, nz;
   long long N;
   T tau0, smago_k, fringe_k;
   int fringe_x0;
 };
 
+// collide the cells of a vector whose bit in `skip` is clear (wall cells keep what they hold)
 template <int Q, typename T>
-__device__ __forceinline__ void aa_collide_vec(const AAArgs<T>& a, long long self, int x0, T (&f)[Q][VecOf<Q, T, COLL_BGK>::V]) {
+__device__ __forceinline__ void aa_collide_vec(const AAArgs<T>& a, long long self, int x0, T (&f)[Q][VecOf<Q, T, COLL_BGK>::V],
+                                               unsigned skip = 0u) {
   constexpr int V = VecOf<Q, T, COLL_BGK>::V;
   T d[V];
 #pragma unroll
@@ -1493,6 +1497,7 @@ __device__ __forceinline__ void aa_collide_vec(const AAArgs<T>& a, long long sel
   if (a.d != nullptr) ld_vec_keep(a.d + self, d);
 #pragma unroll
   for (int v = 0; v < V; ++v) {
+    if ((skip >> v) & 1u) continue;
     T fc[Q];
 #pragma unroll
     for (int i = 0; i < Q; ++i) fc[i] = f[i][v];
@@ -1505,8 +1510,22 @@ __device__ __forceinline__ void aa_collide_vec(const AAArgs<T>& a, long long sel
   }
 }
 
+// which cells of the vector at `self` are walls (bit v), from their class bytes
+template <typename T, int V>
+__device__ __forceinline__ unsigned aa_wall_bits(const uint8_t* __restrict__ cls, long long self) {
+  unsigned w = 0;
+#pragma unroll
+  for (int v = 0; v < V; ++v) w |= is_wall(cls[self + v]) ? (1u << v) : 0u;
+  return w;
+}
+
+// WALLS: the lattice has SOLID cells (halfway bounce-back, R5) and nothing else besides plain fluid.  In the AA pattern the
+// bounce-back link of a cell needs the cell's OWN slots only: the even step is purely local anyway, and in the odd step the
+// population i whose source x - c_i is a wall is read from a[i][x] (where the even step left F_opp(i)(x)) and the population j
+// whose target x + c_j is a wall is written to a[opp(j)][x] -- the same location.  Wall cells' slots are never consumed, so whole
+// vectors are stored whatever their wall lanes hold; their own (inert) values live in the side buffer like in the two-lattice scheme.
 // grid (ceil(nvec / bx), ceil(ny / by), nz), block (bx, by)
-template <int Q, typename T>
+template <int Q, typename T, bool WALLS>
 __global__ void __launch_bounds__(256, 2) k_aa_even(const __grid_constant__ AAArgs<T> a) {
   constexpr Stencil<Q> L{};
   constexpr int V = VecOf<Q, T, COLL_BGK>::V;
@@ -1516,21 +1535,27 @@ __global__ void __launch_bounds__(256, 2) k_aa_even(const __grid_constant__ AAAr
   if (qx >= a.nx / V || y >= a.ny) return;
   const int x0 = qx * V;
   const long long self = (static_cast<long long>(z) * a.ny + y) * a.nx + x0;
+  unsigned walls = 0;
+  if (WALLS) {
+    walls = aa_wall_bits<T, V>(a.cls, self);
+    if (walls == ((1u << V) - 1u)) return;               // walls throughout: nothing to do, nothing to move
+  }
   T f[Q][V];
   T* p = a.a + self;
 #pragma unroll
   for (int i = 0; i < Q; ++i) ld_vec(p + i * a.N, f[i]);
-  aa_collide_vec<Q, T>(a, self, x0, f);
+  aa_collide_vec<Q, T>(a, self, x0, f, walls);
 #pragma unroll
   for (int i = 0; i < Q; ++i) st_vec(p + L.opp[i] * a.N, f[i]);
 }
 
 // grid (1, ceil(ny / by), nz), block (nvec, by): whole rows in x (nvec = nx / V a multiple of 32, nvec * by <= 256)
-template <int Q, typename T>
+template <int Q, typename T, bool WALLS>
 __global__ void __launch_bounds__(256, 2) k_aa_odd(const __grid_constant__ AAArgs<T> a) {
   constexpr Stencil<Q> L{};
   constexpr int V = VecOf<Q, T, COLL_BGK>::V;
   constexpr unsigned FULL = 0xffffffffu;
+  constexpr unsigned VALL = (1u << V) - 1u;
   constexpr int NXP = (Q == 19) ? 5 : 9;                  // populations with c_x = +1 (and as many with c_x = -1)
   __shared__ T edge_r[NXP][8];                           // F_j of the LAST cell of every warp, j with c_x = +1 (goes to the next warp)
   __shared__ T edge_l[NXP][8];                           // F_j of the FIRST cell of every warp, j with c_x = -1 (goes to the previous warp)
@@ -1552,6 +1577,34 @@ __global__ void __launch_bounds__(256, 2) k_aa_odd(const __grid_constant__ AAArg
   const int plane = nx * ny;
   const int dzm = (zm - z) * plane, dzp = (zp - z) * plane;
   const int exl = ((x0 == 0) ? nx - 1 : x0 - 1) - x0, exr = ((x0 + V >= nx) ? 0 : x0 + V) - x0;
+  // WALLS: which own cells are walls / solid-adjacent, and whether the cells left and right of the vector are fluid (they are the
+  // sources of the edge elements this thread stores)
+  unsigned walls = 0, adjb = 0;
+  bool fluid_l = true, fluid_r = true;
+  if (WALLS) {
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const uint8_t c = a.cls[self + v];
+      walls |= is_wall(c) ? (1u << v) : 0u;
+      adjb |= (c & CLS_ADJ) ? (1u << v) : 0u;
+    }
+    fluid_l = !is_wall(a.cls[self + exl]);
+    fluid_r = !is_wall(a.cls[self + exr]);
+    if (!active) { walls = VALL; adjb = 0; fluid_l = fluid_r = false; }
+  }
+  const bool ld = active && walls != VALL;               // a vector of walls throughout loads nothing: nobody consumes its values
+  // the element a shifted row needs from outside the warp -- or from a neighbouring lane that holds walls throughout and therefore
+  // loads nothing (its ROWS of sources may well be fluid): fetched by the lane itself
+  bool own_l = ld && lane == 0, own_r = ld && lane == 31;
+  if (WALLS) {
+    const bool wv_l = __shfl_up_sync(FULL, ld ? 0 : 1, 1) != 0, wv_r = __shfl_down_sync(FULL, ld ? 0 : 1, 1) != 0;
+    own_l = ld && (lane == 0 || wv_l);
+    own_r = ld && (lane == 31 || wv_r);
+  }
+  uint32_t nbm[V];
+#pragma unroll
+  for (int v = 0; v < V; ++v) nbm[v] = 0u;
+  if (WALLS && adjb != 0u) ld_nbmask(a.nbmask + self, nbm);
   T f[Q][V], e[Q];
   // load phase: S_{t+1,i}(x) = a[opp(i)][x - c_i]: the aligned vector of the source row, realigned by one element for c_x = +-1
 #pragma unroll
@@ -1562,27 +1615,37 @@ __global__ void __launch_bounds__(256, 2) k_aa_odd(const __grid_constant__ AAArg
 #pragma unroll
     for (int v = 0; v < V; ++v) f[i][v] = T(0);
     e[i] = T(0);
-    if (active) ld_vec(src, f[i]);
-    if (L.c[i][0] == 1 && active && lane == 0) e[i] = __ldg(src + exl);
-    if (L.c[i][0] == -1 && active && lane == 31) e[i] = __ldg(src + exr);
+    if (ld) ld_vec(src, f[i]);
+    if (L.c[i][0] == 1 && own_l) e[i] = __ldg(src + exl);
+    if (L.c[i][0] == -1 && own_r) e[i] = __ldg(src + exr);
   }
 #pragma unroll
   for (int i = 0; i < Q; ++i) {
     if (L.c[i][0] == 1) {
       T nb = __shfl_up_sync(FULL, f[i][V - 1], 1);
-      if (lane == 0) nb = e[i];
+      if (own_l) nb = e[i];
 #pragma unroll
       for (int v = V - 1; v > 0; --v) f[i][v] = f[i][v - 1];
       f[i][0] = nb;
     } else if (L.c[i][0] == -1) {
       T nb = __shfl_down_sync(FULL, f[i][0], 1);
-      if (lane == 31) nb = e[i];
+      if (own_r) nb = e[i];
 #pragma unroll
       for (int v = 0; v < V - 1; ++v) f[i][v] = f[i][v + 1];
       f[i][V - 1] = nb;
     }
   }
-  if (active) aa_collide_vec<Q, T>(a, self, x0, f);
+  if (WALLS && adjb != 0u) {
+    // R5 in the AA pattern: the population i = opp(j) whose source x + c_j is a wall is the cell's own a[i][x]
+    T* pown = a.a + self;
+#pragma unroll
+    for (int j = 1; j < Q; ++j) {
+#pragma unroll
+      for (int v = 0; v < V; ++v)
+        if (nbm[v] & (1u << j)) f[L.opp[j]][v] = __ldg(pown + static_cast<long long>(L.opp[j]) * N + v);
+    }
+  }
+  if (ld) aa_collide_vec<Q, T>(a, self, x0, f, walls);
   // store phase: F_j(x) goes to a[j][x + c_j]; the aligned vector (j, row + (c_y, c_z), x0) takes F_j(x - c_x)
   {
     int kp = 0, km = 0;
@@ -1596,6 +1659,11 @@ __global__ void __launch_bounds__(256, 2) k_aa_odd(const __grid_constant__ AAArg
   {
     const int wl = ty * wrow + (((tx >> 5) == 0) ? wrow - 1 : (tx >> 5) - 1);          // previous / next warp of the row (periodic)
     const int wr = ty * wrow + (((tx >> 5) == wrow - 1) ? 0 : (tx >> 5) + 1);
+    // WALLS: an element is stored only if the cell it comes from (this row, shifted by c_x) is fluid: what would come out of a wall
+    // cell must not overwrite the slot a fluid cell keeps its bounced population in
+    const unsigned src0 = active ? (~walls & VALL) : 0u;
+    const unsigned srcp = ((src0 << 1) | (fluid_l ? 1u : 0u)) & VALL;                  // c_x = +1: element e comes from cell e - 1
+    const unsigned srcm = (src0 >> 1) | (fluid_r ? (1u << (V - 1)) : 0u);              // c_x = -1: element e comes from cell e + 1
     int kp = 0, km = 0;
 #pragma unroll
     for (int j = 0; j < Q; ++j) {
@@ -1603,6 +1671,7 @@ __global__ void __launch_bounds__(256, 2) k_aa_odd(const __grid_constant__ AAArg
                             static_cast<long long>((L.c[j][2] == 0) ? 0 : ((L.c[j][2] == 1) ? dzp : dzm));
       T* dst = a.a + j * N + self + off;
       T o[V];
+      unsigned ok = src0;
       if (L.c[j][0] == 1) {
         T nb = __shfl_up_sync(FULL, f[j][V - 1], 1);
         if (lane == 0) nb = edge_r[kp][wl];
@@ -1610,6 +1679,7 @@ __global__ void __launch_bounds__(256, 2) k_aa_odd(const __grid_constant__ AAArg
 #pragma unroll
         for (int v = V - 1; v > 0; --v) o[v] = f[j][v - 1];
         o[0] = nb;
+        ok = srcp;
       } else if (L.c[j][0] == -1) {
         T nb = __shfl_down_sync(FULL, f[j][0], 1);
         if (lane == 31) nb = edge_l[km][wr];
@@ -1617,32 +1687,56 @@ __global__ void __launch_bounds__(256, 2) k_aa_odd(const __grid_constant__ AAArg
 #pragma unroll
         for (int v = 0; v < V - 1; ++v) o[v] = f[j][v + 1];
         o[V - 1] = nb;
+        ok = srcm;
       } else {
 #pragma unroll
         for (int v = 0; v < V; ++v) o[v] = f[j][v];
       }
-      if (active) st_vec(dst, o);
+      if (!WALLS) {
+        if (active) st_vec(dst, o);
+      } else if (ok == VALL) {
+        st_vec(dst, o);
+      } else if (ok != 0u) {
+#pragma unroll
+        for (int v = 0; v < V; ++v)
+          if ((ok >> v) & 1u) dst[v] = o[v];
+      }
+    }
+    if (WALLS && adjb != 0u) {
+      // the population j whose target x + c_j is a wall stays in the cell: a[opp(j)][x] (where the next even step reads f_opp(j))
+      T* pown = a.a + self;
+#pragma unroll
+      for (int j = 1; j < Q; ++j) {
+#pragma unroll
+        for (int v = 0; v < V; ++v)
+          if (nbm[v] & (1u << j)) pown[static_cast<long long>(L.opp[j]) * N + v] = f[j][v];
+      }
     }
   }
 }
 
-// the state S_{t+1} out of an array that holds F_t with swapped slots: out[i][x] = a[opp(i)][x - c_i] (materialisation; off the
-// timed path: one thread per value)
+// the state S_{t+1} out of an array that holds F_t with swapped slots: out[i][x] = a[opp(i)][x - c_i], or the cell's own a[i][x]
+// where x - c_i is a wall (materialisation; off the timed path: one thread per cell; wall cells are left to the side buffer)
 template <int Q, typename T>
-__global__ void __launch_bounds__(256) k_aa_unswap(const T* __restrict__ a, T* __restrict__ out, int nx, int ny, int nz, long long N) {
+__global__ void __launch_bounds__(256) k_aa_unswap(const T* __restrict__ a, T* __restrict__ out, int nx, int ny, int nz, long long N,
+                                                   const uint8_t* __restrict__ cls, const uint32_t* __restrict__ nbmask) {
   constexpr Stencil<Q> L{};
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
   const int z = blockIdx.z;
   if (x >= nx || y >= ny) return;
   const long long self = cell_index(x, y, z, nx, ny);
+  const uint8_t c = cls[self];
+  if (is_wall(c)) return;
+  const uint32_t nbm = (c & CLS_ADJ) ? nbmask[self] : 0u;
 #pragma unroll
   for (int i = 0; i < Q; ++i) {
     int sx = x - L.c[i][0], sy = y - L.c[i][1], sz = z - L.c[i][2];
     sx = (sx < 0) ? sx + nx : ((sx >= nx) ? sx - nx : sx);
     sy = (sy < 0) ? sy + ny : ((sy >= ny) ? sy - ny : sy);
     sz = (sz < 0) ? sz + nz : ((sz >= nz) ? sz - nz : sz);
-    out[i * N + self] = a[L.opp[i] * N + cell_index(sx, sy, sz, nx, ny)];
+    const bool own = (i > 0) && ((nbm >> L.opp[i]) & 1u);
+    out[i * N + self] = own ? a[i * N + self] : a[L.opp[i] * N + cell_index(sx, sy, sz, nx, ny)];
   }
 }
 
@@ -1841,7 +1935,7 @@ __global__ void __launch_bounds__(VM_CELLS * VM_SLICES) k_vm_inflow(const uint8_
 }
 
 // counters[0] = invalid flag bytes, [1] = wall cells (SOLID + MOVINGWALL), [2] = masked cells (non-wall, not plain bulk FLUID),
-// [4] = MOVINGWALL cells, [5] = SLIPWALL cells, [6] = WALLMODEL cells, [7] = cells with a slip plane code ([3] belongs to k_mark_list).
+// [4] = MOVINGWALL cells, [5] = SLIPWALL cells, [6] = WALLMODEL cells, [7] = cells with a slip plane code, [8] = non-wall cells of a type other than FLUID ([3] belongs to k_mark_list).
 template <int Q>
 __global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ flags, uint8_t* __restrict__ cls,
                                                   int nx, int ny, int nz, unsigned long long* __restrict__ counters, int wm_special, int slip_planes) {
@@ -1914,6 +2008,7 @@ __global__ void __launch_bounds__(256) k_classify(const uint8_t* __restrict__ fl
   if (type == T_SLIP) atomicAdd(counters + 5, 1ull);
   else if (adj_any || type != T_FLUID) atomicAdd(counters + 2, 1ull);
   if (scode != 0) atomicAdd(counters + 7, 1ull);
+  if (!is_wall(type) && type != T_FLUID) atomicAdd(counters + 8, 1ull);
 }
 
 // nbmask of an accepted classification (a rejected flag array must leave the old geometry intact)

@@ -315,7 +315,8 @@ int launch_aa(lbm_ctx* c, const lbm_params* p, int kind) {
   if (kind == 2) {
     dim3 grid, block;
     launch_dims(c, grid, block);
-    lbm::k_aa_unswap<Q, T><<<grid, block, 0, c->stream>>>(static_cast<const T*>(c->f[c->cur]), static_cast<T*>(c->f[1 - c->cur]), c->nx, c->ny, c->nz, c->N);
+    lbm::k_aa_unswap<Q, T><<<grid, block, 0, c->stream>>>(static_cast<const T*>(c->f[c->cur]), static_cast<T*>(c->f[1 - c->cur]), c->nx, c->ny, c->nz, c->N,
+                                                         c->cls, c->nbmask);
     LBM_CUDA(c, cudaGetLastError());
     c->launches++;
     c->cur = 1 - c->cur;
@@ -325,18 +326,22 @@ int launch_aa(lbm_ctx* c, const lbm_params* p, int kind) {
   lbm::AAArgs<T> a;
   a.a = static_cast<T*>(c->f[c->cur]);
   a.d = sa.d;  a.ub = sa.ub;
+  a.cls = c->cls;  a.nbmask = c->nbmask;
+  const bool walls = c->n_solid > 0;     // SOLID cells with halfway bounce-back (nothing else: inplace_eligible)
   a.nx = c->nx;  a.ny = c->ny;  a.nz = c->nz;  a.N = c->N;
   a.tau0 = sa.tau0;  a.smago_k = sa.smago_k;  a.fringe_k = sa.fringe_k;  a.fringe_x0 = sa.fringe_x0;
   const int nvec = c->nx / V;
   if (kind == 0) {
     dim3 grid, block;
     launch_dims_vec<Q, T, lbm::COLL_BGK>(c, grid, block);
-    lbm::k_aa_even<Q, T><<<grid, block, 0, c->stream>>>(a);
+    if (walls) lbm::k_aa_even<Q, T, true><<<grid, block, 0, c->stream>>>(a);
+    else       lbm::k_aa_even<Q, T, false><<<grid, block, 0, c->stream>>>(a);
   } else {
     int by = 64 / nvec;
     if (by < 1) by = 1;
     dim3 block(nvec, by, 1), grid(1, (c->ny + by - 1) / by, c->nz);
-    lbm::k_aa_odd<Q, T><<<grid, block, 0, c->stream>>>(a);
+    if (walls) lbm::k_aa_odd<Q, T, true><<<grid, block, 0, c->stream>>>(a);
+    else       lbm::k_aa_odd<Q, T, false><<<grid, block, 0, c->stream>>>(a);
   }
   LBM_CUDA(c, cudaGetLastError());
   c->launches++;

@@ -74,13 +74,58 @@ def test_inplace_with_porosity_and_state_reads_in_between(dtype):
     assert field_error(b, ref) <= TOL[dtype]
 
 
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("Q", [19, 27])
+@pytest.mark.parametrize("chunks", [[1], [2], [9], [3, 2, 4]])
+def test_inplace_with_bounce_back_walls_equals_two_lattices_bit_for_bit(Q, dtype, chunks):
+    """config 4 scaled down (periodic box with solid spheres): in the AA pattern a bounce-back link needs the cell's own slots only"""
+    nx = NX[(Q, dtype)]
+    cfg = I.make_config(4, shape=(20, 14, 2 * nx), k_max=4, n_modes=32)
+    cfg["Q"] = Q
+    t = cfg["flags"] & 15
+    assert 0.05 < (t == I.SOLID).mean() < 0.3
+    f, d = oracle_inputs(cfg, dtype)
+    par = P.LbmParams(**cfg["params"])
+    nz, ny, nx_ = cfg["shape"]
+    res = []
+    for inplace in (0, 1):
+        with P.LBM(Q, nx_, ny, nz, dtype) as sim:
+            sim.set_option("inplace", inplace)
+            sim.set_fields(f, None, cfg["flags"])
+            l0 = sim.query("launches")
+            for n in chunks:
+                sim.step(n, par)
+            steps_launches = sim.query("launches") - l0
+            rho = np.empty(f.shape[1:], dtype=f.dtype)
+            u = np.empty((3,) + f.shape[1:], dtype=f.dtype)
+            sim.moments(rho, u)
+            tot = np.array(sim.totals())
+            out = np.empty_like(f)
+            sim.get_populations(out)
+            sim.step(2, par)                                            # and the run goes on after the reads
+            out2 = np.empty_like(f)
+            sim.get_populations(out2)
+        res.append((out, rho, u, tot, out2, steps_launches))
+    a, b = res
+    assert b[5] == sum(chunks)                                          # in place: one launch per step
+    for k in (0, 1, 2, 4):
+        assert np.array_equal(a[k], b[k]), k
+    assert np.abs(a[3] - b[3]).max() <= 1e-6 * abs(a[3][0])
+    mask = ~I.is_wall(cfg["flags"])
+    assert np.array_equal(b[0][:, ~mask], f[:, ~mask])                  # wall cells keep their own values
+    ref = O.step(f.astype(np.float64), flags=cfg["flags"], nsteps=sum(chunks), nthreads=4, **cfg["params"])
+    assert field_error(b[0], ref, mask) <= TOL[dtype]
+
+
 def test_inplace_is_ignored_where_it_does_not_apply():
-    """a wall cell, the HRR form or a row length the row-wide blocks do not take: the two-lattice path runs, same results"""
+    """an inlet / outlet cell, the HRR form or a row length the row-wide blocks do not take: the two-lattice path runs, same results"""
     cfg = I.make_config(2, shape=(8, 6, 128), k_max=4, n_modes=16)
     f, d = oracle_inputs(cfg, "f32")
     flags = np.zeros(cfg["shape"], dtype=np.uint8)
-    flags[3, 2, 40] = I.SOLID
-    par = P.LbmParams(**cfg["params"])
+    flags[1:-1, :, 0] = I.INLET
+    flags[1:-1, :, -1] = I.OUTLET
+    flags[0] = flags[-1] = I.SOLID
+    par = P.LbmParams(**dict(cfg["params"], u_in=(0.03, 0.0, 0.0)))
     hrr = P.LbmParams(**dict(cfg["params"], collision=1, sigma=0.7))
     outs = []
     for inplace in (0, 1):
