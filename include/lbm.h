@@ -210,7 +210,7 @@ int lbm_set_populations_box(lbm_ctx* ctx, int x0, int y0, int z0, int bx, int by
  * and the kinetic energy the Taylor-Green check of config 1 is stated in): out[0] = sum rho, out[1..3] = sum rho u,
  * out[4] = sum rho |u|^2 / 2.  `out`: 5 doubles, host (the call synchronises the stream) or device (asynchronous).  One launch, pulling S_t in registers like lbm_moments:
  * per-thread sums over the cells of a vector in dtype, from the warp level up in fp64 (shuffle tree, one atomicAdd(double)
- * per block into one of 256 slots, the last block adds the slots).  On a sub-domain (lbm_set_halo): the interior cells only.
+ * per block into one of 256 slots, the last block adds the slots: one warp per quantity).  On a sub-domain (lbm_set_halo): the interior cells only.
  * Errors: LBM_EINVAL (NULL ctx / out), LBM_ESTATE (no state), LBM_ECUDA. */
 int lbm_totals(lbm_ctx* ctx, double out[5]);
 
@@ -293,6 +293,8 @@ long long lbm_query(const lbm_ctx* ctx, int what);
  *                           specular pull) run in the vector path, pulling the reflected populations from their own plane; 0: every
  *                           cell next to a slip wall is handled cell by cell in the list blocks.  Decides how flags are
  *                           classified: LBM_ESTATE once a state or geometry has been set
+ *   "totals_waves"  n       lbm_totals runs n whole waves of resident blocks (1 .. 64), each block looping over the z-slices; 0 (default):
+ *                           chosen from the lattice size (about 8 z-iterations per block, 1 .. 16 waves)
  *   "serpentine"    0|1     consecutive launches sweep the z-slices in opposite directions for L2 reuse (default 1)
  *   "inplace"       0|1     1: a lattice of plain fluid cells, with or without resting SOLID cells (halfway bounce-back) but without
  *                           any inlet / outlet / wall-model / moving / slip cell, BGK form, steps IN PLACE on one array (AA pattern: even steps collide locally into the opposite slots, odd

@@ -387,6 +387,7 @@ lbm_ctx* lbm_create(int lattice, int nx, int ny, int nz, int dtype) {
   c->slip_planes = 1;
   c->use_pdl = 2;
   c->use_graph = 0;
+  c->totals_waves = 0;
   c->last = default_params();
   std::snprintf(c->err, sizeof(c->err), "no error");
   const size_t pop = static_cast<size_t>(lattice) * N * dtype;
@@ -693,6 +694,7 @@ static int graph_chunk(lbm_ctx* c, const lbm_params* params, bool* done) {
     if (!c->cap_stream && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
       cudaGetLastError();
       c->use_graph = 0;
+  c->totals_waves = 0;
       return LBM_OK;
     }
     // capture on the private stream; nothing executes, so the bookkeeping the launches advance is put back afterwards
@@ -703,6 +705,7 @@ static int graph_chunk(lbm_ctx* c, const lbm_params* params, bool* done) {
     if (cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
       cudaGetLastError();
       c->use_graph = 0;
+  c->totals_waves = 0;
       return LBM_OK;
     }
     c->stream = c->cap_stream;
@@ -727,6 +730,7 @@ static int graph_chunk(lbm_ctx* c, const lbm_params* params, bool* done) {
     if (ei != cudaSuccess) {
       cudaGetLastError();
       c->use_graph = 0;
+  c->totals_waves = 0;
       return LBM_OK;
     }
     g.valid = true;
@@ -1151,6 +1155,11 @@ int lbm_set_option(lbm_ctx* c, const char* key, long long value) {
       return fail(c, LBM_ESTATE, "slip_planes decides how the flags are classified: set it before lbm_set_fields / lbm_set_geometry");
     c->slip_planes = static_cast<int>(value);
     c->epoch++;
+    return LBM_OK;
+  }
+  if (std::strcmp(key, "totals_waves") == 0) {
+    if (value < 0 || value > 64) return fail(c, LBM_EINVAL, "totals_waves must be in [0, 64]");
+    c->totals_waves = static_cast<int>(value);
     return LBM_OK;
   }
   if (std::strcmp(key, "block_threads") == 0) {

@@ -92,6 +92,7 @@ struct lbm_ctx {
   int hrr_slab;          // HRR form: z-slices per slab of the two-pass step (0 = whole lattice)
   int inplace;           // 1: lattices without any boundary cell step in place (AA pattern), one lattice (option "inplace")
   int slip_planes;       // 1: cells next to a plane slip wall normal to y or z get a slip plane code and run in the vector path (default)
+  int totals_waves;      // lbm_totals: waves of resident blocks in the grid (every block loops over z); 0 = auto
   int wm_prepass;        // 1: wall-model cells run in the vector path, u^B from a pre-pass over their compact list (default)
   int use_pdl;           // programmatic dependent launch of the time-loop kernels: 0 off, 1 every thread waits for the predecessor,
                          // 2 (default) after the wall-model pre-pass only the threads that read its output wait

@@ -843,14 +843,21 @@ __device__ __forceinline__ void reduce_totals(const double (&v)[5], double* __re
   __syncthreads();
   if (tid == 0) s_last = (atomicInc(ticket, nblocks - 1u) == nblocks - 1u) ? 1 : 0;   // wraps to 0 on the last block
   __syncthreads();
-  if (s_last && tid < 5) {
+  if (s_last) {
+    // the last block: every warp takes quantities k = warp, warp + nwarps, ...; its lanes read the slots q = lane, lane + 32, ...
+    // (independent loads, all in flight together -- one thread walking the 256 slots waited for 256 round trips to L2, 45 us),
+    // then a shuffle tree in a fixed order; slots and ticket are left zeroed for the next launch
     __threadfence();
-    double s = 0.0;
-    for (int q = 0; q < nslots; ++q) {
-      s += __ldcg(slots + static_cast<size_t>(q) * 5 + tid);
-      slots[static_cast<size_t>(q) * 5 + tid] = 0.0;
+    for (int k = warp; k < 5; k += nwarps) {
+      double s = 0.0;
+      for (int q = lane; q < nslots; q += 32) {
+        s += __ldcg(slots + static_cast<size_t>(q) * 5 + k);
+        slots[static_cast<size_t>(q) * 5 + k] = 0.0;
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+      if (lane == 0) out[k] = s;
     }
-    out[tid] = s;
   }
 }
 

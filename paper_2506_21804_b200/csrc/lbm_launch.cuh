@@ -149,9 +149,25 @@ int launch_one(lbm_ctx* c, const lbm_params* p, int in, int out, int z0, int nzs
     }
     grid.z = nzs + a.list_z;
     if (grid.z == 0) return LBM_OK;
-    if constexpr (lbm::mode_totals(MODE)) {     // ~16 blocks per SM; every block loops over the z-slices (one reduction per block)
+    if constexpr (lbm::mode_totals(MODE)) {
+      // every block loops over the z-slices (one reduction per block); the grid is a whole number of waves of resident blocks (a
+      // partly filled last wave of these long blocks would cost up to a wave: 2.19 waves measured 0.165 ms on config 3)
+      int per_sm = 8, dev = 0, sms = 148;
+      cudaGetDevice(&dev);
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lbm::k_step_vec<Q, T, MODE, COLL, 0>, block.x * block.y, 0) != cudaSuccess || per_sm < 1) {
+        cudaGetLastError();
+        per_sm = 8;
+      }
       const unsigned per_slice = grid.x * grid.y;
-      const unsigned want = (148u * 16u + per_slice - 1) / per_slice;
+      int waves = c->totals_waves;          // 0 = auto: about 8 z-iterations per block, 1 .. 16 waves (measured: config 3 best at 1 - 4,
+      if (waves <= 0) {                     // 256^3 at 4, 512^3 at 16)
+        const long long all = static_cast<long long>(per_slice) * grid.z;
+        waves = static_cast<int>(all / (8ll * per_sm * sms));
+        waves = waves < 1 ? 1 : (waves > 16 ? 16 : waves);
+      }
+      unsigned want = static_cast<unsigned>(per_sm * sms * waves) / per_slice;
+      if (want < 1) want = 1;
       if (grid.z > want) grid.z = want;
     }
     if (grid.z > 65535u || grid.y > 65535u)
