@@ -171,6 +171,8 @@ def max_over_ranks(x, world, device="cuda"):
         return float(x)
     import torch
     import torch.distributed as dist
+    if dist.get_backend() == "gloo":
+        device = "cpu"
     t = torch.tensor([float(x)], device=device, dtype=torch.float64)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
@@ -309,10 +311,18 @@ def main():
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    # LBM_BENCH_ONE_GPU=1: a dry run of the N > 1 path on ONE GPU (all ranks on cuda:0, halos exchanged through gloo and the host;
+    # nothing in a kernel ever waits for another rank).  It checks the decomposition end to end; its numbers are not a measurement.
+    one_gpu = os.environ.get("LBM_BENCH_ONE_GPU") == "1"
+    if one_gpu:
+        local_rank = 0
     torch.cuda.set_device(local_rank)
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        if one_gpu:
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     number, shape, dtype, extra = workload(args.workload)
     # N > 1: the lattice is cut into z-slabs, one per GPU, with a halo exchange per step.  Weak scaling
@@ -388,7 +398,7 @@ def main():
     def job_totals():
         t = np.array(sim.totals())
         if decomposed:
-            tt = torch.tensor(t, device="cuda", dtype=torch.float64)
+            tt = torch.tensor(t, device="cpu" if dist.get_backend() == "gloo" else "cuda", dtype=torch.float64)
             dist.all_reduce(tt)
             t = tt.cpu().numpy()
         return t
@@ -522,8 +532,9 @@ def main():
                        "solid_cells": n_solid, "masked_cells": sim.query("masked_cells"), "params": cfg["params"],
                        "l2": "inputs larger than L2 (%.2f GB per step)" % (step_bytes / 1e9),
                        "mlups_all_cells": (cells_global if decomposed else world * N) * args.steps / (ms * 1e-3) / 1e6,
-                       "parallelism": ("z-slabs, one per GPU, halo exchange per step over NCCL send/recv (%s scaling): global lattice %s"
-                                       % ("strong" if args.strong else "weak", "x".join(str(v) for v in cfg["shape"][::-1]))) if decomposed
+                       "parallelism": ("z-slabs, one per GPU, halo exchange per step over %s (%s scaling): global lattice %s"
+                                       % ("gloo through the host, ALL RANKS ON ONE GPU: a dry run, not a measurement" if one_gpu else "NCCL send/recv",
+                                          "strong" if args.strong else "weak", "x".join(str(v) for v in cfg["shape"][::-1]))) if decomposed
                                       else ("replicas only" if world > 1 else "single GPU"),
                        "finite": finite, "mass_drift_rel": (tot1[0] - tot0[0]) / tot0[0],
                        "repeats_ms_per_step": [t / args.steps for t in region_ms],

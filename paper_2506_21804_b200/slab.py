@@ -72,6 +72,15 @@ def exchange_faces(slab, send_low, send_high, recv_low, recv_high, group=None):
     high face to the upper one (into its LOW ghost).  Sends and receives are posted in one batch; between the same pair of ranks
     they match in posting order (and by tag where the backend has tags): data travelling DOWN first, then data travelling UP."""
     import torch.distributed as dist
+    if send_low.is_cuda and dist.get_backend(group) == "gloo":
+        # gloo moves host memory only (the CPU tests, and the single-GPU dry run of bench.py's decomposed path): stage through the host
+        hs = [t.cpu() for t in (send_low, send_high, recv_low, recv_high)]
+        exchange_faces(slab, hs[0], hs[1], hs[2], hs[3], group)
+        if slab.lower is not None:
+            recv_low.copy_(hs[2])
+        if slab.upper is not None:
+            recv_high.copy_(hs[3])
+        return
     ops = []
     if slab.lower is not None:
         ops.append(dist.P2POp(dist.isend, send_low, slab.lower, group, 0))        # travels down
