@@ -276,8 +276,11 @@ const char* lbm_last_error(const lbm_ctx* ctx);
  * Returns -1 for an unknown `what` or a NULL ctx. */
 long long lbm_query(const lbm_ctx* ctx, int what);
 
-/* Tuning knobs.  None changes a result (the A/B tests compare populations bit for bit).  Returns LBM_EINVAL for an
- * unknown key or value, LBM_ESTATE where noted.  Keys (every key the library accepts is listed here):
+/* Tuning knobs.  None changes what is computed: "cuda_graph", "pdl", "serpentine", "block_threads", "hrr_slab", "totals_waves"
+ * and "inplace" are schedules / storage schemes (A/B tests compare the populations bit for bit); "wm_prepass", "slip_planes" and
+ * "vector" route some cells through another kernel body with the same arithmetic (tested against each other to rounding and
+ * against the oracle to the parity tolerance).  Returns LBM_EINVAL for an unknown key or value, LBM_ESTATE where noted.  Keys
+ * (every key the library accepts is listed here):
  *   "cuda_graph"    0|1     1: lbm_step replays the steady-state time loop 8 steps at a time from a captured CUDA graph
  *                           (re-captured when parameters, fields or options change); steps that do not fill a chunk, the first
  *                           step of a fresh state, runs with the Vortex Method inlet and sub-domains use plain launches.
@@ -297,8 +300,9 @@ long long lbm_query(const lbm_ctx* ctx, int what);
  *                           chosen from the lattice size (about 8 z-iterations per block, 1 .. 16 waves)
  *   "serpentine"    0|1     consecutive launches sweep the z-slices in opposite directions for L2 reuse (default 1)
  *   "inplace"       0|1     1: a lattice of plain fluid cells, with or without resting SOLID cells (halfway bounce-back) but without
- *                           any inlet / outlet / wall-model / moving / slip cell, BGK form, steps IN PLACE on one array (AA pattern: even steps collide locally into the opposite slots, odd
- *                           steps pull and push through the neighbours); the second lattice is then never
+ *                           any inlet / outlet / wall-model / moving / slip cell, BGK form, steps IN PLACE on one array (AA pattern:
+ *                           even steps collide locally into the opposite slots, odd steps pull and push through the
+ *                           neighbours); the second lattice is then never
  *                           allocated unless a state read after an odd number of steps needs it.  Default 0 (two lattices)
  *   "vector"        0|1     0 forces the scalar kernel (one cell per thread) for every row length (default 1)
  *   "block_threads" 64|128|256   threads per block of the step kernels (default 64)
