@@ -214,6 +214,30 @@ int lbm_set_populations_box(lbm_ctx* ctx, int x0, int y0, int z0, int bx, int by
  * Errors: LBM_EINVAL (NULL ctx / out), LBM_ESTATE (no state), LBM_ECUDA. */
 int lbm_totals(lbm_ctx* ctx, double out[5]);
 
+/* The same totals for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): no context, and no cudaMalloc / cudaFree / allocating library routine anywhere on this call's path.  Same
+ * quantities as lbm_totals (row A9; the conserved moments of Eq. 6, l.97): out[0] = sum rho, out[1..3] = sum rho u,
+ * out[4] = sum rho |u|^2 / 2 over the non-wall cells of the state S_t the caller passes.
+ *   populations : [Q][nz][ny][nx] dtype, DEVICE pointer: the pre-collision populations S_t (what lbm_get_populations writes).
+ *   cell_flags  : [nz][ny][nx] uint8, DEVICE pointer, or NULL => no wall cells.  Flag bytes as in lbm_set_fields; only the type
+ *                 nibble is read (SOLID, MOVINGWALL, SLIPWALL cells do not count) and nothing is validated.
+ *   out         : 5 doubles, DEVICE pointer, written asynchronously on `cuda_stream` (a cudaStream_t as void*; NULL = the legacy
+ *                 default stream).  The caller owns all three buffers; nothing is copied.
+ * Its scratch (one partial sum per block of 8192 cells and quantity, and the ticket that finds the last block) is a file-scope
+ * `static __device__` array of LBM_STATIC_SCRATCH_BYTES that every GPU which loads the library holds until the process exits;
+ * hence the limit nx ny nz <= LBM_STATIC_MAX_CELLS (512^3), beyond which the call returns LBM_EINVAL (use lbm_totals).  The
+ * first call on a device resolves the array's address there (cudaGetSymbolAddress; make that call outside a graph capture).
+ * Every call on a device shares the array: each call clears the ticket on its stream before its launch (the partial sums
+ * need no clearing), but calls that OVERLAP on the same GPU (two streams, two host threads) race on it -- serialise them.
+ * The sums are taken in a fixed order (a function of nx ny nz only), in fp64 from the cell's moments on: repeated calls on the
+ * same data return the same bits.  Works on the current device; the pointers must belong to it.
+ * Errors: LBM_EINVAL (lattice / dtype / sizes, more than LBM_STATIC_MAX_CELLS cells, NULL populations / out, a host or
+ * misaligned pointer), LBM_ECUDA; lbm_last_error(NULL) holds the reason. */
+#define LBM_STATIC_MAX_CELLS 134217728LL
+#define LBM_STATIC_SCRATCH_BYTES 655616
+int lbm_totals_static(int lattice, int nx, int ny, int nz, int dtype, const void* populations, const uint8_t* cell_flags,
+                      double* out, void* cuda_stream);
+
 /* ---- Slab decomposition in z: one context per sub-domain (PAPER.md l.214-218 and Table 1 l.227-239: the
  * paper's scaling runs decompose the lattice over MPI ranks with a halo exchange per step).  The library provides the
  * sub-domain mechanics; the transfer itself (NCCL send/recv, peer copies, or a device copy between two contexts on one GPU)
@@ -262,7 +286,7 @@ int lbm_set_stream(lbm_ctx* ctx, void* cuda_stream);
 int lbm_synchronize(lbm_ctx* ctx);
 
 /* Static or ctx-owned message of the last error; valid until the next call on that ctx.
- * ctx == NULL returns the message of the last failed lbm_create. */
+ * ctx == NULL returns the message of the last failed lbm_create or lbm_totals_static. */
 const char* lbm_last_error(const lbm_ctx* ctx);
 
 /* Introspection used by the harness.  what:

@@ -9,10 +9,10 @@ from .binding import (LBM, LbmError, LbmParams, lbm_create, lbm_destroy, lbm_get
                       lbm_last_error, lbm_moments, lbm_query, lbm_set_fields, lbm_set_geometry, lbm_set_option,
                       lbm_set_stream, lbm_step, lbm_synchronize, lbm_totals, library_path, load_library, lbm_set_inflow,
                       lbm_set_vortices, lbm_get_inflow, lbm_set_porosity, lbm_set_body_velocity, lbm_get_populations_box,
-                      lbm_set_populations_box, lbm_set_halo, lbm_step_halo, lbm_halo_pack, lbm_halo_unpack)
+                      lbm_set_populations_box, lbm_set_halo, lbm_step_halo, lbm_halo_pack, lbm_halo_unpack, lbm_totals_static)
 
 __all__ = ["LBM", "LbmError", "LbmParams", "lbm_create", "lbm_destroy", "lbm_get_populations", "lbm_init_equilibrium",
            "lbm_last_error", "lbm_moments", "lbm_query", "lbm_set_fields", "lbm_set_geometry", "lbm_set_option",
            "lbm_set_stream", "lbm_step", "lbm_synchronize", "lbm_totals", "library_path", "load_library", "lbm_set_inflow",
            "lbm_set_vortices", "lbm_get_inflow", "lbm_set_porosity", "lbm_set_body_velocity", "lbm_get_populations_box",
-           "lbm_set_populations_box", "lbm_set_halo", "lbm_step_halo", "lbm_halo_pack", "lbm_halo_unpack"]
+           "lbm_set_populations_box", "lbm_set_halo", "lbm_step_halo", "lbm_halo_pack", "lbm_halo_unpack", "lbm_totals_static"]

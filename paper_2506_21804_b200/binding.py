@@ -19,7 +19,7 @@ EXPORTS = ["lbm_create", "lbm_destroy", "lbm_set_fields", "lbm_init_equilibrium"
            "lbm_moments", "lbm_get_populations", "lbm_totals", "lbm_set_stream", "lbm_synchronize", "lbm_last_error",
            "lbm_query", "lbm_set_option", "lbm_set_inflow", "lbm_set_vortices", "lbm_get_inflow",
            "lbm_set_porosity", "lbm_set_body_velocity", "lbm_get_populations_box", "lbm_set_populations_box",
-           "lbm_set_halo", "lbm_step_halo", "lbm_halo_pack", "lbm_halo_unpack"]
+           "lbm_set_halo", "lbm_step_halo", "lbm_halo_pack", "lbm_halo_unpack", "lbm_totals_static"]
 
 
 class LbmError(RuntimeError):
@@ -85,6 +85,7 @@ def load_library():
     L.lbm_halo_pack.argtypes = [vp, ip, ip, vp]
     L.lbm_halo_unpack.argtypes = [vp, ip, ip, vp]
     L.lbm_totals.argtypes = [vp, vp]
+    L.lbm_totals_static.argtypes = [ip, ip, ip, ip, ip, vp, vp, vp, vp]
     L.lbm_set_stream.argtypes = [vp, vp]
     L.lbm_synchronize.argtypes = [vp]
     L.lbm_last_error.argtypes = [vp]
@@ -224,6 +225,13 @@ def lbm_totals(ctx, out=None):
     out = (ctypes.c_double * 5)()
     _check(ctx, load_library().lbm_totals(ctx, ctypes.addressof(out)))
     return list(out)
+
+
+def lbm_totals_static(lattice, nx, ny, nz, dtype, populations, cell_flags, out, cuda_stream=None):
+    """The totals of a caller-held state without any allocation (static device scratch; include/lbm.h): device buffers only,
+    `out` = a device buffer of 5 doubles, filled asynchronously on `cuda_stream`"""
+    return _check(None, load_library().lbm_totals_static(lattice, nx, ny, nz, dtype, _ptr(populations), _ptr(cell_flags),
+                                                         _ptr(out), cuda_stream))
 
 
 def lbm_set_stream(ctx, cuda_stream):

@@ -1,6 +1,7 @@
 """Build step for the CUDA library (nvcc, sm_100a only).  `python -m paper_2506_21804_b200.build [--force] [-v]`.
 
-csrc/lbm_api.cu (host side of the C ABI, set-up kernels) + csrc/lbm_inst.cu compiled once per (lattice, dtype, part): seventeen
+csrc/lbm_api.cu (host side of the C ABI, set-up kernels) + csrc/lbm_static.cu (lbm_totals_static: static device scratch, nothing
+allocated) + csrc/lbm_inst.cu compiled once per (lattice, dtype, part): eighteen
 object files, built in parallel, linked into liblbm_b200.so next to this file."""
 import os
 import subprocess
@@ -15,7 +16,7 @@ HEADERS = ["lbm_kernels.cuh", "lbm_launch.cuh", "lbm_ctx.h", os.path.join("..", 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC"]
 # (object name, source, defines)
-UNITS = [("lbm_api", "lbm_api.cu", [])]
+UNITS = [("lbm_api", "lbm_api.cu", []), ("lbm_static", "lbm_static.cu", [])]
 for _q in (19, 27):
     for _t in ("float", "double"):
         for _part in (0, 1, 2, 3):
