@@ -248,6 +248,10 @@ def run_reference(args, rank, world):
     from oracle import oracle as O
     number, shape, dtype, extra = workload(args.workload)
     cores = O.max_threads()
+    if world > 1:
+        # torchrun exports OMP_NUM_THREADS=1 to every rank; rank 0 is the only one that works here, so it takes the host cores it may
+        # run on (the oracle takes its thread count as an argument)
+        cores = max(cores, len(os.sched_getaffinity(0)))
     total = max(args.steps + args.warmup, 1)
     # bounded sample: a reduced instance of the same generator, sized for roughly a minute in total
     cells_budget = max(int(60.0 * 1.0e6 / total), 4096)
