@@ -47,6 +47,9 @@
 //                          reading G10; Eq. 11 (l.94) in full, third-order term = projection on the
 //                          third-order Hermite polynomials the lattice supports (G9); sigma = 0 on
 //                          wall-model cells (l.131); FD velocity = u^ of the same time level (G30-G32)
+//   O2h', collision = 2    the same collision with the FD strain of Eq. 10 taken of u^(x, t - dt), the field of the previous
+//                          level (reading G41: l.172 calls the collision a local cell model at 188 bytes); the first step
+//                          of a call has no history and differences u^(x,t).  Pins L1-L5, tests/test_oracle_hrr_lag.py
 //
 // Pins (tests/test_oracle_*.py, all run with -m "not gpu"): P1 isotropy identities, P2
 // equilibrium fixed point, P3 conservation, P4 Cs=0 == separately written BGK, P5 porous
@@ -603,8 +606,8 @@ int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const u
   p.fringe_len = static_cast<int>(par[15]);  p.fringe_factor = par[16];
   if (p.fringe_len < 0 || p.fringe_factor < 0.0) return -1;
   if (!(p.tau0 > 0.5) || p.cs_smago < 0.0) return -1;
-  if (p.collision != 0 && p.collision != 1) return -1;
-  if (p.collision == 1 && !(p.sigma >= 0.0 && p.sigma <= 1.0)) return -1;
+  if (p.collision != 0 && p.collision != 1 && p.collision != 2) return -1;
+  if (p.collision >= 1 && !(p.sigma >= 0.0 && p.sigma <= 1.0)) return -1;
 #ifdef _OPENMP
   const int nth = (nthreads > 1) ? nthreads : 1;
 #else
@@ -626,7 +629,13 @@ int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const u
   }
   std::vector<double> uB(3 * wm_cells.size(), 0.0);
   std::vector<double> uhat;                                // u^(x,t), [3][N], HRR form only
-  if (p.collision == 1) uhat.assign(3 * static_cast<size_t>(N), 0.0);
+  if (p.collision >= 1) uhat.assign(3 * static_cast<size_t>(N), 0.0);
+  // collision = 2 (reading G41): the HRR form with the FD strain of Eq. 10 taken of u^(x, t - dt), the field of the PREVIOUS
+  // level (a collision that is local but for a stored field: l.172 quotes 188 bytes per collision for a "local cell model").
+  // The state of this form is (S_t, u^_{t-1}); a call starts without history: its first step differences u^(x, t) like
+  // collision = 1, every later step the field of the step before.
+  std::vector<double> uhat_prev;
+  if (p.collision == 2) uhat_prev.assign(3 * static_cast<size_t>(N), 0.0);
   double* cur = f;
   double* nxt = g.data();
 
@@ -659,7 +668,7 @@ int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const u
     // ---- O1b (HRR form): u^(x,t) of every cell, the field the FD strain is taken of (G30) ------
     // Wall cells at rest (SOLID, SLIPWALL): u^ = 0 whatever populations they hold (G30; G37: "the FD stencil sees u^ = 0 on
     // slip wall cells like on any resting wall").
-    if (p.collision == 1) {
+    if (p.collision >= 1) {
 #pragma omp parallel for num_threads(nth) if (nth > 1)
       for (int64_t x = 0; x < N; ++x) {
         const int type = flags ? cell_type(flags[x]) : FLUID;
@@ -684,6 +693,8 @@ int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const u
       }
     }
 
+    // the field Eq. 10 differences: u^ of this level, or (collision = 2, from the second step of the call on) of the previous one
+    const double* ufd = (p.collision == 2 && step > 0) ? uhat_prev.data() : uhat.data();
     // ---- O2: collide ------------------------------------------------------------------------
 #pragma omp parallel for num_threads(nth) if (nth > 1)
     for (int z = 0; z < nz; ++z)
@@ -711,7 +722,7 @@ int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const u
             const double xi = static_cast<double>(xx - (nx - 1 - p.fringe_len)) / p.fringe_len;
             tau0x = 0.5 + (p.tau0 - 0.5) * (1.0 + p.fringe_factor * xi * xi);
           }
-          if (p.collision == 1) {
+          if (p.collision >= 1) {
             // S^FD_ab = (D_a u^_b + D_b u^_a) / 2, D_a g = (g(x+e_a) - g(x-e_a)) / 2; periodic wrap, except
             // that the ghost planes beyond the INLET / OUTLET planes copy those planes (G32)
             const int pos[3] = {xx, y, z}, dim[3] = {nx, ny, nz};
@@ -724,7 +735,7 @@ int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const u
               if (a == 0 && type == INLET) qm[0] = xx;
               const int64_t sp = (static_cast<int64_t>(qp[2]) * ny + qp[1]) * nx + qp[0];
               const int64_t sm = (static_cast<int64_t>(qm[2]) * ny + qm[1]) * nx + qm[0];
-              for (int b = 0; b < 3; ++b) D[a][b] = 0.5 * (uhat[b * N + sp] - uhat[b * N + sm]);
+              for (int b = 0; b < 3; ++b) D[a][b] = 0.5 * (ufd[b * N + sp] - ufd[b * N + sm]);
             }
             double S[3][3];
             for (int a = 0; a < 3; ++a)
@@ -737,6 +748,7 @@ int step_impl(int Q, int nx, int ny, int nz, double* f, const double* d, const u
           for (int i = 0; i < Q; ++i) fstar[i * N + x] = fs[i];
         }
 
+    if (p.collision == 2) uhat_prev = uhat;                  // u^ of this level is the next step's history
     // ---- O3: stream (pull) with halfway bounce-back and outlet clamp -----------------------
 #pragma omp parallel for num_threads(nth) if (nth > 1)
     for (int z = 0; z < nz; ++z)

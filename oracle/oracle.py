@@ -160,7 +160,7 @@ def init_equilibrium(Q, rho, u):
 
 def pack_params(tau0, cs_smago=0.0, use_hlbm=0, u_in=(0.0, 0.0, 0.0), wm_enable=0, wm_kappa=0.41, wm_E=9.8,
                 collision=0, sigma=1.0, u_wall=(0.0, 0.0, 0.0), rho_out=1.0, fringe_len=0, fringe_factor=0.0):
-    """collision: 0 = BGK form (G1), 1 = HRR (Eq. 6-11); sigma = Eq. 7 hybridisation factor; u_wall = velocity of the
+    """collision: 0 = BGK form (G1), 1 = HRR (Eq. 6-11), 2 = HRR with the FD strain of the previous level (G41); sigma = Eq. 7 hybridisation factor; u_wall = velocity of the
     MOVINGWALL cells (G33)."""
     return np.array([tau0, cs_smago, float(use_hlbm), u_in[0], u_in[1], u_in[2], float(wm_enable),
                      wm_kappa, wm_E, float(collision), sigma, u_wall[0], u_wall[1], u_wall[2], rho_out, float(fringe_len), fringe_factor],
