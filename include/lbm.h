@@ -55,7 +55,7 @@ enum { LBM_OK = 0, LBM_EINVAL = -1, LBM_ENOMEM = -2, LBM_ECUDA = -3, LBM_ESTATE 
 enum { LBM_D3Q19 = 19, LBM_D3Q27 = 27 };
 enum { LBM_F32 = 4, LBM_F64 = 8 };
 enum { LBM_FLUID = 0, LBM_SOLID = 1, LBM_INLET = 2, LBM_OUTLET = 3, LBM_WALLMODEL = 4, LBM_MOVINGWALL = 5, LBM_POUTLET = 6, LBM_SLIPWALL = 7 };
-enum { LBM_COLLISION_BGK = 0, LBM_COLLISION_HRR = 1 };
+enum { LBM_COLLISION_BGK = 0, LBM_COLLISION_HRR = 1, LBM_COLLISION_HRR_LAG = 2 };
 enum { LBM_HALO_POPULATIONS = 0, LBM_HALO_UHAT = 1 };
 enum { LBM_SIDE_LOW = 0, LBM_SIDE_HIGH = 1 };
 
@@ -75,7 +75,14 @@ typedef struct {
                      * equilibrium (Eq. 11, G9), recursive-regularised f(1) (Eq. 8-9, G29), finite-
                      * difference part (Eq. 10, G10) hybridised by sigma (Eq. 7); the FD strain is the
                      * central difference of u^(x,t) of the same time level (G30-G32); sigma = 0 on
-                     * WALLMODEL cells when wm_enable (l.131).  Smagorinsky tau_eff as in the BGK form. */
+                     * WALLMODEL cells when wm_enable (l.131).  Smagorinsky tau_eff as in the BGK form.
+                     * LBM_COLLISION_HRR_LAG (2): the same collision with the FD strain of Eq. 10 taken of
+                     * u^(x, t - dt), the field the previous step formed (reading G41; l.172: a local cell
+                     * model at 188 bytes per collision): ONE pass over the lattice per step instead of two.
+                     * The state of this form is (S_t, u^ of the previous level): the first step after
+                     * lbm_set_fields / lbm_init_equilibrium / lbm_set_populations_box / lbm_set_geometry has no
+                     * history and differences u^(x,t) like form 1.  Not with MOVINGWALL cells, not on
+                     * sub-domains (LBM_EINVAL / LBM_ESTATE).                                          */
   double sigma;     /* Eq. 7 hybridisation factor in [0,1]; read only when collision == HRR         */
   double u_wall[3]; /* velocity of the MOVINGWALL cells: the lid of the lid-driven cavity benchmark (l.214).  Halfway
                      * bounce-back off a moving wall (reading G33): the population i returning from the wall gains
@@ -173,7 +180,7 @@ int lbm_get_inflow(lbm_ctx* ctx, void* u);
  * DESIGN.md 5.5) and 3 more values of dtype per cell (allocated on the first HRR step; LBM_ENOMEM if that fails).
  * With option "cuda_graph" steady-state steps are replayed 8 at a time from a captured CUDA graph.  Asynchronous.
  * Errors: LBM_EINVAL (NULL ctx/params, n_steps < 0, tau0 <= 0.5, cs_smago < 0, wm_enable with
- * wm_kappa <= 0 or wm_E <= 0, collision not 0/1, sigma outside [0,1] with HRR, rho_out < 0, fringe_len < 0, fringe_factor < 0), LBM_ESTATE (no state
+ * wm_kappa <= 0 or wm_E <= 0, collision not 0/1/2, sigma outside [0,1] with the HRR forms, rho_out < 0, fringe_len < 0, fringe_factor < 0), LBM_ESTATE (no state
  * set yet), LBM_ECUDA. */
 int lbm_step(lbm_ctx* ctx, int n_steps, const lbm_params* params);
 

@@ -97,7 +97,7 @@ int ensure_lattice1(lbm_ctx* c) {
 
 int launch_step(lbm_ctx* c, const lbm_params* p, int mode, int stage = -1) {
   { int rca = ensure_lattice1(c); if (rca != LBM_OK) return rca; }
-  const bool hrr = p && p->collision == LBM_COLLISION_HRR && mode != lbm::MODE_STREAM;
+  const bool hrr = p && p->collision != LBM_COLLISION_BGK && mode != lbm::MODE_STREAM;
   if (hrr) return LBM_DISPATCH(c, launch_step_hrr, c, p, mode, stage);
   if (stage == 0) return LBM_OK;
   return LBM_DISPATCH(c, launch_step_bgk, c, p, mode);
@@ -121,9 +121,11 @@ int check_params(lbm_ctx* c, const lbm_params* p) {
   if (!(p->u_in[0] < 1.0)) return fail(c, LBM_EINVAL, "lbm_step: u_in[0] = %g must be < 1", p->u_in[0]);
   if (p->rho_out < 0.0) return fail(c, LBM_EINVAL, "lbm_step: rho_out = %g must be > 0 (0 = default 1)", p->rho_out);
   if (p->fringe_len < 0 || !(p->fringe_factor >= 0.0)) return fail(c, LBM_EINVAL, "lbm_step: fringe_len = %d, fringe_factor = %g must be >= 0", p->fringe_len, p->fringe_factor);
-  if (p->collision != LBM_COLLISION_BGK && p->collision != LBM_COLLISION_HRR)
-    return fail(c, LBM_EINVAL, "lbm_step: collision = %d must be 0 (BGK) or 1 (HRR)", p->collision);
-  if (p->collision == LBM_COLLISION_HRR && !(p->sigma >= 0.0 && p->sigma <= 1.0))
+  if (p->collision != LBM_COLLISION_BGK && p->collision != LBM_COLLISION_HRR && p->collision != LBM_COLLISION_HRR_LAG)
+    return fail(c, LBM_EINVAL, "lbm_step: collision = %d must be 0 (BGK), 1 (HRR) or 2 (HRR, FD strain of the previous level)", p->collision);
+  if (p->collision == LBM_COLLISION_HRR_LAG && c && c->n_moving > 0)
+    return fail(c, LBM_EINVAL, "lbm_step: collision = 2 is not available with MOVINGWALL cells (use collision = 1)");
+  if (p->collision != LBM_COLLISION_BGK && !(p->sigma >= 0.0 && p->sigma <= 1.0))
     return fail(c, LBM_EINVAL, "lbm_step: sigma = %g must be in [0,1]", p->sigma);
   return LBM_OK;
 }
@@ -420,7 +422,7 @@ void lbm_destroy(lbm_ctx* c) {
     cudaStreamDestroy(c->vm_stream);
     cudaEventDestroy(c->ev_vm);  cudaEventDestroy(c->ev_step[0]);  cudaEventDestroy(c->ev_step[1]);
   }
-  cudaFree(c->f[0]);  cudaFree(c->f[1]);  cudaFree(c->d);  cudaFree(c->uhat);  cudaFree(c->ub);
+  cudaFree(c->f[0]);  cudaFree(c->f[1]);  cudaFree(c->d);  cudaFree(c->uhat);  cudaFree(c->uhat2);  cudaFree(c->ub);
   cudaFree(c->uin_mean);  cudaFree(c->uin_field[0]);  cudaFree(c->uin_field[1]);  cudaFree(c->vpos);  cudaFree(c->vsign);  cudaFree(c->vgamma);
   cudaFree(c->cls);  cudaFree(c->cls_alt);  cudaFree(c->flags_raw);
   cudaFree(c->counters);  cudaFree(c->totals_dev);  cudaFree(c->staging);
@@ -452,6 +454,7 @@ static int set_geometry_fields(lbm_ctx* c, const void* porosity, const uint8_t* 
   int rc = classify(c, cell_flags);
   if (rc != LBM_OK) return rc;
   c->gamma_dirty = true;   // A and the seeds' cells depend on the flags
+  c->lag_valid = false;    // collision = 2: a new geometry or state has no u^ history (G41)
   if (c->uhat)   // cells that turned SOLID must read u^ = 0 (the UHAT pass does not visit all-SOLID lines)
     LBM_CUDA(c, cudaMemsetAsync(c->uhat, 0, 3 * static_cast<size_t>(c->N) * c->dtype, c->stream));
   if (porosity) {
@@ -499,6 +502,7 @@ int lbm_init_equilibrium(lbm_ctx* c, const void* rho, const void* u) {
   c->cur = 0;
   c->phase = PHASE_PRE;
   c->solid_dirty = false;
+  c->lag_valid = false;
   c->steps = 0;
   { int rci = reset_inflow(c); if (rci != LBM_OK) return rci; }
   return solid_values(c, true);
@@ -763,12 +767,18 @@ static bool inplace_eligible(const lbm_ctx* c, const lbm_params* p) {
 // buffers a step needs beyond the lattices: u^ field (HRR form), u^B of the wall-model cells (pre-pass)
 static int step_buffers(lbm_ctx* c, const lbm_params* params, int n_steps) {
   int rc = LBM_OK;
-  if (params->collision == LBM_COLLISION_HRR && !c->uhat && n_steps > 0) {
+  if (params->collision != LBM_COLLISION_BGK && !c->uhat && n_steps > 0) {
     const size_t bytes = 3 * static_cast<size_t>(c->N) * c->dtype;
     rc = dev_alloc(c, &c->uhat, bytes);
     if (rc != LBM_OK) return rc;
     // SOLID cells of all-SOLID lines are never written by the UHAT pass: u^ = 0 there (resting wall) from here on
     LBM_CUDA(c, cudaMemsetAsync(c->uhat, 0, bytes, c->stream));
+    c->epoch++;
+  }
+  if (params->collision == LBM_COLLISION_HRR_LAG && !c->uhat2 && n_steps > 0) {     // G41: the second u^ buffer
+    rc = dev_alloc(c, &c->uhat2, 3 * static_cast<size_t>(c->N) * c->dtype);
+    if (rc != LBM_OK) return rc;
+    c->lag_valid = false;
     c->epoch++;
   }
   if (params->wm_enable && c->wm_prepass && c->n_wm > 0 && !c->wm_ub && n_steps > 0) {
@@ -813,7 +823,7 @@ int lbm_step(lbm_ctx* c, int n_steps, const lbm_params* params) {
     if (c->phase == PHASE_PRE) {
       rc = launch_step(c, params, lbm::MODE_COLLIDE);          // S_t -> F_t
       c->phase = PHASE_POST;
-    } else if (c->use_graph && !c->uin_mean && n_steps - s >= LBM_GRAPH_CHUNK) {
+    } else if (c->use_graph && !c->uin_mean && params->collision != LBM_COLLISION_HRR_LAG && n_steps - s >= LBM_GRAPH_CHUNK) {
       bool done = false;
       rc = graph_chunk(c, params, &done);
       if (rc != LBM_OK) return rc;
@@ -922,6 +932,7 @@ int lbm_set_populations_box(lbm_ctx* c, int x0, int y0, int z0, int bx, int by, 
   } else {
     rc = materialise(c);                 // the lattice must hold S_t itself (wall cells' own values included)
   }
+  c->lag_valid = false;                  // the state changes under the u^ history of collision = 2 (G41)
   if (rc != LBM_OK) return rc;
   const bool host = !is_device_pointer(populations);
   const void* src = populations;
@@ -1004,6 +1015,7 @@ int lbm_step_halo(lbm_ctx* c, const lbm_params* params, int stage) {
   if (stage != 0 && stage != 1) return fail(c, LBM_EINVAL, "lbm_step_halo: stage = %d must be 0 or 1", stage);
   if (c->phase == PHASE_NONE) return fail(c, LBM_ESTATE, "lbm_step_halo: no state");
   if (c->uin_mean) return fail(c, LBM_ESTATE, "lbm_step_halo: not available with the Vortex Method inlet");
+  if (params->collision == LBM_COLLISION_HRR_LAG) return fail(c, LBM_ESTATE, "lbm_step_halo: collision = 2 is not available on a sub-domain (use collision = 1)");
   if (stage != c->halo_stage) return fail(c, LBM_ESTATE, "lbm_step_halo: stage %d called where stage %d is due", stage, c->halo_stage);
   if (params->wm_enable && c->halo_wm_epoch != c->epoch) {       // the geometry changed since the cut was checked
     rc = check_wm_cut(c, c->ghost_lo, c->ghost_hi);

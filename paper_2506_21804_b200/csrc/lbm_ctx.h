@@ -87,6 +87,11 @@ struct lbm_ctx {
   long long ev_step_level[2];   // time level of the step after which ev_step[k] was recorded (-1: never)
   void* ub;              // prescribed solid velocity u^B [3][N] (lbm_set_body_velocity), nullptr = 0 everywhere
   void* uhat;            // HRR form: u^(x,t) [3][N], allocated on the first HRR step
+  // collision = 2 (G41): two u^ buffers (uhat, uhat2); buffer lag_cur holds u^ of the previous level while lag_valid; lag_active: the
+  // launch being prepared is the fused step of that form (make_args hands the two buffers to the kernel)
+  void* uhat2;
+  bool lag_valid, lag_active;
+  int lag_cur;
   int serpentine;        // 1: consecutive launches sweep z in opposite directions (L2 reuse)
   long long sweep_count; // BGK steps launched so far (parity = direction)
   int hrr_slab;          // HRR form: z-slices per slab of the two-pass step (0 = whole lattice)

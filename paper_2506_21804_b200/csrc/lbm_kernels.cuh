@@ -157,6 +157,9 @@ struct StepArgs {
   int nzs;                        // z-slices of this launch (grid.z = list_z + nzs, except in the totals modes, whose blocks loop over z)
   // HRR form (Eq. 7-11): u^(x,t) of every cell [3][N] (written by the MODE_UHAT_* pass, SOLID cells 0), Eq. 7 factor
   T* __restrict__ uhat;
+  // collision = 2 (reading G41: FD strain of the PREVIOUS level's u^): uhat holds u^(., t - dt), the fused step writes u^(., t) of its
+  // cells into uhat_out (a second [3][N] buffer whose wall entries are already in place); nullptr: the two-pass form
+  T* __restrict__ uhat_out;
   T sigma;
   const double* __restrict__ uin_field;  // [3][nz][ny] per-cell inlet velocity (Vortex Method inlet / mean profile) or nullptr => u_in;
                                          // fp64 for both dtypes: Eq. 21 normalises a gradient of this field (ill-conditioned in fp32)
@@ -326,7 +329,7 @@ __host__ __device__ constexpr double h3(int cx, int cy, int cz, int k) {
 // S[6] = S^FD_xx, yy, zz, xy, xz, yz.
 template <int Q, typename T>
 __device__ __forceinline__ void collide_cell_hrr(T (&f)[Q], T d, T ubx, T uby, T ubz, T tau0, T smago_k, T sigma,
-                                                 const T (&S)[6]) {
+                                                 const T (&S)[6], T& uox, T& uoy, T& uoz) {   // uo: u^(x,t) of the cell (Eq. 12)
   constexpr Stencil<Q> L{};
   constexpr int H = (Q - 1) / 2;
   T rho = f[0], jx = T(0), jy = T(0), jz = T(0);
@@ -351,6 +354,7 @@ __device__ __forceinline__ void collide_cell_hrr(T (&f)[Q], T d, T ubx, T uby, T
   const T ux = keep * (jx * inv_rho) + d * ubx;
   const T uy = keep * (jy * inv_rho) + d * uby;
   const T uz = keep * (jz * inv_rho) + d * ubz;
+  uox = ux;  uoy = uy;  uoz = uz;
   const T qx = rho * ux, qy = rho * uy, qz = rho * uz;
   const T third = rho * T(1.0 / 3.0);
   // a2 (= Pi of the BGK form, now against the third-order equilibrium: same second moment)
@@ -422,6 +426,12 @@ __device__ __forceinline__ void collide_cell_hrr(T (&f)[Q], T d, T ubx, T uby, T
     f[i + H] = even - odd;
   }
   f[0] = rho - (esum + esum);
+}
+
+template <int Q, typename T>
+__device__ __forceinline__ void collide_cell_hrr(T (&f)[Q], T d, T ubx, T uby, T ubz, T tau0, T smago_k, T sigma, const T (&S)[6]) {
+  T a, b, c;
+  collide_cell_hrr<Q, T>(f, d, ubx, uby, ubz, tau0, smago_k, sigma, S, a, b, c);
 }
 
 // O4 / reading R6: regularised velocity inlet on a cell of the plane x = 0 (inward normal +x).
@@ -918,7 +928,13 @@ __device__ __forceinline__ void step_cell_any(const StepArgs<T>& a, int x, int y
     if (COLL == COLL_HRR) {
       T S[6];
       fd_strain_cell<T>(a, x, y, z, type, S);
-      collide_cell_hrr<Q, T>(f, d, ubx, uby, ubz, tau0_at<T>(a, x), a.smago_k, wm ? T(0) : a.sigma, S);   // sigma = 0: l.131
+      T uox, uoy, uoz;
+      collide_cell_hrr<Q, T>(f, d, ubx, uby, ubz, tau0_at<T>(a, x), a.smago_k, wm ? T(0) : a.sigma, S, uox, uoy, uoz);   // sigma = 0: l.131
+      if (a.uhat_out != nullptr) {           // G41: this level's u^ is the next step's history
+        a.uhat_out[self] = uox;
+        a.uhat_out[a.N + self] = uoy;
+        a.uhat_out[2 * a.N + self] = uoz;
+      }
     } else {
       collide_cell<Q, T>(f, d, ubx, uby, ubz, tau0_at<T>(a, x), a.smago_k);
     }
@@ -1431,7 +1447,16 @@ __device__ __forceinline__ void step_vec_body(const StepArgs<T>& a, double (&acc
         }
         const T S[6] = {T(0.5) * D[0][0], T(0.5) * D[1][1], T(0.5) * D[2][2], T(0.25) * (D[0][1] + D[1][0]),
                         T(0.25) * (D[0][2] + D[2][0]), T(0.25) * (D[1][2] + D[2][1])};
-        collide_cell_hrr<Q, T>(fc, d[v], ubx, uby, ubz, tau0_at<T>(a, x0 + v), a.smago_k, wmc ? T(0) : a.sigma, S);   // sigma = 0: l.131
+        T uox, uoy, uoz;
+        collide_cell_hrr<Q, T>(fc, d[v], ubx, uby, ubz, tau0_at<T>(a, x0 + v), a.smago_k, wmc ? T(0) : a.sigma, S, uox, uoy, uoz);   // sigma = 0: l.131
+        if (a.uhat_out != nullptr) {         // G41: this level's u^ is the next step's history (wall cells of the vector: the wall's velocity)
+          const bool wl = (solid_bits >> v) & 1u;
+          const bool mv = ((clsw >> (8 * v)) & CLS_TYPE) == T_MOVING;
+          T* po = a.uhat_out + self + v;
+          po[0] = wl ? (mv ? a.u_wall[0] : T(0)) : uox;
+          po[N] = wl ? (mv ? a.u_wall[1] : T(0)) : uoy;
+          po[2 * N] = wl ? (mv ? a.u_wall[2] : T(0)) : uoz;
+        }
       } else {
         collide_cell<Q, T>(fc, d[v], ubx, uby, ubz, tau0_at<T>(a, x0 + v), a.smago_k);
       }

@@ -51,6 +51,11 @@ lbm::StepArgs<T> make_args(const lbm_ctx* c, const lbm_params* p, int in, int ou
   a.zi0 = zlo(c);
   a.zi1 = zlo(c) + zcount(c);
   a.uhat = static_cast<T*>(c->uhat);
+  a.uhat_out = nullptr;
+  if (c->lag_active) {                 // collision = 2: read the previous level's u^, write this level's
+    a.uhat = static_cast<T*>(c->lag_cur == 0 ? c->uhat : c->uhat2);
+    a.uhat_out = static_cast<T*>(c->lag_cur == 0 ? c->uhat2 : c->uhat);
+  }
   a.sigma = p ? static_cast<T>(p->sigma) : T(1);
   for (int k = 0; k < 3; ++k) a.u_wall[k] = p ? static_cast<T>(p->u_wall[k]) : T(0);
   a.rho_out = (p && p->rho_out > 0.0) ? static_cast<T>(p->rho_out) : T(1);
@@ -220,6 +225,25 @@ int launch_hrr_t(lbm_ctx* c, const lbm_params* p, int in, int out, int stage) {
   const bool halo = (c->ghost_lo + c->ghost_hi) > 0;
   int slab = (c->hrr_slab > 0 && !halo) ? c->hrr_slab : nz;
   int rc = LBM_OK;
+  if (p->collision == LBM_COLLISION_HRR_LAG) {
+    // G41: one pass per step.  Without history (fresh state) the u^ pass forms u^(., t) once, in buffer 0, whose copy gives buffer 1
+    // its wall entries; from then on the fused step reads the buffer the previous step wrote and writes the other one.
+    rc = launch_prepass<Q, T, lbm::mode_pulls(MODE_U)>(c, p, in, out);
+    if (rc != LBM_OK) return rc;
+    if (!c->lag_valid) {
+      rc = launch_one<Q, T, MODE_U, lbm::COLL_BGK>(c, p, in, out, zlo(c), zcount(c), true);
+      if (rc != LBM_OK) return rc;
+      LBM_CUDA(c, cudaMemcpyAsync(c->uhat2, c->uhat, 3 * static_cast<size_t>(c->N) * sizeof(T), cudaMemcpyDeviceToDevice, c->stream));
+      c->lag_cur = 0;
+    }
+    c->lag_active = true;
+    rc = launch_one<Q, T, MODE_S, lbm::COLL_HRR>(c, p, in, out, zlo(c), zcount(c), true);
+    c->lag_active = false;
+    if (rc != LBM_OK) return rc;
+    c->lag_cur = 1 - c->lag_cur;
+    c->lag_valid = true;
+    return LBM_OK;
+  }
   // stages of a step on a sub-domain (lbm_step_halo): 0 = pre-pass + u^ pass (the caller then exchanges the u^ boundary
   // slices), 1 = the fused step pass; stage < 0: the whole step
   if (stage != 1) rc = launch_prepass<Q, T, lbm::mode_pulls(MODE_U)>(c, p, in, out);

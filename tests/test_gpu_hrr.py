@@ -111,6 +111,6 @@ def test_hrr_switching_collision_between_calls_and_vector_off():
 def test_hrr_rejects_bad_sigma_and_collision():
     with P.LBM(19, 8, 8, 8, "f32") as sim:
         sim.init_equilibrium(np.ones((8, 8, 8), np.float32), np.zeros((3, 8, 8, 8), np.float32))
-        for bad in (dict(collision=1, sigma=1.5), dict(collision=1, sigma=-0.1), dict(collision=2)):
+        for bad in (dict(collision=1, sigma=1.5), dict(collision=1, sigma=-0.1), dict(collision=3), dict(collision=2, sigma=1.5)):
             with pytest.raises(P.LbmError):
                 sim.step(1, P.LbmParams(0.6, **bad))
