@@ -57,6 +57,13 @@ WORKLOADS["config3_urban_channel_384x192x128_f64_hrr"] = (3, None, "f64", HRR)
 WORKLOADS["config2_les_periodic_256_f32_hrr"] = (2, None, "f32", HRR)
 WORKLOADS["config4_d3q27_spheres_512_f32_hrr"] = (4, None, "f32", HRR)
 WORKLOADS["config5_urban_cube_512_f32_hrr"] = (5, (512, 512, 512), "f32", HRR)
+# the same collision with the FD strain of the previous level's u^ (collision = 2, reading G41): one pass per step
+HRRLAG = dict(collision=2, sigma=0.7)
+WORKLOADS["config3_urban_channel_384x192x128_f32_hrrlag"] = (3, None, "f32", HRRLAG)
+WORKLOADS["config3_urban_channel_384x192x128_f64_hrrlag"] = (3, None, "f64", HRRLAG)
+WORKLOADS["config2_les_periodic_256_f32_hrrlag"] = (2, None, "f32", HRRLAG)
+WORKLOADS["config4_d3q27_spheres_512_f32_hrrlag"] = (4, None, "f32", HRRLAG)
+WORKLOADS["config5_urban_cube_512_f32_hrrlag"] = (5, (512, 512, 512), "f32", HRRLAG)
 # lid-driven cavity, the paper's own scaling benchmark (fp32): closed box, moving lid
 for _n in (256, 512, 640):
     WORKLOADS["cavity_%d_f32" % _n] = (6, (_n, _n, _n), "f32")
@@ -333,12 +340,13 @@ def main():
     # (default): N copies of the workload's height stacked in z -- the same generator at (N nz, ny, nx) -- so every GPU keeps the
     # workload's own cell count; --strong cuts the workload's own lattice.  Workloads with the Vortex Method inlet (it needs the
     # whole inflow plane) and config 1 run as independent replicas.
-    decomposed = world > 1 and not args.replicas and number != 1 and workload_vm(args.workload, (8, 8, 8)) is None
+    decomposed = (world > 1 and not args.replicas and number != 1 and workload_vm(args.workload, (8, 8, 8)) is None
+                  and (extra or {}).get("collision", 0) != 2)       # (collision = 2 keeps a u^ history per context: replicas)
     if decomposed and not args.strong:
         base = shape or make_cfg(number, None, {})["shape"]
         shape = (base[0] * world, base[1], base[2])
     cfg = make_cfg_named(args.workload, number, shape, extra)
-    hrr = cfg["params"].get("collision", 0) == 1
+    hrr = cfg["params"].get("collision", 0) >= 1
     if args.steps is None:
         args.steps = cfg["steps"]
     Q = cfg["Q"]
