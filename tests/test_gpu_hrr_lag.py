@@ -135,3 +135,15 @@ def test_lag_is_refused_with_a_moving_lid_and_on_sub_domains():
         sim.set_halo(1, 1)
         with pytest.raises(P.LbmError):
             sim.step_halo(P.LbmParams(0.6, collision=2, sigma=0.7), 0)
+
+
+def test_lag_config3_full_size_windows():
+    """bench.py config3_urban_channel_384x192x128_f32_hrrlag at its own size, in the launch configuration bench.py times: light-cone
+    windows (floor with wall-model cells, inlet, outlet, buildings, trees, top) against the oracle on the cropped inputs; the strain
+    reads the previous level's u^, so information moves no faster than in the two-pass form (margin as there)"""
+    from test_gpu_fullsize import W, _check_windows
+    cfg = lag(I.make_config(3), 0.7)
+    nz, ny, nx = cfg["shape"]
+    wins = [(1, 10, 0), (1, 100, nx - W), (nz - 1 - W, 50, 200), (1, 60, 150), (60, 90, 190), (30, ny - 4, 100),
+            (20, 40, 120), (5, 130, 250)]
+    _check_windows(cfg, "f32", wins, (True, False, True), steps=6)
