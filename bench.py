@@ -73,10 +73,12 @@ WORKLOADS["cavity_512_f32_hrr"] = (6, (512, 512, 512), "f32", HRR)
 VM = dict(n_vortices=256, sigma_v=6.0, intensity=0.15)
 WORKLOADS["config3_urban_channel_384x192x128_f32_vm"] = (3, None, "f32", {}, VM)
 WORKLOADS["config3_urban_channel_384x192x128_f32_hrr_vm"] = (3, None, "f32", HRR, VM)
+WORKLOADS["config3_urban_channel_384x192x128_f32_hrrlag_vm"] = (3, None, "f32", HRRLAG, VM)
 # the urban channel in the paper's own boundary set (l.255: fixed-pressure outlet + fringe zone, full-slip outer walls, wall-modelled
 # floor) with the VM inlet; "_hrr_vm" is the paper's HHRRLBM-LES urban set-up as far as the paper defines it
 WORKLOADS["paperbc_urban_channel_384x192x128_f32_vm"] = (7, (128, 192, 384), "f32", {}, VM)
 WORKLOADS["paperbc_urban_channel_384x192x128_f32_hrr_vm"] = (7, (128, 192, 384), "f32", HRR, VM)
+WORKLOADS["paperbc_urban_channel_384x192x128_f32_hrrlag_vm"] = (7, (128, 192, 384), "f32", HRRLAG, VM)
 # moving porous bodies (Eq. 12 with u^B != 0): the trees of config 3 (0 < d < 1, 5 % of the cells) sway with a seeded
 # solid velocity field (lbm_inputs.body_velocity), set once through lbm_set_body_velocity
 BODY = dict(amp=0.02)
@@ -85,6 +87,7 @@ WORKLOADS["config3_urban_channel_384x192x128_f32_hrr_body"] = (3, None, "f32", H
 # the paper's boundary set with the wall model on the building faces too (config 8; SURVEY 8(f)-2 "wall model on building faces")
 WORKLOADS["paperbc_wmfaces_urban_channel_384x192x128_f32_vm"] = (8, (128, 192, 384), "f32", {}, VM)
 WORKLOADS["paperbc_wmfaces_urban_channel_384x192x128_f32_hrr_vm"] = (8, (128, 192, 384), "f32", HRR, VM)
+WORKLOADS["paperbc_wmfaces_urban_channel_384x192x128_f32_hrrlag_vm"] = (8, (128, 192, 384), "f32", HRRLAG, VM)
 # propagation bake-off: the fully periodic LES box of config 2 on two lattices (pull) and in place (AA pattern,
 # option "inplace"); at 768^3 fp64 one population set is 68.9 GB
 INPLACE = dict(inplace=1)

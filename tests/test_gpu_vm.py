@@ -43,7 +43,7 @@ def _gpu(cfg, vm, f, d, dtype, chunks):
 
 
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
-@pytest.mark.parametrize("coll", [0, 1])
+@pytest.mark.parametrize("coll", [0, 1, 2])
 def test_vm_inlet_parity(dtype, coll):
     cfg, vm = _case(extra=dict(collision=coll, sigma=0.7))
     f, d = oracle_inputs(cfg, dtype)
