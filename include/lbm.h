@@ -80,8 +80,8 @@ typedef struct {
                      * u^(x, t - dt), the field the previous step formed (reading G41; l.172: a local cell
                      * model at 188 bytes per collision): ONE pass over the lattice per step instead of two.
                      * The state of this form is (S_t, u^ of the previous level): the first step after
-                     * lbm_set_fields / lbm_init_equilibrium / lbm_set_populations_box / lbm_set_geometry has no
-                     * history and differences u^(x,t) like form 1.  Not with MOVINGWALL cells, not on
+                     * lbm_set_fields / lbm_init_equilibrium / lbm_set_populations_box / lbm_set_geometry, or after
+                     * steps of another form, has no history and differences u^(x,t) like form 1.  Not with MOVINGWALL cells, not on
                      * sub-domains (LBM_EINVAL / LBM_ESTATE).                                          */
   double sigma;     /* Eq. 7 hybridisation factor in [0,1]; read only when collision == HRR         */
   double u_wall[3]; /* velocity of the MOVINGWALL cells: the lid of the lid-driven cavity benchmark (l.214).  Halfway

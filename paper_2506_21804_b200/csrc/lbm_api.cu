@@ -799,6 +799,7 @@ int lbm_step(lbm_ctx* c, int n_steps, const lbm_params* params) {
   if (c->ghost_lo + c->ghost_hi > 0)
     return fail(c, LBM_ESTATE, "lbm_step: the context is a sub-domain with ghost slices (lbm_set_halo): advance it with lbm_step_halo and exchange the halos");
   c->last = *params;
+  if (params->collision != LBM_COLLISION_HRR_LAG && n_steps > 0) c->lag_valid = false;   // G41: steps of another form drop the u^ history
   rc = step_buffers(c, params, n_steps);
   if (rc != LBM_OK) return rc;
   int s = 0;
@@ -1026,6 +1027,7 @@ int lbm_step_halo(lbm_ctx* c, const lbm_params* params, int stage) {
     if (rc != LBM_OK) return rc;
   }
   c->last = *params;
+  c->lag_valid = false;
   rc = step_buffers(c, params, 1);
   if (rc != LBM_OK) return rc;
   const int mode = (c->phase == PHASE_PRE) ? lbm::MODE_COLLIDE : lbm::MODE_STREAM_COLLIDE;

@@ -119,6 +119,18 @@ def test_lag_history_chunks_state_reads_setters_and_launch_count():
         sim.step(3, par)
         sim.get_populations(b)
     assert field_error(b, ref, m) <= TOL["f32"]
+    # ... and steps of another form in between drop the history (the oracle: every call starts without one)
+    kw = dict(d=d.astype(np.float64), flags=cfg["flags"], nthreads=4)
+    r = O.step(f.astype(np.float64), nsteps=2, **kw, **cfg["params"])
+    r = O.step(r, nsteps=1, **kw, **one["params"])
+    r = O.step(r, nsteps=3, **kw, **cfg["params"])
+    with P.LBM(19, nx, ny, nz, "f32") as sim:
+        sim.set_fields(f, d, cfg["flags"])
+        sim.step(2, par)
+        sim.step(1, P.LbmParams(**one["params"]))
+        sim.step(3, par)
+        sim.get_populations(b)
+    assert field_error(b, r, m) <= TOL["f32"]
 
 
 def test_lag_is_refused_with_a_moving_lid_and_on_sub_domains():
