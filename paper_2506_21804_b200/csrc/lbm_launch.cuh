@@ -136,7 +136,8 @@ int launch_one(lbm_ctx* c, const lbm_params* p, int in, int out, int z0, int nzs
   }
   // serpentine sweep (lbm_set_option "serpentine", default 1): BGK steps alternate their direction with the time level; in the
   // HRR form the u^ pass runs downwards and the step pass upwards; a diagnostic pass runs against the last step
-  if (c->serpentine) a.z_reverse = lbm::mode_uhat(MODE) ? 1 : ((COLL == lbm::COLL_HRR) ? 0 : static_cast<int>(c->sweep_count & 1));
+  // (collision = 2 has no u^ pass: its fused steps alternate like the BGK steps)
+  if (c->serpentine) a.z_reverse = lbm::mode_uhat(MODE) ? 1 : ((COLL == lbm::COLL_HRR && !c->lag_active) ? 0 : static_cast<int>(c->sweep_count & 1));
   // programmatic dependent launch for the kernels of the time loop: resident while the predecessor drains.  After the wall-model
   // pre-pass (which itself waited for the lattice) only the threads that read its output wait ("pdl" = 2).
   const bool timeloop = lbm::mode_collides(MODE) || lbm::mode_uhat(MODE);
