@@ -68,6 +68,7 @@ WORKLOADS["config5_urban_cube_512_f32_hrrlag"] = (5, (512, 512, 512), "f32", HRR
 for _n in (256, 512, 640):
     WORKLOADS["cavity_%d_f32" % _n] = (6, (_n, _n, _n), "f32")
 WORKLOADS["cavity_512_f32_hrr"] = (6, (512, 512, 512), "f32", HRR)
+WORKLOADS["cavity_512_f32_hrrlag"] = (6, (512, 512, 512), "f32", HRRLAG)
 # Vortex Method inlet (Eq. 18-21) on the config-3 channel: power-law mean profile, 256 seeded vortices of size 6 cells,
 # intensity 0.15; "_hrr_vm" = the paper's urban set-up as far as this build has it (HRR + Smagorinsky + HLBM + wall model + VM)
 VM = dict(n_vortices=256, sigma_v=6.0, intensity=0.15)

@@ -81,8 +81,8 @@ typedef struct {
                      * model at 188 bytes per collision): ONE pass over the lattice per step instead of two.
                      * The state of this form is (S_t, u^ of the previous level): the first step after
                      * lbm_set_fields / lbm_init_equilibrium / lbm_set_populations_box / lbm_set_geometry, or after
-                     * steps of another form, has no history and differences u^(x,t) like form 1.  Not with MOVINGWALL cells, not on
-                     * sub-domains (LBM_EINVAL / LBM_ESTATE).                                          */
+                     * steps of another form, or with a new u_wall on a lattice with MOVINGWALL cells, has no
+                     * history and differences u^(x,t) like form 1.  Not on sub-domains (LBM_ESTATE).  */
   double sigma;     /* Eq. 7 hybridisation factor in [0,1]; read only when collision == HRR         */
   double u_wall[3]; /* velocity of the MOVINGWALL cells: the lid of the lid-driven cavity benchmark (l.214).  Halfway
                      * bounce-back off a moving wall (reading G33): the population i returning from the wall gains
@@ -177,8 +177,13 @@ int lbm_get_inflow(lbm_ctx* ctx, void* u);
  * BGK form: one fused kernel launch per step on the context's stream, preceded by the wall-model pre-pass over the
  * compact list of WALLMODEL cells when wm_enable and such cells exist (3 values of dtype per cell of device memory for
  * their u^B, allocated on the first such step).  HRR form: two launches per step (u^ pass, then the fused step;
- * DESIGN.md 5.5) and 3 more values of dtype per cell (allocated on the first HRR step; LBM_ENOMEM if that fails).
+ * DESIGN.md 5.5) and 3 more values of dtype per cell (allocated on the first HRR step; LBM_ENOMEM if that fails);
+ * collision = 2: one launch per step and 6 values per cell (the u^ pass runs only on the first step of a history).
  * With option "cuda_graph" steady-state steps are replayed 8 at a time from a captured CUDA graph.  Asynchronous.
+ * When params change from one call to the next: the storage holds the post-collision lattice, the propagation that ends a
+ * step runs as the pull of the NEXT step's launch, so the values the propagation reads from params (u_in, u_wall, rho_out) are
+ * those of the call that pulls.  A state read in between (lbm_get_populations) forms S_t with the params of the last step,
+ * after which a call with new params starts exactly where the method's own order (collide, then stream) would.
  * Errors: LBM_EINVAL (NULL ctx/params, n_steps < 0, tau0 <= 0.5, cs_smago < 0, wm_enable with
  * wm_kappa <= 0 or wm_E <= 0, collision not 0/1/2, sigma outside [0,1] with the HRR forms, rho_out < 0, fringe_len < 0, fringe_factor < 0), LBM_ESTATE (no state
  * set yet), LBM_ECUDA. */

@@ -123,8 +123,6 @@ int check_params(lbm_ctx* c, const lbm_params* p) {
   if (p->fringe_len < 0 || !(p->fringe_factor >= 0.0)) return fail(c, LBM_EINVAL, "lbm_step: fringe_len = %d, fringe_factor = %g must be >= 0", p->fringe_len, p->fringe_factor);
   if (p->collision != LBM_COLLISION_BGK && p->collision != LBM_COLLISION_HRR && p->collision != LBM_COLLISION_HRR_LAG)
     return fail(c, LBM_EINVAL, "lbm_step: collision = %d must be 0 (BGK), 1 (HRR) or 2 (HRR, FD strain of the previous level)", p->collision);
-  if (p->collision == LBM_COLLISION_HRR_LAG && c && c->n_moving > 0)
-    return fail(c, LBM_EINVAL, "lbm_step: collision = 2 is not available with MOVINGWALL cells (use collision = 1)");
   if (p->collision != LBM_COLLISION_BGK && !(p->sigma >= 0.0 && p->sigma <= 1.0))
     return fail(c, LBM_EINVAL, "lbm_step: sigma = %g must be in [0,1]", p->sigma);
   return LBM_OK;
@@ -800,6 +798,11 @@ int lbm_step(lbm_ctx* c, int n_steps, const lbm_params* params) {
     return fail(c, LBM_ESTATE, "lbm_step: the context is a sub-domain with ghost slices (lbm_set_halo): advance it with lbm_step_halo and exchange the halos");
   c->last = *params;
   if (params->collision != LBM_COLLISION_HRR_LAG && n_steps > 0) c->lag_valid = false;   // G41: steps of another form drop the u^ history
+  // ... and so does a new lid velocity: the u^ entries of MOVINGWALL cells in all-wall vectors are written by the u^ pass only
+  if (c->n_moving > 0 && std::memcmp(c->lag_u_wall, params->u_wall, sizeof(c->lag_u_wall)) != 0) {
+    c->lag_valid = false;
+    std::memcpy(c->lag_u_wall, params->u_wall, sizeof(c->lag_u_wall));
+  }
   rc = step_buffers(c, params, n_steps);
   if (rc != LBM_OK) return rc;
   int s = 0;

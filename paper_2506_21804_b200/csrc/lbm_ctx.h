@@ -92,6 +92,7 @@ struct lbm_ctx {
   void* uhat2;
   bool lag_valid, lag_active;
   int lag_cur;
+  double lag_u_wall[3];  // lid velocity the walls' u^ entries were written with
   int serpentine;        // 1: consecutive launches sweep z in opposite directions (L2 reuse)
   long long sweep_count; // BGK steps launched so far (parity = direction)
   int hrr_slab;          // HRR form: z-slices per slab of the two-pass step (0 = whole lattice)
