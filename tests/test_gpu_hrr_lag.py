@@ -172,3 +172,31 @@ def test_lag_config3_full_size_windows():
     wins = [(1, 10, 0), (1, 100, nx - W), (nz - 1 - W, 50, 200), (1, 60, 150), (60, 90, 190), (30, ny - 4, 100),
             (20, 40, 120), (5, 130, 250)]
     _check_windows(cfg, "f32", wins, (True, False, True), steps=6)
+
+
+@pytest.mark.parametrize("key,values", [("serpentine", (1, 0)), ("pdl", (2, 1, 0)), ("block_threads", (64, 128, 256)), ("cuda_graph", (0, 1)),
+                                        ("vector", (1, 0))])
+def test_lag_schedule_knobs_are_bit_identical(key, values):
+    """schedules, not arithmetic ("vector" = 0 routes every cell through the per-cell kernel: agreement to rounding); with
+    "cuda_graph" = 1 the form still steps with plain launches (its u^ buffers swap roles every step)"""
+    cfg = lag(I.make_config(3, shape=(24, 32, 96)), 0.7)
+    f, d = oracle_inputs(cfg, "f32")
+    nz, ny, nx = cfg["shape"]
+    par = P.LbmParams(**cfg["params"])
+    outs = []
+    for v in values:
+        with P.LBM(19, nx, ny, nz, "f32") as sim:
+            sim.set_option(key, v)
+            sim.set_fields(f, d, cfg["flags"])
+            sim.step(11, par)
+            sim.step(9, par)
+            assert sim.query("graph_launches") == 0
+            out = np.empty_like(f)
+            sim.get_populations(out)
+            outs.append(out)
+    for o in outs[1:]:
+        if key == "vector":
+            assert field_error(o, outs[0], nonsolid(cfg)) <= 2e-6
+        else:
+            assert np.array_equal(o, outs[0]), key
+    assert field_error(outs[0], run_oracle(cfg, f, d, 20), nonsolid(cfg)) <= 2 * TOL["f32"]
