@@ -344,8 +344,7 @@ def main():
     # (default): N copies of the workload's height stacked in z -- the same generator at (N nz, ny, nx) -- so every GPU keeps the
     # workload's own cell count; --strong cuts the workload's own lattice.  Workloads with the Vortex Method inlet (it needs the
     # whole inflow plane) and config 1 run as independent replicas.
-    decomposed = (world > 1 and not args.replicas and number != 1 and workload_vm(args.workload, (8, 8, 8)) is None
-                  and (extra or {}).get("collision", 0) != 2)       # (collision = 2 keeps a u^ history per context: replicas)
+    decomposed = world > 1 and not args.replicas and number != 1 and workload_vm(args.workload, (8, 8, 8)) is None
     if decomposed and not args.strong:
         base = shape or make_cfg(number, None, {})["shape"]
         shape = (base[0] * world, base[1], base[2])

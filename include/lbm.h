@@ -82,7 +82,8 @@ typedef struct {
                      * The state of this form is (S_t, u^ of the previous level): the first step after
                      * lbm_set_fields / lbm_init_equilibrium / lbm_set_populations_box / lbm_set_geometry, or after
                      * steps of another form, or with a new u_wall on a lattice with MOVINGWALL cells, has no
-                     * history and differences u^(x,t) like form 1.  Not on sub-domains (LBM_ESTATE).  */
+                     * history and differences u^(x,t) like form 1.  On sub-domains (lbm_step_halo) the u^
+                     * exchange in front of stage 1 carries the previous level's boundary slices.        */
   double sigma;     /* Eq. 7 hybridisation factor in [0,1]; read only when collision == HRR         */
   double u_wall[3]; /* velocity of the MOVINGWALL cells: the lid of the lid-driven cavity benchmark (l.214).  Halfway
                      * bounce-back off a moving wall (reading G33): the population i returning from the wall gains

@@ -1019,7 +1019,6 @@ int lbm_step_halo(lbm_ctx* c, const lbm_params* params, int stage) {
   if (stage != 0 && stage != 1) return fail(c, LBM_EINVAL, "lbm_step_halo: stage = %d must be 0 or 1", stage);
   if (c->phase == PHASE_NONE) return fail(c, LBM_ESTATE, "lbm_step_halo: no state");
   if (c->uin_mean) return fail(c, LBM_ESTATE, "lbm_step_halo: not available with the Vortex Method inlet");
-  if (params->collision == LBM_COLLISION_HRR_LAG) return fail(c, LBM_ESTATE, "lbm_step_halo: collision = 2 is not available on a sub-domain (use collision = 1)");
   if (stage != c->halo_stage) return fail(c, LBM_ESTATE, "lbm_step_halo: stage %d called where stage %d is due", stage, c->halo_stage);
   if (params->wm_enable && c->halo_wm_epoch != c->epoch) {       // the geometry changed since the cut was checked
     rc = check_wm_cut(c, c->ghost_lo, c->ghost_hi);
@@ -1030,7 +1029,11 @@ int lbm_step_halo(lbm_ctx* c, const lbm_params* params, int stage) {
     if (rc != LBM_OK) return rc;
   }
   c->last = *params;
-  c->lag_valid = false;
+  if (params->collision != LBM_COLLISION_HRR_LAG && stage != 1) c->lag_valid = false;   // G41: steps of another form drop the u^ history
+  if (c->n_moving > 0 && stage != 1 && std::memcmp(c->lag_u_wall, params->u_wall, sizeof(c->lag_u_wall)) != 0) {
+    c->lag_valid = false;
+    std::memcpy(c->lag_u_wall, params->u_wall, sizeof(c->lag_u_wall));
+  }
   rc = step_buffers(c, params, 1);
   if (rc != LBM_OK) return rc;
   const int mode = (c->phase == PHASE_PRE) ? lbm::MODE_COLLIDE : lbm::MODE_STREAM_COLLIDE;
@@ -1060,7 +1063,9 @@ static int halo_planes(lbm_ctx* c, const char* who, int what, int side, bool pac
     if (!c->uhat) return fail(c, LBM_ESTATE, "%s: no u^ field (the HRR form has not run yet)", who);
     hp->n = 3;
     hp->idx[0] = 0;  hp->idx[1] = 1;  hp->idx[2] = 2;
-    *field = c->uhat;
+    // collision = 2 (G41): the buffer the next fused step READS -- u^ of the previous level (or, on the first step of a history, the
+    // u^ pass's output), whose ghost slices the exchange fills
+    *field = (c->last.collision == LBM_COLLISION_HRR_LAG && c->uhat2 && c->lag_cur == 1) ? c->uhat2 : c->uhat;
     return LBM_OK;
   }
   // the populations that cross the cut: leaving downwards (c_z = -1) from the low boundary slice, upwards from the high one;

@@ -229,13 +229,19 @@ int launch_hrr_t(lbm_ctx* c, const lbm_params* p, int in, int out, int stage) {
   if (p->collision == LBM_COLLISION_HRR_LAG) {
     // G41: one pass per step.  Without history (fresh state) the u^ pass forms u^(., t) once, in buffer 0, whose copy gives buffer 1
     // its wall entries; from then on the fused step reads the buffer the previous step wrote and writes the other one.
-    rc = launch_prepass<Q, T, lbm::mode_pulls(MODE_U)>(c, p, in, out);
-    if (rc != LBM_OK) return rc;
-    if (!c->lag_valid) {
-      rc = launch_one<Q, T, MODE_U, lbm::COLL_BGK>(c, p, in, out, zlo(c), zcount(c), true);
+    // On a sub-domain (stages): stage 0 = pre-pass (+ the u^ pass of a fresh history); the caller then exchanges the boundary slices
+    // of the buffer the fused step is about to read (lbm_halo_pack / unpack with LBM_HALO_UHAT); stage 1 = the fused step.
+    if (stage != 1) {
+      rc = launch_prepass<Q, T, lbm::mode_pulls(MODE_U)>(c, p, in, out);
       if (rc != LBM_OK) return rc;
-      LBM_CUDA(c, cudaMemcpyAsync(c->uhat2, c->uhat, 3 * static_cast<size_t>(c->N) * sizeof(T), cudaMemcpyDeviceToDevice, c->stream));
-      c->lag_cur = 0;
+      if (!c->lag_valid) {
+        rc = launch_one<Q, T, MODE_U, lbm::COLL_BGK>(c, p, in, out, zlo(c), zcount(c), true);
+        if (rc != LBM_OK) return rc;
+        LBM_CUDA(c, cudaMemcpyAsync(c->uhat2, c->uhat, 3 * static_cast<size_t>(c->N) * sizeof(T), cudaMemcpyDeviceToDevice, c->stream));
+        c->lag_cur = 0;
+        c->lag_valid = true;             // (the history of this step: u^ of its own level)
+      }
+      if (stage == 0) return LBM_OK;
     }
     c->lag_active = true;
     rc = launch_one<Q, T, MODE_S, lbm::COLL_HRR>(c, p, in, out, zlo(c), zcount(c), true);

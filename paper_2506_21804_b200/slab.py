@@ -153,7 +153,7 @@ class SlabLBM:
         """n time steps of this rank's sub-domain, exchanging with the neighbouring ranks (every rank calls it)"""
         if self.slab.world == 1:
             return self.sim.step(n_steps, params)
-        hrr = params.collision == 1
+        hrr = params.collision >= 1        # both HRR forms exchange u^ boundary slices in front of the fused step
         for _ in range(n_steps):
             self.sim.step_halo(params, 0)
             if hrr:
@@ -193,7 +193,7 @@ class LocalGroup:
     def step(self, n_steps, params):
         if self.world == 1:
             return self.parts[0].sim.step(n_steps, params)
-        hrr = params.collision == 1
+        hrr = params.collision >= 1        # both HRR forms exchange u^ boundary slices in front of the fused step
         for _ in range(n_steps):
             for p in self.parts:
                 p.sim.step_halo(params, 0)

@@ -15,6 +15,7 @@ from parity_util import NP_DTYPE, TOL, field_error, nonsolid, oracle_inputs, run
 
 pytestmark = pytest.mark.gpu
 HRR = dict(collision=1, sigma=0.7)
+LAG = dict(collision=2, sigma=0.7)      # the HRR form in one pass (G41): the u^ exchange carries the previous level's boundary slices
 
 
 def _single(cfg, f, d, dtype, chunks):
@@ -66,6 +67,10 @@ CASES = {
     "spheres_d3q27_hrr_f32": (4, (32, 24, 64), HRR, "f32"),
     "cavity_bgk_f32": (6, (33, 24, 64), {}, "f32"),
     "cavity_hrr_f32": (6, (33, 24, 64), HRR, "f32"),
+    "periodic_les_lag_f64": (2, (30, 16, 64), LAG, "f64"),
+    "urban_channel_lag_f32": (3, (41, 24, 96), LAG, "f32"),
+    "spheres_d3q27_lag_f32": (4, (32, 24, 64), LAG, "f32"),
+    "cavity_lag_f32": (6, (33, 24, 64), LAG, "f32"),
     "paper_boundary_set_bgk_f32": (7, (40, 24, 96), {}, "f32"),
     "scalar_rows_bgk_f64": (3, (20, 12, 37), {}, "f64"),           # nx = 37: the one-cell-per-thread kernel
 }

@@ -154,26 +154,6 @@ def test_lag_lid_driven_cavity(dtype):
     assert field_error(out, r, nonsolid(cfg)) <= TOL[dtype]
 
 
-def test_lag_is_refused_on_sub_domains():
-    with P.LBM(19, 32, 16, 10, "f32") as sim:
-        sim.init_equilibrium(np.ones((10, 16, 32), np.float32), np.zeros((3, 10, 16, 32), np.float32))
-        sim.set_halo(1, 1)
-        with pytest.raises(P.LbmError):
-            sim.step_halo(P.LbmParams(0.6, collision=2, sigma=0.7), 0)
-
-
-def test_lag_config3_full_size_windows():
-    """bench.py config3_urban_channel_384x192x128_f32_hrrlag at its own size, in the launch configuration bench.py times: light-cone
-    windows (floor with wall-model cells, inlet, outlet, buildings, trees, top) against the oracle on the cropped inputs; the strain
-    reads the previous level's u^, so information moves no faster than in the two-pass form (margin as there)"""
-    from test_gpu_fullsize import W, _check_windows
-    cfg = lag(I.make_config(3), 0.7)
-    nz, ny, nx = cfg["shape"]
-    wins = [(1, 10, 0), (1, 100, nx - W), (nz - 1 - W, 50, 200), (1, 60, 150), (60, 90, 190), (30, ny - 4, 100),
-            (20, 40, 120), (5, 130, 250)]
-    _check_windows(cfg, "f32", wins, (True, False, True), steps=6)
-
-
 @pytest.mark.parametrize("key,values", [("serpentine", (1, 0)), ("pdl", (2, 1, 0)), ("block_threads", (64, 128, 256)), ("cuda_graph", (0, 1)),
                                         ("vector", (1, 0))])
 def test_lag_schedule_knobs_are_bit_identical(key, values):
